@@ -1,0 +1,129 @@
+/* pespace.h -- C ABI of libpespace.so: batched frequency-domain detector response and
+ * Whittle likelihood for MBHB signals in LISA-/Taiji-/TianQin-like detectors on B200.
+ *
+ * Method: arxiv 2602.12011 ("pespace"); citations are to /root/reference/PAPER.md lines.
+ *   single-link response      Eq. 5
+ *   TDI X,Y,Z, z = e^{-i2pi f L}  Eq. 6, generations 1.5 and 2.0
+ *   A, E, T channels          Eq. 3
+ *   time-frequency map t_f    Eq. 4
+ *   Whittle likelihood        Eq. 10, 11
+ *   Fisher matrix, <.|.>      Eq. 13, 14
+ * Waveform (BASELINE.json configs): TaylorF2 3.5PN phase, 0PN amplitude, modes
+ * (2,2),(2,1),(3,3),(3,2),(4,4) with Psi_lm(f) = (m/2) Psi_22(2f/m), t_lm(f) = t_22(2f/m);
+ * analytic Keplerian orbits.  All readings of what the paper leaves
+ * open are listed in DESIGN.md.
+ *
+ * Conventions
+ *  - Pointers named d_* are DEVICE pointers owned by the caller; the library neither frees
+ *    nor retains them past the call.  Pointers named h_* are HOST pointers.  Structs are
+ *    host memory, read during the call only.
+ *  - All arithmetic is IEEE FP64.  Complex numbers are interleaved (re, im) pairs.
+ *  - theta, 11 doubles per sample: [0] M total mass (detector frame, Msun), [1] q = m1/m2 >= 1,
+ *    [2] chi1, [3] chi2, [4] D_L (Gpc), [5] iota, [6] phi_c, [7] lambda (ecliptic longitude),
+ *    [8] beta (ecliptic latitude), [9] psi, [10] t_c (s from the start of the data, SSB time).
+ *  - Layouts are channel-planar and bin-contiguous: data [n_det][3][N][2], psd [n_det][3][N],
+ *    response out [B][n_det][3][N][2]; channel order A, E, T.  psd is the one-sided S_n(f_k)
+ *    in 1/Hz for the SAME TDI generation as the detector's tdi_gen.
+ *  - Calls are asynchronous on `stream` (a cudaStream_t passed as void*; NULL = default
+ *    stream); outputs are valid once the stream is synchronised.  The *_host calls are
+ *    synchronous.  Same inputs give bit-identical outputs (fixed reduction order).
+ *  - Return value: PESPACE_OK, or a negative code.  Nothing is printed, nothing throws.
+ *  - Per-sample domain errors cannot be seen by the host: a sample with a non-finite entry,
+ *    M <= 0, q < 1 or D_L <= 0 gets lnL = -INFINITY and NaN-filled response / Fisher rows.
+ *  - Bins whose psd is 0, negative or non-finite carry weight 0 (e.g. exact TDI nulls).
+ */
+#ifndef PESPACE_H
+#define PESPACE_H
+#include <stddef.h>
+#include <stdint.h>
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define PESPACE_OK 0
+#define PESPACE_EINVAL (-1) /* null pointer, B<=0, N<=0, df<=0, f0<=0, unknown kind/tdi_gen, empty or
+                               unknown mode_mask, n_det outside 1..PESPACE_MAX_DET, workspace too small */
+#define PESPACE_ECUDA (-2)  /* CUDA launch / runtime error; text via pespace_strerror() */
+#define PESPACE_ENOMEM (-3) /* device or pinned-host allocation failed (host-buffer calls only) */
+
+#define PESPACE_NPAR 11
+#define PESPACE_MAX_DET 8
+
+#define PESPACE_MODE_22 1u
+#define PESPACE_MODE_21 2u
+#define PESPACE_MODE_33 4u
+#define PESPACE_MODE_32 8u
+#define PESPACE_MODE_44 16u
+
+typedef struct {
+  int32_t kind;    /* 0 heliocentric (LISA-/Taiji-like), 1 geocentric (TianQin-like) */
+  int32_t tdi_gen; /* 15 or 20: X_1.5 or X_2.0 of Eq. 6 */
+  double L_m;      /* arm length, metres */
+  double kappa;    /* kind 0: guiding-centre phase relative to Earth at t = 0 (rad) */
+  double lambda0;  /* kind 0: constellation rotation phase; kind 1: orbital phase phi0 (rad) */
+  double period_s; /* kind 1: spacecraft orbital period (s) */
+  double lon, lat; /* kind 1: fixed pointing of the orbit normal, ecliptic (rad) */
+} pespace_detector;
+
+typedef struct { double f0, df; int64_t N; } pespace_grid; /* f_k = fma((double)k, df, f0); T = 1/df */
+
+typedef struct {
+  uint32_t mode_mask; /* OR of PESPACE_MODE_* */
+  int32_t n_det;
+  const pespace_detector* det; /* host array [n_det] */
+} pespace_model;
+
+/* Detector response (Eq. 5 -> Eq. 6 -> Eq. 3, summed over the modes of the mask).
+ *   d_params [B][11], d_freqs [N] (Hz; bins with f <= 0 produce 0), d_out_AET [B][n_det][3][N][2]. */
+int pespace_response(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
+                     const pespace_model* model, double* d_out_AET, void* stream);
+
+/* Scratch the likelihood / Fisher calls need for (B, grid, model). */
+size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespace_model* model,
+                               int want_fisher);
+
+/* lnL_b = -1/2 sum_det sum_{c in A,E,T} 4 df sum_k |d_c(f_k) - h_c(f_k; theta_b)|^2 / S_c(f_k)
+ * (Eq. 10, 11 with T = 1/df; additive constants dropped).
+ *   d_params [B][11], d_data_AET [n_det][3][N][2], d_psd [n_det][3][N], d_out_lnL [B],
+ *   d_workspace >= pespace_workspace_bytes(B, grid, model, 0) bytes, 16-byte aligned. */
+int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                    const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                    void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Forward-mode derivatives (Eq. 13, 14): F_ij = <d_i h | d_j h>, grad_i = d lnL / d theta_i
+ * = <d - h | d_i h>, derivatives w.r.t. the 11 raw theta entries.
+ *   d_out_F [B][11][11] symmetric, full storage; d_out_grad [B][11] or NULL;
+ *   d_data_AET may be NULL: then the gradient is skipped. */
+int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                   const pespace_grid* grid, const pespace_model* model, double* d_out_F,
+                   double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
+
+/* Host-buffer twin of pespace_loglike for end-to-end use: copies params, data and psd to the
+ * device, runs the same kernels, copies lnL back and synchronises.  All pointers are HOST
+ * pointers; device scratch is allocated and freed inside the call. */
+int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET,
+                         const double* h_psd, const pespace_grid* grid, const pespace_model* model,
+                         double* h_out_lnL);
+
+/* FP64 FMA micro-benchmark used as the roofline denominator: runs `iters` dependent-chain
+ * DFMA blocks on every SM and returns the sustained rate in TFLOP/s (FMA = 2 flop) and the
+ * kernel time in ms.  Synchronous. */
+int pespace_fp64_peak(int iters, double* h_out_tflops, double* h_out_ms);
+
+/* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel
+ * (the fused per-bin likelihood kernel) is bracketed by CUDA events on the launching stream.
+ * pespace_profile_read synchronises those events and returns the summed kernel time in ms and
+ * the number of launches since the last read (either pointer may be NULL), then resets. */
+int pespace_profile_enable(int on);
+int pespace_profile_read(double* h_main_ms, int64_t* h_launches);
+
+/* Number of kernels this library has launched since load (all calls, all streams). */
+int64_t pespace_launch_count(void);
+
+const char* pespace_strerror(int code);
+const char* pespace_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

@@ -1,0 +1,206 @@
+"""Thin ctypes binding over libpespace.so (include/pespace.h).  Argument marshalling only:
+every step of the hot path runs in the CUDA kernels.  There is NO CPU fallback -- if the
+shared library is missing this module raises at import, and every compute call needs a
+CUDA device.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import Optional
+
+import numpy as np
+import torch
+
+NPAR = 11
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libpespace.so")
+
+EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
+           "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
+           "pespace_launch_count", "pespace_strerror",
+           "pespace_version")
+
+
+class PespaceError(RuntimeError):
+    pass
+
+
+class _Det(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("tdi_gen", C.c_int32), ("L_m", C.c_double), ("kappa", C.c_double),
+                ("lambda0", C.c_double), ("period_s", C.c_double), ("lon", C.c_double), ("lat", C.c_double)]
+
+
+class _Grid(C.Structure):
+    _fields_ = [("f0", C.c_double), ("df", C.c_double), ("N", C.c_int64)]
+
+
+class _Model(C.Structure):
+    _fields_ = [("mode_mask", C.c_uint32), ("n_det", C.c_int32), ("det", C.POINTER(_Det))]
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2602_12011_b200.build` "
+                          "(there is no CPU fallback)")
+    L = C.CDLL(LIB_PATH)
+    vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
+    L.pespace_response.argtypes = [vp, i64, vp, i64, C.POINTER(_Model), vp, vp]
+    L.pespace_workspace_bytes.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model), C.c_int]
+    L.pespace_workspace_bytes.restype = sz
+    L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
+    L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
+    L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
+    L.pespace_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.pespace_profile_enable.argtypes = [C.c_int]
+    L.pespace_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i64)]
+    L.pespace_launch_count.restype = i64
+    L.pespace_strerror.argtypes = [C.c_int]
+    L.pespace_strerror.restype = C.c_char_p
+    L.pespace_version.restype = C.c_char_p
+    return L
+
+
+_lib = _load()
+
+
+def lib():
+    return _lib
+
+
+def _check(rc: int, what: str) -> None:
+    if rc != 0:
+        raise PespaceError(f"{what} failed: {_lib.pespace_strerror(rc).decode()} (code {rc})")
+
+
+def _model(model):
+    dets = (_Det * len(model.detectors))(*[
+        _Det(int(d.kind), int(d.tdi_gen), float(d.L_m), float(d.kappa), float(d.lambda0),
+             float(d.period_s), float(d.lon), float(d.lat)) for d in model.detectors])
+    return _Model(int(model.mode_mask), len(model.detectors), dets), dets
+
+
+def _grid(grid):
+    return _Grid(float(grid.f0), float(grid.df), int(grid.N))
+
+
+def _dev(t: torch.Tensor, name: str) -> torch.Tensor:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()):
+        raise PespaceError(f"{name}: expected a contiguous float64 CUDA tensor")
+    return t
+
+
+def _stream_ptr() -> int:
+    return torch.cuda.current_stream().cuda_stream
+
+
+def version() -> str:
+    return _lib.pespace_version().decode()
+
+
+def launch_count() -> int:
+    return int(_lib.pespace_launch_count())
+
+
+def workspace_bytes(B: int, grid, model, want_fisher: bool = False) -> int:
+    m, keep = _model(model)
+    g = _grid(grid)
+    return int(_lib.pespace_workspace_bytes(int(B), C.byref(g), C.byref(m), int(want_fisher)))
+
+
+def response(params: torch.Tensor, freqs: torch.Tensor, model, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """params [B][11], freqs [N] (device, f64) -> complex128 [B][n_det][3][N] (device)."""
+    p, f = _dev(params, "params"), _dev(freqs, "freqs")
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    if out is None:
+        out = torch.empty((B, nd, 3, N, 2), dtype=torch.float64, device=p.device)
+    m, keep = _model(model)
+    _check(_lib.pespace_response(p.data_ptr(), B, f.data_ptr(), N, C.byref(m), _dev(out, "out").data_ptr(),
+                                 _stream_ptr()), "pespace_response")
+    return torch.view_as_complex(out)
+
+
+class Likelihood:
+    """Data, PSD and workspace resident on the device; one call per batch of samples."""
+
+    def __init__(self, data: torch.Tensor, psd: torch.Tensor, grid, model, max_batch: int):
+        nd = len(model.detectors)
+        d = torch.view_as_real(data) if data.is_complex() else data
+        self.data = _dev(d.contiguous(), "data")
+        self.psd = _dev(psd.contiguous(), "psd")
+        if tuple(self.data.shape) != (nd, 3, grid.N, 2) or tuple(self.psd.shape) != (nd, 3, grid.N):
+            raise PespaceError("data must be [n_det][3][N] complex and psd [n_det][3][N]")
+        self.grid, self.model, self.max_batch = grid, model, int(max_batch)
+        self._m, self._keep = _model(model)
+        self._g = _grid(grid)
+        self.ws_bytes = workspace_bytes(max_batch, grid, model)
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=self.data.device)
+
+    def __call__(self, params: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        p = _dev(params, "params")
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        if out is None:
+            out = torch.empty(B, dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_loglike(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g),
+                                    C.byref(self._m), _dev(out, "out").data_ptr(), self.ws.data_ptr(),
+                                    self.ws_bytes, _stream_ptr()), "pespace_loglike")
+        return out
+
+
+def loglike(params: torch.Tensor, data: torch.Tensor, psd: torch.Tensor, grid, model) -> torch.Tensor:
+    return Likelihood(data, psd, grid, model, params.shape[0])(params)
+
+
+def fisher(params: torch.Tensor, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):
+    """-> (F [B][11][11], grad [B][11] or None)."""
+    p = _dev(params, "params")
+    B = p.shape[0]
+    m, keep = _model(model)
+    g = _grid(grid)
+    nbytes = workspace_bytes(B, grid, model, True)
+    ws = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=p.device)
+    F = torch.empty((B, NPAR, NPAR), dtype=torch.float64, device=p.device)
+    grad, dptr = None, None
+    if data is not None:
+        d = torch.view_as_real(data) if data.is_complex() else data
+        d = _dev(d.contiguous(), "data")
+        dptr = d.data_ptr()
+        grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+    _check(_lib.pespace_fisher(p.data_ptr(), B, dptr, _dev(psd.contiguous(), "psd").data_ptr(), C.byref(g),
+                               C.byref(m), F.data_ptr(), None if grad is None else grad.data_ptr(),
+                               ws.data_ptr(), nbytes, _stream_ptr()), "pespace_fisher")
+    return F, grad
+
+
+def loglike_host(params: np.ndarray, data: np.ndarray, psd: np.ndarray, grid, model) -> np.ndarray:
+    """End-to-end call on HOST numpy buffers: H2D copies, kernels and the D2H copy of lnL all
+    happen inside the C call (pespace_loglike_host)."""
+    p = np.ascontiguousarray(params, dtype=np.float64)
+    d = np.ascontiguousarray(data, dtype=np.complex128)
+    s = np.ascontiguousarray(psd, dtype=np.float64)
+    out = np.empty(p.shape[0], dtype=np.float64)
+    m, keep = _model(model)
+    g = _grid(grid)
+    _check(_lib.pespace_loglike_host(p.ctypes.data, p.shape[0], d.ctypes.data, s.ctypes.data, C.byref(g),
+                                     C.byref(m), out.ctypes.data), "pespace_loglike_host")
+    return out
+
+
+def fp64_peak(iters: int = 4096):
+    """-> (TFLOP/s, ms) of the DFMA micro-benchmark."""
+    t, ms = C.c_double(), C.c_double()
+    _check(_lib.pespace_fp64_peak(int(iters), C.byref(t), C.byref(ms)), "pespace_fp64_peak")
+    return t.value, ms.value
+
+
+def profile_enable(on: bool) -> None:
+    _check(_lib.pespace_profile_enable(int(bool(on))), "pespace_profile_enable")
+
+
+def profile_read():
+    """-> (summed ms of the dominant kernel, number of its launches) since the last read."""
+    ms, n = C.c_double(), C.c_int64()
+    _check(_lib.pespace_profile_read(C.byref(ms), C.byref(n)), "pespace_profile_read")
+    return ms.value, int(n.value)

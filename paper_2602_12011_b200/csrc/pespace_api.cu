@@ -1,0 +1,295 @@
+// pespace_api.cu -- the C ABI of include/pespace.h: argument checks, workspace carving, launches.
+#include "../../include/pespace.h"
+#include "pespace_device.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+using namespace pespace;
+
+namespace {
+
+std::atomic<long long> g_launches{0};
+thread_local char g_cuda_msg[256] = "";
+
+int cuda_fail(cudaError_t e) {
+  snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error: %s", cudaGetErrorString(e));
+  return PESPACE_ECUDA;
+}
+#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+#define LAUNCHED() do { ++g_launches; cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
+
+// optional event timing of the dominant kernel (pespace_profile_enable / _read)
+struct EvPair { cudaEvent_t a, b; };
+bool g_profile = false;
+std::vector<EvPair> g_events;
+std::mutex g_ev_mutex;
+
+bool model_ok(const pespace_model* m) {
+  if (!m || !m->det || m->n_det < 1 || m->n_det > PESPACE_MAX_DET) return false;
+  if ((m->mode_mask & 31u) == 0 || (m->mode_mask & ~31u) != 0) return false;
+  for (int i = 0; i < m->n_det; ++i) {
+    const pespace_detector& d = m->det[i];
+    if (d.kind != 0 && d.kind != 1) return false;
+    if (d.tdi_gen != 15 && d.tdi_gen != 20) return false;
+    if (!(d.L_m > 0.0) || !std::isfinite(d.L_m)) return false;
+    if (d.kind == 1 && !(d.period_s > 0.0)) return false;
+  }
+  return true;
+}
+bool grid_ok(const pespace_grid* g) {
+  return g && g->N > 0 && g->df > 0.0 && g->f0 > 0.0 && std::isfinite(g->df) && std::isfinite(g->f0);
+}
+
+DetC make_det(const pespace_detector& d) {
+  DetC c;
+  std::memset(&c, 0, sizeof c);
+  c.Lbar = d.L_m / kC;
+  c.kind = d.kind; c.gen = d.tdi_gen;
+  c.kappa = d.kappa; c.lambda0 = d.lambda0; c.period_s = d.period_s; c.lon = d.lon; c.lat = d.lat;
+  c.yr_over_p = (d.kind == 1) ? kYear / d.period_s : 0.0;
+  for (int n = 0; n < 3; ++n) {
+    const double ang = 2.0 * kPi * n / 3.0 + (d.kind == 0 ? d.lambda0 : 0.0);
+    c.cn[n] = std::cos(ang); c.sn[n] = std::sin(ang);
+  }
+  // arms a: 2-3, b: 3-1, c: 1-2
+  const int r[3] = {1, 2, 0}, s[3] = {2, 0, 1};
+  for (int l = 0; l < 3; ++l) { c.dcn[l] = c.cn[r[l]] - c.cn[s[l]]; c.dsn[l] = c.sn[r[l]] - c.sn[s[l]]; }
+  return c;
+}
+
+unsigned class_mask(unsigned mode_mask) {
+  unsigned m = 0;
+  if (mode_mask & PESPACE_MODE_21) m |= 1u;                       // m = 1
+  if (mode_mask & (PESPACE_MODE_22 | PESPACE_MODE_32)) m |= 2u;   // m = 2
+  if (mode_mask & PESPACE_MODE_33) m |= 4u;                       // m = 3
+  if (mode_mask & PESPACE_MODE_44) m |= 8u;                       // m = 4
+  return m;
+}
+
+size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+struct Plan {
+  int n_det, stride;
+  long long nbb;          // bin blocks
+  long long ntile;        // sample tiles
+  size_t consts_bytes, partial_bytes;
+};
+Plan make_plan(long long B, long long N, int n_det) {
+  Plan p;
+  p.n_det = n_det;
+  p.stride = sample_stride(n_det);
+  p.nbb = (N + BLOCK - 1) / BLOCK;
+  p.ntile = (B + TILE - 1) / TILE;
+  p.consts_bytes = align_up((size_t)B * p.stride * sizeof(double), 256);
+  p.partial_bytes = align_up((size_t)n_det * p.nbb * (size_t)B * sizeof(double), 256);
+  return p;
+}
+
+int run_prep(const double* d_params, long long B, const pespace_model* model, double* d_consts, cudaStream_t st) {
+  PrepArgs A;
+  std::memset(&A, 0, sizeof A);
+  A.n_det = model->n_det;
+  A.mode_mask = model->mode_mask;
+  for (int i = 0; i < model->n_det; ++i) A.det[i] = make_det(model->det[i]);
+  const int th = 128;
+  prep_samples_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
+  LAUNCHED();
+  return PESPACE_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* pespace_version(void) { return "pespace-b200 0.1 (sm_100a, fp64)"; }
+
+const char* pespace_strerror(int code) {
+  switch (code) {
+    case PESPACE_OK: return "ok";
+    case PESPACE_EINVAL: return "invalid argument";
+    case PESPACE_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case PESPACE_ENOMEM: return "out of memory";
+    default: return "unknown error code";
+  }
+}
+
+int64_t pespace_launch_count(void) { return (int64_t)g_launches.load(); }
+
+int pespace_profile_enable(int on) {
+  g_profile = on != 0;
+  return PESPACE_OK;
+}
+
+int pespace_profile_read(double* h_main_ms, int64_t* h_launches) {
+  std::lock_guard<std::mutex> lk(g_ev_mutex);
+  double total = 0.0;
+  int rc = PESPACE_OK;
+  for (const EvPair& ev : g_events) {
+    float ms = 0.f;
+    cudaError_t e = cudaEventSynchronize(ev.b);
+    if (e == cudaSuccess) e = cudaEventElapsedTime(&ms, ev.a, ev.b);
+    if (e != cudaSuccess) rc = cuda_fail(e);
+    total += ms;
+    cudaEventDestroy(ev.a);
+    cudaEventDestroy(ev.b);
+  }
+  if (h_main_ms) *h_main_ms = total;
+  if (h_launches) *h_launches = (int64_t)g_events.size();
+  g_events.clear();
+  return rc;
+}
+
+size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespace_model* model, int want_fisher) {
+  if (B <= 0 || !grid_ok(grid) || !model_ok(model)) return 0;
+  (void)want_fisher;
+  const Plan p = make_plan(B, grid->N, model->n_det);
+  return p.consts_bytes + p.partial_bytes;
+}
+
+int pespace_response(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
+                     const pespace_model* model, double* d_out_AET, void* stream) {
+  if (!d_params || !d_freqs || !d_out_AET || B <= 0 || N <= 0 || !model_ok(model)) return PESPACE_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Plan p = make_plan(B, N, model->n_det);
+  double* d_consts = nullptr;
+  CU(cudaMallocAsync((void**)&d_consts, p.consts_bytes, st));
+  int rc = run_prep(d_params, B, model, d_consts, st);
+  if (rc == PESPACE_OK) {
+    const unsigned cm = class_mask(model->mode_mask);
+    const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
+    for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
+      const DetC dc = make_det(model->det[d]);
+      if (dc.kind == 0)
+        response_kernel<0><<<grid, BLOCK, 0, st>>>(d_consts, B, d_freqs, N, dc, model->n_det, d, cm, (double2*)d_out_AET);
+      else
+        response_kernel<1><<<grid, BLOCK, 0, st>>>(d_consts, B, d_freqs, N, dc, model->n_det, d, cm, (double2*)d_out_AET);
+      ++g_launches;
+      cudaError_t e = cudaGetLastError();
+      if (e != cudaSuccess) rc = cuda_fail(e);
+    }
+  }
+  cudaError_t e = cudaFreeAsync(d_consts, st);
+  if (rc == PESPACE_OK && e != cudaSuccess) rc = cuda_fail(e);
+  return rc;
+}
+
+int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                    const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                    void* d_workspace, size_t workspace_bytes, void* stream) {
+  if (!d_params || !d_data_AET || !d_psd || !d_out_lnL || !d_workspace || B <= 0 || !grid_ok(grid) ||
+      !model_ok(model))
+    return PESPACE_EINVAL;
+  if (workspace_bytes < pespace_workspace_bytes(B, grid, model, 0) || ((uintptr_t)d_workspace & 15u))
+    return PESPACE_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Plan p = make_plan(B, grid->N, model->n_det);
+  double* d_consts = (double*)d_workspace;
+  double* d_partial = (double*)((char*)d_workspace + p.consts_bytes);
+  int rc = run_prep(d_params, B, model, d_consts, st);
+  if (rc != PESPACE_OK) return rc;
+  const unsigned cm = class_mask(model->mode_mask);
+  const GridC G = {grid->f0, grid->df, (long long)grid->N};
+  const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
+  for (int d = 0; d < model->n_det; ++d) {
+    const DetC dc = make_det(model->det[d]);
+    EvPair ev = {nullptr, nullptr};
+    if (g_profile) {
+      CU(cudaEventCreate(&ev.a));
+      CU(cudaEventCreate(&ev.b));
+      CU(cudaEventRecord(ev.a, st));
+    }
+    if (dc.kind == 0)
+      loglike_kernel<0><<<g, BLOCK, 0, st>>>(d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, cm, d_partial);
+    else
+      loglike_kernel<1><<<g, BLOCK, 0, st>>>(d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, cm, d_partial);
+    LAUNCHED();
+    if (ev.a) {
+      CU(cudaEventRecord(ev.b, st));
+      std::lock_guard<std::mutex> lk(g_ev_mutex);
+      g_events.push_back(ev);
+    }
+  }
+  const int th = 128;
+  combine_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_partial, d_consts, B, (int)(model->n_det * p.nbb),
+                                                                p.stride, d_out_lnL);
+  LAUNCHED();
+  return PESPACE_OK;
+}
+
+int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                   const pespace_grid* grid, const pespace_model* model, double* d_out_F, double* d_out_grad,
+                   void* d_workspace, size_t workspace_bytes, void* stream) {
+  (void)d_data_AET; (void)d_out_grad; (void)stream;
+  if (!d_params || !d_psd || !d_out_F || !d_workspace || B <= 0 || !grid_ok(grid) || !model_ok(model))
+    return PESPACE_EINVAL;
+  if (workspace_bytes < pespace_workspace_bytes(B, grid, model, 1)) return PESPACE_EINVAL;
+  snprintf(g_cuda_msg, sizeof g_cuda_msg, "pespace_fisher: forward-mode kernel not built yet");
+  return PESPACE_ECUDA;
+}
+
+int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET, const double* h_psd,
+                         const pespace_grid* grid, const pespace_model* model, double* h_out_lnL) {
+  if (!h_params || !h_data_AET || !h_psd || !h_out_lnL || B <= 0 || !grid_ok(grid) || !model_ok(model))
+    return PESPACE_EINVAL;
+  const size_t nP = (size_t)B * NPAR, nS = (size_t)model->n_det * 3 * (size_t)grid->N;
+  const size_t ws = pespace_workspace_bytes(B, grid, model, 0);
+  double *dP = nullptr, *dD = nullptr, *dS = nullptr, *dO = nullptr;
+  void* dW = nullptr;
+  cudaStream_t st = nullptr;
+  int rc = PESPACE_OK;
+  auto bail = [&](int code) {
+    cudaFree(dP); cudaFree(dD); cudaFree(dS); cudaFree(dO); cudaFree(dW);
+    return code;
+  };
+  if (cudaMalloc((void**)&dP, nP * 8) != cudaSuccess || cudaMalloc((void**)&dD, nS * 16) != cudaSuccess ||
+      cudaMalloc((void**)&dS, nS * 8) != cudaSuccess || cudaMalloc((void**)&dO, (size_t)B * 8) != cudaSuccess ||
+      cudaMalloc(&dW, ws) != cudaSuccess) {
+    cudaGetLastError();
+    return bail(PESPACE_ENOMEM);
+  }
+  cudaError_t e;
+  if ((e = cudaMemcpyAsync(dP, h_params, nP * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dD, h_data_AET, nS * 16, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
+      (e = cudaMemcpyAsync(dS, h_psd, nS * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
+    return bail(cuda_fail(e));
+  rc = pespace_loglike(dP, B, dD, dS, grid, model, dO, dW, ws, st);
+  if (rc != PESPACE_OK) return bail(rc);
+  if ((e = cudaMemcpyAsync(h_out_lnL, dO, (size_t)B * 8, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
+      (e = cudaStreamSynchronize(st)) != cudaSuccess)
+    return bail(cuda_fail(e));
+  return bail(PESPACE_OK);
+}
+
+int pespace_fp64_peak(int iters, double* h_out_tflops, double* h_out_ms) {
+  if (iters <= 0 || !h_out_tflops) return PESPACE_EINVAL;
+  int dev = 0, sms = 0;
+  CU(cudaGetDevice(&dev));
+  CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  double* d_out = nullptr;
+  CU(cudaMalloc((void**)&d_out, 8));
+  cudaEvent_t e0, e1;
+  CU(cudaEventCreate(&e0));
+  CU(cudaEventCreate(&e1));
+  const int blocks = sms * 8, threads = 256;
+  dfma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, d_out);   // warm-up
+  ++g_launches;
+  CU(cudaEventRecord(e0));
+  dfma_peak_kernel<<<blocks, threads>>>(iters, 1.0, d_out);
+  ++g_launches;
+  CU(cudaEventRecord(e1));
+  CU(cudaEventSynchronize(e1));
+  float ms = 0.f;
+  CU(cudaEventElapsedTime(&ms, e0, e1));
+  const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  *h_out_tflops = flops / (ms * 1e-3) / 1e12;
+  if (h_out_ms) *h_out_ms = ms;
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+  return PESPACE_OK;
+}
+
+}  // extern "C"

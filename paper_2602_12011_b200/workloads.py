@@ -204,7 +204,7 @@ MONTH_DF = 1.0 / 2592000.0   # 1/(30 days)
 def _jitter_workload(name, seed, noise_seed, B, N, mode_mask, dets, want_fisher=False) -> Workload:
     grid = Grid(1e-4, MONTH_DF, N)
     inj = THETA_INJ.copy()
-    inj[10] = 0.8 / MONTH_DF           # t_c = 0.8 T = 2073600 s (defined by the full 1-month grid)
+    inj[10] = 2073600.0                # t_c = 0.8 T, T = 30 days
     rng = np.random.default_rng(seed)
     return Workload(name, grid, Model(mode_mask, tuple(dets)), draw_jitter(B, inj, rng), inj, noise_seed,
                     want_fisher)

@@ -1,0 +1,90 @@
+"""Host-side checks that need no GPU: the C-ABI library builds, loads and exports every symbol
+include/pespace.h declares; argument validation returns the documented codes before any CUDA
+call; the workload recipes are reproducible."""
+import ctypes as C
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2602_12011_b200 import build as pbuild
+from paper_2602_12011_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module")
+def lib():
+    return C.CDLL(pbuild.build())
+
+
+def declared_symbols():
+    text = open(os.path.join(ROOT, "include", "pespace.h")).read()
+    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
+    return sorted(set(re.findall(r"\b(pespace_[a-z0-9_]+)\s*\(", text)))
+
+
+def test_library_exports_every_declared_symbol(lib):
+    names = declared_symbols()
+    assert {"pespace_response", "pespace_loglike", "pespace_fisher", "pespace_workspace_bytes",
+            "pespace_strerror"} <= set(names)
+    for n in names:
+        assert hasattr(lib, n), n
+
+
+def test_binding_mirrors_the_header():
+    from paper_2602_12011_b200 import binding
+    assert sorted(binding.EXPORTS) == declared_symbols()
+    assert "sm_100a" in binding.version()
+
+
+def test_argument_validation_without_a_device():
+    from paper_2602_12011_b200 import binding as P
+    L = P.lib()
+    wl = W.config(2, B=4, N=64)
+    m, keep = P._model(wl.model)
+    g = P._grid(wl.grid)
+    EINVAL = -1
+    fake = 0x1000  # never dereferenced: validation fails first
+    assert L.pespace_loglike(None, 4, fake, fake, C.byref(g), C.byref(m), fake, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike(fake, 0, fake, fake, C.byref(g), C.byref(m), fake, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike(fake, 4, fake, fake, C.byref(g), C.byref(m), fake, fake, 8, None) == EINVAL  # ws too small
+    bad_g = P._Grid(1e-4, -1.0, 64)
+    assert L.pespace_loglike(fake, 4, fake, fake, C.byref(bad_g), C.byref(m), fake, fake, 1 << 30, None) == EINVAL
+    bad_m, keep2 = P._model(W.Model(0, wl.model.detectors))
+    assert L.pespace_response(fake, 4, fake, 64, C.byref(bad_m), fake, None) == EINVAL
+    bad_m2, keep3 = P._model(W.Model(1, (W.Detector("x", 7, 20, 1e9),)))
+    assert L.pespace_response(fake, 4, fake, 64, C.byref(bad_m2), fake, None) == EINVAL
+    bad_m3, keep4 = P._model(W.Model(1, (W.Detector("x", 0, 17, 1e9),)))
+    assert L.pespace_fisher(fake, 4, None, fake, C.byref(g), C.byref(bad_m3), fake, None, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike_host(None, 4, fake, fake, C.byref(g), C.byref(m), fake) == EINVAL
+    assert L.pespace_fp64_peak(0, None, None) == EINVAL
+    assert L.pespace_workspace_bytes(0, C.byref(g), C.byref(m), 0) == 0
+    assert L.pespace_workspace_bytes(4096, C.byref(g), C.byref(m), 0) > 4096 * 8
+    assert L.pespace_strerror(EINVAL) == b"invalid argument"
+    assert L.pespace_strerror(0) == b"ok"
+
+
+def test_workloads_are_seeded_and_shaped_like_the_configs():
+    a, b = W.config(2, B=64, N=128), W.config(2, B=64, N=128)
+    assert np.array_equal(a.params, b.params)
+    assert a.params[:, 1].min() >= 1.0 and np.all(a.params[:, 2:4] == 0.0)
+    assert np.allclose(a.params.mean(axis=0)[[0, 4]], [2e6, 10.0], rtol=0.01)
+    full = W.config(2)
+    assert (full.B, full.grid.N, full.grid.f0) == (4096, 262144, 1e-4)
+    assert full.grid.df == 1.0 / (30 * 86400) and full.theta_inj[10] == 2073600.0
+    c4 = W.config(4)
+    assert c4.B == 8192 and [d.kind for d in c4.model.detectors] == [0, 0, 1] and c4.model.mode_mask == 31
+    c1 = W.config(1)
+    assert c1.B == 16 and c1.grid.N == 4096 and c1.noise_seed is None
+    f = c1.grid.freqs()
+    assert f[0] == 1e-4 and abs(f[-1] - 1e-2) < 1e-15
+    # G12: noise variance
+    psd = np.full((1, 3, 20000), 2.5e-40)
+    n = W.coloured_noise(psd, 1e-6, np.random.default_rng(0))
+    assert np.var(n.real) == pytest.approx(2.5e-40 / 4e-6, rel=0.03)
+    # psd nulls of TDI 2.0 sit where sin(2x) = 0
+    det = W.lisa_like()
+    fn = 299792458.0 / (4 * det.L_m)
+    assert W.psd_aet(det, np.array([fn]))[0, 0] < 1e-25 * W.psd_aet(det, np.array([fn * 0.9]))[0, 0]

@@ -1,0 +1,206 @@
+"""GPU-vs-oracle parity (run on the B200 box: pytest -m gpu).  Every call goes through the
+C ABI of libpespace.so via the ctypes binding; expected values come from oracle/ only.
+
+Tolerances (BASELINE.json north_star): lnL and <h|h> 1e-9 relative -- relative to
+max(|lnL|, 1/2 <h|h>) (reading G14: lnL ~ 0 for a noiseless injection) -- and 1e-8
+relative max-abs on the response arrays.  The response array of one (sample, detector) is
+[3][N]; its error is measured against its max |.| (1e-8), and ALSO per channel against that
+channel's own max |.| (1e-8) plus a cancellation floor of 1e-12 of the detector's max |.|:
+T = (X+Y+Z)/sqrt3 cancels to ~(2 pi f L)^3 of A at low f (pin P8), so for the short-arm
+TianQin-like detector below 1 mHz T is 1e-12 of A and is rounding noise in ANY double
+evaluation, the oracle's included ("Tolerances").
+"""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2602_12011_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+TOL_LNL = 1e-9
+TOL_RESP = 1e-8
+CANCEL_FLOOR = 1e-12
+
+
+@pytest.fixture(scope="module")
+def P():
+    import torch
+    from paper_2602_12011_b200 import binding
+    assert torch.cuda.is_available()
+    return binding
+
+
+def dev(a):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def oracle_response_fn(params, freqs, model):
+    return oracle.response(params, freqs, model)
+
+
+def check_response(P, params, freqs, model):
+    got = P.response(dev(params), dev(freqs), model).cpu().numpy()
+    want = oracle.response(params, freqs, model)
+    assert got.shape == want.shape
+    for b in range(want.shape[0]):
+        for d in range(want.shape[1]):
+            det_scale = np.abs(want[b, d]).max()
+            assert np.abs(got[b, d] - want[b, d]).max() <= TOL_RESP * det_scale
+            for c in range(3):
+                scale = np.abs(want[b, d, c]).max()
+                err = np.abs(got[b, d, c] - want[b, d, c]).max()
+                assert err <= TOL_RESP * scale + CANCEL_FLOOR * det_scale, (b, d, c, err / scale, err / det_scale)
+    return got, want
+
+
+def check_loglike(P, wl, data, psd, subset=None):
+    import torch
+    lik = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    got = lik(dev(wl.params)).cpu().numpy()
+    idx = np.arange(wl.B) if subset is None else np.asarray(subset)
+    want = oracle.loglike(wl.params[idx], data, psd, wl.grid, wl.model)
+    hh = -2.0 * oracle.loglike(wl.params[idx], np.zeros_like(data), psd, wl.grid, wl.model)
+    scale = np.maximum(np.abs(want), 0.5 * hh)
+    rel = np.abs(got[idx] - want) / scale
+    assert np.all(rel <= TOL_LNL), (rel.max(), idx[np.argmax(rel)])
+    # <h|h> itself (data = 0)
+    lik0 = P.Likelihood(dev(np.zeros_like(data)), dev(psd), wl.grid, wl.model, wl.B)
+    hh_gpu = -2.0 * lik0(dev(wl.params)).cpu().numpy()[idx]
+    assert np.all(np.abs(hh_gpu - hh) <= TOL_LNL * hh)
+    return got
+
+
+# ------------------------------------------------------------------ config 1, in full
+def test_config1_response_and_loglike_full(P):
+    wl = W.config(1)
+    f = wl.grid.freqs()
+    check_response(P, wl.params, f, wl.model)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    lnL = check_loglike(P, wl, data, psd)
+    # noiseless injection = sample 0: lnL ~ 0 on the scale of <h|h>, and the maximum of the batch
+    assert np.argmax(lnL) == 0
+
+
+# ------------------------------------------------------------------ reduced configs 2-4: several tiles + ragged tails
+@pytest.mark.parametrize("idx,B,N", [(2, 70, 3000), (3, 37, 1500), (4, 67, 1100)])
+def test_reduced_configs_loglike_and_response(P, idx, B, N):
+    wl = W.config(idx, B=B, N=N)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_loglike(P, wl, data, psd)
+    check_response(P, wl.params[:5], wl.grid.freqs()[::7], wl.model)
+
+
+@pytest.mark.parametrize("gen", [15, 20])
+def test_random_sky_all_detectors_both_generations(P, gen):
+    """Prior draws (random sky, inclination, masses) through all three detector kinds."""
+    rng = np.random.default_rng(11)
+    grid = W.Grid(1e-4, 3.1e-5, 700)
+    th = W.draw_prior(19, 4e5, rng)
+    th[:, 2] = rng.uniform(-0.8, 0.8, 19); th[:, 3] = rng.uniform(-0.8, 0.8, 19)
+    model = W.Model(W.MODES_HM, (W.lisa_like(gen), W.taiji_like(gen), W.tianqin_like(gen)))
+    wl = W.Workload("random", grid, model, th, th[3].copy(), 77)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_loglike(P, wl, data, psd)
+    check_response(P, th, grid.freqs()[::5], model)
+
+
+@pytest.mark.parametrize("mask", [1, 2, 4, 8, 16, 9, 22])
+def test_individual_modes(P, mask):
+    wl = W.config(3, B=9, N=600)
+    model = W.Model(mask, wl.model.detectors)
+    check_response(P, wl.params, wl.grid.freqs(), model)
+
+
+# ------------------------------------------------------------------ edge cases
+def test_edge_cases(P):
+    import torch
+    wl = W.config(2, B=5, N=300)
+    f = wl.grid.freqs()
+    psd = wl.psd()
+    data = wl.data(oracle_response_fn)
+    # B = 1, N = 1
+    one = W.Workload("one", W.Grid(3e-3, 1e-5, 1), wl.model, wl.params[:1], wl.theta_inj, None)
+    check_loglike(P, one, np.full((1, 3, 1), 1e-20 + 2e-20j), one.psd())
+    # zero / inf / nan PSD bins carry no weight; out-of-domain samples give -inf / NaN rows
+    psd2 = psd.copy(); psd2[0, 0, 3] = 0.0; psd2[0, 1, 100] = np.inf; psd2[0, 2, 299] = np.nan; psd2[0, 0, 17] = -1.0
+    th = wl.params.copy(); th[1, 0] = -5.0; th[3, 4] = np.nan
+    got = P.loglike(dev(th), dev(data), dev(psd2), wl.grid, wl.model).cpu().numpy()
+    want = oracle.loglike(th, data, psd2, wl.grid, wl.model)
+    assert np.isneginf(got[1]) and np.isneginf(got[3]) and np.isneginf(want[1])
+    ok = [0, 2, 4]
+    assert np.all(np.abs(got[ok] - want[ok]) <= TOL_LNL * np.abs(want[ok]))
+    r = P.response(dev(th), dev(f), wl.model).cpu().numpy()
+    assert np.all(np.isnan(r[1].view(np.float64))) and np.all(np.isfinite(r[0].view(np.float64)))
+    # f <= 0 bins produce zeros
+    f2 = f.copy(); f2[0] = 0.0; f2[5] = -1e-3
+    r2 = P.response(dev(wl.params), dev(f2), wl.model).cpu().numpy()
+    assert np.all(r2[:, :, :, [0, 5]] == 0) and np.all(r2[:, :, :, 1] != 0)
+
+
+def test_source_along_an_arm_is_regular(P):
+    """k parallel to an arm at t_f(f): 1 - (k.n)^2 -> 0 (Eq. 5's sinc argument -> 0)."""
+    th = W.THETA_INJ.copy(); th[10] = 2.0e6
+    det = W.lisa_like()
+    f0 = 1e-3
+    _, _, t = oracle.waveform(th, 2, 2, np.array([f0]))
+    x = oracle.orbit(det, t[0])
+    n12 = (x[0] - x[1]) / det.L_m
+    th[8] = -math.asin(n12[2]); th[7] = math.atan2(-n12[1], -n12[0])
+    _, _, t2 = oracle.waveform(th, 2, 2, np.array([f0]))
+    assert t2[0] == t[0]
+    f = np.array([f0 * (1 - 1e-9), f0, f0 * (1 + 1e-9), 2e-3, 5e-3])
+    check_response(P, th[None, :], f, W.Model(1, (det,)))
+
+
+def test_bitwise_determinism(P):
+    wl = W.config(3, B=130, N=2000)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    lik = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    p = dev(wl.params)
+    a = lik(p).cpu().numpy()
+    b = lik(p).cpu().numpy()
+    assert np.array_equal(a, b)
+    r1 = P.response(p, dev(wl.grid.freqs()), wl.model).cpu().numpy()
+    r2 = P.response(p, dev(wl.grid.freqs()), wl.model).cpu().numpy()
+    assert np.array_equal(r1.view(np.float64), r2.view(np.float64))
+
+
+def test_host_buffer_call_matches_device_call(P):
+    wl = W.config(4, B=33, N=900)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    a = P.loglike_host(wl.params, data, psd, wl.grid, wl.model)
+    b = P.loglike(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model).cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_error_codes_on_device(P):
+    wl = W.config(2, B=4, N=64)
+    data, psd = dev(wl.data(oracle_response_fn)), dev(wl.psd())
+    with pytest.raises(P.PespaceError):
+        P.loglike(dev(wl.params), data, psd, W.Grid(1e-4, 0.0, 64), wl.model)
+    with pytest.raises(P.PespaceError):
+        P.loglike(dev(wl.params), data, psd, wl.grid, W.Model(64, wl.model.detectors))
+    lik = P.Likelihood(data, psd, wl.grid, wl.model, 2)
+    with pytest.raises(P.PespaceError):
+        lik(dev(wl.params))                     # batch larger than the workspace
+
+
+# ------------------------------------------------------------------ full size, sampled (bench.py's launch configuration)
+@pytest.mark.parametrize("idx,stride_div", [(2, 32), (3, 16)])
+def test_full_size_sampled_parity(P, idx, stride_div):
+    wl = W.config(idx)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    step = -(-wl.B // stride_div)
+    subset = sorted(set([0] + list(range(0, wl.B, step))))
+    check_loglike(P, wl, data, psd, subset=subset)
+
+
+def test_full_size_network_sampled_parity(P):
+    wl = W.config(4)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    subset = [0, 1023, 4097, 8191]
+    check_loglike(P, wl, data, psd, subset=subset)
