@@ -62,6 +62,26 @@ DetC make_det(const pespace_detector& d) {
   return c;
 }
 
+// ---- kernel dispatch on (detector kind, mode-class mask); all 15 masks are instantiated
+template <int KIND, unsigned CM>
+void launch_loglike(dim3 g, cudaStream_t st, const double* consts, long long B, const double2* data, const double* psd,
+                    GridC G, const DetC& dc, int n_det, int det, double* partial) {
+  loglike_kernel<KIND, CM><<<g, BLOCK, 0, st>>>(consts, B, data, psd, G, dc, n_det, det, partial);
+}
+template <int KIND, unsigned CM>
+void launch_response(dim3 g, cudaStream_t st, const double* consts, long long B, const double* freqs, long long N,
+                     const DetC& dc, int n_det, int det, double2* out) {
+  response_kernel<KIND, CM><<<g, BLOCK, 0, st>>>(consts, B, freqs, N, dc, n_det, det, out);
+}
+using LoglikeFn = void (*)(dim3, cudaStream_t, const double*, long long, const double2*, const double*, GridC,
+                           const DetC&, int, int, double*);
+using ResponseFn = void (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&, int,
+                            int, double2*);
+#define PESPACE_ROW(F, K) {nullptr, F<K, 1>, F<K, 2>, F<K, 3>, F<K, 4>, F<K, 5>, F<K, 6>, F<K, 7>, F<K, 8>, \
+                           F<K, 9>, F<K, 10>, F<K, 11>, F<K, 12>, F<K, 13>, F<K, 14>, F<K, 15>}
+const LoglikeFn kLoglike[2][16] = {PESPACE_ROW(launch_loglike, 0), PESPACE_ROW(launch_loglike, 1)};
+const ResponseFn kResponse[2][16] = {PESPACE_ROW(launch_response, 0), PESPACE_ROW(launch_response, 1)};
+
 unsigned class_mask(unsigned mode_mask) {
   unsigned m = 0;
   if (mode_mask & PESPACE_MODE_21) m |= 1u;                       // m = 1
@@ -164,10 +184,7 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
     const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
     for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
       const DetC dc = make_det(model->det[d]);
-      if (dc.kind == 0)
-        response_kernel<0><<<grid, BLOCK, 0, st>>>(d_consts, B, d_freqs, N, dc, model->n_det, d, cm, (double2*)d_out_AET);
-      else
-        response_kernel<1><<<grid, BLOCK, 0, st>>>(d_consts, B, d_freqs, N, dc, model->n_det, d, cm, (double2*)d_out_AET);
+      kResponse[dc.kind][cm](grid, st, d_consts, B, d_freqs, N, dc, model->n_det, d, (double2*)d_out_AET);
       ++g_launches;
       cudaError_t e = cudaGetLastError();
       if (e != cudaSuccess) rc = cuda_fail(e);
@@ -203,10 +220,7 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
       CU(cudaEventCreate(&ev.b));
       CU(cudaEventRecord(ev.a, st));
     }
-    if (dc.kind == 0)
-      loglike_kernel<0><<<g, BLOCK, 0, st>>>(d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, cm, d_partial);
-    else
-      loglike_kernel<1><<<g, BLOCK, 0, st>>>(d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, cm, d_partial);
+    kLoglike[dc.kind][cm](g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial);
     LAUNCHED();
     if (ev.a) {
       CU(cudaEventRecord(ev.b, st));

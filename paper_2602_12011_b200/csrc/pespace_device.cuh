@@ -58,13 +58,6 @@ constexpr int SMEM_STRIDE = D_BASE + D_STRIDE;   // one sample, one detector
 static_assert(SMEM_STRIDE == 64, "sample block is 64 doubles");
 __host__ __device__ constexpr int sample_stride(int n_det) { return D_BASE + D_STRIDE * n_det; }
 
-// ---- per-mode-class constants, class index = m - 1
-struct ModeClassC { double cb, ln3, s83, mh; };   // (2/m)^{1/3}, ln(2/m)/3, (m/2)^{8/3}, m/2
-__constant__ ModeClassC c_mc[4] = {
-    {1.2599210498948731648, 0.23104906018664843647, 0.1574901312368591456, 0.5},
-    {1.0, 0.0, 1.0, 1.0},
-    {0.87358046473629886905, -0.13515503603605479399, 2.948334068485008683, 1.5},
-    {0.79370052598409973738, -0.23104906018664843647, 6.349604207872797899, 2.0}};
 // (m/2)^{7/6} for the amplitude (host/prep side)
 __device__ constexpr double kM76[4] = {0.44544935907016965237, 1.0, 1.6048697909004944263, 2.2449240966187459629};
 
@@ -81,11 +74,54 @@ struct DetC {
 struct GridC { double f0, df; long long N; };
 
 // ---- per-bin constants (registers)
-struct BinC { double f, cf, lnf3, fm53, fm83, fm76, sth, cth; };
+struct BinC { double f4, cf, lnf3, fm53, fm83, fm76, sth, cth; };   // f4 = 4 f
+
+// ---- FP64 helpers written for this kernel (the library sincospi/division carry quadrant,
+// special-value and slow-path logic that the FP64-bound inner loop cannot afford)
+
+// sin and cos of (pi/2) x, x in QUARTER TURNS, |x| < 2^30.  Octant reduction y = x - rint(x),
+// then near-minimax polynomials in y^2 on |y| <= 1/2 (max abs error 1.2e-16 / 1.8e-16,
+// coefficients from a Chebyshev-node fit in 60-digit arithmetic).
+__device__ __forceinline__ void sincos_qt(double x, double& s_out, double& c_out) {
+  const double qf = rint(x);
+  const double y = x - qf;
+  const int q = __double2int_rn(qf);
+  const double z = y * y;
+  double ps = fma(5.633933781537854e-08, z, -3.59864335298231e-06);
+  ps = fma(ps, z, 0.0001604411507421909);
+  ps = fma(ps, z, -0.004681754132340976);
+  ps = fma(ps, z, 0.07969262624604301);
+  ps = fma(ps, z, -0.6459640975062443);
+  ps = fma(ps, z, 1.5707963267948966);
+  ps *= y;
+  double pc = fma(4.6552961874867623e-07, z, -2.520013526428479e-05);
+  pc = fma(pc, z, 0.000919259950041661);
+  pc = fma(pc, z, -0.02086348073494657);
+  pc = fma(pc, z, 0.25366950789986475);
+  pc = fma(pc, z, -1.2337005501361513);
+  pc = fma(pc, z, 1.0);
+  // quadrant: q odd swaps, sign of sin = bit1(q), sign of cos = bit1(q+1); applied on the high words
+  const bool odd = q & 1;
+  int sh = __double2hiint(odd ? pc : ps), sl = __double2loint(odd ? pc : ps);
+  int ch = __double2hiint(odd ? ps : pc), cl = __double2loint(odd ? ps : pc);
+  sh ^= (q & 2) << 30;
+  ch ^= ((q + 1) & 2) << 30;
+  s_out = __hiloint2double(sh, sl);
+  c_out = __hiloint2double(ch, cl);
+}
+
+// 1/x for x > 0: hardware seed (rcp.approx.ftz.f64, ~2^-20) + one cubic Newton step (3 DFMA)
+__device__ __forceinline__ double rcp_pos(double x) {
+  double r;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+  const double e = fma(-x, r, 1.0);
+  const double t = fma(e, e, e);
+  return fma(r, t, r);
+}
 
 __device__ __forceinline__ BinC make_bin(double f, double Lbar) {
   BinC b;
-  b.f = f;
+  b.f4 = 4.0 * f;
   b.cf = cbrt(f);
   b.lnf3 = log(f) * (1.0 / 3.0);
   const double cf2 = b.cf * b.cf;
@@ -112,127 +148,139 @@ __device__ __forceinline__ void tdi_prefactor(const BinC& b, int gen, double& gr
 }
 
 // ---------------------------------------------------------------------------------------------
-// X, Y, Z of one (sample, bin, detector), all mode classes of `cmask`, WITHOUT the common factor
-// g z f^{-7/6}.  sc -> this sample's constant block in shared memory.
-template <int KIND>
-__device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
-                                         unsigned cmask, double (&S)[6]) {
+// One mode class (m = MC + 1) of one (sample, bin, detector): adds its X, Y, Z (without the common
+// factor g z f^{-7/6}) to S.  All phases are carried in QUARTER TURNS (the prep kernel scales the
+// polynomial coefficients by 4) so that sincos_qt needs no multiply.
+template <int KIND, int MC, bool FIRST>
+__device__ __forceinline__ void eval_class(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
+                                           double va, double La, double ftc4, double (&S)[6]) {
+  // compile-time class constants: (2/m)^{1/3}, ln(2/m)/3, (m/2)^{8/3}, m/2
+  constexpr double CB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
+  constexpr double LN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
+  constexpr double S83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
+  constexpr double MH[4] = {0.5, 1.0, 1.5, 2.0};
+  // ---- S2/S3: v, ln v, phase and t_lm
+  const double v = (MC == 1) ? va : va * CB[MC];
+  const double L = (MC == 1) ? La : La + LN3[MC];
+  const double v2 = v * v;
+  double P = fma(sc[W_P7], v, fma(sc[W_P6L], L, sc[W_P6]));
+  P = fma(P, v, fma(sc[W_P5L], L, sc[W_P5]));
+  P = fma(P, v, sc[W_P4]);
+  P = fma(P, v, sc[W_P3]);
+  P = fma(P, v, sc[W_P2]);
+  P = fma(P, v2, sc[W_P0]);
+  double Q = fma(sc[W_Q7], v, fma(sc[W_Q6L], L, sc[W_Q6]));
+  Q = fma(Q, v, sc[W_Q5]);
+  Q = fma(Q, v, sc[W_Q4]);
+  Q = fma(Q, v, sc[W_Q3]);
+  Q = fma(Q, v, sc[W_Q2]);
+  Q = fma(Q, v2, sc[W_Q0]);
+  double psi = ((MC == 1) ? bc.fm53 : S83[MC] * bc.fm53) * P;     // PN phase, quarter turns (up to ~4e5)
+  psi -= 4.0 * rint(0.25 * psi);                                   // mod 4 quarter turns, exact
+  psi += fma(MH[MC], sc[W_PH0], ftc4);                             // + 4 [f t_c - (m/2)(phi_c/pi + 1/8)]
+  const double tau = ((MC == 1) ? bc.fm83 : S83[MC] * bc.fm83) * Q;   // 4 (t_lm - t_c) / yr
+
+  // ---- amplitude x polarisation content of the class: vp (a + b v^2)
+  const double* ka = sc + W_KA + 4 * MC;
+  double CKp, CKc;
+  if (MC == 1) { CKp = fma(ka[1], v2, ka[0]); CKc = fma(ka[3], v2, ka[2]); }
+  else if (MC == 3) { CKp = v2 * ka[0]; CKc = v2 * ka[2]; }
+  else { CKp = v * ka[0]; CKc = v * ka[2]; }
+
+  // ---- S4: orbit phase(s) and the two rotating combinations G1, G2 of each of k, u', v'
+  double G1k, G2k, G1u, G2u, G1v, G2v, kR;
+  if (KIND == 0) {
+    double sa, ca;
+    sincos_qt(sc[D_BASE] + tau, sa, ca);
+    const double c2 = fma(2.0 * ca, ca, -1.0), s2 = 2.0 * sa * ca;
+    const double* w = sc + S_K;
+    G1k = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
+    G2k = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
+    w = sc + S_U;
+    G1u = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
+    G2u = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
+    w = sc + S_V;
+    G1v = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
+    G2v = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
+    kR = fma(sc[S_DX], ca, sc[S_DY] * sa);
+  } else {
+    double sE, cE, sp, cp;
+    sincos_qt(sc[D_BASE] + tau, sE, cE);
+    sincos_qt(fma(tau, dc.yr_over_p, sc[D_BASE + 1]), sp, cp);
+    const double* w = sc + D_BASE + 2;
+    G1k = fma(w[0], cp, w[1] * sp); G2k = fma(w[1], cp, -w[0] * sp);
+    G1u = fma(w[2], cp, w[3] * sp); G2u = fma(w[3], cp, -w[2] * sp);
+    G1v = fma(w[4], cp, w[5] * sp); G2v = fma(w[5], cp, -w[4] * sp);
+    kR = fma(sc[S_DX], cE, sc[S_DY] * sE);
+  }
+  // k.delta_n / L for the three spacecraft, k.n_l for the arms a: 2-3, b: 3-1, c: 1-2
+  const double nu0 = fma(dc.cn[0], G1k, dc.sn[0] * G2k);
+  const double nu1 = fma(dc.cn[1], G1k, dc.sn[1] * G2k);
+  const double nu2 = fma(dc.cn[2], G1k, dc.sn[2] * G2k);
+  const double ka_ = nu1 - nu2, kb_ = nu2 - nu0, kc_ = nu0 - nu1;   // k.n_23, k.n_31, k.n_12
+
+  // ---- S5: W_l = amplitude * (n_l.P.n_l) / (1 - (k.n_l)^2), with 1-(k.n)^2 = (u'.n)^2 + (v'.n)^2
+  double Wr[3], Wi[3];
 #pragma unroll
-  for (int i = 0; i < 6; ++i) S[i] = 0.0;
-  const double a = sc[W_A], lnA = sc[W_LNA], tc = sc[W_TC];
-  // f t_c in turns, fractional part, with the rounding error of the product recovered by fma
-  const double p = bc.f * tc;
-  const double ftc = (p - rint(p)) + fma(bc.f, tc, -p);
-  const double va = a * bc.cf, La = lnA + bc.lnf3;
+  for (int l = 0; l < 3; ++l) {
+    const double uu = fma(dc.dcn[l], G1u, dc.dsn[l] * G2u);
+    const double vv = fma(dc.dcn[l], G1v, dc.dsn[l] * G2v);
+    const double v2_ = vv * vv;
+    const double D = fma(uu, uu, v2_);
+    const double rD = (D > 0.0) ? rcp_pos(D) : 0.0;
+    Wr[l] = (CKp * rD) * fma(uu, uu, -v2_);
+    Wi[l] = (CKc * rD) * (uu * vv);
+  }
 
-#pragma unroll 1
-  for (int mc = 0; mc < 4; ++mc) {
-    if (!((cmask >> mc) & 1u)) continue;
-    const ModeClassC M = c_mc[mc];
-    // ---- S2/S3: v, ln v, phase and t_lm
-    const double v = va * M.cb, L = La + M.ln3, v2 = v * v;
-    double P = fma(sc[W_P7], v, fma(sc[W_P6L], L, sc[W_P6]));
-    P = fma(P, v, fma(sc[W_P5L], L, sc[W_P5]));
-    P = fma(P, v, sc[W_P4]);
-    P = fma(P, v, sc[W_P3]);
-    P = fma(P, v, sc[W_P2]);
-    P = fma(P, v2, sc[W_P0]);
-    double Q = fma(sc[W_Q7], v, fma(sc[W_Q6L], L, sc[W_Q6]));
-    Q = fma(Q, v, sc[W_Q5]);
-    Q = fma(Q, v, sc[W_Q4]);
-    Q = fma(Q, v, sc[W_Q3]);
-    Q = fma(Q, v, sc[W_Q2]);
-    Q = fma(Q, v2, sc[W_Q0]);
-    double psi = (M.s83 * bc.fm53) * P;                 // PN phase, turns (up to ~1e5)
-    psi -= rint(psi);
-    psi += fma(M.mh, sc[W_PH0], ftc);                   // + f t_c - (m/2)(phi_c/pi + 1/8)
-    const double tau = (M.s83 * bc.fm83) * Q;           // (t_lm - t_c) / yr
-
-    // ---- amplitude x polarisation content of the class: vp (a + b v^2)
-    const double vp = (mc == 1) ? 1.0 : ((mc == 3) ? v2 : v);
-    const double* ka = sc + W_KA + 4 * mc;
-    const double CKp = vp * fma(ka[1], v2, ka[0]);
-    const double CKc = vp * fma(ka[3], v2, ka[2]);
-
-    // ---- S4: orbit phase(s) and the two rotating combinations G1, G2 of each of k, u', v'
-    double G1k, G2k, G1u, G2u, G1v, G2v, kR;
-    if (KIND == 0) {
-      double al = sc[D_BASE] + tau;
-      al -= rint(al);
-      double sa, ca;
-      sincospi(2.0 * al, &sa, &ca);
-      const double c2 = fma(2.0 * ca, ca, -1.0), s2 = 2.0 * sa * ca;
-      const double* w = sc + S_K;
-      G1k = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
-      G2k = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
-      w = sc + S_U;
-      G1u = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
-      G2u = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
-      w = sc + S_V;
-      G1v = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
-      G2v = fma(w[0], s2, fma(-w[1], c2, fma(w[2], sa, w[4])));
-      kR = fma(sc[S_DX], ca, sc[S_DY] * sa);
+  // ---- S6: h_lm E_n = exp(-i (pi/2) (psi + 4 f k.x_n)) for the three spacecraft
+  double Er[3], Ei[3];
+  {
+    const double nun[3] = {nu0, nu1, nu2};
+#pragma unroll
+    for (int n = 0; n < 3; ++n) {
+      double s, c;
+      sincos_qt(fma(bc.f4, fma(dc.Lbar, nun[n], kR), psi), s, c);
+      Er[n] = c; Ei[n] = s;          // note: Ei holds +sin; the minus sign is carried below
+    }
+  }
+  // ---- S7: brackets  B(r,s,kap) = kap (E_s - cos(th) E_r) - i sin(th) E_r  and the TDI sums, with
+  // E = Er - i Ei and W = Wr - i Wi:   Re(W B) = Wr Br - Wi Bi',  -Im(W B) = Wr Bi' + Wi Br
+  // (Bi' = -Im B).  S accumulates (Re, -Im); the sign is restored when the residual is formed.
+  auto add = [&](double& Sr, double& Si, int r, int s_, double kap, double wr, double wi, bool init) {
+    const double br = fma(kap, fma(-bc.cth, Er[r], Er[s_]), -bc.sth * Ei[r]);
+    const double bi = fma(kap, fma(-bc.cth, Ei[r], Ei[s_]), bc.sth * Er[r]);
+    if (init) {
+      Sr = fma(wr, br, -wi * bi);
+      Si = fma(wr, bi, wi * br);
     } else {
-      double aE = sc[D_BASE] + tau;
-      aE -= rint(aE);
-      double ph = fma(tau, dc.yr_over_p, sc[D_BASE + 1]);
-      ph -= rint(ph);
-      double sE, cE, sp, cp;
-      sincospi(2.0 * aE, &sE, &cE);
-      sincospi(2.0 * ph, &sp, &cp);
-      const double* w = sc + D_BASE + 2;
-      G1k = fma(w[0], cp, w[1] * sp); G2k = fma(w[1], cp, -w[0] * sp);
-      G1u = fma(w[2], cp, w[3] * sp); G2u = fma(w[3], cp, -w[2] * sp);
-      G1v = fma(w[4], cp, w[5] * sp); G2v = fma(w[5], cp, -w[4] * sp);
-      kR = fma(sc[S_DX], cE, sc[S_DY] * sE);
-    }
-    // k.delta_n / L for the three spacecraft, k.n_l for the arms a: 2-3, b: 3-1, c: 1-2
-    const double nu0 = fma(dc.cn[0], G1k, dc.sn[0] * G2k);
-    const double nu1 = fma(dc.cn[1], G1k, dc.sn[1] * G2k);
-    const double nu2 = fma(dc.cn[2], G1k, dc.sn[2] * G2k);
-    const double ka_ = nu1 - nu2, kb_ = nu2 - nu0, kc_ = nu0 - nu1;   // k.n_23, k.n_31, k.n_12
-
-    // ---- S5: W_l = amplitude * (n_l.P.n_l) / (1 - (k.n_l)^2), with 1-(k.n)^2 = (u'.n)^2 + (v'.n)^2
-    double Wr[3], Wi[3];
-#pragma unroll
-    for (int l = 0; l < 3; ++l) {
-      const double uu = fma(dc.dcn[l], G1u, dc.dsn[l] * G2u);
-      const double vv = fma(dc.dcn[l], G1v, dc.dsn[l] * G2v);
-      const double v2_ = vv * vv;
-      const double D = fma(uu, uu, v2_);
-      const double rD = (D > 0.0) ? 1.0 / D : 0.0;
-      Wr[l] = CKp * (fma(uu, uu, -v2_) * rD);
-      Wi[l] = -CKc * ((uu * vv) * rD);
-    }
-
-    // ---- S6: h_lm E_n = exp(-2 pi i (psi + f k.x_n)) for the three spacecraft
-    double Er[3], Ei[3];
-    {
-      const double nun[3] = {nu0, nu1, nu2};
-#pragma unroll
-      for (int n = 0; n < 3; ++n) {
-        double ph = fma(bc.f, fma(dc.Lbar, nun[n], kR), psi);
-        ph -= rint(ph);
-        double s, c;
-        sincospi(2.0 * ph, &s, &c);
-        Er[n] = c; Ei[n] = -s;
-      }
-    }
-    // ---- S7: brackets  B(r,s,kap) = kap (E_s - cos(th) E_r) - i sin(th) E_r  and the TDI sums
-    auto add = [&](double& Sr, double& Si, int r, int s, double kap, double wr, double wi) {
-      const double br = fma(kap, fma(-bc.cth, Er[r], Er[s]), bc.sth * Ei[r]);
-      const double bi = fma(kap, fma(-bc.cth, Ei[r], Ei[s]), -bc.sth * Er[r]);
       Sr = fma(wr, br, fma(-wi, bi, Sr));
       Si = fma(wr, bi, fma(wi, br, Si));
-    };
-    // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2)
-    add(S[0], S[1], 0, 2, -kb_, Wr[1], Wi[1]);     // X: + W_b B(1,3,k13)
-    add(S[0], S[1], 0, 1, kc_, -Wr[2], -Wi[2]);    //    - W_c B(1,2,k12)
-    add(S[2], S[3], 1, 0, -kc_, Wr[2], Wi[2]);     // Y: + W_c B(2,1,k21)
-    add(S[2], S[3], 1, 2, ka_, -Wr[0], -Wi[0]);    //    - W_a B(2,3,k23)
-    add(S[4], S[5], 2, 1, -ka_, Wr[0], Wi[0]);     // Z: + W_a B(3,2,k32)
-    add(S[4], S[5], 2, 0, kb_, -Wr[1], -Wi[1]);    //    - W_b B(3,1,k31)
-  }
+    }
+  };
+  // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2)
+  add(S[0], S[1], 0, 2, -kb_, Wr[1], Wi[1], FIRST);   // X: + W_b B(1,3,k13)
+  add(S[0], S[1], 0, 1, kc_, -Wr[2], -Wi[2], false);  //    - W_c B(1,2,k12)
+  add(S[2], S[3], 1, 0, -kc_, Wr[2], Wi[2], FIRST);   // Y: + W_c B(2,1,k21)
+  add(S[2], S[3], 1, 2, ka_, -Wr[0], -Wi[0], false);  //    - W_a B(2,3,k23)
+  add(S[4], S[5], 2, 1, -ka_, Wr[0], Wi[0], FIRST);   // Z: + W_a B(3,2,k32)
+  add(S[4], S[5], 2, 0, kb_, -Wr[1], -Wi[1], false);  //    - W_b B(3,1,k31)
+}
+
+// X, Y, Z of one (sample, bin, detector) summed over the mode classes of CMASK (compile time;
+// bit m-1 set = class m present).  Returns (Re, -Im) pairs in S.
+template <int KIND, unsigned CMASK>
+__device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
+                                         double (&S)[6]) {
+  const double tc = sc[W_TC];
+  // 4 f t_c in quarter turns mod 4, with the rounding error of the product recovered by fma
+  const double p = bc.f4 * tc;
+  const double ftc4 = (p - 4.0 * rint(0.25 * p)) + fma(bc.f4, tc, -p);
+  const double va = sc[W_A] * bc.cf, La = sc[W_LNA] + bc.lnf3;
+  constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
+  if (c0) eval_class<KIND, 0, true>(bc, sc, dc, va, La, ftc4, S);
+  if (c1) eval_class<KIND, 1, !c0>(bc, sc, dc, va, La, ftc4, S);
+  if (c2) eval_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, va, La, ftc4, S);
+  if (c3) eval_class<KIND, 3, !(c0 || c1 || c2)>(bc, sc, dc, va, La, ftc4, S);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -275,7 +323,7 @@ __global__ void prep_samples_kernel(const double* __restrict__ params, long long
   const double Ds = DL * (kGpc / kC);
   const double a = cbrt(kPi * Ms);
   o[W_A] = a; o[W_LNA] = log(a); o[W_TC] = tc;
-  o[W_PH0] = -(phic / kPi + 0.125);
+  o[W_PH0] = -4.0 * (phic / kPi + 0.125);              // quarter turns
   o[W_VALID] = 1.0;
   // TaylorF2 3.5PN coefficients, spin terms per G3
   const double pi2 = kPi * kPi;
@@ -291,10 +339,10 @@ __global__ void prep_samples_kernel(const double* __restrict__ params, long long
   const double ph6l = -6848.0 / 21.0;
   const double ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta * eta);
   const double a5 = 1.0 / (a * a * a * a * a);
-  const double cP = 3.0 / (256.0 * kPi * eta) * a5;          // Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
+  const double cP = 4.0 * 3.0 / (256.0 * kPi * eta) * a5;    // 4 Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
   o[W_P0] = cP; o[W_P2] = cP * ph2; o[W_P3] = cP * ph3; o[W_P4] = cP * ph4;
   o[W_P5] = cP * ph5a; o[W_P5L] = cP * 3.0 * ph5a; o[W_P6] = cP * ph6a; o[W_P6L] = cP * ph6l; o[W_P7] = cP * ph7;
-  const double cQ = cP / (3.0 * kYear);                       // (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
+  const double cQ = cP / (3.0 * kYear);                       // 4 (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
   o[W_Q0] = -5.0 * cQ; o[W_Q2] = -3.0 * cQ * ph2; o[W_Q3] = -2.0 * cQ * ph3; o[W_Q4] = -cQ * ph4;
   o[W_Q5] = 3.0 * cQ * ph5a; o[W_Q6] = cQ * (ph6a + ph6l); o[W_Q6L] = cQ * ph6l; o[W_Q7] = 2.0 * cQ * ph7;
   // amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
@@ -342,12 +390,12 @@ __global__ void prep_samples_kernel(const double* __restrict__ params, long long
     double a0 = tc / kYear;
     a0 -= rint(a0);
     if (D.kind == 0) {
-      d[0] = a0 + D.kappa / (2.0 * kPi);
+      d[0] = 4.0 * (a0 + D.kappa / (2.0 * kPi));
     } else {
-      d[0] = a0;
+      d[0] = 4.0 * a0;
       double p0 = tc / D.period_s;
       p0 -= rint(p0);
-      d[1] = p0 + D.lambda0 / (2.0 * kPi);
+      d[1] = 4.0 * (p0 + D.lambda0 / (2.0 * kPi));
       const double cL = cos(D.lon), sL = sin(D.lon), cB = cos(D.lat), sB = sin(D.lat);
       const double nh[3] = {cB * cL, cB * sL, sB};
       const double e1[3] = {-sL, cL, 0.0};
@@ -380,10 +428,12 @@ __device__ __forceinline__ void stage_tile(double* smem, const double* __restric
 }
 
 // K_main: grid (bin blocks, sample tiles); one launch per detector.
-template <int KIND>
-__global__ void __launch_bounds__(BLOCK)
+constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1) + ((m >> 3) & 1); }
+
+template <int KIND, unsigned CMASK>
+__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? 3 : 2)
 loglike_kernel(const double* __restrict__ consts, long long B, const double2* __restrict__ data,
-               const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det, unsigned cmask,
+               const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
                double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
   __shared__ double smem[TILE * SMEM_STRIDE];
   __shared__ double red[BLOCK / 32][TILE];
@@ -408,7 +458,7 @@ loglike_kernel(const double* __restrict__ consts, long long B, const double2* __
     const bool use = live && isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
     const double sc_ = use ? nrm[c] / g2 : 0.0;
     dr[c] = (d.x * gr + d.y * gi) * sc_;          // d * conj(g) / |g|^2 * nrm
-    di[c] = (d.y * gr - d.x * gi) * sc_;
+    di[c] = (d.x * gi - d.y * gr) * sc_;          // MINUS the imaginary part: eval_xyz returns (Re, -Im)
     w[c] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
   }
   __syncthreads();
@@ -417,7 +467,7 @@ loglike_kernel(const double* __restrict__ consts, long long B, const double2* __
   const int ns = (int)min((long long)TILE, B - b0);
   for (int s = 0; s < ns; ++s) {
     double S[6];
-    eval_xyz<KIND>(bc, smem + s * SMEM_STRIDE, dc, cmask, S);
+    eval_xyz<KIND, CMASK>(bc, smem + s * SMEM_STRIDE, dc, S);
     const double Ar = S[4] - S[0], Ai = S[5] - S[1];                         // Z - X
     const double Er_ = S[0] - 2.0 * S[2] + S[4], Ei_ = S[1] - 2.0 * S[3] + S[5];   // X - 2Y + Z
     const double Tr = S[0] + S[2] + S[4], Ti = S[1] + S[3] + S[5];           // X + Y + Z
@@ -451,10 +501,10 @@ __global__ void combine_kernel(const double* __restrict__ partial, const double*
 }
 
 // pespace_response: same body, writes A, E, T (with the common factor restored).
-template <int KIND>
+template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK)
 response_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ freqs, long long N,
-                DetC dc, int n_det, int det, unsigned cmask, double2* __restrict__ out /* [B][n_det][3][N] */) {
+                DetC dc, int n_det, int det, double2* __restrict__ out /* [B][n_det][3][N] */) {
   __shared__ double smem[TILE * SMEM_STRIDE];
   const long long b0 = (long long)blockIdx.y * TILE;
   stage_tile(smem, consts, b0, B, n_det, det);
@@ -471,11 +521,11 @@ response_kernel(const double* __restrict__ consts, long long B, const double* __
   for (int s = 0; s < ns; ++s) {
     const double* sc = smem + s * SMEM_STRIDE;
     double S[6];
-    eval_xyz<KIND>(bc, sc, dc, cmask, S);
-    double ch[6];
-    ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[5] - S[1]) * i2;
-    ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = (S[1] - 2.0 * S[3] + S[5]) * i6;
-    ch[4] = (S[0] + S[2] + S[4]) * i3; ch[5] = (S[1] + S[3] + S[5]) * i3;
+    eval_xyz<KIND, CMASK>(bc, sc, dc, S);
+    double ch[6];                                      // S holds (Re, -Im)
+    ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
+    ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;
+    ch[4] = (S[0] + S[2] + S[4]) * i3; ch[5] = -(S[1] + S[3] + S[5]) * i3;
     if (!live) continue;
     const bool valid = sc[W_VALID] != 0.0;
 #pragma unroll

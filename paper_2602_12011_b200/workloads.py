@@ -210,9 +210,19 @@ def _jitter_workload(name, seed, noise_seed, B, N, mode_mask, dets, want_fisher=
                     want_fisher)
 
 
-def config(idx: int, B: Optional[int] = None, N: Optional[int] = None) -> Workload:
-    """BASELINE.json configs 1-5.  B / N override the size (reduced parity cases keep
-    f0, df and the draw recipe, and take the first B draws / first N bins)."""
+CONFIG_SEEDS = {1: (0, None), 2: (1, 101), 3: (1, 101), 4: (3, 103), 5: (4, 104)}   # (params, noise)
+
+
+def config(idx: int, B: Optional[int] = None, N: Optional[int] = None,
+           param_seed: Optional[int] = None) -> Workload:
+    """BASELINE.json configs 1-5.  B / N override the size (reduced parity cases keep f0, df
+    and the draw recipe with B draws / the first N bins); param_seed overrides the seed of
+    the parameter draws only (one batch per rank or per step in bench.py)."""
+    if param_seed is not None and idx != 1:
+        base = config(idx, B, N)
+        rng = np.random.default_rng(param_seed)
+        base.params = draw_jitter(base.B, base.theta_inj, rng)
+        return base
     if idx == 1:
         n = 4096 if N is None else N
         grid_full_df = (1e-2 - 1e-4) / 4095
