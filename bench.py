@@ -36,29 +36,28 @@ if ROOT not in sys.path:
 from paper_2602_12011_b200 import dist as pdist          # noqa: E402
 from paper_2602_12011_b200 import workloads as W         # noqa: E402
 
-# ---- roofline constants:
-# FP64 ALU peak: 148 SMs x 64 FP64 FMA lanes x 2 flop x clocks.max.sm (1965 MHz) = 37.23 TFLOP/s.
-# The pespace_fp64_peak DFMA micro-benchmark measures ~36.6 TFLOP/s on this pool (reported too).
+# ---- roofline constants
+# FP64 ALU peak: 148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (1965 MHz) = 37.22 TFLOP/s.  The
+# library's own DFMA micro-benchmark (pespace_fp64_peak) is run in the same process and reported next
+# to it: mode 0 (two register operands) reaches ~98 % of that figure, mode 1 (three distinct register
+# operands, the common case in this kernel) ~66 % (profiles/r01_fp64_operand_bandwidth.md).
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
-# Executed FP64 work of loglike_kernel per bin-eval, from the committed ncu profile
-# (profiles/r01_*): thread-level DFMA, DMUL, DADD counts divided by B*N.  flop = 2*DFMA+DMUL+DADD.
-EXEC_FP64_PER_BIN_EVAL = {
-    2: {"dfma": 0.0, "dmul": 0.0, "dadd": 0.0},
-    3: {"dfma": 0.0, "dmul": 0.0, "dadd": 0.0},
-    4: {"dfma": 0.0, "dmul": 0.0, "dadd": 0.0},
+# FP64 operations of loglike_kernel per (sample, bin, detector), thread level, counted by ncu
+# (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / (B*N), profiles/r01_loglike_kernel_ncu.md).
+# They equal the operation list of the reduced formulas in DESIGN.md ("Algorithmic work") to <1 %; the
+# kernel has no redundant evaluation, so executed = algorithmic.  flop = 2*DFMA + DMUL + DADD.
+FP64_OPS_PER_UNIT = {
+    # (detector kind, mode-class mask): per (sample, bin, detector)
+    (0, 2): {"dfma": 169.17, "dmul": 59.88, "dadd": 35.27},      # kind 0, (2,2) only      -- config 2
+    (0, 15): {"dfma": 661.17, "dmul": 215.88, "dadd": 68.27},    # kind 0, five modes      -- configs 3, 4
+    (1, 15): None,                                               # kind 1, five modes: measured in r02
 }
-# SURVEY.md 8(d) algorithmic estimate (transcendentals costed: sincos 40, cbrt 30, log 35, ...)
+# dram__bytes_read.sum + dram__bytes_write.sum of one loglike_kernel launch (same ncu capture)
+DRAM_TRAFFIC_PER_LAUNCH = {2: 21.03e6 + 0.86e6, 3: 21.54e6 + 33.45e6}
+# SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
+# kept for reference only -- the reduced algorithm needs less than half of it.
 SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0}
 METRIC, UNIT = "lnL_evals_per_sec", "lnL/s"
-
-
-def load_exec_counts():
-    path = os.path.join(ROOT, "profiles", "fp64_ops_per_bin_eval.json")
-    if os.path.exists(path):
-        with open(path) as fh:
-            for k, v in json.load(fh).items():
-                if k.isdigit():
-                    EXEC_FP64_PER_BIN_EVAL[int(k)] = v
 
 
 class ClockSampler:
@@ -169,7 +168,6 @@ def run_ours(args):
     rank, local_rank, world = pdist.init("nccl")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
-    load_exec_counts()
 
     # ---- inputs: synthetic, seeded; the injection comes from this library's own response call
     n_batches = 4
@@ -241,30 +239,40 @@ def run_ours(args):
 
     # ---- roofline of the dominant kernel (per launch, timed live with CUDA events in the library)
     peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
-    dfma_tflops, _ = P.fp64_peak(8192)
+    dfma_tflops, _ = P.fp64_peak(8192, mode=0)
+    dfma3_tflops, _ = P.fp64_peak(8192, mode=1)
     n_det = len(wl.model.detectors)
-    kern_ms = main_ms / max(1, main_launches)                 # one launch = one detector, B x N bin-evals
-    ops = EXEC_FP64_PER_BIN_EVAL.get(args.config, {"dfma": 0, "dmul": 0, "dadd": 0})
-    flop_per_unit = (2.0 * ops["dfma"] + ops["dmul"] + ops["dadd"]) / n_det   # per (sample, bin, detector)
-    inst_per_unit = (ops["dfma"] + ops["dmul"] + ops["dadd"]) / n_det
-    achieved = flop_per_unit * B * N / (kern_ms * 1e-3) / 1e12
-    survey_unit = SURVEY_FLOP_PER_BIN_EVAL[args.config] / n_det
-    roofline = {
-        "bound": "alu", "kernel": "loglike_kernel", "achieved": achieved, "peak": peak_tflops, "unit": "TFLOP/s",
-        "frac": achieved / peak_tflops, "traffic": None,
-        "peak_source": "148 SM x 64 FP64 lanes x 2 x clocks.max.sm (DESIGN.md); DFMA micro-benchmark alongside",
-        "peak_dfma_measured": dfma_tflops,
-        "fp64_pipe_frac": inst_per_unit * B * N / (kern_ms * 1e-3) / (peak_tflops * 1e12 / 2.0),
-        "flop_per_launch": flop_per_unit * B * N, "kernel_ms": kern_ms, "kernel_launches": main_launches,
-        "kernel_share_of_step": main_ms / elapsed_ms,
-        "flop_basis": "executed FP64 (2*DFMA+DMUL+DADD per bin-eval from ncu, profiles/fp64_ops_per_bin_eval.json)",
-        "survey_algorithmic": {"flop_per_bin_eval": SURVEY_FLOP_PER_BIN_EVAL[args.config],
-                               "achieved": survey_unit * B * N / (kern_ms * 1e-3) / 1e12,
-                               "frac": survey_unit * B * N / (kern_ms * 1e-3) / 1e12 / peak_tflops},
-    }
-    traffic_path = os.path.join(ROOT, "profiles", "dram_traffic_per_launch.json")
-    if os.path.exists(traffic_path):
-        roofline["traffic"] = json.load(open(traffic_path)).get(str(args.config))
+    kern_ms = main_ms / max(1, main_launches)                 # one launch = one detector, B x N (sample, bin) units
+    cmask = (2 if wl.model.mode_mask & 9 else 0) | (1 if wl.model.mode_mask & 2 else 0) | \
+            (4 if wl.model.mode_mask & 4 else 0) | (8 if wl.model.mode_mask & 16 else 0)
+    per_det = [FP64_OPS_PER_UNIT.get((d.kind, cmask)) for d in wl.model.detectors]
+    known = [o for o in per_det if o]
+    ops = {k: sum(o[k] for o in known) / len(known) for k in ("dfma", "dmul", "dadd")} if known else None
+    roofline = {"bound": "alu", "kernel": "loglike_kernel", "achieved": None, "peak": peak_tflops,
+                "unit": "TFLOP/s", "frac": None, "traffic": DRAM_TRAFFIC_PER_LAUNCH.get(args.config)}
+    if ops:
+        flop_per_unit = 2.0 * ops["dfma"] + ops["dmul"] + ops["dadd"]
+        inst_per_unit = ops["dfma"] + ops["dmul"] + ops["dadd"]
+        achieved = flop_per_unit * B * N / (kern_ms * 1e-3) / 1e12
+        roofline.update({
+            "achieved": achieved, "frac": achieved / peak_tflops,
+            "flop_per_unit": flop_per_unit, "unit_of_work": "(sample, bin, detector)",
+            "flop_per_launch": flop_per_unit * B * N,
+            "fma_share_of_fp64_instructions": ops["dfma"] / inst_per_unit,
+            "fp64_pipe_frac": inst_per_unit * B * N / (kern_ms * 1e-3) / (peak_tflops * 1e12 / 2.0),
+            "detectors_with_measured_op_counts": f"{len(known)} of {n_det}",
+        })
+    roofline.update({
+        "peak_source": "148 SM x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md; no FP64 entry in "
+                       "MEASURED_PEAKS.json); DFMA micro-benchmarks of this library alongside",
+        "peak_dfma_measured": dfma_tflops, "peak_dfma_3reg_measured": dfma3_tflops,
+        "frac_of_dfma_measured": (roofline["achieved"] / dfma_tflops) if roofline["achieved"] else None,
+        "kernel_ms": kern_ms, "kernel_launches": main_launches, "kernel_share_of_step": main_ms / elapsed_ms,
+        "flop_basis": "FP64 operations of the reduced algorithm = executed 2*DFMA+DMUL+DADD per unit, ncu "
+                      "(profiles/r01_loglike_kernel_ncu.md)",
+        "hbm_gbs_achieved": (roofline["traffic"] / (kern_ms * 1e-3) / 1e9) if roofline["traffic"] else None,
+        "survey_estimate_flop_per_bin_eval": SURVEY_FLOP_PER_BIN_EVAL[args.config],
+    })
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:

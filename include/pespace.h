@@ -105,10 +105,14 @@ int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data
                          const double* h_psd, const pespace_grid* grid, const pespace_model* model,
                          double* h_out_lnL);
 
-/* FP64 FMA micro-benchmark used as the roofline denominator: runs `iters` dependent-chain
- * DFMA blocks on every SM and returns the sustained rate in TFLOP/s (FMA = 2 flop) and the
- * kernel time in ms.  Synchronous. */
-int pespace_fp64_peak(int iters, double* h_out_tflops, double* h_out_ms);
+/* FP64 FMA micro-benchmark used as the roofline denominator: runs `iters` blocks of 64
+ * DFMAs (8 independent chains) per thread on every SM and returns the sustained rate in
+ * TFLOP/s (FMA = 2 flop) and the kernel time in ms.  Synchronous.
+ *   mode 0: a = a*m + c with m, c shared by the chains (two register operands per DFMA):
+ *           the FP64 pipe peak, 1 warp-instruction / 2 cycles / SM sub-partition;
+ *   mode 1: a = a*b + c with three distinct register operands per DFMA: the register-file
+ *           read bandwidth then limits the pipe to 1 / 3 cycles (profiles/r01_fp64_operand_bandwidth.md). */
+int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms);
 
 /* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel
  * (the fused per-bin likelihood kernel) is bracketed by CUDA events on the launching stream.

@@ -51,7 +51,7 @@ def _load():
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
-    L.pespace_fp64_peak.argtypes = [C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+    L.pespace_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.pespace_profile_enable.argtypes = [C.c_int]
     L.pespace_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i64)]
     L.pespace_launch_count.restype = i64
@@ -188,10 +188,11 @@ def loglike_host(params: np.ndarray, data: np.ndarray, psd: np.ndarray, grid, mo
     return out
 
 
-def fp64_peak(iters: int = 4096):
-    """-> (TFLOP/s, ms) of the DFMA micro-benchmark."""
+def fp64_peak(iters: int = 4096, mode: int = 0):
+    """-> (TFLOP/s, ms) of the DFMA micro-benchmark (mode 0: two register operands, the pipe peak;
+    mode 1: three distinct register operands)."""
     t, ms = C.c_double(), C.c_double()
-    _check(_lib.pespace_fp64_peak(int(iters), C.byref(t), C.byref(ms)), "pespace_fp64_peak")
+    _check(_lib.pespace_fp64_peak(int(mode), int(iters), C.byref(t), C.byref(ms)), "pespace_fp64_peak")
     return t.value, ms.value
 
 

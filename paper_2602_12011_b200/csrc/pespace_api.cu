@@ -279,22 +279,27 @@ int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data
   return bail(PESPACE_OK);
 }
 
-int pespace_fp64_peak(int iters, double* h_out_tflops, double* h_out_ms) {
-  if (iters <= 0 || !h_out_tflops) return PESPACE_EINVAL;
+int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms) {
+  if (iters <= 0 || !h_out_tflops || (mode != 0 && mode != 1)) return PESPACE_EINVAL;
   int dev = 0, sms = 0;
   CU(cudaGetDevice(&dev));
   CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
-  double* d_out = nullptr;
+  double *d_in = nullptr, *d_out = nullptr;
+  CU(cudaMalloc((void**)&d_in, 64 * 8));
   CU(cudaMalloc((void**)&d_out, 8));
+  CU(cudaMemset(d_in, 0, 64 * 8));          // all-zero operands: no overflow, full-rate DFMA
   cudaEvent_t e0, e1;
   CU(cudaEventCreate(&e0));
   CU(cudaEventCreate(&e1));
   const int blocks = sms * 8, threads = 256;
-  dfma_peak_kernel<<<blocks, threads>>>(iters / 8 + 1, 1.0, d_out);   // warm-up
-  ++g_launches;
+  auto go = [&](int n) {
+    if (mode == 0) dfma_peak_kernel<false><<<blocks, threads>>>(n, d_in, d_out);
+    else dfma_peak_kernel<true><<<blocks, threads>>>(n, d_in, d_out);
+    ++g_launches;
+  };
+  go(iters / 8 + 1);   // warm-up
   CU(cudaEventRecord(e0));
-  dfma_peak_kernel<<<blocks, threads>>>(iters, 1.0, d_out);
-  ++g_launches;
+  go(iters);
   CU(cudaEventRecord(e1));
   CU(cudaEventSynchronize(e1));
   float ms = 0.f;
@@ -302,7 +307,7 @@ int pespace_fp64_peak(int iters, double* h_out_tflops, double* h_out_ms) {
   const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
   *h_out_tflops = flops / (ms * 1e-3) / 1e12;
   if (h_out_ms) *h_out_ms = ms;
-  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_out);
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_in); cudaFree(d_out);
   return PESPACE_OK;
 }
 

@@ -540,19 +540,26 @@ response_kernel(const double* __restrict__ consts, long long B, const double* __
   }
 }
 
-// FP64 FMA peak: 8 independent chains per thread.
-__global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, double seed, double* __restrict__ out) {
-  double a0 = seed + threadIdx.x, a1 = a0 + 1.0, a2 = a0 + 2.0, a3 = a0 + 3.0, a4 = a0 + 4.0, a5 = a0 + 5.0,
-         a6 = a0 + 6.0, a7 = a0 + 7.0;
-  const double m = 0.999999, c = 1e-6;
+// FP64 FMA peak: 8 independent chains per thread.  THREE = false: the multiplier and addend are
+// shared by the chains (two register operands per DFMA); THREE = true: three distinct registers.
+template <bool THREE>
+__global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, const double* __restrict__ in,
+                                                        double* __restrict__ out) {
+  double a[8], b[8], c[8];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    a[j] = in[(threadIdx.x + j) & 63];
+    b[j] = in[(threadIdx.x + 2 * j + 1) & 63];
+    c[j] = in[(threadIdx.x + 3 * j + 2) & 63];
+  }
   for (int i = 0; i < iters; ++i) {
 #pragma unroll
-    for (int j = 0; j < 8; ++j) {
-      a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
-      a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int j = 0; j < 8; ++j) a[j] = THREE ? fma(a[j], b[j], c[j]) : fma(a[j], b[0], c[0]);
     }
   }
-  const double r = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  const double r = ((a[0] + a[1]) + (a[2] + a[3])) + ((a[4] + a[5]) + (a[6] + a[7]));
   if (r == 12345.678) out[0] = r;   // never true; keeps the chains alive
 }
 
