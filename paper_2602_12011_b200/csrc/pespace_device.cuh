@@ -21,6 +21,8 @@
 #include <cuda_runtime.h>
 #include <math_constants.h>
 
+#include "pespace_dual.cuh"
+
 namespace pespace {
 
 constexpr int NPAR = 11;
@@ -284,130 +286,145 @@ __device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restric
 }
 
 // ---------------------------------------------------------------------------------------------
-// S1: per-sample constants.  One thread per sample; plain double-precision library math.
+// S1: per-sample constants.  One thread per sample; plain double-precision library math.  The body
+// is written once on a scalar type T: double for the likelihood / response path, Du<7> (tangents
+// w.r.t. M, q, chi1, chi2, iota, lambda, beta) for the Fisher path.  `put(idx, value)` stores one
+// constant of the sample block.
 struct PrepArgs { DetC det[8]; int n_det; unsigned mode_mask; };
 
-__device__ __forceinline__ void swsh_pairs(double iota, double Yp[5], double Ym[5]) {
+template <class T>
+__device__ __forceinline__ void swsh_pairs(const T& iota, T Yp[5], T Ym[5]) {
   // -2Y_lm(iota, 0) closed forms for (2,2),(2,1),(3,3),(3,2),(4,4) and their -m partners
-  const double c = cos(iota), s = sin(iota), C = cos(0.5 * iota), Sh = sin(0.5 * iota);
+  const T c = p_cos(iota), s = p_sin(iota), C = p_cos(iota * 0.5), Sh = p_sin(iota * 0.5);
   const double n22 = 0.15769578262626000302, n21 = 0.31539156525252000603;
   const double n33 = 1.8281831978578629446, n3 = 1.4927053303604615657;
-  const double C2 = C * C, S2 = Sh * Sh;
-  Yp[0] = n22 * (1.0 + c) * (1.0 + c);        Ym[0] = n22 * (1.0 - c) * (1.0 - c);
-  Yp[1] = n21 * s * (1.0 + c);                Ym[1] = n21 * s * (1.0 - c);
-  Yp[2] = -n33 * C2 * C2 * C * Sh;            Ym[2] = n33 * C * S2 * S2 * Sh;
-  Yp[3] = n3 * C2 * C2 * (3.0 * c - 2.0) * 0.5;  Ym[3] = n3 * S2 * S2 * (3.0 * c + 2.0) * 0.5;
-  Yp[4] = 3.0 * n3 * C2 * C2 * C2 * S2;       Ym[4] = 3.0 * n3 * C2 * S2 * S2 * S2;
+  const T C2 = C * C, S2 = Sh * Sh;
+  Yp[0] = n22 * ((1.0 + c) * (1.0 + c));        Ym[0] = n22 * ((1.0 - c) * (1.0 - c));
+  Yp[1] = n21 * (s * (1.0 + c));                Ym[1] = n21 * (s * (1.0 - c));
+  Yp[2] = -n33 * (C2 * C2 * C * Sh);            Ym[2] = n33 * (C * S2 * S2 * Sh);
+  Yp[3] = (n3 * 0.5) * (C2 * C2 * (3.0 * c - 2.0));  Ym[3] = (n3 * 0.5) * (S2 * S2 * (3.0 * c + 2.0));
+  Yp[4] = (3.0 * n3) * (C2 * C2 * C2 * S2);     Ym[4] = (3.0 * n3) * (C2 * S2 * S2 * S2);
 }
 
-__global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
-                                    double* __restrict__ consts) {
-  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (b >= B) return;
-  const double* th = params + b * NPAR;
-  const int stride = sample_stride(A.n_det);
-  double* o = consts + b * stride;
+__device__ __forceinline__ bool sample_in_domain(const double* th) {
   bool ok = true;
   for (int i = 0; i < NPAR; ++i) ok = ok && isfinite(th[i]);
-  ok = ok && th[0] > 0.0 && th[1] >= 1.0 && th[4] > 0.0;
-  if (!ok) {
-    for (int i = 0; i < stride; ++i) o[i] = 0.0;
-    o[W_A] = 1.0; o[W_VALID] = 0.0;
-    return;
-  }
-  const double M = th[0], q = th[1], chi1 = th[2], chi2 = th[3], DL = th[4], iota = th[5], phic = th[6],
-               lam = th[7], bet = th[8], pol = th[9], tc = th[10];
-  const double Ms = M * (kGMsun / (kC * kC * kC));
-  const double eta = q / ((1.0 + q) * (1.0 + q)), delta = (q - 1.0) / (q + 1.0);
-  const double mu1 = q / (1.0 + q), mu2 = 1.0 / (1.0 + q);
-  const double Ds = DL * (kGpc / kC);
-  const double a = cbrt(kPi * Ms);
-  o[W_A] = a; o[W_LNA] = log(a); o[W_TC] = tc;
-  o[W_PH0] = -4.0 * (phic / kPi + 0.125);              // quarter turns
-  o[W_VALID] = 1.0;
+  return ok && th[0] > 0.0 && th[1] >= 1.0 && th[4] > 0.0;
+}
+
+template <class T, class Put>
+__device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
+  const T M = th[0], q = th[1], chi1 = th[2], chi2 = th[3], DL = th[4], iota = th[5], phic = th[6],
+          lam = th[7], bet = th[8], pol = th[9], tc = th[10];
+  const T Ms = M * (kGMsun / (kC * kC * kC));
+  const T eta = q / ((1.0 + q) * (1.0 + q)), delta = (q - 1.0) / (q + 1.0);
+  const T mu1 = q / (1.0 + q), mu2 = 1.0 / (1.0 + q);
+  const T Ds = DL * (kGpc / kC);
+  const T a = p_cbrt(kPi * Ms);
+  put(W_A, a); put(W_LNA, p_log(a)); put(W_TC, tc);
+  put(W_PH0, -4.0 * (phic / kPi + 0.125));              // quarter turns
+  put(W_VALID, T(1.0));
   // TaylorF2 3.5PN coefficients, spin terms per G3
   const double pi2 = kPi * kPi;
-  const double bso = (113.0 / 12.0 * mu1 * mu1 + 6.25 * eta) * chi1 + (113.0 / 12.0 * mu2 * mu2 + 6.25 * eta) * chi2;
-  const double sss = 79.0 / 8.0 * eta * chi1 * chi2;
-  const double ph2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
-  const double ph3 = -16.0 * kPi + 4.0 * bso;
-  const double ph4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * eta * eta - 10.0 * sss;
-  const double ph5a = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);          // phi5 = ph5a (1 + 3 ln v)
-  const double ph6a = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * pi2 - 6848.0 / 21.0 * kEuler +
-                      eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi2) + 76055.0 / 1728.0 * eta * eta -
-                      127825.0 / 1296.0 * eta * eta * eta - 6848.0 / 21.0 * log(4.0);   // phi6 = ph6a - 6848/21 ln v
+  const T bso = (113.0 / 12.0 * (mu1 * mu1) + 6.25 * eta) * chi1 + (113.0 / 12.0 * (mu2 * mu2) + 6.25 * eta) * chi2;
+  const T sss = 79.0 / 8.0 * (eta * chi1 * chi2);
+  const T ph2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
+  const T ph3 = -16.0 * kPi + 4.0 * bso;
+  const T ph4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * (eta * eta) - 10.0 * sss;
+  const T ph5a = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);          // phi5 = ph5a (1 + 3 ln v)
+  const T ph6a = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * pi2 - 6848.0 / 21.0 * kEuler +
+                 eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi2) + 76055.0 / 1728.0 * (eta * eta) -
+                 127825.0 / 1296.0 * (eta * eta * eta) - 6848.0 / 21.0 * log(4.0);   // phi6 = ph6a - 6848/21 ln v
   const double ph6l = -6848.0 / 21.0;
-  const double ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * eta * eta);
-  const double a5 = 1.0 / (a * a * a * a * a);
-  const double cP = 4.0 * 3.0 / (256.0 * kPi * eta) * a5;    // 4 Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
-  o[W_P0] = cP; o[W_P2] = cP * ph2; o[W_P3] = cP * ph3; o[W_P4] = cP * ph4;
-  o[W_P5] = cP * ph5a; o[W_P5L] = cP * 3.0 * ph5a; o[W_P6] = cP * ph6a; o[W_P6L] = cP * ph6l; o[W_P7] = cP * ph7;
-  const double cQ = cP / (3.0 * kYear);                       // 4 (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
-  o[W_Q0] = -5.0 * cQ; o[W_Q2] = -3.0 * cQ * ph2; o[W_Q3] = -2.0 * cQ * ph3; o[W_Q4] = -cQ * ph4;
-  o[W_Q5] = 3.0 * cQ * ph5a; o[W_Q6] = cQ * (ph6a + ph6l); o[W_Q6L] = cQ * ph6l; o[W_Q7] = 2.0 * cQ * ph7;
+  const T ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * (eta * eta));
+  const T a5 = 1.0 / (a * a * a * a * a);
+  const T cP = 4.0 * 3.0 / (256.0 * kPi * eta) * a5;    // 4 Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
+  put(W_P0, cP); put(W_P2, cP * ph2); put(W_P3, cP * ph3); put(W_P4, cP * ph4);
+  put(W_P5, cP * ph5a); put(W_P5L, cP * 3.0 * ph5a); put(W_P6, cP * ph6a); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
+  const T cQ = cP / (3.0 * kYear);                       // 4 (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
+  put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
+  put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l)); put(W_Q6L, cQ * ph6l); put(W_Q7, 2.0 * cQ * ph7);
   // amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
-  const double amp0 = sqrt(2.0 * eta / 3.0) * 0.82630748711075811083 * (Ms * Ms / Ds) / (Ms * sqrt(cbrt(Ms)));
+  const T amp0 = p_sqrt(2.0 * eta / 3.0) * 0.82630748711075811083 * (Ms * Ms / Ds) / (Ms * p_sqrt(p_cbrt(Ms)));
   const double s57 = sqrt(5.0 / 7.0);
-  const double clm[5] = {1.0, delta / 3.0, 0.75 * sqrt(15.0 / 14.0) * delta, s57 / 3.0 * (1.0 - 3.0 * eta),
-                         8.0 / 9.0 * s57 * (1.0 - 3.0 * eta)};
+  const T clm[5] = {T(1.0), delta / 3.0, 0.75 * sqrt(15.0 / 14.0) * delta, s57 / 3.0 * (1.0 - 3.0 * eta),
+                    8.0 / 9.0 * s57 * (1.0 - 3.0 * eta)};
   const int mm[5] = {2, 1, 3, 2, 4}, ll[5] = {2, 2, 3, 3, 4};
-  double Yp[5], Ym[5];
+  T Yp[5], Ym[5];
   swsh_pairs(iota, Yp, Ym);
-  for (int i = 0; i < 16; ++i) o[W_KA + i] = 0.0;
+  T kam[16];
+  for (int i = 0; i < 16; ++i) kam[i] = T(0.0);
   for (int i = 0; i < 5; ++i) {
     if (!((A.mode_mask >> i) & 1u)) continue;
     const int m = mm[i];
     const double sg = (ll[i] & 1) ? -1.0 : 1.0;
-    const double Alm = sqrt(2.0 / m) * clm[i] * amp0 * kM76[m - 1];
-    const double Kp = 0.5 * (Yp[i] + sg * Ym[i]);           // K+ (real)
-    const double Kc = 0.5 * (Yp[i] - sg * Ym[i]);           // Kx = -i Kc
-    double* ka = o + W_KA + 4 * (m - 1);
-    const int slot = (i == 3) ? 1 : 0;                      // (3,2) rides on the m=2 class with an extra v^2
-    ka[slot] = Alm * Kp;
-    ka[2 + slot] = 2.0 * Alm * Kc;                          // factor 2 of n.e_x.n = 2 (n.u)(n.v)
+    const T Alm = sqrt(2.0 / m) * clm[i] * amp0 * kM76[m - 1];
+    const T Kp = 0.5 * (Yp[i] + sg * Ym[i]);           // K+ (real)
+    const T Kc = 0.5 * (Yp[i] - sg * Ym[i]);           // Kx = -i Kc
+    const int slot = (i == 3) ? 1 : 0;                 // (3,2) rides on the m=2 class with an extra v^2
+    kam[4 * (m - 1) + slot] = Alm * Kp;
+    kam[4 * (m - 1) + 2 + slot] = 2.0 * Alm * Kc;      // factor 2 of n.e_x.n = 2 (n.u)(n.v)
   }
+  for (int i = 0; i < 16; ++i) put(W_KA + i, kam[i]);
   // frame (O7) with the polarisation angle absorbed into the basis: u' = cos(psi) u + sin(psi) v, ...
-  const double cl = cos(lam), sl = sin(lam), cb = cos(bet), sb = sin(bet), cp = cos(pol), sp = sin(pol);
-  const double k[3] = {-cb * cl, -cb * sl, -sb};
-  const double u[3] = {sl, -cl, 0.0};
-  const double v[3] = {-sb * cl, -sb * sl, cb};
-  double up[3], vp[3];
-  for (int i = 0; i < 3; ++i) { up[i] = cp * u[i] + sp * v[i]; vp[i] = -sp * u[i] + cp * v[i]; }
+  const T cl = p_cos(lam), sl = p_sin(lam), cb = p_cos(bet), sb = p_sin(bet), cp = p_cos(pol), sp = p_sin(pol);
+  const T k[3] = {-(cb * cl), -(cb * sl), -sb};
+  const T u[3] = {sl, -cl, T(0.0)};
+  const T v[3] = {-(sb * cl), -(sb * sl), cb};
+  T up[3], vp[3];
+  for (int i = 0; i < 3; ++i) { up[i] = cp * u[i] + sp * v[i]; vp[i] = cp * v[i] - sp * u[i]; }
   const double r43 = 1.0 / (4.0 * sqrt(3.0));
-  const double* W3[3] = {k, up, vp};
+  const T* W3[3] = {k, up, vp};
   const int off[3] = {S_K, S_U, S_V};
   for (int j = 0; j < 3; ++j) {
-    const double* w = W3[j];
-    double* d = o + off[j];
-    d[0] = w[0] * r43; d[1] = w[1] * r43; d[2] = -0.5 * w[2];
-    d[3] = -3.0 * w[0] * r43; d[4] = -3.0 * w[1] * r43;
+    const T* w = W3[j];
+    put(off[j] + 0, w[0] * r43); put(off[j] + 1, w[1] * r43); put(off[j] + 2, -0.5 * w[2]);
+    put(off[j] + 3, -3.0 * r43 * w[0]); put(off[j] + 4, -3.0 * r43 * w[1]);
   }
-  o[S_DX] = (kAU / kC) * k[0]; o[S_DY] = (kAU / kC) * k[1]; o[S_PAD] = 0.0;
+  put(S_DX, (kAU / kC) * k[0]); put(S_DY, (kAU / kC) * k[1]); put(S_PAD, T(0.0));
+  const double tcv = p_val(tc);
   for (int dI = 0; dI < A.n_det; ++dI) {
     const DetC& D = A.det[dI];
-    double* d = o + D_BASE + D_STRIDE * dI;
-    for (int i = 0; i < D_STRIDE; ++i) d[i] = 0.0;
-    double a0 = tc / kYear;
+    const int base = D_BASE + D_STRIDE * dI;
+    double a0 = tcv / kYear;
     a0 -= rint(a0);
     if (D.kind == 0) {
-      d[0] = 4.0 * (a0 + D.kappa / (2.0 * kPi));
+      put(base, T(4.0 * (a0 + D.kappa / (2.0 * kPi))));
+      for (int i = 1; i < D_STRIDE; ++i) put(base + i, T(0.0));
     } else {
-      d[0] = 4.0 * a0;
-      double p0 = tc / D.period_s;
+      put(base, T(4.0 * a0));
+      double p0 = tcv / D.period_s;
       p0 -= rint(p0);
-      d[1] = 4.0 * (p0 + D.lambda0 / (2.0 * kPi));
+      put(base + 1, T(4.0 * (p0 + D.lambda0 / (2.0 * kPi))));
       const double cL = cos(D.lon), sL = sin(D.lon), cB = cos(D.lat), sB = sin(D.lat);
       const double nh[3] = {cB * cL, cB * sL, sB};
       const double e1[3] = {-sL, cL, 0.0};
       const double e2[3] = {nh[1] * e1[2] - nh[2] * e1[1], nh[2] * e1[0] - nh[0] * e1[2], nh[0] * e1[1] - nh[1] * e1[0]};
       const double r3 = 1.0 / sqrt(3.0);
       for (int j = 0; j < 3; ++j) {
-        const double* w = W3[j];
-        d[2 + 2 * j] = r3 * (w[0] * e1[0] + w[1] * e1[1] + w[2] * e1[2]);
-        d[3 + 2 * j] = r3 * (w[0] * e2[0] + w[1] * e2[1] + w[2] * e2[2]);
+        const T* w = W3[j];
+        put(base + 2 + 2 * j, r3 * (w[0] * e1[0] + w[1] * e1[1] + w[2] * e1[2]));
+        put(base + 3 + 2 * j, r3 * (w[0] * e2[0] + w[1] * e2[1] + w[2] * e2[2]));
       }
     }
   }
+}
+
+__global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
+                                    double* __restrict__ consts) {
+  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= B) return;
+  const double* thp = params + b * NPAR;
+  const int stride = sample_stride(A.n_det);
+  double* o = consts + b * stride;
+  if (!sample_in_domain(thp)) {
+    for (int i = 0; i < stride; ++i) o[i] = 0.0;
+    o[W_A] = 1.0; o[W_VALID] = 0.0;
+    return;
+  }
+  double th[NPAR];
+  for (int i = 0; i < NPAR; ++i) th[i] = thp[i];
+  prep_sample<double>(th, A, [o](int idx, double val) { o[idx] = val; });
 }
 
 // ---------------------------------------------------------------------------------------------
