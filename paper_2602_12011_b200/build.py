@@ -1,17 +1,23 @@
-"""Build libpespace.so in-tree with nvcc for sm_100a (python -m paper_2602_12011_b200.build)."""
+"""Build libpespace.so in-tree with nvcc for sm_100a (python -m paper_2602_12011_b200.build).
+
+Every .cu under csrc/ is one translation unit; they are compiled in parallel to build/*.o and
+linked into paper_2602_12011_b200/libpespace.so."""
+import concurrent.futures as cf
+import glob
 import os
 import subprocess
 import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
+OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpespace.so")
-SOURCES = [os.path.join(CSRC, "pespace_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, "pespace_device.cuh"),
-                  os.path.join(os.path.dirname(HERE), "include", "pespace.h")]
+SOURCES = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
+DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(CSRC, "*.hpp"))) + \
+    [os.path.join(os.path.dirname(HERE), "include", "pespace.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "-shared", "--fmad=true", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"]
 
 
 def nvcc() -> str:
@@ -19,15 +25,34 @@ def nvcc() -> str:
     return cand if os.path.exists(cand) else "nvcc"
 
 
+def _compile(src: str, verbose: bool) -> str:
+    obj = os.path.join(OBJ, os.path.basename(src)[:-3] + ".o")
+    newest = max(os.path.getmtime(p) for p in DEPS)
+    if os.path.exists(obj) and os.path.getmtime(obj) >= newest:
+        return obj
+    res = subprocess.run([nvcc(), *NVCC_FLAGS, "-c", src, "-o", obj], capture_output=True, text=True)
+    if verbose or res.returncode != 0:
+        sys.stderr.write(res.stdout + res.stderr)
+    if res.returncode != 0:
+        raise RuntimeError(f"nvcc failed on {os.path.basename(src)}")
+    return obj
+
+
 def build(force: bool = False, verbose: bool = False) -> str:
     stale = not os.path.exists(LIB) or os.path.getmtime(LIB) < max(os.path.getmtime(p) for p in DEPS)
     if force or stale:
-        cmd = [nvcc(), *NVCC_FLAGS, *SOURCES, "-o", LIB]
-        res = subprocess.run(cmd, capture_output=True, text=True)
+        os.makedirs(OBJ, exist_ok=True)
+        if force:
+            for o in glob.glob(os.path.join(OBJ, "*.o")):
+                os.unlink(o)
+        with cf.ThreadPoolExecutor(max_workers=max(1, min(len(SOURCES), os.cpu_count() or 1))) as ex:
+            objs = list(ex.map(lambda s: _compile(s, verbose), SOURCES))
+        res = subprocess.run([nvcc(), "-shared", "-gencode", "arch=compute_100a,code=sm_100a", *objs, "-o", LIB],
+                             capture_output=True, text=True)
         if verbose or res.returncode != 0:
             sys.stderr.write(res.stdout + res.stderr)
         if res.returncode != 0:
-            raise RuntimeError("nvcc failed building libpespace.so")
+            raise RuntimeError("nvcc failed linking libpespace.so")
     return LIB
 
 

@@ -1,66 +1,29 @@
 // pespace_api.cu -- the C ABI of include/pespace.h: argument checks, workspace carving, launches.
-#include "../../include/pespace.h"
-#include "pespace_device.cuh"
+#include "pespace_host.hpp"
 
-#include <atomic>
-#include <cmath>
-#include <cstdio>
-#include <cstring>
 #include <mutex>
 #include <vector>
 
 using namespace pespace;
+using namespace pespace::host;
+
+namespace pespace {
+namespace host {
+std::atomic<long long> g_launches{0};
+char* cuda_msg() {
+  static thread_local char msg[256] = "";
+  return msg;
+}
+}  // namespace host
+}  // namespace pespace
 
 namespace {
-
-std::atomic<long long> g_launches{0};
-thread_local char g_cuda_msg[256] = "";
-
-int cuda_fail(cudaError_t e) {
-  snprintf(g_cuda_msg, sizeof g_cuda_msg, "CUDA error: %s", cudaGetErrorString(e));
-  return PESPACE_ECUDA;
-}
-#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
-#define LAUNCHED() do { ++g_launches; cudaError_t e_ = cudaGetLastError(); if (e_ != cudaSuccess) return cuda_fail(e_); } while (0)
 
 // optional event timing of the dominant kernel (pespace_profile_enable / _read)
 struct EvPair { cudaEvent_t a, b; };
 bool g_profile = false;
 std::vector<EvPair> g_events;
 std::mutex g_ev_mutex;
-
-bool model_ok(const pespace_model* m) {
-  if (!m || !m->det || m->n_det < 1 || m->n_det > PESPACE_MAX_DET) return false;
-  if ((m->mode_mask & 31u) == 0 || (m->mode_mask & ~31u) != 0) return false;
-  for (int i = 0; i < m->n_det; ++i) {
-    const pespace_detector& d = m->det[i];
-    if (d.kind != 0 && d.kind != 1) return false;
-    if (d.tdi_gen != 15 && d.tdi_gen != 20) return false;
-    if (!(d.L_m > 0.0) || !std::isfinite(d.L_m)) return false;
-    if (d.kind == 1 && !(d.period_s > 0.0)) return false;
-  }
-  return true;
-}
-bool grid_ok(const pespace_grid* g) {
-  return g && g->N > 0 && g->df > 0.0 && g->f0 > 0.0 && std::isfinite(g->df) && std::isfinite(g->f0);
-}
-
-DetC make_det(const pespace_detector& d) {
-  DetC c;
-  std::memset(&c, 0, sizeof c);
-  c.Lbar = d.L_m / kC;
-  c.kind = d.kind; c.gen = d.tdi_gen;
-  c.kappa = d.kappa; c.lambda0 = d.lambda0; c.period_s = d.period_s; c.lon = d.lon; c.lat = d.lat;
-  c.yr_over_p = (d.kind == 1) ? kYear / d.period_s : 0.0;
-  for (int n = 0; n < 3; ++n) {
-    const double ang = 2.0 * kPi * n / 3.0 + (d.kind == 0 ? d.lambda0 : 0.0);
-    c.cn[n] = std::cos(ang); c.sn[n] = std::sin(ang);
-  }
-  // arms a: 2-3, b: 3-1, c: 1-2
-  const int r[3] = {1, 2, 0}, s[3] = {2, 0, 1};
-  for (int l = 0; l < 3; ++l) { c.dcn[l] = c.cn[r[l]] - c.cn[s[l]]; c.dsn[l] = c.sn[r[l]] - c.sn[s[l]]; }
-  return c;
-}
 
 // ---- kernel dispatch on (detector kind, mode-class mask); all 15 masks are instantiated
 template <int KIND, unsigned CM>
@@ -82,17 +45,6 @@ using ResponseFn = void (*)(dim3, cudaStream_t, const double*, long long, const 
 const LoglikeFn kLoglike[2][16] = {PESPACE_ROW(launch_loglike, 0), PESPACE_ROW(launch_loglike, 1)};
 const ResponseFn kResponse[2][16] = {PESPACE_ROW(launch_response, 0), PESPACE_ROW(launch_response, 1)};
 
-unsigned class_mask(unsigned mode_mask) {
-  unsigned m = 0;
-  if (mode_mask & PESPACE_MODE_21) m |= 1u;                       // m = 1
-  if (mode_mask & (PESPACE_MODE_22 | PESPACE_MODE_32)) m |= 2u;   // m = 2
-  if (mode_mask & PESPACE_MODE_33) m |= 4u;                       // m = 3
-  if (mode_mask & PESPACE_MODE_44) m |= 8u;                       // m = 4
-  return m;
-}
-
-size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
-
 struct Plan {
   int n_det, stride;
   long long nbb;          // bin blocks
@@ -111,11 +63,7 @@ Plan make_plan(long long B, long long N, int n_det) {
 }
 
 int run_prep(const double* d_params, long long B, const pespace_model* model, double* d_consts, cudaStream_t st) {
-  PrepArgs A;
-  std::memset(&A, 0, sizeof A);
-  A.n_det = model->n_det;
-  A.mode_mask = model->mode_mask;
-  for (int i = 0; i < model->n_det; ++i) A.det[i] = make_det(model->det[i]);
+  const PrepArgs A = make_prep_args(model);
   const int th = 128;
   prep_samples_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
   LAUNCHED();
@@ -132,7 +80,7 @@ const char* pespace_strerror(int code) {
   switch (code) {
     case PESPACE_OK: return "ok";
     case PESPACE_EINVAL: return "invalid argument";
-    case PESPACE_ECUDA: return g_cuda_msg[0] ? g_cuda_msg : "CUDA error";
+    case PESPACE_ECUDA: return cuda_msg()[0] ? cuda_msg() : "CUDA error";
     case PESPACE_ENOMEM: return "out of memory";
     default: return "unknown error code";
   }
@@ -166,7 +114,7 @@ int pespace_profile_read(double* h_main_ms, int64_t* h_launches) {
 
 size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespace_model* model, int want_fisher) {
   if (B <= 0 || !grid_ok(grid) || !model_ok(model)) return 0;
-  (void)want_fisher;
+  if (want_fisher) return fisher_workspace_bytes(B, grid->N, model->n_det);
   const Plan p = make_plan(B, grid->N, model->n_det);
   return p.consts_bytes + p.partial_bytes;
 }
@@ -233,17 +181,6 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
                                                                 p.stride, d_out_lnL);
   LAUNCHED();
   return PESPACE_OK;
-}
-
-int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
-                   const pespace_grid* grid, const pespace_model* model, double* d_out_F, double* d_out_grad,
-                   void* d_workspace, size_t workspace_bytes, void* stream) {
-  (void)d_data_AET; (void)d_out_grad; (void)stream;
-  if (!d_params || !d_psd || !d_out_F || !d_workspace || B <= 0 || !grid_ok(grid) || !model_ok(model))
-    return PESPACE_EINVAL;
-  if (workspace_bytes < pespace_workspace_bytes(B, grid, model, 1)) return PESPACE_EINVAL;
-  snprintf(g_cuda_msg, sizeof g_cuda_msg, "pespace_fisher: forward-mode kernel not built yet");
-  return PESPACE_ECUDA;
 }
 
 int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET, const double* h_psd,

@@ -410,7 +410,7 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   }
 }
 
-__global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
+static __global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
                                     double* __restrict__ consts) {
   const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;
@@ -508,7 +508,7 @@ loglike_kernel(const double* __restrict__ consts, long long B, const double2* __
 }
 
 // K_combine: fixed-order sum over (detector, bin block); lnL = -1/2 sum; out-of-domain -> -inf.
-__global__ void combine_kernel(const double* __restrict__ partial, const double* __restrict__ consts, long long B,
+static __global__ void combine_kernel(const double* __restrict__ partial, const double* __restrict__ consts, long long B,
                                int n_slices, int stride, double* __restrict__ out) {
   const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (b >= B) return;

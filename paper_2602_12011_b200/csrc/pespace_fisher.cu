@@ -1,0 +1,83 @@
+// pespace_fisher.cu -- pespace_fisher of include/pespace.h: forward-mode derivatives (S10).
+#include "pespace_host.hpp"
+#include "pespace_fisher.cuh"
+
+using namespace pespace;
+using namespace pespace::host;
+
+namespace {
+
+template <int KIND, unsigned CM>
+cudaError_t launch_fisher(dim3 g, cudaStream_t st, const double* consts, long long B, const double2* data,
+                          const double* psd, GridC G, const DetC& dc, int n_det, int det, double* partial) {
+  static bool configured = false;        // per instantiation; the attribute is per function and idempotent
+  if (!configured) {
+    cudaError_t e = cudaFuncSetAttribute(fisher_kernel<KIND, CM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                         (int)fisher_smem_bytes());
+    if (e != cudaSuccess) return e;
+    configured = true;
+  }
+  fisher_kernel<KIND, CM><<<g, FBLOCK, fisher_smem_bytes(), st>>>(consts, B, data, psd, G, dc, n_det, det, partial);
+  return cudaSuccess;
+}
+using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double2*, const double*, GridC,
+                                 const DetC&, int, int, double*);
+#define PESPACE_ROW(F, K) {nullptr, F<K, 1>, F<K, 2>, F<K, 3>, F<K, 4>, F<K, 5>, F<K, 6>, F<K, 7>, F<K, 8>, \
+                           F<K, 9>, F<K, 10>, F<K, 11>, F<K, 12>, F<K, 13>, F<K, 14>, F<K, 15>}
+const FisherFn kFisher[2][16] = {PESPACE_ROW(launch_fisher, 0), PESPACE_ROW(launch_fisher, 1)};
+
+struct FisherPlan {
+  long long nbx, ntile;
+  size_t consts_bytes, partial_bytes;
+};
+FisherPlan make_fisher_plan(long long B, long long N, int n_det) {
+  FisherPlan p;
+  p.nbx = (N + (long long)FBLOCK * FCHUNKS - 1) / ((long long)FBLOCK * FCHUNKS);
+  p.ntile = (B + FTILE - 1) / FTILE;
+  p.consts_bytes = align_up((size_t)B * fisher_const_stride(n_det) * sizeof(double), 256);
+  p.partial_bytes = align_up((size_t)n_det * p.nbx * (size_t)B * NG * sizeof(double), 256);
+  return p;
+}
+
+}  // namespace
+
+namespace pespace {
+namespace host {
+size_t fisher_workspace_bytes(long long B, long long N, int n_det) {
+  const FisherPlan p = make_fisher_plan(B, N, n_det);
+  return p.consts_bytes + p.partial_bytes;
+}
+}  // namespace host
+}  // namespace pespace
+
+extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                              const pespace_grid* grid, const pespace_model* model, double* d_out_F,
+                              double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream) {
+  if (!d_params || !d_psd || !d_out_F || !d_workspace || B <= 0 || !grid_ok(grid) || !model_ok(model))
+    return PESPACE_EINVAL;
+  if (d_out_grad && !d_data_AET) return PESPACE_EINVAL;       // the gradient needs the data
+  if (workspace_bytes < fisher_workspace_bytes(B, grid->N, model->n_det) || ((uintptr_t)d_workspace & 15u))
+    return PESPACE_EINVAL;
+  const FisherPlan p = make_fisher_plan(B, grid->N, model->n_det);
+  if (p.ntile > 65535) return PESPACE_EINVAL;                 // gridDim.y
+  cudaStream_t st = (cudaStream_t)stream;
+  double* d_consts = (double*)d_workspace;
+  double* d_partial = (double*)((char*)d_workspace + p.consts_bytes);
+  const PrepArgs A = make_prep_args(model);
+  const int th = 64;
+  prep_samples_du_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
+  LAUNCHED();
+  const unsigned cm = class_mask(model->mode_mask);
+  const GridC G = {grid->f0, grid->df, (long long)grid->N};
+  const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
+  for (int d = 0; d < model->n_det; ++d) {
+    const DetC dc = make_det(model->det[d]);
+    CU(kFisher[dc.kind][cm](g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial));
+    LAUNCHED();
+  }
+  const long long nt = (long long)B * NG;
+  combine_fisher_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(
+      d_partial, d_consts, B, (int)(model->n_det * p.nbx), fisher_const_stride(model->n_det), d_out_F, d_out_grad);
+  LAUNCHED();
+  return PESPACE_OK;
+}

@@ -1,0 +1,465 @@
+// pespace_fisher.cuh -- forward-mode derivative kernel (S10): F_ij = <d_i h | d_j h> and
+// grad_i = <d - h | d_i h> (Eq. 13, 14; "forward mode").
+//
+// The 11 tangents of h are NOT propagated as an 11-wide dual number.  Per mode class the response is
+//     h_class = CKp Hp + i CKc Hc            (conjugate representation, as in pespace_device.cuh)
+// with real amplitudes CKp, CKc (functions of M, q, D_L, iota and of v) and two complex TDI sums Hp, Hc
+// built with the real arm weights xi_+/D and (n.u')(n.v')/D.  The parameters enter through
+//   * the amplitudes                       (M, q, iota, D_L)          -> linear in Hp, Hc
+//   * the phase psi of the class           (M, q, chi1, chi2, phi_c, t_c) -> i (pi/2) dpsi * h_class
+//   * the time t_lm at which the orbit is evaluated (M, q, chi1, chi2, t_c) -> ONE geometric tangent
+//   * the sky position                     (lambda, beta)             -> two geometric tangents
+//   * the polarisation angle               d Hp = 4 Hc, d Hc = -Hp    -> linear in Hp, Hc
+// so the per-bin geometry runs on a 3-tangent dual number (orbit angle, lambda, beta), the phase and
+// time polynomials on a 4-tangent one (M, q, chi1, chi2), and everything else is closed form.
+//
+// Launch geometry: block = 128 threads = 128 consecutive bins ("chunk"); a block walks FCHUNKS chunks and a
+// tile of FTILE samples.  The 12 x 3 complex numbers (value + 11 tangents of X, Y, Z) of one (sample, bin)
+// are accumulated over the mode classes in shared memory (thread-private columns), then the upper triangle
+// of the 12 x 12 Gram matrix of (residual, d_1 h, ..., d_11 h) -- 78 numbers -- is formed per thread and
+// reduced over the warp by a halving butterfly (93 shuffles instead of 78 x 5), fixed order throughout.
+#pragma once
+#include "pespace_device.cuh"
+
+namespace pespace {
+
+constexpr int FBLOCK = 128;   // threads = bins per chunk
+constexpr int FTILE = 4;      // samples per block
+constexpr int FCHUNKS = 16;   // chunks per block
+constexpr int NT = 12;        // value + 11 tangents
+constexpr int NJ = NT * 6;    // x (X, Y, Z) x (re, im)
+constexpr int NG = 78;        // upper triangle of the 12 x 12 Gram matrix
+constexpr int NGP = 96;       // padded to 3 x 32 for the butterfly
+constexpr int DUW = 8;        // doubles per constant: value + tangents (M, q, chi1, chi2, iota, lambda, beta)
+constexpr int FS_STRIDE = SMEM_STRIDE * DUW;   // one sample, one detector, in shared memory
+constexpr double kHalfPi = 1.57079632679489661923;
+
+__host__ __device__ constexpr int fisher_const_stride(int n_det) { return sample_stride(n_det) * DUW; }
+constexpr size_t fisher_smem_bytes() {
+  return sizeof(double) * ((size_t)NJ * FBLOCK + (size_t)FTILE * FS_STRIDE + (size_t)(FBLOCK / 32) * FTILE * NGP);
+}
+
+// ---- constant accessors: sc points at one sample block [SMEM_STRIDE][DUW]
+__device__ __forceinline__ double cv(const double* sc, int idx) { return sc[idx * DUW]; }
+__device__ __forceinline__ double ct(const double* sc, int idx, int t) { return sc[idx * DUW + 1 + t]; }
+// tangents (M, q, chi1, chi2)
+__device__ __forceinline__ Du<4> c4(const double* sc, int idx) {
+  Du<4> r;
+  const double* p = sc + idx * DUW;
+  r.v = p[0]; r.d[0] = p[1]; r.d[1] = p[2]; r.d[2] = p[3]; r.d[3] = p[4];
+  return r;
+}
+// geometry directions (orbit angle, lambda, beta): constants carry lambda, beta only
+__device__ __forceinline__ Du<3> cg(const double* sc, int idx) {
+  Du<3> r;
+  const double* p = sc + idx * DUW;
+  r.v = p[0]; r.d[0] = 0.0; r.d[1] = p[6]; r.d[2] = p[7];
+  return r;
+}
+// amplitude directions (M, q, iota)
+__device__ __forceinline__ Du<3> ca3(const double* sc, int idx) {
+  Du<3> r;
+  const double* p = sc + idx * DUW;
+  r.v = p[0]; r.d[0] = p[1]; r.d[1] = p[2]; r.d[2] = p[5];
+  return r;
+}
+// a Du<3> with only the orbit-angle tangent
+__device__ __forceinline__ Du<3> ang(double v, double d0) {
+  Du<3> r;
+  r.v = v; r.d[0] = d0; r.d[1] = 0.0; r.d[2] = 0.0;
+  return r;
+}
+
+// phase-like scalars of one class handed from stage A to stage C
+struct ClassScal {
+  double psi;        // phase, quarter turns (reduced)
+  double tau;        // 4 (t_lm - t_c) / yr
+  double dpsi[4];    // (pi/2) d psi / d (M, q, chi1, chi2): radians per unit parameter
+  double dtau[4];    // (pi/2) d tau / d (M, q, chi1, chi2): radians of orbit angle per unit parameter
+  Du<3> CKp, CKc;    // amplitudes, tangents (M, q, iota)
+};
+
+template <int MC>
+__device__ __forceinline__ void fisher_stage_a(const BinC& bc, const double* __restrict__ sc, double ftc4,
+                                               ClassScal& o) {
+  constexpr double CB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
+  constexpr double LN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
+  constexpr double S83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
+  constexpr double MH[4] = {0.5, 1.0, 1.5, 2.0};
+  const double sv = bc.cf * CB[MC];
+  Du<4> v(0.0), L(0.0);
+  v.v = cv(sc, W_A) * sv; v.d[0] = ct(sc, W_A, 0) * sv;
+  L.v = cv(sc, W_LNA) + bc.lnf3 + LN3[MC]; L.d[0] = ct(sc, W_LNA, 0);
+  const Du<4> v2 = v * v;
+  Du<4> P = dfma(c4(sc, W_P7), v, dfma(c4(sc, W_P6L), L, c4(sc, W_P6)));
+  P = dfma(P, v, dfma(c4(sc, W_P5L), L, c4(sc, W_P5)));
+  P = dfma(P, v, c4(sc, W_P4));
+  P = dfma(P, v, c4(sc, W_P3));
+  P = dfma(P, v, c4(sc, W_P2));
+  P = dfma(P, v2, c4(sc, W_P0));
+  Du<4> Q = dfma(c4(sc, W_Q7), v, dfma(c4(sc, W_Q6L), L, c4(sc, W_Q6)));
+  Q = dfma(Q, v, c4(sc, W_Q5));
+  Q = dfma(Q, v, c4(sc, W_Q4));
+  Q = dfma(Q, v, c4(sc, W_Q3));
+  Q = dfma(Q, v, c4(sc, W_Q2));
+  Q = dfma(Q, v2, c4(sc, W_Q0));
+  const double sp = S83[MC] * bc.fm53, sq = S83[MC] * bc.fm83;
+  double psi = sp * P.v;
+  psi -= 4.0 * rint(0.25 * psi);
+  o.psi = psi + fma(MH[MC], cv(sc, W_PH0), ftc4);
+  o.tau = sq * Q.v;
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    o.dpsi[i] = (kHalfPi * sp) * P.d[i];
+    o.dtau[i] = (kHalfPi * sq) * Q.d[i];
+  }
+  // amplitude x polarisation content, tangents (M, q, iota); v carries M only
+  Du<3> va(0.0);
+  va.v = v.v; va.d[0] = v.d[0];
+  const int ka = W_KA + 4 * MC;
+  if (MC == 1) {
+    const Du<3> va2 = va * va;
+    o.CKp = dfma(ca3(sc, ka + 1), va2, ca3(sc, ka));
+    o.CKc = dfma(ca3(sc, ka + 3), va2, ca3(sc, ka + 2));
+  } else if (MC == 3) {
+    const Du<3> va2 = va * va;
+    o.CKp = va2 * ca3(sc, ka);
+    o.CKc = va2 * ca3(sc, ka + 2);
+  } else {
+    o.CKp = va * ca3(sc, ka);
+    o.CKc = va * ca3(sc, ka + 2);
+  }
+}
+
+// J accumulation: column of this thread in shared memory, J[(p * 6 + comp * 2 + ri) * FBLOCK]
+template <bool FIRST>
+__device__ __forceinline__ void jadd(double* J, int p, int comp, double re, double im) {
+  double* a = J + ((p * 6 + comp * 2) * FBLOCK);
+  if (FIRST) { a[0] = re; a[FBLOCK] = im; }
+  else { a[0] += re; a[FBLOCK] += im; }
+}
+
+// One mode class of one (sample, bin, detector): adds value and tangents of (X, Y, Z) to J.
+// Tangent order p = 1..11 follows theta: M, q, chi1, chi2, D_L, iota, phi_c, lambda, beta, psi, t_c
+// (D_L is filled in after the class loop: d h / d D_L = -h / D_L).
+template <int KIND, int MC, bool FIRST>
+__device__ __forceinline__ void fisher_class(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
+                                             double ftc4, double* __restrict__ J) {
+  using G = Du<3>;
+  constexpr double MM[4] = {1.0, 2.0, 3.0, 4.0};
+  ClassScal cs;
+  fisher_stage_a<MC>(bc, sc, ftc4, cs);
+
+  // ---- S4 on (value, d/d alpha [rad], d/d lambda, d/d beta)
+  G G1k, G2k, G1u, G2u, G1v, G2v, kR;
+  if (KIND == 0) {
+    double sa, ca;
+    sincos_qt(cv(sc, D_BASE) + cs.tau, sa, ca);
+    const double c2v = fma(2.0 * ca, ca, -1.0), s2v = 2.0 * sa * ca;
+    const G sA = ang(sa, ca), cA = ang(ca, -sa), s2 = ang(s2v, 2.0 * c2v), c2 = ang(c2v, -2.0 * s2v);
+    auto rot = [&](int off, G& g1, G& g2) {
+      const G w0 = cg(sc, off), w1 = cg(sc, off + 1), w2 = cg(sc, off + 2);
+      g1 = dfma(w0, c2, dfma(w1, s2, dfma(w2, cA, cg(sc, off + 3))));
+      g2 = dfma(w0, s2, dfma(w2, sA, cg(sc, off + 4)) - w1 * c2);
+    };
+    rot(S_K, G1k, G2k);
+    rot(S_U, G1u, G2u);
+    rot(S_V, G1v, G2v);
+    kR = dfma(cg(sc, S_DX), cA, cg(sc, S_DY) * sA);
+  } else {
+    double sE, cE, sp, cp;
+    sincos_qt(cv(sc, D_BASE) + cs.tau, sE, cE);
+    sincos_qt(fma(cs.tau, dc.yr_over_p, cv(sc, D_BASE + 1)), sp, cp);
+    const G sEg = ang(sE, cE), cEg = ang(cE, -sE);
+    const G spg = ang(sp, dc.yr_over_p * cp), cpg = ang(cp, -dc.yr_over_p * sp);
+    auto rot = [&](int off, G& g1, G& g2) {
+      const G w0 = cg(sc, off), w1 = cg(sc, off + 1);
+      g1 = dfma(w0, cpg, w1 * spg);
+      g2 = dfma(w1, cpg, -(w0 * spg));
+    };
+    rot(D_BASE + 2, G1k, G2k);
+    rot(D_BASE + 4, G1u, G2u);
+    rot(D_BASE + 6, G1v, G2v);
+    kR = dfma(cg(sc, S_DX), cEg, cg(sc, S_DY) * sEg);
+  }
+  G nu[3];
+#pragma unroll
+  for (int n = 0; n < 3; ++n) nu[n] = dfma(dc.cn[n], G1k, dc.sn[n] * G2k);
+  G kap[3];                                   // k.n_23, k.n_31, k.n_12
+  kap[0] = nu[1] - nu[2]; kap[1] = nu[2] - nu[0]; kap[2] = nu[0] - nu[1];
+
+  // ---- S5: real arm weights xi_+/D and (n.u')(n.v')/D
+  G Wp[3], Wc[3];
+#pragma unroll
+  for (int l = 0; l < 3; ++l) {
+    const G uu = dfma(dc.dcn[l], G1u, dc.dsn[l] * G2u);
+    const G vv = dfma(dc.dcn[l], G1v, dc.dsn[l] * G2v);
+    const G v2_ = vv * vv;
+    const G D = dfma(uu, uu, v2_);
+    G rD;
+    rD.v = (D.v > 0.0) ? rcp_pos(D.v) : 0.0;
+    const double m2 = -rD.v * rD.v;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) rD.d[i] = m2 * D.d[i];
+    Wp[l] = rD * (uu * uu - v2_);
+    Wc[l] = rD * (uu * vv);
+  }
+
+  // ---- S6: E_n = exp(+i (pi/2) (psi + 4 f k.x_n)) (conjugate representation)
+  G Er[3], Ei[3];
+#pragma unroll
+  for (int n = 0; n < 3; ++n) {
+    const G ph = dfma(dc.Lbar, nu[n], kR);
+    double s, c;
+    sincos_qt(fma(bc.f4, ph.v, cs.psi), s, c);
+    Er[n].v = c; Ei[n].v = s;
+    const double sc4 = kHalfPi * bc.f4;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const double t = sc4 * ph.d[i];
+      Er[n].d[i] = -s * t;
+      Ei[n].d[i] = c * t;
+    }
+  }
+
+  // ---- S7 + tangent assembly, one of X, Y, Z at a time
+  auto bracket = [&](int r, int s_, const G& kp, G& br, G& bi) {
+    br = dfma(kp, dfma(-bc.cth, Er[r], Er[s_]), (-bc.sth) * Ei[r]);
+    bi = dfma(kp, dfma(-bc.cth, Ei[r], Ei[s_]), bc.sth * Er[r]);
+  };
+  auto component = [&](int comp, int r, int s1, const G& k1, int l1, int s2, const G& k2, int l2) {
+    // H = W[l1] B(r, s1, k1) - W[l2] B(r, s2, k2)
+    G b1r, b1i, b2r, b2i;
+    bracket(r, s1, k1, b1r, b1i);
+    bracket(r, s2, k2, b2r, b2i);
+    const G Hpr = Wp[l1] * b1r - Wp[l2] * b2r, Hpi = Wp[l1] * b1i - Wp[l2] * b2i;
+    const G Hcr = Wc[l1] * b1r - Wc[l2] * b2r, Hci = Wc[l1] * b1i - Wc[l2] * b2i;
+    const double kp = cs.CKp.v, kc = cs.CKc.v;
+    const double hr = fma(kp, Hpr.v, -kc * Hci.v), hi = fma(kp, Hpi.v, kc * Hcr.v);      // CKp Hp + i CKc Hc
+    double Tr[3], Ti[3];
+#pragma unroll
+    for (int g = 0; g < 3; ++g) {
+      Tr[g] = fma(kp, Hpr.d[g], -kc * Hci.d[g]);
+      Ti[g] = fma(kp, Hpi.d[g], kc * Hcr.d[g]);
+    }
+    jadd<FIRST>(J, 0, comp, hr, hi);
+    // M, q: amplitude + phase + orbit time;  chi1, chi2: phase + orbit time
+#pragma unroll
+    for (int i = 0; i < 2; ++i) {
+      const double ap = cs.CKp.d[i], ac = cs.CKc.d[i];
+      const double re = fma(ap, Hpr.v, fma(-ac, Hci.v, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0])));
+      const double im = fma(ap, Hpi.v, fma(ac, Hcr.v, fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0])));
+      jadd<FIRST>(J, 1 + i, comp, re, im);
+    }
+#pragma unroll
+    for (int i = 2; i < 4; ++i)
+      jadd<FIRST>(J, 1 + i, comp, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0]), fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0]));
+    // iota: amplitudes only
+    jadd<FIRST>(J, 6, comp, fma(cs.CKp.d[2], Hpr.v, -cs.CKc.d[2] * Hci.v), fma(cs.CKp.d[2], Hpi.v, cs.CKc.d[2] * Hcr.v));
+    // phi_c: d psi = -(4/pi) (m/2) quarter turns -> -m i h
+    jadd<FIRST>(J, 7, comp, MM[MC] * hi, -MM[MC] * hr);
+    // lambda, beta
+    jadd<FIRST>(J, 8, comp, Tr[1], Ti[1]);
+    jadd<FIRST>(J, 9, comp, Tr[2], Ti[2]);
+    // polarisation angle: d Hp = 4 Hc, d Hc = -Hp
+    jadd<FIRST>(J, 10, comp, fma(4.0 * kp, Hcr.v, kc * Hpi.v), fma(4.0 * kp, Hci.v, -kc * Hpr.v));
+    // t_c: phase 2 pi f, orbit angle 2 pi / yr
+    const double wp = kHalfPi * bc.f4, wt = kHalfPi * 4.0 / kYear;
+    jadd<FIRST>(J, 11, comp, fma(-wp, hi, wt * Tr[0]), fma(wp, hr, wt * Ti[0]));
+  };
+  // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2); same terms as eval_class
+  component(0, 0, 2, -kap[1], 1, 1, kap[2], 2);    // X = W_b B(1,3,k13) - W_c B(1,2,k12)
+  component(1, 1, 0, -kap[2], 2, 2, kap[0], 0);    // Y = W_c B(2,1,k21) - W_a B(2,3,k23)
+  component(2, 2, 1, -kap[0], 0, 0, kap[1], 1);    // Z = W_a B(3,2,k32) - W_b B(3,1,k31)
+}
+
+// ---- per-sample constants with tangents: consts_du [B][sample_stride(n_det)][DUW]
+static __global__ void prep_samples_du_kernel(const double* __restrict__ params, long long B, PrepArgs A,
+                                       double* __restrict__ consts) {
+  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (b >= B) return;
+  const double* thp = params + b * NPAR;
+  const int stride = sample_stride(A.n_det);
+  double* o = consts + b * (long long)stride * DUW;
+  if (!sample_in_domain(thp)) {
+    for (int i = 0; i < stride * DUW; ++i) o[i] = 0.0;
+    o[W_A * DUW] = 1.0;
+    return;
+  }
+  // tangent slots: M, q, chi1, chi2, iota, lambda, beta.  D_L, phi_c, psi and t_c are closed form.
+  const int slot[NPAR] = {0, 1, 2, 3, -1, 4, -1, 5, 6, -1, -1};
+  Du<7> th[NPAR];
+  for (int i = 0; i < NPAR; ++i) {
+    th[i] = Du<7>(thp[i]);
+    if (slot[i] >= 0) th[i].d[slot[i]] = 1.0;
+  }
+  prep_sample<Du<7>>(th, A, [o](int idx, const Du<7>& val) {
+    double* p = o + idx * DUW;
+    p[0] = val.v;
+    for (int t = 0; t < 7; ++t) p[1 + t] = val.d[t];
+  });
+  o[S_PAD * DUW] = -1.0 / thp[4];        // d h / d D_L = -h / D_L
+}
+
+__device__ __forceinline__ void stage_tile_du(double* smem, const double* __restrict__ consts, long long b0,
+                                              long long B, int n_det, int det) {
+  const int stride = sample_stride(n_det);
+  for (int i = threadIdx.x; i < FTILE * FS_STRIDE; i += blockDim.x) {
+    const int s = i / FS_STRIDE, r = i % FS_STRIDE, j = r / DUW, t = r % DUW;
+    long long b = b0 + s;
+    if (b >= B) b = B - 1;
+    const int src = (j < D_BASE) ? j : (D_BASE + D_STRIDE * det + (j - D_BASE));
+    smem[i] = consts[(b * stride + src) * DUW + t];
+  }
+}
+
+// index of (p, q), p <= q, in the packed upper triangle of the 12 x 12 Gram matrix
+__host__ __device__ constexpr int gram_index(int p, int q) { return p * NT - p * (p - 1) / 2 + (q - p); }
+
+// Halving butterfly: on entry every lane holds NGP values; on exit lane l holds, in a[0..2], the sums over the
+// warp of the values with index  j + 48 b4 + 24 b3 + 12 b2 + 6 b1 + 3 b0  (b_i = bit i of l), j = 0..2.
+template <int HALF, int OFF>
+__device__ __forceinline__ void butterfly_level(double (&a)[NGP], int lane) {
+  const bool up = lane & OFF;
+#pragma unroll
+  for (int i = 0; i < HALF; ++i) {
+    const double keep = up ? a[i + HALF] : a[i];
+    const double send = up ? a[i] : a[i + HALF];
+    a[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
+  }
+}
+__host__ __device__ inline int butterfly_slot_index(int lane, int j) {
+  return j + 48 * ((lane >> 4) & 1) + 24 * ((lane >> 3) & 1) + 12 * ((lane >> 2) & 1) + 6 * ((lane >> 1) & 1) +
+         3 * (lane & 1);
+}
+
+template <int KIND, unsigned CMASK>
+__global__ void __launch_bounds__(FBLOCK, 2)
+fisher_kernel(const double* __restrict__ consts, long long B, const double2* __restrict__ data /* may be null */,
+              const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
+              double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
+  extern __shared__ double fsm[];
+  double* Jsm = fsm;                                   // [NJ][FBLOCK]
+  double* csm = Jsm + NJ * FBLOCK;                     // [FTILE][SMEM_STRIDE][DUW]
+  double* red = csm + FTILE * FS_STRIDE;               // [warps][FTILE][NGP]
+  const long long b0 = (long long)blockIdx.y * FTILE;
+  stage_tile_du(csm, consts, b0, B, n_det, det);
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int i = threadIdx.x; i < (FBLOCK / 32) * FTILE * NGP; i += FBLOCK) red[i] = 0.0;
+  __syncthreads();
+  double* J = Jsm + threadIdx.x;
+  const int ns = (int)min((long long)FTILE, B - b0);
+  constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
+
+  for (int ch = 0; ch < FCHUNKS; ++ch) {
+    const long long kbase = ((long long)blockIdx.x * FCHUNKS + ch) * FBLOCK;
+    if (kbase >= G.N) break;
+    const long long k = kbase + threadIdx.x;
+    const bool live = k < G.N;
+    const long long kk = live ? k : G.N - 1;
+    const BinC bc = make_bin(fma((double)kk, G.df, G.f0), dc.Lbar);
+    double gr, gi;
+    tdi_prefactor(bc, dc.gen, gr, gi);
+    const double g2 = gr * gr + gi * gi;
+    const double nrm[3] = {1.4142135623730950488, 2.4494897427831780982, 1.7320508075688772935};
+    double dr[3], di[3], w[3];
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      const size_t idx = ((size_t)det * 3 + c) * (size_t)G.N + (size_t)kk;
+      double2 d = make_double2(0.0, 0.0);
+      if (data) d = data[idx];
+      const double Sn = psd[idx];
+      const bool use = live && isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
+      const double sc_ = use ? nrm[c] / g2 : 0.0;
+      dr[c] = (d.x * gr + d.y * gi) * sc_;
+      di[c] = (d.x * gi - d.y * gr) * sc_;
+      w[c] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+    }
+    for (int s = 0; s < ns; ++s) {
+      const double* sc = csm + s * FS_STRIDE;
+      const double tc = cv(sc, W_TC);
+      const double p = bc.f4 * tc;
+      const double ftc4 = (p - 4.0 * rint(0.25 * p)) + fma(bc.f4, tc, -p);
+      if (c0) fisher_class<KIND, 0, true>(bc, sc, dc, ftc4, J);
+      if (c1) fisher_class<KIND, 1, !c0>(bc, sc, dc, ftc4, J);
+      if (c2) fisher_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, ftc4, J);
+      if (c3) fisher_class<KIND, 3, !(c0 || c1 || c2)>(bc, sc, dc, ftc4, J);
+      // Gram matrix of a_0 = d - h, a_p = d_p h (p = 1..11) over the channels A, E, T
+      const double mDL = cv(sc, S_PAD);
+      double a[NGP];
+#pragma unroll
+      for (int i = 0; i < NGP; ++i) a[i] = 0.0;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        double ar[NT], ai[NT];
+#pragma unroll
+        for (int pp = 0; pp < NT; ++pp) {
+          if (pp == 5) continue;
+          const double* jp = J + pp * 6 * FBLOCK;
+          const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
+                       zi = jp[5 * FBLOCK];
+          if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
+          else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
+          else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
+        }
+        ar[5] = mDL * ar[0]; ai[5] = mDL * ai[0];
+        ar[0] = dr[c] - ar[0]; ai[0] = di[c] - ai[0];
+#pragma unroll
+        for (int pp = 0; pp < NT; ++pp) {
+          const double wr = w[c] * ar[pp], wi = w[c] * ai[pp];
+#pragma unroll
+          for (int q = pp; q < NT; ++q) {
+            const int gi_ = gram_index(pp, q);
+            a[gi_] = fma(wr, ar[q], fma(wi, ai[q], a[gi_]));
+          }
+        }
+      }
+      butterfly_level<48, 16>(a, lane);
+      butterfly_level<24, 8>(a, lane);
+      butterfly_level<12, 4>(a, lane);
+      butterfly_level<6, 2>(a, lane);
+      butterfly_level<3, 1>(a, lane);
+      double* r = red + ((warp * FTILE + s) * NGP + lane * 3);
+      r[0] += a[0]; r[1] += a[1]; r[2] += a[2];
+    }
+  }
+  __syncthreads();
+  // cross-warp sum in fixed order; thread t < 96 owns slot (lane = t / 3, j = t % 3)
+  if (threadIdx.x < NGP) {
+    const int gidx = butterfly_slot_index(threadIdx.x / 3, threadIdx.x % 3);
+    if (gidx < NG) {
+      for (int s = 0; s < ns; ++s) {
+        double t = 0.0;
+#pragma unroll
+        for (int wv = 0; wv < FBLOCK / 32; ++wv) t += red[(wv * FTILE + s) * NGP + threadIdx.x];
+        partial[(((size_t)det * gridDim.x + blockIdx.x) * (size_t)B + (size_t)(b0 + s)) * NG + gidx] = t;
+      }
+    }
+  }
+}
+
+// second pass: fixed-order sum over (detector, bin block); scatter to F (symmetric, full) and grad.
+static __global__ void combine_fisher_kernel(const double* __restrict__ partial, const double* __restrict__ consts,
+                                      long long B, int n_slices, int const_stride, double* __restrict__ outF,
+                                      double* __restrict__ out_grad) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= B * NG) return;
+  const long long b = t / NG;
+  const int idx = (int)(t % NG);
+  double sum = 0.0;
+  for (int i = 0; i < n_slices; ++i) sum += partial[((size_t)i * (size_t)B + (size_t)b) * NG + idx];
+  // W_A is 1 with all tangents 0 only for out-of-domain samples (prep_samples_du_kernel)
+  const bool valid = consts[(size_t)b * const_stride + W_A * DUW + 1] != 0.0;
+  if (!valid) sum = CUDART_NAN;
+  int p = 0, rem = idx;
+  while (rem >= NT - p) { rem -= NT - p; ++p; }
+  const int q = p + rem;
+  if (p == 0) {
+    if (q > 0 && out_grad) out_grad[b * NPAR + (q - 1)] = sum;
+  } else {
+    outF[(b * NPAR + (p - 1)) * NPAR + (q - 1)] = sum;
+    outF[(b * NPAR + (q - 1)) * NPAR + (p - 1)] = sum;
+  }
+}
+
+}  // namespace pespace

@@ -1,0 +1,83 @@
+// pespace_host.hpp -- host-side helpers shared by the translation units of libpespace.so
+// (argument checks, detector constants, launch bookkeeping).  Not part of the public ABI.
+#pragma once
+#include "../../include/pespace.h"
+#include "pespace_device.cuh"
+
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+namespace pespace {
+namespace host {
+
+extern std::atomic<long long> g_launches;
+char* cuda_msg();   // thread-local message buffer behind pespace_strerror(PESPACE_ECUDA), 256 bytes
+
+inline int cuda_fail(cudaError_t e) {
+  snprintf(cuda_msg(), 256, "CUDA error: %s", cudaGetErrorString(e));
+  return PESPACE_ECUDA;
+}
+#define CU(x) do { cudaError_t e_ = (x); if (e_ != cudaSuccess) return ::pespace::host::cuda_fail(e_); } while (0)
+#define LAUNCHED() do { ++::pespace::host::g_launches; cudaError_t e_ = cudaGetLastError(); \
+                        if (e_ != cudaSuccess) return ::pespace::host::cuda_fail(e_); } while (0)
+
+inline bool model_ok(const pespace_model* m) {
+  if (!m || !m->det || m->n_det < 1 || m->n_det > PESPACE_MAX_DET) return false;
+  if ((m->mode_mask & 31u) == 0 || (m->mode_mask & ~31u) != 0) return false;
+  for (int i = 0; i < m->n_det; ++i) {
+    const pespace_detector& d = m->det[i];
+    if (d.kind != 0 && d.kind != 1) return false;
+    if (d.tdi_gen != 15 && d.tdi_gen != 20) return false;
+    if (!(d.L_m > 0.0) || !std::isfinite(d.L_m)) return false;
+    if (d.kind == 1 && !(d.period_s > 0.0)) return false;
+  }
+  return true;
+}
+inline bool grid_ok(const pespace_grid* g) {
+  return g && g->N > 0 && g->df > 0.0 && g->f0 > 0.0 && std::isfinite(g->df) && std::isfinite(g->f0);
+}
+
+inline DetC make_det(const pespace_detector& d) {
+  DetC c;
+  std::memset(&c, 0, sizeof c);
+  c.Lbar = d.L_m / kC;
+  c.kind = d.kind; c.gen = d.tdi_gen;
+  c.kappa = d.kappa; c.lambda0 = d.lambda0; c.period_s = d.period_s; c.lon = d.lon; c.lat = d.lat;
+  c.yr_over_p = (d.kind == 1) ? kYear / d.period_s : 0.0;
+  for (int n = 0; n < 3; ++n) {
+    const double ang = 2.0 * kPi * n / 3.0 + (d.kind == 0 ? d.lambda0 : 0.0);
+    c.cn[n] = std::cos(ang); c.sn[n] = std::sin(ang);
+  }
+  // arms a: 2-3, b: 3-1, c: 1-2
+  const int r[3] = {1, 2, 0}, s[3] = {2, 0, 1};
+  for (int l = 0; l < 3; ++l) { c.dcn[l] = c.cn[r[l]] - c.cn[s[l]]; c.dsn[l] = c.sn[r[l]] - c.sn[s[l]]; }
+  return c;
+}
+
+inline PrepArgs make_prep_args(const pespace_model* model) {
+  PrepArgs A;
+  std::memset(&A, 0, sizeof A);
+  A.n_det = model->n_det;
+  A.mode_mask = model->mode_mask;
+  for (int i = 0; i < model->n_det; ++i) A.det[i] = make_det(model->det[i]);
+  return A;
+}
+
+inline unsigned class_mask(unsigned mode_mask) {
+  unsigned m = 0;
+  if (mode_mask & PESPACE_MODE_21) m |= 1u;                       // m = 1
+  if (mode_mask & (PESPACE_MODE_22 | PESPACE_MODE_32)) m |= 2u;   // m = 2
+  if (mode_mask & PESPACE_MODE_33) m |= 4u;                       // m = 3
+  if (mode_mask & PESPACE_MODE_44) m |= 8u;                       // m = 4
+  return m;
+}
+
+inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
+
+// Fisher path (pespace_fisher.cu)
+size_t fisher_workspace_bytes(long long B, long long N, int n_det);
+
+}  // namespace host
+}  // namespace pespace

@@ -204,3 +204,108 @@ def test_full_size_network_sampled_parity(P):
     data, psd = wl.data(oracle_response_fn), wl.psd()
     subset = [0, 1023, 4097, 8191]
     check_loglike(P, wl, data, psd, subset=subset)
+
+
+# ------------------------------------------------------------------ S10: forward-mode derivatives (Eq. 13, 14)
+# Tolerance: the Fisher matrix is a Gram matrix of the tangents d_i h, so an entry is
+# compared on the Cauchy-Schwarz scale of its row and column, |dF_ij| <= 1e-9 sqrt(F_ii F_jj); the gradient
+# <d - h | d_i h> on the scale sqrt(F_ii <d-h|d-h>).  1e-9 is the north-star tolerance of <h|h>.
+TOL_F = 1e-9
+
+
+def check_fisher(P, wl, data, psd, subset=None, with_grad=True):
+    idx = np.arange(wl.B) if subset is None else np.asarray(subset)
+    F, g = P.fisher(dev(wl.params), dev(data) if with_grad else None, dev(psd), wl.grid, wl.model)
+    F = F.cpu().numpy()
+    Fo, go = oracle.fisher(wl.params[idx], data if with_grad else None, psd, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    assert np.all(d > 0)
+    errF = np.abs(F[idx] - Fo) / (d[:, :, None] * d[:, None, :])
+    assert errF.max() <= TOL_F, errF.max()
+    assert np.array_equal(F, F.transpose(0, 2, 1))
+    if with_grad:
+        rr = -2.0 * oracle.loglike(wl.params[idx], data, psd, wl.grid, wl.model)
+        errg = np.abs(g.cpu().numpy()[idx] - go) / (d * np.sqrt(rr)[:, None])
+        assert errg.max() <= TOL_F, errg.max()
+    else:
+        assert g is None
+    return F
+
+
+def test_fisher_config1_full(P):
+    wl = W.config(1)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    # noiseless data = h(sample 0): every other sample has a non-zero residual; sample 0 has d - h = 0 and
+    # its gradient is compared on the scale of the batch
+    F, g = P.fisher(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model)
+    Fo, go = oracle.fisher(wl.params, data, psd, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    assert (np.abs(F.cpu().numpy() - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
+    rr = -2.0 * oracle.loglike(wl.params, data, psd, wl.grid, wl.model)
+    hh = -2.0 * oracle.loglike(wl.params, np.zeros_like(data), psd, wl.grid, wl.model)
+    scale = d * np.sqrt(np.maximum(rr, hh))[:, None]
+    assert (np.abs(g.cpu().numpy() - go) / scale).max() <= TOL_F
+
+
+@pytest.mark.parametrize("idx,B,N", [(2, 11, 5000), (3, 6, 2100), (5, 9, 2300)])
+def test_fisher_reduced_configs(P, idx, B, N):
+    """several chunks (128 bins), several blocks (2048 bins), ragged tails in bins and samples"""
+    wl = W.config(idx, B=B, N=N)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_fisher(P, wl, data, psd)
+    check_fisher(P, wl, data, psd, with_grad=False)
+
+
+@pytest.mark.parametrize("gen", [15, 20])
+def test_fisher_random_sky_spinning(P, gen):
+    rng = np.random.default_rng(5)
+    th = W.draw_prior(9, 4e5, rng)
+    th[:, 2] = rng.uniform(-0.8, 0.8, 9); th[:, 3] = rng.uniform(-0.8, 0.8, 9)
+    model = W.Model(W.MODES_HM, (W.lisa_like(gen), W.taiji_like(gen), W.tianqin_like(gen)))
+    wl = W.Workload("random", W.Grid(1e-4, 3.1e-5, 700), model, th, th[3].copy(), 77)
+    check_fisher(P, wl, wl.data(oracle_response_fn), wl.psd())
+
+
+@pytest.mark.parametrize("mask", [2, 4, 8, 16, 9, 22])
+def test_fisher_individual_modes(P, mask):
+    wl = W.config(3, B=5, N=400)
+    wl = W.Workload("modes", wl.grid, W.Model(mask, wl.model.detectors), wl.params, wl.theta_inj, 5)
+    check_fisher(P, wl, wl.data(oracle_response_fn), wl.psd())
+
+
+def test_fisher_edge_cases_and_determinism(P):
+    wl = W.config(5, B=6, N=300)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    psd2 = psd.copy(); psd2[0, 0, 3] = 0.0; psd2[1, 1, 100] = np.inf; psd2[2, 2, 299] = np.nan
+    th = wl.params.copy(); th[1, 0] = -5.0; th[4, 4] = np.nan
+    F, g = P.fisher(dev(th), dev(data), dev(psd2), wl.grid, wl.model)
+    F2, g2 = P.fisher(dev(th), dev(data), dev(psd2), wl.grid, wl.model)
+    F, g = F.cpu().numpy(), g.cpu().numpy()
+    assert np.array_equal(F, F2.cpu().numpy(), equal_nan=True) and np.array_equal(g, g2.cpu().numpy(), equal_nan=True)
+    assert np.all(np.isnan(F[[1, 4]])) and np.all(np.isnan(g[[1, 4]]))
+    ok = [0, 2, 3, 5]
+    Fo, go = oracle.fisher(th[ok], data, psd2, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    assert (np.abs(F[ok] - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
+
+
+def test_fisher_gradient_is_the_derivative_of_loglike(P):
+    """d lnL / d theta_i from pespace_fisher against a central difference of pespace_loglike (GPU only):
+    ties the two entry points together at a size where the oracle would take minutes."""
+    wl = W.config(3, B=4, N=20000)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    _, g = P.fisher(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model)
+    g = g.cpu().numpy()
+    lik = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    for i, h in [(4, 1e-6), (5, 1e-7), (6, 1e-7), (9, 1e-7)]:      # D_L, iota, phi_c, psi
+        tp, tm = wl.params.copy(), wl.params.copy()
+        tp[:, i] += h; tm[:, i] -= h
+        fd = (lik(dev(tp)).cpu().numpy() - lik(dev(tm)).cpu().numpy()) / (2 * h)
+        assert np.allclose(fd, g[:, i], rtol=2e-5, atol=1e-3 * np.abs(g[:, i]).max()), (i, fd, g[:, i])
+
+
+def test_fisher_full_size_sampled_parity(P):
+    """config 5 at full size (B = 256 x N = 262144, three detectors, five modes), oracle on 4 samples"""
+    wl = W.config(5)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_fisher(P, wl, data, psd, subset=[0, 85, 170, 255])
