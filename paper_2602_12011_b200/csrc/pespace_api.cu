@@ -26,20 +26,35 @@ std::vector<EvPair> g_events;
 std::mutex g_ev_mutex;
 
 // ---- kernel dispatch on (detector kind, mode-class mask); all 15 masks are instantiated
-template <int KIND, unsigned CM>
-void launch_loglike(dim3 g, cudaStream_t st, const double* consts, long long B, const double2* data, const double* psd,
-                    GridC G, const DetC& dc, int n_det, int det, double* partial) {
-  loglike_kernel<KIND, CM><<<g, BLOCK, 0, st>>>(consts, B, data, psd, G, dc, n_det, det, partial);
+// the kernels use 50 KB of dynamic shared memory (trig table + sample tile): opt in once per instantiation
+template <class K>
+cudaError_t opt_in_smem(K kernel, bool& done) {
+  if (done) return cudaSuccess;
+  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kernel_smem_bytes());
+  done = e == cudaSuccess;
+  return e;
 }
 template <int KIND, unsigned CM>
-void launch_response(dim3 g, cudaStream_t st, const double* consts, long long B, const double* freqs, long long N,
-                     const DetC& dc, int n_det, int det, double2* out) {
-  response_kernel<KIND, CM><<<g, BLOCK, 0, st>>>(consts, B, freqs, N, dc, n_det, det, out);
+cudaError_t launch_loglike(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
+                           const double2* data, const double* psd, GridC G, const DetC& dc, int n_det, int det,
+                           double* partial) {
+  static bool configured = false;
+  if (cudaError_t e = opt_in_smem(loglike_kernel<KIND, CM>, configured); e != cudaSuccess) return e;
+  loglike_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, data, psd, G, dc, n_det, det, partial);
+  return cudaSuccess;
 }
-using LoglikeFn = void (*)(dim3, cudaStream_t, const double*, long long, const double2*, const double*, GridC,
-                           const DetC&, int, int, double*);
-using ResponseFn = void (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&, int,
-                            int, double2*);
+template <int KIND, unsigned CM>
+cudaError_t launch_response(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
+                            const double* freqs, long long N, const DetC& dc, int n_det, int det, double2* out) {
+  static bool configured = false;
+  if (cudaError_t e = opt_in_smem(response_kernel<KIND, CM>, configured); e != cudaSuccess) return e;
+  response_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, freqs, N, dc, n_det, det, out);
+  return cudaSuccess;
+}
+using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double2*,
+                                  const double*, GridC, const DetC&, int, int, double*);
+using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
+                                   long long, const DetC&, int, int, double2*);
 #define PESPACE_ROW(F, K) {nullptr, F<K, 1>, F<K, 2>, F<K, 3>, F<K, 4>, F<K, 5>, F<K, 6>, F<K, 7>, F<K, 8>, \
                            F<K, 9>, F<K, 10>, F<K, 11>, F<K, 12>, F<K, 13>, F<K, 14>, F<K, 15>}
 const LoglikeFn kLoglike[2][16] = {PESPACE_ROW(launch_loglike, 0), PESPACE_ROW(launch_loglike, 1)};
@@ -49,7 +64,7 @@ struct Plan {
   int n_det, stride;
   long long nbb;          // bin blocks
   long long ntile;        // sample tiles
-  size_t consts_bytes, partial_bytes;
+  size_t trig_bytes, consts_bytes, partial_bytes;      // workspace: [trig table | sample constants | block partials]
 };
 Plan make_plan(long long B, long long N, int n_det) {
   Plan p;
@@ -57,15 +72,17 @@ Plan make_plan(long long B, long long N, int n_det) {
   p.stride = sample_stride(n_det);
   p.nbb = (N + BLOCK - 1) / BLOCK;
   p.ntile = (B + TILE - 1) / TILE;
+  p.trig_bytes = align_up((size_t)NTAB * sizeof(double2), 256);
   p.consts_bytes = align_up((size_t)B * p.stride * sizeof(double), 256);
   p.partial_bytes = align_up((size_t)n_det * p.nbb * (size_t)B * sizeof(double), 256);
   return p;
 }
 
-int run_prep(const double* d_params, long long B, const pespace_model* model, double* d_consts, cudaStream_t st) {
+int run_prep(const double* d_params, long long B, const pespace_model* model, double* d_consts, double2* d_trig,
+             cudaStream_t st) {
   const PrepArgs A = make_prep_args(model);
   const int th = 128;
-  prep_samples_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
+  prep_samples_kernel<<<(unsigned)((prep_threads(B) + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts, d_trig);
   LAUNCHED();
   return PESPACE_OK;
 }
@@ -116,7 +133,7 @@ size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespac
   if (B <= 0 || !grid_ok(grid) || !model_ok(model)) return 0;
   if (want_fisher) return fisher_workspace_bytes(B, grid->N, model->n_det);
   const Plan p = make_plan(B, grid->N, model->n_det);
-  return p.consts_bytes + p.partial_bytes;
+  return p.trig_bytes + p.consts_bytes + p.partial_bytes;
 }
 
 int pespace_response(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
@@ -124,21 +141,24 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
   if (!d_params || !d_freqs || !d_out_AET || B <= 0 || N <= 0 || !model_ok(model)) return PESPACE_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   const Plan p = make_plan(B, N, model->n_det);
-  double* d_consts = nullptr;
-  CU(cudaMallocAsync((void**)&d_consts, p.consts_bytes, st));
-  int rc = run_prep(d_params, B, model, d_consts, st);
+  char* d_scratch = nullptr;
+  CU(cudaMallocAsync((void**)&d_scratch, p.trig_bytes + p.consts_bytes, st));
+  double2* d_trig = (double2*)d_scratch;
+  double* d_consts = (double*)(d_scratch + p.trig_bytes);
+  int rc = run_prep(d_params, B, model, d_consts, d_trig, st);
   if (rc == PESPACE_OK) {
     const unsigned cm = class_mask(model->mode_mask);
     const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
     for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
       const DetC dc = make_det(model->det[d]);
-      kResponse[dc.kind][cm](grid, st, d_consts, B, d_freqs, N, dc, model->n_det, d, (double2*)d_out_AET);
+      cudaError_t e = kResponse[dc.kind][cm](grid, st, d_consts, d_trig, B, d_freqs, N, dc, model->n_det, d,
+                                             (double2*)d_out_AET);
       ++g_launches;
-      cudaError_t e = cudaGetLastError();
+      if (e == cudaSuccess) e = cudaGetLastError();
       if (e != cudaSuccess) rc = cuda_fail(e);
     }
   }
-  cudaError_t e = cudaFreeAsync(d_consts, st);
+  cudaError_t e = cudaFreeAsync(d_scratch, st);
   if (rc == PESPACE_OK && e != cudaSuccess) rc = cuda_fail(e);
   return rc;
 }
@@ -153,9 +173,10 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
     return PESPACE_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   const Plan p = make_plan(B, grid->N, model->n_det);
-  double* d_consts = (double*)d_workspace;
-  double* d_partial = (double*)((char*)d_workspace + p.consts_bytes);
-  int rc = run_prep(d_params, B, model, d_consts, st);
+  double2* d_trig = (double2*)d_workspace;
+  double* d_consts = (double*)((char*)d_workspace + p.trig_bytes);
+  double* d_partial = (double*)((char*)d_workspace + p.trig_bytes + p.consts_bytes);
+  int rc = run_prep(d_params, B, model, d_consts, d_trig, st);
   if (rc != PESPACE_OK) return rc;
   const unsigned cm = class_mask(model->mode_mask);
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
@@ -168,7 +189,8 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
       CU(cudaEventCreate(&ev.b));
       CU(cudaEventRecord(ev.a, st));
     }
-    kLoglike[dc.kind][cm](g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial);
+    CU(kLoglike[dc.kind][cm](g, st, d_consts, d_trig, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d,
+                             d_partial));
     LAUNCHED();
     if (ev.a) {
       CU(cudaEventRecord(ev.b, st));

@@ -36,6 +36,14 @@ constexpr double kYear = 31558149.763545603;
 constexpr double kEuler = 0.5772156649015329;
 constexpr double kPi = 3.14159265358979323846;
 
+// ---- phase units.  Every phase of the inner loop is carried in units of 1/1024 turn ("pu"): range
+// reduction is then a subtraction of a multiple of 1024, the integer part of a phase indexes a
+// 1024-entry sine/cosine table directly, and no multiplication by 2 pi ever happens per bin.
+constexpr double kTurn = 1024.0;                 // pu per turn
+constexpr double kRadPerPu = 2.0 * kPi / kTurn;  // radians per pu
+constexpr int NTAB = 1024;                       // table entries per turn (one per pu)
+constexpr double kMagic = 6755399441055744.0;    // 1.5 * 2^52: x + kMagic rounds x to an integer (|x| < 2^51)
+
 // ---- per-sample constant block (doubles)
 enum : int {
   W_A = 0,      // (pi Ms)^{1/3}
@@ -76,10 +84,13 @@ struct DetC {
 struct GridC { double f0, df; long long N; };
 
 // ---- per-bin constants (registers)
-struct BinC { double f4, cf, lnf3, fm53, fm83, fm76, sth, cth; };   // f4 = 4 f
+struct BinC { double fT, cf, lnf3, fm53, fm83, fm76, sth, cth; };   // fT = kTurn f
 
 // ---- FP64 helpers written for this kernel (the library sincospi/division carry quadrant,
 // special-value and slow-path logic that the FP64-bound inner loop cannot afford)
+
+// round to nearest integer without FRND/F2I (quarter-rate conversion unit): two full-rate DADDs
+__device__ __forceinline__ double rint_magic(double x) { return (x + kMagic) - kMagic; }
 
 // sin and cos of (pi/2) x, x in QUARTER TURNS, |x| < 2^30.  Octant reduction y = x - rint(x),
 // then near-minimax polynomials in y^2 on |y| <= 1/2 (max abs error 1.2e-16 / 1.8e-16,
@@ -121,9 +132,39 @@ __device__ __forceinline__ double rcp_pos(double x) {
   return fma(r, t, r);
 }
 
+// sin and cos of a phase u in pu (|u| < 2^31) from the 1024-entry table T[j] = (sin, cos)(2 pi j / 1024)
+// in shared memory: j = rint(u) mod 1024 (low word of u + kMagic), y = u - rint(u) in [-1/2, 1/2] pu,
+// i.e. |theta| <= pi/1024, where sin(theta) = y (A1 + A3 y^2) and cos(theta) - 1 = y^2 (B2 + B4 y^2)
+// (Taylor with the theta^5 term economised onto the lower ones: max error 1.4e-16 / 1.2e-18), then
+// the angle-addition formulas.  12 FP64 instructions, no quadrant logic, no conversion instructions.
+constexpr double kHh = 0.5 * kRadPerPu;   // half-width of the reduced interval, radians
+constexpr double kA1 = kRadPerPu * (1.0 - (5.0 / 16.0) * (kHh * kHh * kHh * kHh) / 120.0);
+constexpr double kA3 = kRadPerPu * kRadPerPu * kRadPerPu * (-1.0 / 6.0 + (5.0 / 4.0) * (kHh * kHh) / 120.0);
+constexpr double kB2 = -0.5 * kRadPerPu * kRadPerPu;
+constexpr double kB4 = kRadPerPu * kRadPerPu * kRadPerPu * kRadPerPu / 24.0;
+
+__device__ __forceinline__ void sincos_tab(double u, const double2* __restrict__ tab, double& s_out, double& c_out) {
+  const double t = u + kMagic;
+  const double y = u - (t - kMagic);
+  const double2 T = tab[__double2loint(t) & (NTAB - 1)];
+  const double z = y * y;
+  const double sl = y * fma(kA3, z, kA1);
+  const double cl = z * fma(kB4, z, kB2);
+  s_out = fma(T.y, sl, fma(T.x, cl, T.x));
+  c_out = fma(-T.x, sl, fma(T.y, cl, T.y));
+}
+
+// phase in pu -> sin, cos; TAB selects the table (likelihood / response kernels) or the polynomial
+// (kernels whose shared memory is spoken for)
+template <bool TAB>
+__device__ __forceinline__ void sincos_pu(double u, const double2* __restrict__ tab, double& s_out, double& c_out) {
+  if constexpr (TAB) sincos_tab(u, tab, s_out, c_out);
+  else sincos_qt(u * (4.0 / kTurn), s_out, c_out);
+}
+
 __device__ __forceinline__ BinC make_bin(double f, double Lbar) {
   BinC b;
-  b.f4 = 4.0 * f;
+  b.fT = kTurn * f;
   b.cf = cbrt(f);
   b.lnf3 = log(f) * (1.0 / 3.0);
   const double cf2 = b.cf * b.cf;
@@ -151,11 +192,12 @@ __device__ __forceinline__ void tdi_prefactor(const BinC& b, int gen, double& gr
 
 // ---------------------------------------------------------------------------------------------
 // One mode class (m = MC + 1) of one (sample, bin, detector): adds its X, Y, Z (without the common
-// factor g z f^{-7/6}) to S.  All phases are carried in QUARTER TURNS (the prep kernel scales the
-// polynomial coefficients by 4) so that sincos_qt needs no multiply.
-template <int KIND, int MC, bool FIRST>
+// factor g z f^{-7/6}) to S.  All phases are carried in pu = 1/1024 turn (the prep kernel scales the
+// polynomial coefficients by kTurn) so that the sine/cosine evaluation needs no multiply.
+template <int KIND, int MC, bool FIRST, bool TAB>
 __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
-                                           double va, double La, double ftc4, double (&S)[6]) {
+                                           const double2* __restrict__ tab, double va, double La, double ftc,
+                                           double (&S)[6]) {
   // compile-time class constants: (2/m)^{1/3}, ln(2/m)/3, (m/2)^{8/3}, m/2
   constexpr double CB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
   constexpr double LN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
@@ -177,10 +219,10 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
   Q = fma(Q, v, sc[W_Q3]);
   Q = fma(Q, v, sc[W_Q2]);
   Q = fma(Q, v2, sc[W_Q0]);
-  double psi = ((MC == 1) ? bc.fm53 : S83[MC] * bc.fm53) * P;     // PN phase, quarter turns (up to ~4e5)
-  psi -= 4.0 * rint(0.25 * psi);                                   // mod 4 quarter turns, exact
-  psi += fma(MH[MC], sc[W_PH0], ftc4);                             // + 4 [f t_c - (m/2)(phi_c/pi + 1/8)]
-  const double tau = ((MC == 1) ? bc.fm83 : S83[MC] * bc.fm83) * Q;   // 4 (t_lm - t_c) / yr
+  double psi = ((MC == 1) ? bc.fm53 : S83[MC] * bc.fm53) * P;     // PN phase, pu (up to ~1e8 and beyond)
+  psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);         // mod one turn, exact
+  psi += fma(MH[MC], sc[W_PH0], ftc);                              // + kTurn [f t_c - (m/2)(phi_c/pi + 1/8)]
+  const double tau = ((MC == 1) ? bc.fm83 : S83[MC] * bc.fm83) * Q;   // kTurn (t_lm - t_c) / yr
 
   // ---- amplitude x polarisation content of the class: vp (a + b v^2)
   const double* ka = sc + W_KA + 4 * MC;
@@ -193,7 +235,7 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
   double G1k, G2k, G1u, G2u, G1v, G2v, kR;
   if (KIND == 0) {
     double sa, ca;
-    sincos_qt(sc[D_BASE] + tau, sa, ca);
+    sincos_pu<TAB>(sc[D_BASE] + tau, tab, sa, ca);
     const double c2 = fma(2.0 * ca, ca, -1.0), s2 = 2.0 * sa * ca;
     const double* w = sc + S_K;
     G1k = fma(w[0], c2, fma(w[1], s2, fma(w[2], ca, w[3])));
@@ -207,8 +249,8 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
     kR = fma(sc[S_DX], ca, sc[S_DY] * sa);
   } else {
     double sE, cE, sp, cp;
-    sincos_qt(sc[D_BASE] + tau, sE, cE);
-    sincos_qt(fma(tau, dc.yr_over_p, sc[D_BASE + 1]), sp, cp);
+    sincos_pu<TAB>(sc[D_BASE] + tau, tab, sE, cE);
+    sincos_pu<TAB>(fma(tau, dc.yr_over_p, sc[D_BASE + 1]), tab, sp, cp);
     const double* w = sc + D_BASE + 2;
     G1k = fma(w[0], cp, w[1] * sp); G2k = fma(w[1], cp, -w[0] * sp);
     G1u = fma(w[2], cp, w[3] * sp); G2u = fma(w[3], cp, -w[2] * sp);
@@ -234,14 +276,14 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
     Wi[l] = (CKc * rD) * (uu * vv);
   }
 
-  // ---- S6: h_lm E_n = exp(-i (pi/2) (psi + 4 f k.x_n)) for the three spacecraft
+  // ---- S6: h_lm E_n = exp(-i (2 pi / kTurn) (psi + kTurn f k.x_n)) for the three spacecraft
   double Er[3], Ei[3];
   {
     const double nun[3] = {nu0, nu1, nu2};
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
       double s, c;
-      sincos_qt(fma(bc.f4, fma(dc.Lbar, nun[n], kR), psi), s, c);
+      sincos_pu<TAB>(fma(bc.fT, fma(dc.Lbar, nun[n], kR), psi), tab, s, c);
       Er[n] = c; Ei[n] = s;          // note: Ei holds +sin; the minus sign is carried below
     }
   }
@@ -270,19 +312,19 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
 
 // X, Y, Z of one (sample, bin, detector) summed over the mode classes of CMASK (compile time;
 // bit m-1 set = class m present).  Returns (Re, -Im) pairs in S.
-template <int KIND, unsigned CMASK>
+template <int KIND, unsigned CMASK, bool TAB>
 __device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
-                                         double (&S)[6]) {
+                                         const double2* __restrict__ tab, double (&S)[6]) {
   const double tc = sc[W_TC];
-  // 4 f t_c in quarter turns mod 4, with the rounding error of the product recovered by fma
-  const double p = bc.f4 * tc;
-  const double ftc4 = (p - 4.0 * rint(0.25 * p)) + fma(bc.f4, tc, -p);
+  // kTurn f t_c in pu mod one turn, with the rounding error of the product recovered by fma
+  const double p = bc.fT * tc;
+  const double ftc = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
   const double va = sc[W_A] * bc.cf, La = sc[W_LNA] + bc.lnf3;
   constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
-  if (c0) eval_class<KIND, 0, true>(bc, sc, dc, va, La, ftc4, S);
-  if (c1) eval_class<KIND, 1, !c0>(bc, sc, dc, va, La, ftc4, S);
-  if (c2) eval_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, va, La, ftc4, S);
-  if (c3) eval_class<KIND, 3, !(c0 || c1 || c2)>(bc, sc, dc, va, La, ftc4, S);
+  if (c0) eval_class<KIND, 0, true, TAB>(bc, sc, dc, tab, va, La, ftc, S);
+  if (c1) eval_class<KIND, 1, !c0, TAB>(bc, sc, dc, tab, va, La, ftc, S);
+  if (c2) eval_class<KIND, 2, !(c0 || c1), TAB>(bc, sc, dc, tab, va, La, ftc, S);
+  if (c3) eval_class<KIND, 3, !(c0 || c1 || c2), TAB>(bc, sc, dc, tab, va, La, ftc, S);
 }
 
 // ---------------------------------------------------------------------------------------------
@@ -322,7 +364,7 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   const T Ds = DL * (kGpc / kC);
   const T a = p_cbrt(kPi * Ms);
   put(W_A, a); put(W_LNA, p_log(a)); put(W_TC, tc);
-  put(W_PH0, -4.0 * (phic / kPi + 0.125));              // quarter turns
+  put(W_PH0, -kTurn * (phic / kPi + 0.125));            // pu, for m/2 = 1
   put(W_VALID, T(1.0));
   // TaylorF2 3.5PN coefficients, spin terms per G3
   const double pi2 = kPi * kPi;
@@ -338,10 +380,10 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   const double ph6l = -6848.0 / 21.0;
   const T ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * (eta * eta));
   const T a5 = 1.0 / (a * a * a * a * a);
-  const T cP = 4.0 * 3.0 / (256.0 * kPi * eta) * a5;    // 4 Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
+  const T cP = kTurn * 3.0 / (256.0 * kPi * eta) * a5;  // kTurn Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
   put(W_P0, cP); put(W_P2, cP * ph2); put(W_P3, cP * ph3); put(W_P4, cP * ph4);
   put(W_P5, cP * ph5a); put(W_P5L, cP * 3.0 * ph5a); put(W_P6, cP * ph6a); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
-  const T cQ = cP / (3.0 * kYear);                       // 4 (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
+  const T cQ = cP / (3.0 * kYear);                       // kTurn (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
   put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
   put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l)); put(W_Q6L, cQ * ph6l); put(W_Q7, 2.0 * cQ * ph7);
   // amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
@@ -389,13 +431,13 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
     double a0 = tcv / kYear;
     a0 -= rint(a0);
     if (D.kind == 0) {
-      put(base, T(4.0 * (a0 + D.kappa / (2.0 * kPi))));
+      put(base, T(kTurn * (a0 + D.kappa / (2.0 * kPi))));
       for (int i = 1; i < D_STRIDE; ++i) put(base + i, T(0.0));
     } else {
-      put(base, T(4.0 * a0));
+      put(base, T(kTurn * a0));
       double p0 = tcv / D.period_s;
       p0 -= rint(p0);
-      put(base + 1, T(4.0 * (p0 + D.lambda0 / (2.0 * kPi))));
+      put(base + 1, T(kTurn * (p0 + D.lambda0 / (2.0 * kPi))));
       const double cL = cos(D.lon), sL = sin(D.lon), cB = cos(D.lat), sB = sin(D.lat);
       const double nh[3] = {cB * cL, cB * sL, sB};
       const double e1[3] = {-sL, cL, 0.0};
@@ -410,9 +452,21 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   }
 }
 
+// sine/cosine table of sincos_tab: trig[j] = (sin, cos)(2 pi j / NTAB), |error| <= 1 ulp (sincospi)
+__device__ __forceinline__ void fill_trig_entry(double2* __restrict__ trig, long long j) {
+  if (trig && j < NTAB) {
+    double s, c;
+    sincospi((double)j * (2.0 / NTAB), &s, &c);
+    trig[j] = make_double2(s, c);
+  }
+}
+__host__ __device__ constexpr long long prep_threads(long long B) { return B > NTAB ? B : (long long)NTAB; }
+
+// grid covers prep_threads(B) threads: thread j < NTAB also writes table entry j (trig may be null)
 static __global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
-                                    double* __restrict__ consts) {
+                                    double* __restrict__ consts, double2* __restrict__ trig) {
   const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  fill_trig_entry(trig, b);
   if (b >= B) return;
   const double* thp = params + b * NPAR;
   const int stride = sample_stride(A.n_det);
@@ -430,6 +484,15 @@ static __global__ void prep_samples_kernel(const double* __restrict__ params, lo
 // ---------------------------------------------------------------------------------------------
 constexpr int BLOCK = 256;      // threads = bins per block
 constexpr int TILE = 64;        // samples staged in shared memory per block
+
+// dynamic shared memory of the likelihood / response kernels: [trig table | sample constants | warp partials]
+extern __shared__ __align__(16) unsigned char pespace_dyn_smem[];
+constexpr size_t kernel_smem_bytes() {
+  return sizeof(double) * ((size_t)2 * NTAB + (size_t)TILE * SMEM_STRIDE + (size_t)(BLOCK / 32) * TILE);
+}
+__device__ __forceinline__ void stage_trig(double2* tab, const double2* __restrict__ trig) {
+  for (int i = threadIdx.x; i < NTAB; i += blockDim.x) tab[i] = trig[i];
+}
 
 __device__ __forceinline__ void stage_tile(double* smem, const double* __restrict__ consts, long long b0,
                                            long long B, int n_det, int det) {
@@ -449,12 +512,14 @@ constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 
 
 template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? 3 : 2)
-loglike_kernel(const double* __restrict__ consts, long long B, const double2* __restrict__ data,
-               const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
+loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
+               const double2* __restrict__ data, const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
                double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
-  __shared__ double smem[TILE * SMEM_STRIDE];
-  __shared__ double red[BLOCK / 32][TILE];
+  double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
+  double* smem = reinterpret_cast<double*>(tab + NTAB);
+  double (*red)[TILE] = reinterpret_cast<double (*)[TILE]>(smem + TILE * SMEM_STRIDE);
   const long long b0 = (long long)blockIdx.y * TILE;
+  stage_trig(tab, trig);
   stage_tile(smem, consts, b0, B, n_det, det);
 
   const long long k = (long long)blockIdx.x * BLOCK + threadIdx.x;
@@ -484,7 +549,7 @@ loglike_kernel(const double* __restrict__ consts, long long B, const double2* __
   const int ns = (int)min((long long)TILE, B - b0);
   for (int s = 0; s < ns; ++s) {
     double S[6];
-    eval_xyz<KIND, CMASK>(bc, smem + s * SMEM_STRIDE, dc, S);
+    eval_xyz<KIND, CMASK, true>(bc, smem + s * SMEM_STRIDE, dc, tab, S);
     const double Ar = S[4] - S[0], Ai = S[5] - S[1];                         // Z - X
     const double Er_ = S[0] - 2.0 * S[2] + S[4], Ei_ = S[1] - 2.0 * S[3] + S[5];   // X - 2Y + Z
     const double Tr = S[0] + S[2] + S[4], Ti = S[1] + S[3] + S[5];           // X + Y + Z
@@ -520,10 +585,13 @@ static __global__ void combine_kernel(const double* __restrict__ partial, const 
 // pespace_response: same body, writes A, E, T (with the common factor restored).
 template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK)
-response_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ freqs, long long N,
-                DetC dc, int n_det, int det, double2* __restrict__ out /* [B][n_det][3][N] */) {
-  __shared__ double smem[TILE * SMEM_STRIDE];
+response_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
+                const double* __restrict__ freqs, long long N, DetC dc, int n_det, int det,
+                double2* __restrict__ out /* [B][n_det][3][N] */) {
+  double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
+  double* smem = reinterpret_cast<double*>(tab + NTAB);
   const long long b0 = (long long)blockIdx.y * TILE;
+  stage_trig(tab, trig);
   stage_tile(smem, consts, b0, B, n_det, det);
   const long long k = (long long)blockIdx.x * BLOCK + threadIdx.x;
   const bool live = k < N;
@@ -538,7 +606,7 @@ response_kernel(const double* __restrict__ consts, long long B, const double* __
   for (int s = 0; s < ns; ++s) {
     const double* sc = smem + s * SMEM_STRIDE;
     double S[6];
-    eval_xyz<KIND, CMASK>(bc, sc, dc, S);
+    eval_xyz<KIND, CMASK, true>(bc, sc, dc, tab, S);
     double ch[6];                                      // S holds (Re, -Im)
     ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
     ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;

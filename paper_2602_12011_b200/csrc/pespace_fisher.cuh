@@ -32,7 +32,6 @@ constexpr int NG = 78;        // upper triangle of the 12 x 12 Gram matrix
 constexpr int NGP = 96;       // padded to 3 x 32 for the butterfly
 constexpr int DUW = 8;        // doubles per constant: value + tangents (M, q, chi1, chi2, iota, lambda, beta)
 constexpr int FS_STRIDE = SMEM_STRIDE * DUW;   // one sample, one detector, in shared memory
-constexpr double kHalfPi = 1.57079632679489661923;
 
 __host__ __device__ constexpr int fisher_const_stride(int n_det) { return sample_stride(n_det) * DUW; }
 constexpr size_t fisher_smem_bytes() {
@@ -72,10 +71,10 @@ __device__ __forceinline__ Du<3> ang(double v, double d0) {
 
 // phase-like scalars of one class handed from stage A to stage C
 struct ClassScal {
-  double psi;        // phase, quarter turns (reduced)
-  double tau;        // 4 (t_lm - t_c) / yr
-  double dpsi[4];    // (pi/2) d psi / d (M, q, chi1, chi2): radians per unit parameter
-  double dtau[4];    // (pi/2) d tau / d (M, q, chi1, chi2): radians of orbit angle per unit parameter
+  double psi;        // phase, pu (reduced)
+  double tau;        // kTurn (t_lm - t_c) / yr
+  double dpsi[4];    // (2 pi/kTurn) d psi / d (M, q, chi1, chi2): radians per unit parameter
+  double dtau[4];    // (2 pi/kTurn) d tau / d (M, q, chi1, chi2): radians of orbit angle per unit parameter
   Du<3> CKp, CKc;    // amplitudes, tangents (M, q, iota)
 };
 
@@ -105,13 +104,13 @@ __device__ __forceinline__ void fisher_stage_a(const BinC& bc, const double* __r
   Q = dfma(Q, v2, c4(sc, W_Q0));
   const double sp = S83[MC] * bc.fm53, sq = S83[MC] * bc.fm83;
   double psi = sp * P.v;
-  psi -= 4.0 * rint(0.25 * psi);
+  psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);
   o.psi = psi + fma(MH[MC], cv(sc, W_PH0), ftc4);
   o.tau = sq * Q.v;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
-    o.dpsi[i] = (kHalfPi * sp) * P.d[i];
-    o.dtau[i] = (kHalfPi * sq) * Q.d[i];
+    o.dpsi[i] = (kRadPerPu * sp) * P.d[i];
+    o.dtau[i] = (kRadPerPu * sq) * Q.d[i];
   }
   // amplitude x polarisation content, tangents (M, q, iota); v carries M only
   Du<3> va(0.0);
@@ -154,7 +153,7 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
   G G1k, G2k, G1u, G2u, G1v, G2v, kR;
   if (KIND == 0) {
     double sa, ca;
-    sincos_qt(cv(sc, D_BASE) + cs.tau, sa, ca);
+    sincos_pu<false>(cv(sc, D_BASE) + cs.tau, nullptr, sa, ca);
     const double c2v = fma(2.0 * ca, ca, -1.0), s2v = 2.0 * sa * ca;
     const G sA = ang(sa, ca), cA = ang(ca, -sa), s2 = ang(s2v, 2.0 * c2v), c2 = ang(c2v, -2.0 * s2v);
     auto rot = [&](int off, G& g1, G& g2) {
@@ -168,8 +167,8 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
     kR = dfma(cg(sc, S_DX), cA, cg(sc, S_DY) * sA);
   } else {
     double sE, cE, sp, cp;
-    sincos_qt(cv(sc, D_BASE) + cs.tau, sE, cE);
-    sincos_qt(fma(cs.tau, dc.yr_over_p, cv(sc, D_BASE + 1)), sp, cp);
+    sincos_pu<false>(cv(sc, D_BASE) + cs.tau, nullptr, sE, cE);
+    sincos_pu<false>(fma(cs.tau, dc.yr_over_p, cv(sc, D_BASE + 1)), nullptr, sp, cp);
     const G sEg = ang(sE, cE), cEg = ang(cE, -sE);
     const G spg = ang(sp, dc.yr_over_p * cp), cpg = ang(cp, -dc.yr_over_p * sp);
     auto rot = [&](int off, G& g1, G& g2) {
@@ -205,15 +204,15 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
     Wc[l] = rD * (uu * vv);
   }
 
-  // ---- S6: E_n = exp(+i (pi/2) (psi + 4 f k.x_n)) (conjugate representation)
+  // ---- S6: E_n = exp(+i (2 pi/kTurn) (psi + kTurn f k.x_n)) (conjugate representation)
   G Er[3], Ei[3];
 #pragma unroll
   for (int n = 0; n < 3; ++n) {
     const G ph = dfma(dc.Lbar, nu[n], kR);
     double s, c;
-    sincos_qt(fma(bc.f4, ph.v, cs.psi), s, c);
+    sincos_pu<false>(fma(bc.fT, ph.v, cs.psi), nullptr, s, c);
     Er[n].v = c; Ei[n].v = s;
-    const double sc4 = kHalfPi * bc.f4;
+    const double sc4 = kRadPerPu * bc.fT;
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
       const double t = sc4 * ph.d[i];
@@ -256,7 +255,7 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
       jadd<FIRST>(J, 1 + i, comp, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0]), fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0]));
     // iota: amplitudes only
     jadd<FIRST>(J, 6, comp, fma(cs.CKp.d[2], Hpr.v, -cs.CKc.d[2] * Hci.v), fma(cs.CKp.d[2], Hpi.v, cs.CKc.d[2] * Hcr.v));
-    // phi_c: d psi = -(4/pi) (m/2) quarter turns -> -m i h
+    // phi_c: d psi = -m d phi_c (radians) -> -m i h
     jadd<FIRST>(J, 7, comp, MM[MC] * hi, -MM[MC] * hr);
     // lambda, beta
     jadd<FIRST>(J, 8, comp, Tr[1], Ti[1]);
@@ -264,7 +263,7 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
     // polarisation angle: d Hp = 4 Hc, d Hc = -Hp
     jadd<FIRST>(J, 10, comp, fma(4.0 * kp, Hcr.v, kc * Hpi.v), fma(4.0 * kp, Hci.v, -kc * Hpr.v));
     // t_c: phase 2 pi f, orbit angle 2 pi / yr
-    const double wp = kHalfPi * bc.f4, wt = kHalfPi * 4.0 / kYear;
+    const double wp = kRadPerPu * bc.fT, wt = kRadPerPu * kTurn / kYear;
     jadd<FIRST>(J, 11, comp, fma(-wp, hi, wt * Tr[0]), fma(wp, hr, wt * Ti[0]));
   };
   // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2); same terms as eval_class
@@ -378,8 +377,8 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
     for (int s = 0; s < ns; ++s) {
       const double* sc = csm + s * FS_STRIDE;
       const double tc = cv(sc, W_TC);
-      const double p = bc.f4 * tc;
-      const double ftc4 = (p - 4.0 * rint(0.25 * p)) + fma(bc.f4, tc, -p);
+      const double p = bc.fT * tc;
+      const double ftc4 = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
       if (c0) fisher_class<KIND, 0, true>(bc, sc, dc, ftc4, J);
       if (c1) fisher_class<KIND, 1, !c0>(bc, sc, dc, ftc4, J);
       if (c2) fisher_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, ftc4, J);
