@@ -1,5 +1,5 @@
 // pespace_api.cu -- the C ABI of include/pespace.h: argument checks, workspace carving, launches.
-#include "pespace_host.hpp"
+#include "pespace_launch.hpp"
 
 #include <mutex>
 #include <vector>
@@ -24,41 +24,6 @@ struct EvPair { cudaEvent_t a, b; };
 bool g_profile = false;
 std::vector<EvPair> g_events;
 std::mutex g_ev_mutex;
-
-// ---- kernel dispatch on (detector kind, mode-class mask); all 15 masks are instantiated
-// the kernels use 50 KB of dynamic shared memory (trig table + sample tile): opt in once per instantiation
-template <class K>
-cudaError_t opt_in_smem(K kernel, bool& done) {
-  if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kernel_smem_bytes());
-  done = e == cudaSuccess;
-  return e;
-}
-template <int KIND, unsigned CM>
-cudaError_t launch_loglike(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
-                           const double2* data, const double* psd, GridC G, const DetC& dc, int n_det, int det,
-                           double* partial) {
-  static bool configured = false;
-  if (cudaError_t e = opt_in_smem(loglike_kernel<KIND, CM>, configured); e != cudaSuccess) return e;
-  loglike_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, data, psd, G, dc, n_det, det, partial);
-  return cudaSuccess;
-}
-template <int KIND, unsigned CM>
-cudaError_t launch_response(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
-                            const double* freqs, long long N, const DetC& dc, int n_det, int det, double2* out) {
-  static bool configured = false;
-  if (cudaError_t e = opt_in_smem(response_kernel<KIND, CM>, configured); e != cudaSuccess) return e;
-  response_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, freqs, N, dc, n_det, det, out);
-  return cudaSuccess;
-}
-using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double2*,
-                                  const double*, GridC, const DetC&, int, int, double*);
-using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
-                                   long long, const DetC&, int, int, double2*);
-#define PESPACE_ROW(F, K) {nullptr, F<K, 1>, F<K, 2>, F<K, 3>, F<K, 4>, F<K, 5>, F<K, 6>, F<K, 7>, F<K, 8>, \
-                           F<K, 9>, F<K, 10>, F<K, 11>, F<K, 12>, F<K, 13>, F<K, 14>, F<K, 15>}
-const LoglikeFn kLoglike[2][16] = {PESPACE_ROW(launch_loglike, 0), PESPACE_ROW(launch_loglike, 1)};
-const ResponseFn kResponse[2][16] = {PESPACE_ROW(launch_response, 0), PESPACE_ROW(launch_response, 1)};
 
 struct Plan {
   int n_det, stride;
@@ -151,7 +116,7 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
     const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
     for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
       const DetC dc = make_det(model->det[d]);
-      cudaError_t e = kResponse[dc.kind][cm](grid, st, d_consts, d_trig, B, d_freqs, N, dc, model->n_det, d,
+      cudaError_t e = response_launcher(dc.kind, cm)(grid, st, d_consts, d_trig, B, d_freqs, N, dc, model->n_det, d,
                                              (double2*)d_out_AET);
       ++g_launches;
       if (e == cudaSuccess) e = cudaGetLastError();
@@ -189,7 +154,7 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
       CU(cudaEventCreate(&ev.b));
       CU(cudaEventRecord(ev.a, st));
     }
-    CU(kLoglike[dc.kind][cm](g, st, d_consts, d_trig, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d,
+    CU(loglike_launcher(dc.kind, cm)(g, st, d_consts, d_trig, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d,
                              d_partial));
     LAUNCHED();
     if (ev.a) {

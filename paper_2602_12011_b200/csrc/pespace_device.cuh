@@ -54,16 +54,21 @@ enum : int {
   W_Q0, W_Q2, W_Q3, W_Q4, W_Q5, W_Q6, W_Q6L, W_Q7,          // (t_lm - t_c)/yr polynomial
   W_VALID,      // 1.0 valid, 0.0 out of domain
   W_KA,         // [4 mode classes][a+, b+, ax, bx]
-  S_K = W_KA + 16,  // k/(4 sqrt3): x, y, -z/2*..., -3x, -3y   (5 each; kind 0 geometry)
+  W_MDL = W_KA + 16,   // -1 / D_L (Fisher path)
+  W_PAD,
+  D_BASE,           // per detector, D_STRIDE doubles
+  // offsets of the staged (one detector) view; the block of detector d starts at D_BASE + d D_STRIDE
+  S_K = D_BASE + 2,    // kind 0: k/(4 sqrt3): x, y, -z/2*..., -3x, -3y  (5 each), in the frame rotated by lambda0
   S_U = S_K + 5,
   S_V = S_U + 5,
-  S_DX = S_V + 5,   // (AU/c) k_x, (AU/c) k_y: Doppler phase of the guiding centre
+  S_DX = S_V + 5,      // (AU/c) k_x, (AU/c) k_y: Doppler phase of the guiding centre (kind 0: rotated frame)
   S_DY,
-  S_PAD,
-  D_BASE,           // per detector, D_STRIDE doubles
 };
-constexpr int D_STRIDE = 8;
-// kind 0: [0] alpha0 (turns).  kind 1: [0] alphaE0, [1] phi0 (turns), [2..7] (w.e1, w.e2)/sqrt3 for w = k, u', v'
+constexpr int D_STRIDE = 24;
+// kind 0: [0] alpha0 - lambda0 (pu), [2..16] S_K, S_U, S_V, [17..18] S_DX, S_DY.  The constellation with rotation
+//         phase lambda0 is the lambda0 = 0 constellation at orbital phase alpha - lambda0, rotated about z by lambda0:
+//         the rotation is applied to k, u', v' here, so the kernels only ever see spacecraft at 0, 120, 240 degrees.
+// kind 1: [0] alphaE0, [1] phi0 (pu), [2..7] (w.e1, w.e2)/sqrt3 for w = k, u', v', [17..18] S_DX, S_DY
 constexpr int SMEM_STRIDE = D_BASE + D_STRIDE;   // one sample, one detector
 static_assert(SMEM_STRIDE == 64, "sample block is 64 doubles");
 __host__ __device__ constexpr int sample_stride(int n_det) { return D_BASE + D_STRIDE * n_det; }
@@ -74,8 +79,6 @@ __device__ constexpr double kM76[4] = {0.44544935907016965237, 1.0, 1.6048697909
 // ---- per-detector constants (kernel parameter)
 struct DetC {
   double Lbar;        // L / c  (s)
-  double cn[3], sn[3];   // kind 0: cos/sin beta_n; kind 1: cos/sin 2 pi (n-1)/3
-  double dcn[3], dsn[3]; // arm differences, arms a: 2-3, b: 3-1, c: 1-2
   double yr_over_p;   // kind 1
   double kappa, lambda0, period_s, lon, lat;   // raw, for the prep kernel
   int kind, gen;
@@ -257,18 +260,22 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
     G1v = fma(w[4], cp, w[5] * sp); G2v = fma(w[5], cp, -w[4] * sp);
     kR = fma(sc[S_DX], cE, sc[S_DY] * sE);
   }
-  // k.delta_n / L for the three spacecraft, k.n_l for the arms a: 2-3, b: 3-1, c: 1-2
-  const double nu0 = fma(dc.cn[0], G1k, dc.sn[0] * G2k);
-  const double nu1 = fma(dc.cn[1], G1k, dc.sn[1] * G2k);
-  const double nu2 = fma(dc.cn[2], G1k, dc.sn[2] * G2k);
-  const double ka_ = nu1 - nu2, kb_ = nu2 - nu0, kc_ = nu0 - nu1;   // k.n_23, k.n_31, k.n_12
+  // Spacecraft n sits at angle 2 pi (n-1)/3 (cos = 1, -1/2, -1/2; sin = 0, r, -r with r = sqrt3/2), so
+  // w.delta_n / L = (G1, -G1/2 + r G2, -G1/2 - r G2) and along the arms a: 2-3, b: 3-1, c: 1-2
+  // w.n_l = (2 r G2, -3/2 G1 - r G2, 3/2 G1 - r G2): literal coefficients, no per-detector constants.
+  constexpr double R3H = 0.86602540378443864676;
+  const double tk = R3H * G2k;
+  const double nu0 = G1k, nu1 = fma(-0.5, G1k, tk), nu2 = fma(-0.5, G1k, -tk);     // k.delta_n / L
+  const double ka_ = tk + tk, kb_ = fma(-1.5, G1k, -tk), kc_ = fma(1.5, G1k, -tk);  // k.n_23, k.n_31, k.n_12
+  const double tu = R3H * G2u, tv = R3H * G2v;
+  const double ul[3] = {tu + tu, fma(-1.5, G1u, -tu), fma(1.5, G1u, -tu)};
+  const double vl[3] = {tv + tv, fma(-1.5, G1v, -tv), fma(1.5, G1v, -tv)};
 
   // ---- S5: W_l = amplitude * (n_l.P.n_l) / (1 - (k.n_l)^2), with 1-(k.n)^2 = (u'.n)^2 + (v'.n)^2
   double Wr[3], Wi[3];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
-    const double uu = fma(dc.dcn[l], G1u, dc.dsn[l] * G2u);
-    const double vv = fma(dc.dcn[l], G1v, dc.dsn[l] * G2v);
+    const double uu = ul[l], vv = vl[l];
     const double v2_ = vv * vv;
     const double D = fma(uu, uu, v2_);
     const double rD = (D > 0.0) ? rcp_pos(D) : 0.0;
@@ -417,23 +424,28 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   for (int i = 0; i < 3; ++i) { up[i] = cp * u[i] + sp * v[i]; vp[i] = cp * v[i] - sp * u[i]; }
   const double r43 = 1.0 / (4.0 * sqrt(3.0));
   const T* W3[3] = {k, up, vp};
-  const int off[3] = {S_K, S_U, S_V};
-  for (int j = 0; j < 3; ++j) {
-    const T* w = W3[j];
-    put(off[j] + 0, w[0] * r43); put(off[j] + 1, w[1] * r43); put(off[j] + 2, -0.5 * w[2]);
-    put(off[j] + 3, -3.0 * r43 * w[0]); put(off[j] + 4, -3.0 * r43 * w[1]);
-  }
-  put(S_DX, (kAU / kC) * k[0]); put(S_DY, (kAU / kC) * k[1]); put(S_PAD, T(0.0));
+  const int off[3] = {S_K - D_BASE, S_U - D_BASE, S_V - D_BASE};
+  put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
   const double tcv = p_val(tc);
   for (int dI = 0; dI < A.n_det; ++dI) {
     const DetC& D = A.det[dI];
     const int base = D_BASE + D_STRIDE * dI;
+    for (int i = 0; i < D_STRIDE; ++i) put(base + i, T(0.0));
     double a0 = tcv / kYear;
     a0 -= rint(a0);
     if (D.kind == 0) {
-      put(base, T(kTurn * (a0 + D.kappa / (2.0 * kPi))));
-      for (int i = 1; i < D_STRIDE; ++i) put(base + i, T(0.0));
+      // orbital phase and sky basis in the frame rotated about z by lambda0 (see the layout note above)
+      put(base, T(kTurn * (a0 + (D.kappa - D.lambda0) / (2.0 * kPi))));
+      const double cL0 = cos(D.lambda0), sL0 = sin(D.lambda0);
+      for (int j = 0; j < 3; ++j) {
+        const T* w = W3[j];
+        const T wx = cL0 * w[0] + sL0 * w[1], wy = cL0 * w[1] - sL0 * w[0];
+        put(base + off[j] + 0, wx * r43); put(base + off[j] + 1, wy * r43); put(base + off[j] + 2, -0.5 * w[2]);
+        put(base + off[j] + 3, -3.0 * r43 * wx); put(base + off[j] + 4, -3.0 * r43 * wy);
+        if (j == 0) { put(base + (S_DX - D_BASE), (kAU / kC) * wx); put(base + (S_DY - D_BASE), (kAU / kC) * wy); }
+      }
     } else {
+      put(base + (S_DX - D_BASE), (kAU / kC) * k[0]); put(base + (S_DY - D_BASE), (kAU / kC) * k[1]);
       put(base, T(kTurn * a0));
       double p0 = tcv / D.period_s;
       p0 -= rint(p0);

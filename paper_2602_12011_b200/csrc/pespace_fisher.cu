@@ -1,30 +1,11 @@
 // pespace_fisher.cu -- pespace_fisher of include/pespace.h: forward-mode derivatives (S10).
-#include "pespace_host.hpp"
+#include "pespace_launch.hpp"
 #include "pespace_fisher.cuh"
 
 using namespace pespace;
 using namespace pespace::host;
 
 namespace {
-
-template <int KIND, unsigned CM>
-cudaError_t launch_fisher(dim3 g, cudaStream_t st, const double* consts, long long B, const double2* data,
-                          const double* psd, GridC G, const DetC& dc, int n_det, int det, double* partial) {
-  static bool configured = false;        // per instantiation; the attribute is per function and idempotent
-  if (!configured) {
-    cudaError_t e = cudaFuncSetAttribute(fisher_kernel<KIND, CM>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                         (int)fisher_smem_bytes());
-    if (e != cudaSuccess) return e;
-    configured = true;
-  }
-  fisher_kernel<KIND, CM><<<g, FBLOCK, fisher_smem_bytes(), st>>>(consts, B, data, psd, G, dc, n_det, det, partial);
-  return cudaSuccess;
-}
-using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double2*, const double*, GridC,
-                                 const DetC&, int, int, double*);
-#define PESPACE_ROW(F, K) {nullptr, F<K, 1>, F<K, 2>, F<K, 3>, F<K, 4>, F<K, 5>, F<K, 6>, F<K, 7>, F<K, 8>, \
-                           F<K, 9>, F<K, 10>, F<K, 11>, F<K, 12>, F<K, 13>, F<K, 14>, F<K, 15>}
-const FisherFn kFisher[2][16] = {PESPACE_ROW(launch_fisher, 0), PESPACE_ROW(launch_fisher, 1)};
 
 struct FisherPlan {
   long long nbx, ntile;
@@ -72,7 +53,7 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
   const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
-    CU(kFisher[dc.kind][cm](g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial));
+    CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial));
     LAUNCHED();
   }
   const long long nt = (long long)B * NG;

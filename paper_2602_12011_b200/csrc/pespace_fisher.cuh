@@ -181,18 +181,22 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
     rot(D_BASE + 6, G1v, G2v);
     kR = dfma(cg(sc, S_DX), cEg, cg(sc, S_DY) * sEg);
   }
+  // spacecraft at 0, 120, 240 degrees (lambda0 is absorbed by the per-sample constants): same literal
+  // coefficients as eval_class
+  constexpr double R3H = 0.86602540378443864676;
+  const G tk = R3H * G2k, tu = R3H * G2u, tv = R3H * G2v;
   G nu[3];
-#pragma unroll
-  for (int n = 0; n < 3; ++n) nu[n] = dfma(dc.cn[n], G1k, dc.sn[n] * G2k);
+  nu[0] = G1k; nu[1] = dfma(-0.5, G1k, tk); nu[2] = dfma(-0.5, G1k, -tk);
   G kap[3];                                   // k.n_23, k.n_31, k.n_12
-  kap[0] = nu[1] - nu[2]; kap[1] = nu[2] - nu[0]; kap[2] = nu[0] - nu[1];
+  kap[0] = tk + tk; kap[1] = dfma(-1.5, G1k, -tk); kap[2] = dfma(1.5, G1k, -tk);
+  const G ul[3] = {tu + tu, dfma(-1.5, G1u, -tu), dfma(1.5, G1u, -tu)};
+  const G vl[3] = {tv + tv, dfma(-1.5, G1v, -tv), dfma(1.5, G1v, -tv)};
 
   // ---- S5: real arm weights xi_+/D and (n.u')(n.v')/D
   G Wp[3], Wc[3];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
-    const G uu = dfma(dc.dcn[l], G1u, dc.dsn[l] * G2u);
-    const G vv = dfma(dc.dcn[l], G1v, dc.dsn[l] * G2v);
+    const G uu = ul[l], vv = vl[l];
     const G v2_ = vv * vv;
     const G D = dfma(uu, uu, v2_);
     G rD;
@@ -297,7 +301,6 @@ static __global__ void prep_samples_du_kernel(const double* __restrict__ params,
     p[0] = val.v;
     for (int t = 0; t < 7; ++t) p[1 + t] = val.d[t];
   });
-  o[S_PAD * DUW] = -1.0 / thp[4];        // d h / d D_L = -h / D_L
 }
 
 __device__ __forceinline__ void stage_tile_du(double* smem, const double* __restrict__ consts, long long b0,
@@ -384,7 +387,7 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
       if (c2) fisher_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, ftc4, J);
       if (c3) fisher_class<KIND, 3, !(c0 || c1 || c2)>(bc, sc, dc, ftc4, J);
       // Gram matrix of a_0 = d - h, a_p = d_p h (p = 1..11) over the channels A, E, T
-      const double mDL = cv(sc, S_PAD);
+      const double mDL = cv(sc, W_MDL);      // d h / d D_L = -h / D_L
       double a[NGP];
 #pragma unroll
       for (int i = 0; i < NGP; ++i) a[i] = 0.0;

@@ -46,13 +46,6 @@ inline DetC make_det(const pespace_detector& d) {
   c.kind = d.kind; c.gen = d.tdi_gen;
   c.kappa = d.kappa; c.lambda0 = d.lambda0; c.period_s = d.period_s; c.lon = d.lon; c.lat = d.lat;
   c.yr_over_p = (d.kind == 1) ? kYear / d.period_s : 0.0;
-  for (int n = 0; n < 3; ++n) {
-    const double ang = 2.0 * kPi * n / 3.0 + (d.kind == 0 ? d.lambda0 : 0.0);
-    c.cn[n] = std::cos(ang); c.sn[n] = std::sin(ang);
-  }
-  // arms a: 2-3, b: 3-1, c: 1-2
-  const int r[3] = {1, 2, 0}, s[3] = {2, 0, 1};
-  for (int l = 0; l < 3; ++l) { c.dcn[l] = c.cn[r[l]] - c.cn[s[l]]; c.dsn[l] = c.sn[r[l]] - c.sn[s[l]]; }
   return c;
 }
 

@@ -108,6 +108,22 @@ def test_random_sky_all_detectors_both_generations(P, gen):
     check_response(P, th, grid.freqs()[::5], model)
 
 
+def test_nonzero_constellation_phases(P):
+    """lambda0 != 0 (kind 0: constellation rotation phase, absorbed into the per-sample constants by a frame
+    rotation; kind 1: orbital phase phi0), two kind-0 detectors with DIFFERENT lambda0 in one model."""
+    import dataclasses
+    rng = np.random.default_rng(23)
+    th = W.draw_prior(7, 4e5, rng)
+    dets = (dataclasses.replace(W.lisa_like(), lambda0=0.7), dataclasses.replace(W.taiji_like(15), lambda0=-2.1),
+            dataclasses.replace(W.tianqin_like(), lambda0=1.1))
+    model = W.Model(W.MODES_HM, dets)
+    wl = W.Workload("phases", W.Grid(1e-4, 2.9e-5, 600), model, th, th[2].copy(), 78)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_response(P, th, wl.grid.freqs()[::3], model)
+    check_loglike(P, wl, data, psd)
+    check_fisher(P, wl, data, psd)
+
+
 @pytest.mark.parametrize("mask", [1, 2, 4, 8, 16, 9, 22])
 def test_individual_modes(P, mask):
     wl = W.config(3, B=9, N=600)
