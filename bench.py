@@ -47,17 +47,21 @@ SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # They equal the operation list of the reduced formulas in DESIGN.md ("Algorithmic work") to <1 %; the
 # kernel has no redundant evaluation, so executed = algorithmic.  flop = 2*DFMA + DMUL + DADD.
 FP64_OPS_PER_UNIT = {
-    # (detector kind, mode-class mask): per (sample, bin, detector)
-    (0, 2): {"dfma": 169.17, "dmul": 59.88, "dadd": 35.27},      # kind 0, (2,2) only      -- config 2
-    (0, 15): {"dfma": 661.17, "dmul": 215.88, "dadd": 68.27},    # kind 0, five modes      -- configs 3, 4
-    (1, 15): None,                                               # kind 1, five modes: measured in r02
+    # (kernel, detector kind, mode-class mask): per (sample, bin, detector)
+    ("loglike", 0, 2): {"dfma": 169.17, "dmul": 59.88, "dadd": 35.27},      # kind 0, (2,2) only  -- config 2
+    ("loglike", 0, 15): {"dfma": 661.17, "dmul": 215.88, "dadd": 68.27},    # kind 0, five modes  -- configs 3, 4
+    ("loglike", 1, 15): None,                                               # kind 1, five modes  -- config 4
+    ("fisher", 0, 15): None,                                                # config 5
+    ("fisher", 1, 15): None,
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one loglike_kernel launch (same ncu capture)
 DRAM_TRAFFIC_PER_LAUNCH = {2: 21.03e6 + 0.86e6, 3: 21.54e6 + 33.45e6}
 # SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
 # kept for reference only -- the reduced algorithm needs less than half of it.
-SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0}
+SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0, 5: 100000.0}
+OPS_SOURCE = "profiles/r01_loglike_kernel_ncu.md"
 METRIC, UNIT = "lnL_evals_per_sec", "lnL/s"
+FISHER_METRIC, FISHER_UNIT = "fisher_evals_per_sec", "F/s"     # --config 5 only (S10: F and grad per sample)
 
 
 class ClockSampler:
@@ -108,24 +112,40 @@ class ClockSampler:
                 "samples": len(sm), "reasons": sorted(reasons)}
 
 
-def oracle_timed(wl, n_samples, steps: int, warmup: int, target_s: float = 12.0):
-    """Time the oracle, as it stands, on `n_samples` samples x all N bins per step.
-    n_samples=None: sized from a one-sample-per-core calibration pass for ~target_s of wall time."""
+FISHER_REF_BINS = 8192   # the oracle's Fisher pass costs ~45 core-seconds per sample at N = 262144: time a bin subset
+
+
+def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0):
+    """Time the oracle, as it stands, on a bounded sample of the workload: `n_samples` samples (None: sized from a
+    one-sample-per-core calibration pass for ~target_s of wall time) x all N bins per step; for the Fisher path
+    (config 5) x the first FISHER_REF_BINS bins, the rate scaled by FISHER_REF_BINS / N (the cost per bin is uniform).
+    -> (rate in full-N evaluations/s, seconds per step, cores, description of the sample)."""
     import oracle
+    fisher = config == 5
+    full = W.config(config)
+    wl = W.config(config, N=FISHER_REF_BINS) if fisher else full
+    scale = wl.grid.N / full.grid.N
     psd = wl.psd()
     data = wl.data(lambda p, fr, m: oracle.response(p, fr, m))
     cores = oracle.get_threads()
+    if fisher:
+        call = lambda p: oracle.fisher(p, data, psd, wl.grid, wl.model)
+    else:
+        call = lambda p: oracle.loglike(p, data, psd, wl.grid, wl.model)
     t0 = time.perf_counter()
-    oracle.loglike(wl.params[:cores], data, psd, wl.grid, wl.model)          # warm-up + calibration
+    call(wl.params[:cores])                                                  # warm-up + calibration
     t_cal = time.perf_counter() - t0
     if n_samples is None:
         n_samples = int(min(wl.B, max(cores, cores * round(target_s / max(t_cal, 1e-3)))))
     idx = np.linspace(0, wl.B - 1, n_samples).astype(int)
     t0 = time.perf_counter()
     for _ in range(steps):
-        oracle.loglike(wl.params[idx], data, psd, wl.grid, wl.model)
+        call(wl.params[idx])
     dt = time.perf_counter() - t0
-    return n_samples * steps / dt, dt / steps, cores, n_samples
+    bins = f"all {wl.grid.N} bins" if not fisher else f"the first {wl.grid.N} of {full.grid.N} bins (rate scaled by {scale:.5f})"
+    desc = (f"{n_samples} of {full.B} samples (evenly spaced) x {bins} per pass, {steps} pass(es), "
+            f"{dt / steps:.1f} s per pass, OpenMP over samples")
+    return n_samples * steps / dt * scale, dt / steps, cores, desc
 
 
 def run_reference(args):
@@ -133,9 +153,10 @@ def run_reference(args):
     if rank != 0:
         return
     wl = W.config(args.config)
-    rate, sec_per_step, cores, n = oracle_timed(wl, args.ref_samples, args.steps, min(args.warmup, 1),
-                                                target_s=max(2.0, 60.0 / max(1, args.steps)))
-    sample = f"{n} of {wl.B} samples (evenly spaced) x all {wl.grid.N} bins per step, OpenMP over samples"
+    fisher_mode = args.config == 5
+    METRIC, UNIT = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (globals()["METRIC"], globals()["UNIT"])
+    rate, sec_per_step, cores, sample = oracle_timed(args.config, args.ref_samples, args.steps,
+                                                     target_s=max(2.0, 60.0 / max(1, args.steps)))
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3,
@@ -170,6 +191,7 @@ def run_ours(args):
     device = torch.device("cuda", local_rank)
 
     # ---- inputs: synthetic, seeded; the injection comes from this library's own response call
+    fisher_mode = args.config == 5
     n_batches = 4
     wls = [W.config(args.config, param_seed=pdist.rank_seed(1000 + i, rank)) for i in range(n_batches)]
     wl = wls[0]
@@ -179,16 +201,26 @@ def run_ours(args):
     def gpu_response(p, fr, m):
         return P.response(torch.from_numpy(np.ascontiguousarray(p)).to(device), freqs_d, m).cpu().numpy()
 
-    data_h = np.ascontiguousarray(wl.data(gpu_response))
-    psd_h = np.ascontiguousarray(wl.psd())
-    lik = P.Likelihood(torch.from_numpy(data_h).to(device), torch.from_numpy(psd_h).to(device), wl.grid, wl.model, B)
-    params_d = [torch.from_numpy(w.params).to(device) for w in wls]
-    out_d = torch.empty(B, dtype=torch.float64, device=device)
+    # host copies live in pinned memory: the e2e leg copies them to the device every step
+    data_h = torch.from_numpy(np.ascontiguousarray(wl.data(gpu_response))).pin_memory()
+    psd_h = torch.from_numpy(np.ascontiguousarray(wl.psd())).pin_memory()
+    params_h = [torch.from_numpy(np.ascontiguousarray(w.params)).pin_memory() for w in wls]
+    params_d = [p.to(device) for p in params_h]
+    if fisher_mode:
+        fis = P.Fisher(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
+        F_d = torch.empty((B, P.NPAR, P.NPAR), dtype=torch.float64, device=device)
+        g_d = torch.empty((B, P.NPAR), dtype=torch.float64, device=device)
+    else:
+        lik = P.Likelihood(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
+        out_d = torch.empty(B, dtype=torch.float64, device=device)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
 
     def step(i):
         flush.zero_()
-        lik(params_d[i % n_batches], out_d)
+        if fisher_mode:
+            fis(params_d[i % n_batches], F_d, g_d)
+        else:
+            lik(params_d[i % n_batches], out_d)
 
     for i in range(args.warmup):
         step(i)
@@ -214,30 +246,50 @@ def run_ours(args):
     main_ms, main_launches = P.profile_read()
     P.profile_enable(False)
     clocks = sampler.stop()
-    lnL_last = out_d.cpu().numpy()
-    if not np.all(np.isfinite(lnL_last)):
-        raise SystemExit("bench.py: non-finite lnL in the timed region")
+    last = (F_d if fisher_mode else out_d).cpu().numpy()
+    if not np.all(np.isfinite(last)):
+        raise SystemExit("bench.py: non-finite result in the timed region")
 
     max_ms, total_units = pdist.aggregate(elapsed_ms, B * args.steps, device)
     value = total_units / (max_ms * 1e-3)
 
-    # ---- e2e: host buffers through pespace_loglike_host (copies inside the call)
+    # ---- e2e: HOST buffers through the C ABI (pespace_session_*): every step copies that step's inputs
+    # (theta, data set, PSD) from pinned host memory to the device and reads the result back, all inside
+    # the timed region.  e2e_resident_data: the sampler-facing use, data set copied once, theta per step.
     e2e_steps = max(1, min(args.steps, 10))
-    P.loglike_host(wls[0].params, data_h, psd_h, wl.grid, wl.model)        # warm-up
-    pdist.barrier(device)
-    t0 = time.perf_counter()
-    for i in range(e2e_steps):
-        lnL_host = P.loglike_host(wls[i % n_batches].params, data_h, psd_h, wl.grid, wl.model)
-    torch.cuda.synchronize()
-    e2e_ms = (time.perf_counter() - t0) * 1e3
-    e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
-    h2d = wl.params.nbytes + data_h.nbytes + psd_h.nbytes
-    d2h = lnL_host.nbytes
+    ses = P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
+    res_h = torch.empty((B, P.NPAR, P.NPAR) if fisher_mode else (B,), dtype=torch.float64).pin_memory()
+    grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
+
+    def e2e_step(i, copy_data):
+        if copy_data:
+            ses.set_data(data_h, psd_h)
+        if fisher_mode:
+            ses.fisher(params_h[i % n_batches], True, res_h, grad_h)
+        else:
+            ses.loglike(params_h[i % n_batches], res_h)
+
+    e2e = {}
+    for key, copy_data in (("full", True), ("resident", False)):
+        e2e_step(0, True)                                                   # warm-up
+        pdist.barrier(device)
+        t0 = time.perf_counter()
+        for i in range(e2e_steps):
+            e2e_step(i, copy_data)
+        e2e_ms = (time.perf_counter() - t0) * 1e3                           # the calls are synchronous
+        e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
+        e2e[key] = e2e_units / (e2e_max_ms * 1e-3)
+    ses.close()
+    nbytes = lambda t: t.numel() * t.element_size()
+    h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h)
+    d2h = nbytes(res_h) + (nbytes(grad_h) if fisher_mode else 0)
 
     if rank != 0:
         return
 
     # ---- roofline of the dominant kernel (per launch, timed live with CUDA events in the library)
+    kernel = "fisher" if fisher_mode else "loglike"
+    metric, unit = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (METRIC, UNIT)
     peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     dfma_tflops, _ = P.fp64_peak(8192, mode=0)
     dfma3_tflops, _ = P.fp64_peak(8192, mode=1)
@@ -245,22 +297,28 @@ def run_ours(args):
     kern_ms = main_ms / max(1, main_launches)                 # one launch = one detector, B x N (sample, bin) units
     cmask = (2 if wl.model.mode_mask & 9 else 0) | (1 if wl.model.mode_mask & 2 else 0) | \
             (4 if wl.model.mode_mask & 4 else 0) | (8 if wl.model.mode_mask & 16 else 0)
-    per_det = [FP64_OPS_PER_UNIT.get((d.kind, cmask)) for d in wl.model.detectors]
+    per_det = [FP64_OPS_PER_UNIT.get((kernel, d.kind, cmask)) for d in wl.model.detectors]
     known = [o for o in per_det if o]
-    ops = {k: sum(o[k] for o in known) / len(known) for k in ("dfma", "dmul", "dadd")} if known else None
-    roofline = {"bound": "alu", "kernel": "loglike_kernel", "achieved": None, "peak": peak_tflops,
+    ops = {k: sum(o[k] for o in known) / len(known) for k in ("dfma", "dmul", "dadd")} if len(known) == n_det else None
+    roofline = {"bound": "alu", "kernel": f"{kernel}_kernel", "achieved": None, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": None, "traffic": DRAM_TRAFFIC_PER_LAUNCH.get(args.config)}
     if ops:
         flop_per_unit = 2.0 * ops["dfma"] + ops["dmul"] + ops["dadd"]
         inst_per_unit = ops["dfma"] + ops["dmul"] + ops["dadd"]
         achieved = flop_per_unit * B * N / (kern_ms * 1e-3) / 1e12
+        # issue cost on the FP64 pipe (profiles/r01_fp64_operand_bandwidth.md): one 64-bit register operand
+        # per cycle and SM sub-partition, at least 2 cycles per instruction -> a DFMA with three distinct
+        # register operands takes 3 cycles.  The bound below charges every DFMA 3 cycles and DMUL/DADD 2.
+        cyc = 3.0 * ops["dfma"] + 2.0 * (ops["dmul"] + ops["dadd"])
+        t_operand = cyc * (B * N / 32.0) / (SM_COUNT * 4) / ((clocks.get("sm_max_mhz") or 1965.0) * 1e6)
         roofline.update({
             "achieved": achieved, "frac": achieved / peak_tflops,
             "flop_per_unit": flop_per_unit, "unit_of_work": "(sample, bin, detector)",
             "flop_per_launch": flop_per_unit * B * N,
             "fma_share_of_fp64_instructions": ops["dfma"] / inst_per_unit,
             "fp64_pipe_frac": inst_per_unit * B * N / (kern_ms * 1e-3) / (peak_tflops * 1e12 / 2.0),
-            "detectors_with_measured_op_counts": f"{len(known)} of {n_det}",
+            "operand_bandwidth_bound_ms": t_operand * 1e3,
+            "frac_of_operand_bandwidth_bound": t_operand * 1e3 / kern_ms,
         })
     roofline.update({
         "peak_source": "148 SM x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md; no FP64 entry in "
@@ -268,33 +326,34 @@ def run_ours(args):
         "peak_dfma_measured": dfma_tflops, "peak_dfma_3reg_measured": dfma3_tflops,
         "frac_of_dfma_measured": (roofline["achieved"] / dfma_tflops) if roofline["achieved"] else None,
         "kernel_ms": kern_ms, "kernel_launches": main_launches, "kernel_share_of_step": main_ms / elapsed_ms,
-        "flop_basis": "FP64 operations of the reduced algorithm = executed 2*DFMA+DMUL+DADD per unit, ncu "
-                      "(profiles/r01_loglike_kernel_ncu.md)",
+        "flop_basis": "FP64 operations of the reduced algorithm = executed 2*DFMA+DMUL+DADD per unit, averaged over "
+                      f"the detectors, ncu ({OPS_SOURCE})",
         "hbm_gbs_achieved": (roofline["traffic"] / (kern_ms * 1e-3) / 1e9) if roofline["traffic"] else None,
-        "survey_estimate_flop_per_bin_eval": SURVEY_FLOP_PER_BIN_EVAL[args.config],
+        "survey_estimate_flop_per_bin_eval": SURVEY_FLOP_PER_BIN_EVAL.get(args.config),
     })
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
-        rate, sec, cores, n_ref = oracle_timed(W.config(args.config), args.ref_samples, 1, 1)
-        cpu_baseline = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
-                        "sample": f"{n_ref} of {B} samples (evenly spaced) x all {N} bins, one pass, "
-                                  f"{sec:.1f} s, OpenMP over samples"}
+        rate, sec, cores, desc = oracle_timed(args.config, args.ref_samples, 1)
+        cpu_baseline = {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": desc}
 
     line = {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": "f64", "data": "synthetic",
         "bin_evals_per_sec": value * N,
         "config": workload_config(wl, args, l2="256 MiB buffer rewritten before every step, inside the timed region"),
         "clocks": clocks,
-        "e2e": {"value": e2e_units / (e2e_max_ms * 1e-3), "unit": UNIT, "h2d_bytes_per_step": int(h2d),
+        "e2e": {"value": e2e["full"], "unit": unit, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-                "api": "pespace_loglike_host (pageable host buffers; cudaMalloc/free inside the call)"},
+                "api": "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
+                       " per step: theta, data set and PSD copied from pinned host memory, result read back",
+                "value_resident_data": e2e["resident"],
+                "resident_data_note": "same call with the data set copied once (sampler use): theta in, result out"},
         "gpu_launches": int(launches),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
-        "lnL_check": {"min": float(lnL_last.min()), "max": float(lnL_last.max())},
+        "result_check": {"min": float(last.min()), "max": float(last.max())},
     }
     print(json.dumps(line), flush=True)
 
@@ -305,7 +364,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
-    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4])
+    ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
     ap.add_argument("--ref-samples", type=int, default=None,
                     help="samples per oracle pass (default: sized for ~15 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

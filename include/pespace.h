@@ -98,9 +98,33 @@ int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, 
                    const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                    double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
 
-/* Host-buffer twin of pespace_loglike for end-to-end use: copies params, data and psd to the
- * device, runs the same kernels, copies lnL back and synchronises.  All pointers are HOST
- * pointers; device scratch is allocated and freed inside the call. */
+/* ---- Host-buffer entry points (a sampler evaluates many batches of theta against
+ * ONE data set).  A session owns a stream and keeps the data set, the PSD, the workspace
+ * and the result buffers resident on the device between calls; each call then moves only theta in
+ * and lnL (or F, grad) out.  The arithmetic is that of pespace_loglike / pespace_fisher, launched on
+ * the session's stream.  All pointers are HOST pointers (pinned memory makes the copies DMA
+ * transfers; pageable memory works); the calls are synchronous: outputs are valid, and input
+ * buffers may be reused, on return.  A session is not thread-safe; use one per thread. */
+typedef struct pespace_session pespace_session;
+
+/* Allocates device buffers for batches of up to max_B samples on the current device.  want_fisher != 0
+ * also sizes the pespace_session_fisher buffers.  *out is NULL on failure (PESPACE_EINVAL,
+ * PESPACE_ENOMEM). */
+int pespace_session_create(const pespace_grid* grid, const pespace_model* model, int64_t max_B,
+                           int want_fisher, pespace_session** out);
+/* Copies the data set h_data_AET [n_det][3][N][2] and / or the PSD h_psd [n_det][3][N] to the
+ * device (either pointer may be NULL: that array is left as it is). */
+int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const double* h_psd);
+/* h_params [B][11] -> h_out_lnL [B], B <= max_B.  PESPACE_EINVAL before data and PSD are set. */
+int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL);
+/* h_params [B][11] -> h_out_F [B][11][11] and, if h_out_grad != NULL, h_out_grad [B][11] (needs the
+ * data set; the Fisher matrix alone needs only the PSD). */
+int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
+                           double* h_out_grad);
+/* Waits for the session's stream and frees everything the session owns. */
+int pespace_session_destroy(pespace_session* s);
+
+/* One-shot host-buffer twin of pespace_loglike: session create + set_data + loglike + destroy. */
 int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET,
                          const double* h_psd, const pespace_grid* grid, const pespace_model* model,
                          double* h_out_lnL);
@@ -115,7 +139,8 @@ int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms);
 
 /* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel
- * (the fused per-bin likelihood kernel) is bracketed by CUDA events on the launching stream.
+ * (the fused per-bin likelihood kernel, or the Fisher kernel) is bracketed by CUDA events on the
+ * launching stream.
  * pespace_profile_read synchronises those events and returns the summed kernel time in ms and
  * the number of launches since the last read (either pointer may be NULL), then resets. */
 int pespace_profile_enable(int on);

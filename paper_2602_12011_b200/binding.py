@@ -17,6 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
+           "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike",
+           "pespace_session_fisher", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
            "pespace_launch_count", "pespace_strerror",
            "pespace_version")
@@ -51,6 +53,11 @@ def _load():
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
+    L.pespace_session_create.argtypes = [C.POINTER(_Grid), C.POINTER(_Model), i64, C.c_int, C.POINTER(vp)]
+    L.pespace_session_set_data.argtypes = [vp, vp, vp]
+    L.pespace_session_loglike.argtypes = [vp, vp, i64, vp]
+    L.pespace_session_fisher.argtypes = [vp, vp, i64, vp, vp]
+    L.pespace_session_destroy.argtypes = [vp]
     L.pespace_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.pespace_profile_enable.argtypes = [C.c_int]
     L.pespace_profile_read.argtypes = [C.POINTER(C.c_double), C.POINTER(i64)]
@@ -153,25 +160,42 @@ def loglike(params: torch.Tensor, data: torch.Tensor, psd: torch.Tensor, grid, m
     return Likelihood(data, psd, grid, model, params.shape[0])(params)
 
 
+class Fisher:
+    """Data (optional), PSD, workspace and outputs resident on the device; one pespace_fisher call per batch."""
+
+    def __init__(self, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model, max_batch: int):
+        self.psd = _dev(psd.contiguous(), "psd")
+        self.data = None
+        if data is not None:
+            d = torch.view_as_real(data) if data.is_complex() else data
+            self.data = _dev(d.contiguous(), "data")
+        self.grid, self.model, self.max_batch = grid, model, int(max_batch)
+        self._m, self._keep = _model(model)
+        self._g = _grid(grid)
+        self.ws_bytes = workspace_bytes(max_batch, grid, model, True)
+        self.ws = torch.empty(max(self.ws_bytes, 16), dtype=torch.uint8, device=self.psd.device)
+
+    def __call__(self, params: torch.Tensor, out_F: Optional[torch.Tensor] = None,
+                 out_grad: Optional[torch.Tensor] = None):
+        p = _dev(params, "params")
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        if out_F is None:
+            out_F = torch.empty((B, NPAR, NPAR), dtype=torch.float64, device=p.device)
+        if self.data is not None and out_grad is None:
+            out_grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_fisher(p.data_ptr(), B, None if self.data is None else self.data.data_ptr(),
+                                   self.psd.data_ptr(), C.byref(self._g), C.byref(self._m),
+                                   _dev(out_F, "out_F").data_ptr(),
+                                   None if self.data is None else _dev(out_grad, "out_grad").data_ptr(),
+                                   self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_fisher")
+        return out_F, (out_grad if self.data is not None else None)
+
+
 def fisher(params: torch.Tensor, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):
     """-> (F [B][11][11], grad [B][11] or None)."""
-    p = _dev(params, "params")
-    B = p.shape[0]
-    m, keep = _model(model)
-    g = _grid(grid)
-    nbytes = workspace_bytes(B, grid, model, True)
-    ws = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=p.device)
-    F = torch.empty((B, NPAR, NPAR), dtype=torch.float64, device=p.device)
-    grad, dptr = None, None
-    if data is not None:
-        d = torch.view_as_real(data) if data.is_complex() else data
-        d = _dev(d.contiguous(), "data")
-        dptr = d.data_ptr()
-        grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
-    _check(_lib.pespace_fisher(p.data_ptr(), B, dptr, _dev(psd.contiguous(), "psd").data_ptr(), C.byref(g),
-                               C.byref(m), F.data_ptr(), None if grad is None else grad.data_ptr(),
-                               ws.data_ptr(), nbytes, _stream_ptr()), "pespace_fisher")
-    return F, grad
+    return Fisher(data, psd, grid, model, params.shape[0])(params)
 
 
 def loglike_host(params: np.ndarray, data: np.ndarray, psd: np.ndarray, grid, model) -> np.ndarray:
@@ -186,6 +210,71 @@ def loglike_host(params: np.ndarray, data: np.ndarray, psd: np.ndarray, grid, mo
     _check(_lib.pespace_loglike_host(p.ctypes.data, p.shape[0], d.ctypes.data, s.ctypes.data, C.byref(g),
                                      C.byref(m), out.ctypes.data), "pespace_loglike_host")
     return out
+
+
+def _host_ptr(a, dtype, name: str):
+    """Address of a contiguous host buffer: numpy array or CPU torch tensor (pinned or pageable)."""
+    if isinstance(a, torch.Tensor):
+        want = torch.complex128 if dtype == np.complex128 else torch.float64
+        if a.is_cuda or a.dtype != want or not a.is_contiguous():
+            raise PespaceError(f"{name}: expected a contiguous host tensor of {want}")
+        return a.data_ptr(), a
+    b = np.ascontiguousarray(a, dtype=dtype)
+    return b.ctypes.data, b
+
+
+class Session:
+    """Host-buffer API (pespace_session_*): data set, PSD and scratch stay on the device; a call copies
+    theta in and lnL (or F, grad) out.  Inputs and outputs are numpy arrays or CPU torch tensors."""
+
+    def __init__(self, grid, model, max_batch: int, want_fisher: bool = False):
+        m, self._keep = _model(model)
+        g = _grid(grid)
+        h = C.c_void_p()
+        _check(_lib.pespace_session_create(C.byref(g), C.byref(m), int(max_batch), int(want_fisher), C.byref(h)),
+               "pespace_session_create")
+        self._h, self.grid, self.model, self.max_batch = h, grid, model, int(max_batch)
+
+    def set_data(self, data=None, psd=None) -> None:
+        dp = sp = None
+        if data is not None:
+            dp, keep_d = _host_ptr(data, np.complex128, "data")
+        if psd is not None:
+            sp, keep_s = _host_ptr(psd, np.float64, "psd")
+        _check(_lib.pespace_session_set_data(self._h, dp, sp), "pespace_session_set_data")
+
+    def loglike(self, params, out=None):
+        pp, p = _host_ptr(params, np.float64, "params")
+        if out is None:
+            out = np.empty(p.shape[0], dtype=np.float64)
+        op, o = _host_ptr(out, np.float64, "out")
+        _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
+        return out
+
+    def fisher(self, params, with_grad: bool = True, out_F=None, out_grad=None):
+        pp, p = _host_ptr(params, np.float64, "params")
+        B = int(p.shape[0])
+        if out_F is None:
+            out_F = np.empty((B, NPAR, NPAR), dtype=np.float64)
+        if with_grad and out_grad is None:
+            out_grad = np.empty((B, NPAR), dtype=np.float64)
+        Fp, keep_F = _host_ptr(out_F, np.float64, "out_F")
+        gp = None
+        if with_grad:
+            gp, keep_g = _host_ptr(out_grad, np.float64, "out_grad")
+        _check(_lib.pespace_session_fisher(self._h, pp, B, Fp, gp), "pespace_session_fisher")
+        return out_F, (out_grad if with_grad else None)
+
+    def close(self) -> None:
+        if self._h is not None and self._h.value:
+            h, self._h = self._h, None
+            _check(_lib.pespace_session_destroy(h), "pespace_session_destroy")
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
 
 
 def fp64_peak(iters: int = 4096, mode: int = 0):

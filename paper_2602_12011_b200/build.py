@@ -17,7 +17,7 @@ DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.gl
     [os.path.join(os.path.dirname(HERE), "include", "pespace.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
-              "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"]
+              "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"] + os.environ.get("PESPACE_NVCC_EXTRA", "").split()
 
 
 def nvcc() -> str:

@@ -19,8 +19,6 @@ char* cuda_msg() {
 
 namespace {
 
-// optional event timing of the dominant kernel (pespace_profile_enable / _read)
-struct EvPair { cudaEvent_t a, b; };
 bool g_profile = false;
 std::vector<EvPair> g_events;
 std::mutex g_ev_mutex;
@@ -29,7 +27,8 @@ struct Plan {
   int n_det, stride;
   long long nbb;          // bin blocks
   long long ntile;        // sample tiles
-  size_t trig_bytes, consts_bytes, partial_bytes;      // workspace: [trig table | sample constants | block partials]
+  size_t trig_bytes, consts_bytes, partial_bytes, bins_bytes;   // workspace: [trig table | sample constants | block
+                                                                // partials | per-bin table (likelihood only)]
 };
 Plan make_plan(long long B, long long N, int n_det) {
   Plan p;
@@ -40,6 +39,7 @@ Plan make_plan(long long B, long long N, int n_det) {
   p.trig_bytes = align_up((size_t)NTAB * sizeof(double2), 256);
   p.consts_bytes = align_up((size_t)B * p.stride * sizeof(double), 256);
   p.partial_bytes = align_up((size_t)n_det * p.nbb * (size_t)B * sizeof(double), 256);
+  p.bins_bytes = align_up((size_t)n_det * NBF * (size_t)N * sizeof(double), 256);
   return p;
 }
 
@@ -53,6 +53,26 @@ int run_prep(const double* d_params, long long B, const pespace_model* model, do
 }
 
 }  // namespace
+
+namespace pespace {
+namespace host {
+int prof_begin(EvPair& ev, cudaStream_t st) {
+  ev = EvPair();
+  if (!g_profile) return PESPACE_OK;
+  CU(cudaEventCreate(&ev.a));
+  CU(cudaEventCreate(&ev.b));
+  CU(cudaEventRecord(ev.a, st));
+  return PESPACE_OK;
+}
+int prof_end(EvPair& ev, cudaStream_t st) {
+  if (!ev.a) return PESPACE_OK;
+  CU(cudaEventRecord(ev.b, st));
+  std::lock_guard<std::mutex> lk(g_ev_mutex);
+  g_events.push_back(ev);
+  return PESPACE_OK;
+}
+}  // namespace host
+}  // namespace pespace
 
 extern "C" {
 
@@ -98,7 +118,7 @@ size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespac
   if (B <= 0 || !grid_ok(grid) || !model_ok(model)) return 0;
   if (want_fisher) return fisher_workspace_bytes(B, grid->N, model->n_det);
   const Plan p = make_plan(B, grid->N, model->n_det);
-  return p.trig_bytes + p.consts_bytes + p.partial_bytes;
+  return p.trig_bytes + p.consts_bytes + p.partial_bytes + p.bins_bytes;
 }
 
 int pespace_response(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
@@ -141,66 +161,32 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
   double2* d_trig = (double2*)d_workspace;
   double* d_consts = (double*)((char*)d_workspace + p.trig_bytes);
   double* d_partial = (double*)((char*)d_workspace + p.trig_bytes + p.consts_bytes);
+  double* d_bins = (double*)((char*)d_workspace + p.trig_bytes + p.consts_bytes + p.partial_bytes);
   int rc = run_prep(d_params, B, model, d_consts, d_trig, st);
   if (rc != PESPACE_OK) return rc;
   const unsigned cm = class_mask(model->mode_mask);
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
+  {
+    // S0: per-bin table of this data set, once per call
+    const PrepArgs A = make_prep_args(model);
+    const dim3 gb((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det);
+    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, d_bins);
+    LAUNCHED();
+  }
   const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
-    EvPair ev = {nullptr, nullptr};
-    if (g_profile) {
-      CU(cudaEventCreate(&ev.a));
-      CU(cudaEventCreate(&ev.b));
-      CU(cudaEventRecord(ev.a, st));
-    }
-    CU(loglike_launcher(dc.kind, cm)(g, st, d_consts, d_trig, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d,
-                             d_partial));
+    EvPair ev;
+    if (int rc2 = prof_begin(ev, st); rc2 != PESPACE_OK) return rc2;
+    CU(loglike_launcher(dc.kind, cm)(g, st, d_consts, d_trig, B, d_bins, G.N, dc, model->n_det, d, d_partial));
     LAUNCHED();
-    if (ev.a) {
-      CU(cudaEventRecord(ev.b, st));
-      std::lock_guard<std::mutex> lk(g_ev_mutex);
-      g_events.push_back(ev);
-    }
+    if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
   }
   const int th = 128;
   combine_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_partial, d_consts, B, (int)(model->n_det * p.nbb),
                                                                 p.stride, d_out_lnL);
   LAUNCHED();
   return PESPACE_OK;
-}
-
-int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET, const double* h_psd,
-                         const pespace_grid* grid, const pespace_model* model, double* h_out_lnL) {
-  if (!h_params || !h_data_AET || !h_psd || !h_out_lnL || B <= 0 || !grid_ok(grid) || !model_ok(model))
-    return PESPACE_EINVAL;
-  const size_t nP = (size_t)B * NPAR, nS = (size_t)model->n_det * 3 * (size_t)grid->N;
-  const size_t ws = pespace_workspace_bytes(B, grid, model, 0);
-  double *dP = nullptr, *dD = nullptr, *dS = nullptr, *dO = nullptr;
-  void* dW = nullptr;
-  cudaStream_t st = nullptr;
-  int rc = PESPACE_OK;
-  auto bail = [&](int code) {
-    cudaFree(dP); cudaFree(dD); cudaFree(dS); cudaFree(dO); cudaFree(dW);
-    return code;
-  };
-  if (cudaMalloc((void**)&dP, nP * 8) != cudaSuccess || cudaMalloc((void**)&dD, nS * 16) != cudaSuccess ||
-      cudaMalloc((void**)&dS, nS * 8) != cudaSuccess || cudaMalloc((void**)&dO, (size_t)B * 8) != cudaSuccess ||
-      cudaMalloc(&dW, ws) != cudaSuccess) {
-    cudaGetLastError();
-    return bail(PESPACE_ENOMEM);
-  }
-  cudaError_t e;
-  if ((e = cudaMemcpyAsync(dP, h_params, nP * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dD, h_data_AET, nS * 16, cudaMemcpyHostToDevice, st)) != cudaSuccess ||
-      (e = cudaMemcpyAsync(dS, h_psd, nS * 8, cudaMemcpyHostToDevice, st)) != cudaSuccess)
-    return bail(cuda_fail(e));
-  rc = pespace_loglike(dP, B, dD, dS, grid, model, dO, dW, ws, st);
-  if (rc != PESPACE_OK) return bail(rc);
-  if ((e = cudaMemcpyAsync(h_out_lnL, dO, (size_t)B * 8, cudaMemcpyDeviceToHost, st)) != cudaSuccess ||
-      (e = cudaStreamSynchronize(st)) != cudaSuccess)
-    return bail(cuda_fail(e));
-  return bail(PESPACE_OK);
 }
 
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms) {

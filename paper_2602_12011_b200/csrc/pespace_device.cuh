@@ -140,6 +140,8 @@ __device__ __forceinline__ double rcp_pos(double x) {
 // i.e. |theta| <= pi/1024, where sin(theta) = y (A1 + A3 y^2) and cos(theta) - 1 = y^2 (B2 + B4 y^2)
 // (Taylor with the theta^5 term economised onto the lower ones: max error 1.4e-16 / 1.2e-18), then
 // the angle-addition formulas.  12 FP64 instructions, no quadrant logic, no conversion instructions.
+// (Evaluating the two small terms in FP32 was tried and dropped: every non-FP64 instruction costs an issue
+// cycle that the FP64 pipe cannot use, and the 1e-12 error shows in the cancelling T channel.)
 constexpr double kHh = 0.5 * kRadPerPu;   // half-width of the reduced interval, radians
 constexpr double kA1 = kRadPerPu * (1.0 - (5.0 / 16.0) * (kHh * kHh * kHh * kHh) / 120.0);
 constexpr double kA3 = kRadPerPu * kRadPerPu * kRadPerPu * (-1.0 / 6.0 + (5.0 / 4.0) * (kHh * kHh) / 120.0);
@@ -519,13 +521,51 @@ __device__ __forceinline__ void stage_tile(double* smem, const double* __restric
   }
 }
 
+// S0: per-bin table of one data set, written once per pespace_loglike call and read by every
+// sample tile: [n_det][NBF][N] doubles = the per-bin factors of make_bin and the data / weights with
+// g z f^{-7/6} and the 1/sqrt2, 1/sqrt6, 1/sqrt3 of Eq. 3 folded in (Eq. 10: w = 4 df / S_n).
+enum : int { BF_FT = 0, BF_CF, BF_LNF3, BF_FM53, BF_FM83, BF_STH, BF_CTH, BF_DR, BF_DI = BF_DR + 3, BF_W = BF_DI + 3,
+             NBF = BF_W + 3 };
+static_assert(NBF == 16, "bin record is 16 doubles");
+
+static __global__ void prep_bins_kernel(const double2* __restrict__ data, const double* __restrict__ psd, GridC G,
+                                        PrepArgs A, double* __restrict__ bins /* [n_det][NBF][N] */) {
+  const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int det = blockIdx.y;
+  if (k >= G.N) return;
+  const DetC& dc = A.det[det];
+  const BinC bc = make_bin(fma((double)k, G.df, G.f0), dc.Lbar);
+  double gr, gi;
+  tdi_prefactor(bc, dc.gen, gr, gi);
+  const double g2 = gr * gr + gi * gi;
+  double* o = bins + (size_t)det * NBF * (size_t)G.N + (size_t)k;
+  const size_t N = (size_t)G.N;
+  o[BF_FT * N] = bc.fT; o[BF_CF * N] = bc.cf; o[BF_LNF3 * N] = bc.lnf3; o[BF_FM53 * N] = bc.fm53;
+  o[BF_FM83 * N] = bc.fm83; o[BF_STH * N] = bc.sth; o[BF_CTH * N] = bc.cth;
+  const double nrm[3] = {1.4142135623730950488, 2.4494897427831780982, 1.7320508075688772935};
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    const size_t idx = ((size_t)det * 3 + c) * N + (size_t)k;
+    const double2 d = data[idx];
+    const double Sn = psd[idx];
+    const bool use = isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
+    const double sc_ = use ? nrm[c] / g2 : 0.0;
+    o[(BF_DR + c) * N] = (d.x * gr + d.y * gi) * sc_;          // d * conj(g) / |g|^2 * nrm
+    o[(BF_DI + c) * N] = (d.x * gi - d.y * gr) * sc_;          // MINUS the imaginary part: eval_xyz returns (Re, -Im)
+    o[(BF_W + c) * N] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+  }
+}
+
 // K_main: grid (bin blocks, sample tiles); one launch per detector.
 constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1) + ((m >> 3) & 1); }
 
 template <int KIND, unsigned CMASK>
-__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? 3 : 2)
+#ifndef PESPACE_MINB1
+#define PESPACE_MINB1 3
+#endif
+__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? PESPACE_MINB1 : 2)
 loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
-               const double2* __restrict__ data, const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
+               const double* __restrict__ bins /* [n_det][NBF][N] */, long long N, DetC dc, int n_det, int det,
                double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
   double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
   double* smem = reinterpret_cast<double*>(tab + NTAB);
@@ -535,25 +575,16 @@ loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ tr
   stage_tile(smem, consts, b0, B, n_det, det);
 
   const long long k = (long long)blockIdx.x * BLOCK + threadIdx.x;
-  const bool live = k < G.N;
-  const long long kk = live ? k : G.N - 1;
-  const BinC bc = make_bin(fma((double)kk, G.df, G.f0), dc.Lbar);
-  double gr, gi;
-  tdi_prefactor(bc, dc.gen, gr, gi);
-  const double g2 = gr * gr + gi * gi;
-  // fold g z f^{-7/6} and the 1/sqrt2, 1/sqrt6, 1/sqrt3 of Eq. 3 into data and weights
-  const double nrm[3] = {1.4142135623730950488, 2.4494897427831780982, 1.7320508075688772935};
+  const bool live = k < N;
+  const double* bp = bins + (size_t)det * NBF * (size_t)N + (size_t)(live ? k : N - 1);
+  BinC bc;
+  bc.fT = bp[BF_FT * N]; bc.cf = bp[BF_CF * N]; bc.lnf3 = bp[BF_LNF3 * N]; bc.fm53 = bp[BF_FM53 * N];
+  bc.fm83 = bp[BF_FM83 * N]; bc.sth = bp[BF_STH * N]; bc.cth = bp[BF_CTH * N]; bc.fm76 = 0.0;
   double dr[3], di[3], w[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const size_t idx = ((size_t)det * 3 + c) * (size_t)G.N + (size_t)kk;
-    const double2 d = data[idx];
-    const double Sn = psd[idx];
-    const bool use = live && isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
-    const double sc_ = use ? nrm[c] / g2 : 0.0;
-    dr[c] = (d.x * gr + d.y * gi) * sc_;          // d * conj(g) / |g|^2 * nrm
-    di[c] = (d.x * gi - d.y * gr) * sc_;          // MINUS the imaginary part: eval_xyz returns (Re, -Im)
-    w[c] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+    dr[c] = bp[(BF_DR + c) * N]; di[c] = bp[(BF_DI + c) * N];
+    w[c] = live ? bp[(BF_W + c) * N] : 0.0;
   }
   __syncthreads();
 

@@ -53,8 +53,11 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
   const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
+    EvPair ev;
+    if (int rc = prof_begin(ev, st); rc != PESPACE_OK) return rc;
     CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial));
     LAUNCHED();
+    if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }
   const long long nt = (long long)B * NG;
   combine_fisher_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(

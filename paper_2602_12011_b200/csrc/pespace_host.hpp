@@ -69,6 +69,11 @@ inline unsigned class_mask(unsigned mode_mask) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// optional event timing of the dominant kernels (pespace_profile_enable / _read); defined in pespace_api.cu
+struct EvPair { cudaEvent_t a = nullptr, b = nullptr; };
+int prof_begin(EvPair& ev, cudaStream_t st);   // no-op unless profiling is enabled
+int prof_end(EvPair& ev, cudaStream_t st);
+
 // Fisher path (pespace_fisher.cu)
 size_t fisher_workspace_bytes(long long B, long long N, int n_det);
 

@@ -23,11 +23,10 @@ cudaError_t opt_in_smem(K kernel, size_t bytes, bool& done) {
 #if PESPACE_INST_WHAT == 0
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
-                   const double2* data, const double* psd, GridC G, const DetC& dc, int n_det, int det,
-                   double* partial) {
+                   const double* bins, long long N, const DetC& dc, int n_det, int det, double* partial) {
   static bool configured = false;
   if (cudaError_t e = opt_in_smem(loglike_kernel<KIND, CM>, kernel_smem_bytes(), configured); e != cudaSuccess) return e;
-  loglike_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, data, psd, G, dc, n_det, det, partial);
+  loglike_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, bins, N, dc, n_det, det, partial);
   return cudaSuccess;
 }
 using Fn = LoglikeFn;

@@ -8,8 +8,8 @@
 namespace pespace {
 namespace host {
 
-using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double2*,
-                                  const double*, GridC, const DetC&, int, int, double*);
+using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
+                                  long long, const DetC&, int, int, double*);
 using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
                                    long long, const DetC&, int, int, double2*);
 using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double2*, const double*, GridC,

@@ -1,0 +1,136 @@
+// pespace_session.cu -- host-buffer entry points of include/pespace.h.  A session keeps the data set, the
+// PSD, the workspace and the result buffers resident on the device between calls (the
+// sampler-facing use is many batches of theta against ONE data set), so that a call moves only theta in and
+// lnL (or F, grad) out.  Every step of the path still runs in the kernels behind pespace_loglike /
+// pespace_fisher; this file only owns memory, a stream and the copies.
+#include "pespace_host.hpp"
+
+#include <new>
+#include <vector>
+
+using namespace pespace;
+using namespace pespace::host;
+
+struct pespace_session {
+  pespace_grid grid;
+  pespace_model model;
+  std::vector<pespace_detector> det;
+  long long max_B = 0;
+  int want_fisher = 0;
+  bool have_data = false, have_psd = false;
+  cudaStream_t st = nullptr;
+  double *d_params = nullptr, *d_data = nullptr, *d_psd = nullptr, *d_lnL = nullptr, *d_F = nullptr, *d_grad = nullptr;
+  void *d_ws = nullptr, *d_ws_f = nullptr;
+  size_t ws_bytes = 0, ws_f_bytes = 0;
+  size_t n_series() const { return (size_t)model.n_det * 3 * (size_t)grid.N; }
+};
+
+namespace {
+
+void release(pespace_session* s) {
+  if (!s) return;
+  cudaFree(s->d_params); cudaFree(s->d_data); cudaFree(s->d_psd); cudaFree(s->d_lnL); cudaFree(s->d_F);
+  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f);
+  if (s->st) cudaStreamDestroy(s->st);
+  delete s;
+}
+
+}  // namespace
+
+extern "C" {
+
+int pespace_session_create(const pespace_grid* grid, const pespace_model* model, int64_t max_B, int want_fisher,
+                           pespace_session** out) {
+  if (!out) return PESPACE_EINVAL;
+  *out = nullptr;
+  if (max_B <= 0 || !grid_ok(grid) || !model_ok(model)) return PESPACE_EINVAL;
+  pespace_session* s = new (std::nothrow) pespace_session();
+  if (!s) return PESPACE_ENOMEM;
+  s->grid = *grid;
+  s->det.assign(model->det, model->det + model->n_det);
+  s->model = *model;
+  s->model.det = s->det.data();
+  s->max_B = max_B;
+  s->want_fisher = want_fisher != 0;
+  s->ws_bytes = pespace_workspace_bytes(max_B, grid, &s->model, 0);
+  s->ws_f_bytes = want_fisher ? pespace_workspace_bytes(max_B, grid, &s->model, 1) : 0;
+  const size_t nS = s->n_series();
+  bool ok = cudaStreamCreateWithFlags(&s->st, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaMalloc((void**)&s->d_params, (size_t)max_B * NPAR * 8) == cudaSuccess &&
+            cudaMalloc((void**)&s->d_data, nS * 16) == cudaSuccess &&
+            cudaMalloc((void**)&s->d_psd, nS * 8) == cudaSuccess &&
+            cudaMalloc((void**)&s->d_lnL, (size_t)max_B * 8) == cudaSuccess &&
+            cudaMalloc(&s->d_ws, s->ws_bytes) == cudaSuccess;
+  if (ok && want_fisher)
+    ok = cudaMalloc((void**)&s->d_F, (size_t)max_B * NPAR * NPAR * 8) == cudaSuccess &&
+         cudaMalloc((void**)&s->d_grad, (size_t)max_B * NPAR * 8) == cudaSuccess &&
+         cudaMalloc(&s->d_ws_f, s->ws_f_bytes) == cudaSuccess;
+  if (!ok) {
+    cudaGetLastError();
+    release(s);
+    return PESPACE_ENOMEM;
+  }
+  *out = s;
+  return PESPACE_OK;
+}
+
+int pespace_session_destroy(pespace_session* s) {
+  if (!s) return PESPACE_EINVAL;
+  cudaError_t e = cudaStreamSynchronize(s->st);
+  release(s);
+  return e == cudaSuccess ? PESPACE_OK : cuda_fail(e);
+}
+
+int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const double* h_psd) {
+  if (!s || (!h_data_AET && !h_psd)) return PESPACE_EINVAL;
+  const size_t nS = s->n_series();
+  if (h_data_AET) {
+    CU(cudaMemcpyAsync(s->d_data, h_data_AET, nS * 16, cudaMemcpyHostToDevice, s->st));
+    s->have_data = true;
+  }
+  if (h_psd) {
+    CU(cudaMemcpyAsync(s->d_psd, h_psd, nS * 8, cudaMemcpyHostToDevice, s->st));
+    s->have_psd = true;
+  }
+  CU(cudaStreamSynchronize(s->st));   // the caller may reuse its buffers on return
+  return PESPACE_OK;
+}
+
+int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL) {
+  if (!s || !h_params || !h_out_lnL || B <= 0 || B > s->max_B || !s->have_data || !s->have_psd) return PESPACE_EINVAL;
+  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  const int rc = pespace_loglike(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL, s->d_ws,
+                                 s->ws_bytes, s->st);
+  if (rc != PESPACE_OK) return rc;
+  CU(cudaMemcpyAsync(h_out_lnL, s->d_lnL, (size_t)B * 8, cudaMemcpyDeviceToHost, s->st));
+  CU(cudaStreamSynchronize(s->st));
+  return PESPACE_OK;
+}
+
+int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
+                           double* h_out_grad) {
+  if (!s || !s->want_fisher || !h_params || !h_out_F || B <= 0 || B > s->max_B || !s->have_psd) return PESPACE_EINVAL;
+  if (h_out_grad && !s->have_data) return PESPACE_EINVAL;
+  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  const int rc = pespace_fisher(s->d_params, B, h_out_grad ? s->d_data : nullptr, s->d_psd, &s->grid, &s->model,
+                                s->d_F, h_out_grad ? s->d_grad : nullptr, s->d_ws_f, s->ws_f_bytes, s->st);
+  if (rc != PESPACE_OK) return rc;
+  CU(cudaMemcpyAsync(h_out_F, s->d_F, (size_t)B * NPAR * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
+  if (h_out_grad) CU(cudaMemcpyAsync(h_out_grad, s->d_grad, (size_t)B * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
+  CU(cudaStreamSynchronize(s->st));
+  return PESPACE_OK;
+}
+
+int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET, const double* h_psd,
+                         const pespace_grid* grid, const pespace_model* model, double* h_out_lnL) {
+  if (!h_params || !h_data_AET || !h_psd || !h_out_lnL) return PESPACE_EINVAL;
+  pespace_session* s = nullptr;
+  int rc = pespace_session_create(grid, model, B, 0, &s);
+  if (rc != PESPACE_OK) return rc;
+  rc = pespace_session_set_data(s, h_data_AET, h_psd);
+  if (rc == PESPACE_OK) rc = pespace_session_loglike(s, h_params, B, h_out_lnL);
+  const int rc2 = pespace_session_destroy(s);
+  return rc != PESPACE_OK ? rc : rc2;
+}
+
+}  // extern "C"

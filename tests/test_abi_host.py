@@ -88,3 +88,26 @@ def test_workloads_are_seeded_and_shaped_like_the_configs():
     det = W.lisa_like()
     fn = 299792458.0 / (4 * det.L_m)
     assert W.psd_aet(det, np.array([fn]))[0, 0] < 1e-25 * W.psd_aet(det, np.array([fn * 0.9]))[0, 0]
+
+
+def test_session_argument_validation_without_a_device():
+    """pespace_session_* reject bad arguments before any CUDA call (include/pespace.h, host-buffer entry points)."""
+    from paper_2602_12011_b200 import binding as P
+    L = P.lib()
+    wl = W.config(2, B=4, N=64)
+    m, keep = P._model(wl.model)
+    g = P._grid(wl.grid)
+    EINVAL = -1
+    h = C.c_void_p(0x1234)
+    assert L.pespace_session_create(C.byref(g), C.byref(m), 0, 0, C.byref(h)) == EINVAL
+    assert not h.value                                            # *out is NULL on failure
+    bad_g = P._Grid(1e-4, 0.0, 64)
+    assert L.pespace_session_create(C.byref(bad_g), C.byref(m), 4, 0, C.byref(h)) == EINVAL
+    bad_m, keep2 = P._model(W.Model(64, wl.model.detectors))
+    assert L.pespace_session_create(C.byref(g), C.byref(bad_m), 4, 1, C.byref(h)) == EINVAL
+    assert L.pespace_session_create(C.byref(g), C.byref(m), 4, 0, None) == EINVAL
+    assert L.pespace_session_set_data(None, None, None) == EINVAL
+    assert L.pespace_session_loglike(None, None, 4, None) == EINVAL
+    assert L.pespace_session_fisher(None, None, 4, None, None) == EINVAL
+    assert L.pespace_session_destroy(None) == EINVAL
+    assert L.pespace_loglike_host(None, 4, None, None, C.byref(g), C.byref(m), None) == EINVAL

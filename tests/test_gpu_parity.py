@@ -193,6 +193,39 @@ def test_host_buffer_call_matches_device_call(P):
     assert np.array_equal(a, b)
 
 
+def test_session_matches_device_calls_and_oracle(P):
+    """pespace_session_*: host buffers in, host buffers out; same kernels, so bit-identical to the device-pointer
+    calls, and within tolerance of the oracle.  Pinned torch tensors and numpy arrays are both accepted."""
+    import torch
+    wl = W.config(4, B=37, N=1100)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    ses = P.Session(wl.grid, wl.model, 64, want_fisher=True)
+    with pytest.raises(P.PespaceError):
+        ses.loglike(wl.params)                                   # no data yet
+    ses.set_data(None, psd)
+    F0, none = ses.fisher(wl.params, with_grad=False)             # the Fisher matrix needs only the PSD
+    assert none is None
+    with pytest.raises(P.PespaceError):
+        ses.fisher(wl.params, with_grad=True)                    # the gradient needs the data
+    ses.set_data(torch.from_numpy(data).pin_memory(), None)
+    a = ses.loglike(wl.params)
+    b = P.loglike(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model).cpu().numpy()
+    assert np.array_equal(a, b)
+    want = oracle.loglike(wl.params, data, psd, wl.grid, wl.model)
+    assert np.all(np.abs(a - want) <= TOL_LNL * np.abs(want))
+    out = torch.empty(20, dtype=torch.float64).pin_memory()
+    ses.loglike(torch.from_numpy(wl.params[:20]).pin_memory(), out)   # smaller batch, pinned buffers
+    assert np.array_equal(out.numpy(), a[:20])
+    F, g = ses.fisher(wl.params)
+    Fd, gd = P.fisher(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model)
+    assert np.array_equal(F, Fd.cpu().numpy()) and np.array_equal(g, gd.cpu().numpy())
+    assert np.array_equal(F0, F)
+    with pytest.raises(P.PespaceError):
+        ses.loglike(np.tile(wl.params, (2, 1)))                  # batch larger than max_B
+    ses.close()
+    ses.close()                                                  # idempotent
+
+
 def test_error_codes_on_device(P):
     wl = W.config(2, B=4, N=64)
     data, psd = dev(wl.data(oracle_response_fn)), dev(wl.psd())
