@@ -78,13 +78,18 @@ struct ClassScal {
   Du<3> CKp, CKc;    // amplitudes, tangents (M, q, iota)
 };
 
-template <int MC>
-__device__ __forceinline__ void fisher_stage_a(const BinC& bc, const double* __restrict__ sc, double ftc4,
+// class constants, indexed by m - 1 at run time (the class loop of the Fisher kernel is NOT unrolled: the unrolled
+// body was 154 KB of code per kernel and stalled on instruction fetch, profiles/r01_fisher_kernel_ncu.md)
+__constant__ double kClassCB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
+__constant__ double kClassLN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
+__constant__ double kClassS83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
+
+__device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const double* __restrict__ sc, double ftc4,
                                                ClassScal& o) {
-  constexpr double CB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
-  constexpr double LN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
-  constexpr double S83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
-  constexpr double MH[4] = {0.5, 1.0, 1.5, 2.0};
+  const double* CB = kClassCB;
+  const double* LN3 = kClassLN3;
+  const double* S83 = kClassS83;
+  const double MHmc = 0.5 * (double)(MC + 1);
   const double sv = bc.cf * CB[MC];
   Du<4> v(0.0), L(0.0);
   v.v = cv(sc, W_A) * sv; v.d[0] = ct(sc, W_A, 0) * sv;
@@ -105,7 +110,7 @@ __device__ __forceinline__ void fisher_stage_a(const BinC& bc, const double* __r
   const double sp = S83[MC] * bc.fm53, sq = S83[MC] * bc.fm83;
   double psi = sp * P.v;
   psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);
-  o.psi = psi + fma(MH[MC], cv(sc, W_PH0), ftc4);
+  o.psi = psi + fma(MHmc, cv(sc, W_PH0), ftc4);
   o.tau = sq * Q.v;
 #pragma unroll
   for (int i = 0; i < 4; ++i) {
@@ -131,23 +136,22 @@ __device__ __forceinline__ void fisher_stage_a(const BinC& bc, const double* __r
 }
 
 // J accumulation: column of this thread in shared memory, J[(p * 6 + comp * 2 + ri) * FBLOCK]
-template <bool FIRST>
-__device__ __forceinline__ void jadd(double* J, int p, int comp, double re, double im) {
+__device__ __forceinline__ void jadd(bool first, double* J, int p, int comp, double re, double im) {
   double* a = J + ((p * 6 + comp * 2) * FBLOCK);
-  if (FIRST) { a[0] = re; a[FBLOCK] = im; }
+  if (first) { a[0] = re; a[FBLOCK] = im; }
   else { a[0] += re; a[FBLOCK] += im; }
 }
 
 // One mode class of one (sample, bin, detector): adds value and tangents of (X, Y, Z) to J.
 // Tangent order p = 1..11 follows theta: M, q, chi1, chi2, D_L, iota, phi_c, lambda, beta, psi, t_c
 // (D_L is filled in after the class loop: d h / d D_L = -h / D_L).
-template <int KIND, int MC, bool FIRST>
-__device__ __forceinline__ void fisher_class(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
-                                             double ftc4, double* __restrict__ J) {
+template <int KIND>
+__device__ __forceinline__ void fisher_class(int MC, bool FIRST, const BinC& bc, const double* __restrict__ sc,
+                                          const DetC& dc, double ftc4, double* __restrict__ J) {
   using G = Du<3>;
-  constexpr double MM[4] = {1.0, 2.0, 3.0, 4.0};
+  const double MMmc = (double)(MC + 1);
   ClassScal cs;
-  fisher_stage_a<MC>(bc, sc, ftc4, cs);
+  fisher_stage_a(MC, bc, sc, ftc4, cs);
 
   // ---- S4 on (value, d/d alpha [rad], d/d lambda, d/d beta)
   G G1k, G2k, G1u, G2u, G1v, G2v, kR;
@@ -245,30 +249,30 @@ __device__ __forceinline__ void fisher_class(const BinC& bc, const double* __res
       Tr[g] = fma(kp, Hpr.d[g], -kc * Hci.d[g]);
       Ti[g] = fma(kp, Hpi.d[g], kc * Hcr.d[g]);
     }
-    jadd<FIRST>(J, 0, comp, hr, hi);
+    jadd(FIRST, J, 0, comp, hr, hi);
     // M, q: amplitude + phase + orbit time;  chi1, chi2: phase + orbit time
 #pragma unroll
     for (int i = 0; i < 2; ++i) {
       const double ap = cs.CKp.d[i], ac = cs.CKc.d[i];
       const double re = fma(ap, Hpr.v, fma(-ac, Hci.v, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0])));
       const double im = fma(ap, Hpi.v, fma(ac, Hcr.v, fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0])));
-      jadd<FIRST>(J, 1 + i, comp, re, im);
+      jadd(FIRST, J, 1 + i, comp, re, im);
     }
 #pragma unroll
     for (int i = 2; i < 4; ++i)
-      jadd<FIRST>(J, 1 + i, comp, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0]), fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0]));
+      jadd(FIRST, J, 1 + i, comp, fma(-cs.dpsi[i], hi, cs.dtau[i] * Tr[0]), fma(cs.dpsi[i], hr, cs.dtau[i] * Ti[0]));
     // iota: amplitudes only
-    jadd<FIRST>(J, 6, comp, fma(cs.CKp.d[2], Hpr.v, -cs.CKc.d[2] * Hci.v), fma(cs.CKp.d[2], Hpi.v, cs.CKc.d[2] * Hcr.v));
+    jadd(FIRST, J, 6, comp, fma(cs.CKp.d[2], Hpr.v, -cs.CKc.d[2] * Hci.v), fma(cs.CKp.d[2], Hpi.v, cs.CKc.d[2] * Hcr.v));
     // phi_c: d psi = -m d phi_c (radians) -> -m i h
-    jadd<FIRST>(J, 7, comp, MM[MC] * hi, -MM[MC] * hr);
+    jadd(FIRST, J, 7, comp, MMmc * hi, -MMmc * hr);
     // lambda, beta
-    jadd<FIRST>(J, 8, comp, Tr[1], Ti[1]);
-    jadd<FIRST>(J, 9, comp, Tr[2], Ti[2]);
+    jadd(FIRST, J, 8, comp, Tr[1], Ti[1]);
+    jadd(FIRST, J, 9, comp, Tr[2], Ti[2]);
     // polarisation angle: d Hp = 4 Hc, d Hc = -Hp
-    jadd<FIRST>(J, 10, comp, fma(4.0 * kp, Hcr.v, kc * Hpi.v), fma(4.0 * kp, Hci.v, -kc * Hpr.v));
+    jadd(FIRST, J, 10, comp, fma(4.0 * kp, Hcr.v, kc * Hpi.v), fma(4.0 * kp, Hci.v, -kc * Hpr.v));
     // t_c: phase 2 pi f, orbit angle 2 pi / yr
     const double wp = kRadPerPu * bc.fT, wt = kRadPerPu * kTurn / kYear;
-    jadd<FIRST>(J, 11, comp, fma(-wp, hi, wt * Tr[0]), fma(wp, hr, wt * Ti[0]));
+    jadd(FIRST, J, 11, comp, fma(-wp, hi, wt * Tr[0]), fma(wp, hr, wt * Ti[0]));
   };
   // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2); same terms as eval_class
   component(0, 0, 2, -kap[1], 1, 1, kap[2], 2);    // X = W_b B(1,3,k13) - W_c B(1,2,k12)
@@ -351,8 +355,6 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
   __syncthreads();
   double* J = Jsm + threadIdx.x;
   const int ns = (int)min((long long)FTILE, B - b0);
-  constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
-
   for (int ch = 0; ch < FCHUNKS; ++ch) {
     const long long kbase = ((long long)blockIdx.x * FCHUNKS + ch) * FBLOCK;
     if (kbase >= G.N) break;
@@ -382,10 +384,15 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
       const double tc = cv(sc, W_TC);
       const double p = bc.fT * tc;
       const double ftc4 = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
-      if (c0) fisher_class<KIND, 0, true>(bc, sc, dc, ftc4, J);
-      if (c1) fisher_class<KIND, 1, !c0>(bc, sc, dc, ftc4, J);
-      if (c2) fisher_class<KIND, 2, !(c0 || c1)>(bc, sc, dc, ftc4, J);
-      if (c3) fisher_class<KIND, 3, !(c0 || c1 || c2)>(bc, sc, dc, ftc4, J);
+      {
+        bool first = true;
+#pragma unroll 1
+        for (int mc = 0; mc < 4; ++mc) {
+          if (!((CMASK >> mc) & 1u)) continue;
+          fisher_class<KIND>(mc, first, bc, sc, dc, ftc4, J);
+          first = false;
+        }
+      }
       // Gram matrix of a_0 = d - h, a_p = d_p h (p = 1..11) over the channels A, E, T
       const double mDL = cv(sc, W_MDL);      // d h / d D_L = -h / D_L
       double a[NGP];
