@@ -546,7 +546,7 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const size_t idx = ((size_t)det * 3 + c) * N + (size_t)k;
-    const double2 d = data[idx];
+    const double2 d = data ? data[idx] : make_double2(0.0, 0.0);     // no data set: Fisher matrix only
     const double Sn = psd[idx];
     const bool use = isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
     const double sc_ = use ? nrm[c] / g2 : 0.0;

@@ -9,7 +9,7 @@ namespace {
 
 struct FisherPlan {
   long long nbx, ntile;
-  size_t consts_bytes, partial_bytes;
+  size_t consts_bytes, partial_bytes, bins_bytes;     // workspace: [sample constants | block partials | per-bin table]
 };
 FisherPlan make_fisher_plan(long long B, long long N, int n_det) {
   FisherPlan p;
@@ -17,6 +17,7 @@ FisherPlan make_fisher_plan(long long B, long long N, int n_det) {
   p.ntile = (B + FTILE - 1) / FTILE;
   p.consts_bytes = align_up((size_t)B * fisher_const_stride(n_det) * sizeof(double), 256);
   p.partial_bytes = align_up((size_t)n_det * p.nbx * (size_t)B * NG * sizeof(double), 256);
+  p.bins_bytes = align_up((size_t)n_det * NBF * (size_t)N * sizeof(double), 256);
   return p;
 }
 
@@ -26,7 +27,7 @@ namespace pespace {
 namespace host {
 size_t fisher_workspace_bytes(long long B, long long N, int n_det) {
   const FisherPlan p = make_fisher_plan(B, N, n_det);
-  return p.consts_bytes + p.partial_bytes;
+  return p.consts_bytes + p.partial_bytes + p.bins_bytes;
 }
 }  // namespace host
 }  // namespace pespace
@@ -44,18 +45,25 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
   cudaStream_t st = (cudaStream_t)stream;
   double* d_consts = (double*)d_workspace;
   double* d_partial = (double*)((char*)d_workspace + p.consts_bytes);
+  double* d_bins = (double*)((char*)d_workspace + p.consts_bytes + p.partial_bytes);
   const PrepArgs A = make_prep_args(model);
   const int th = 64;
   prep_samples_du_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
   LAUNCHED();
   const unsigned cm = class_mask(model->mode_mask);
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
+  {
+    // S0: per-bin table of this data set (d_data_AET == NULL: zeros, Fisher matrix only)
+    const dim3 gb((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det);
+    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, d_bins);
+    LAUNCHED();
+  }
   const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc = prof_begin(ev, st); rc != PESPACE_OK) return rc;
-    CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, (const double2*)d_data_AET, d_psd, G, dc, model->n_det, d, d_partial));
+    CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, d_bins, G.N, dc, model->n_det, d, d_partial));
     LAUNCHED();
     if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }

@@ -17,7 +17,7 @@
 // tile of FTILE samples.  The 12 x 3 complex numbers (value + 11 tangents of X, Y, Z) of one (sample, bin)
 // are accumulated over the mode classes in shared memory (thread-private columns), then the upper triangle
 // of the 12 x 12 Gram matrix of (residual, d_1 h, ..., d_11 h) -- 78 numbers -- is formed per thread and
-// reduced over the warp by a halving butterfly (93 shuffles instead of 78 x 5), fixed order throughout.
+// reduced over the warp by a halving butterfly (96 shuffles instead of 78 x 5), fixed order throughout.
 #pragma once
 #include "pespace_device.cuh"
 
@@ -29,7 +29,7 @@ constexpr int FCHUNKS = 16;   // chunks per block
 constexpr int NT = 12;        // value + 11 tangents
 constexpr int NJ = NT * 6;    // x (X, Y, Z) x (re, im)
 constexpr int NG = 78;        // upper triangle of the 12 x 12 Gram matrix
-constexpr int NGP = 96;       // padded to 3 x 32 for the butterfly
+constexpr int NGP = 96;       // padded: two passes of 48 accumulators
 constexpr int DUW = 8;        // doubles per constant: value + tangents (M, q, chi1, chi2, iota, lambda, beta)
 constexpr int FS_STRIDE = SMEM_STRIDE * DUW;   // one sample, one detector, in shared memory
 
@@ -322,10 +322,16 @@ __device__ __forceinline__ void stage_tile_du(double* smem, const double* __rest
 // index of (p, q), p <= q, in the packed upper triangle of the 12 x 12 Gram matrix
 __host__ __device__ constexpr int gram_index(int p, int q) { return p * NT - p * (p - 1) / 2 + (q - p); }
 
-// Halving butterfly: on entry every lane holds NGP values; on exit lane l holds, in a[0..2], the sums over the
-// warp of the values with index  j + 48 b4 + 24 b3 + 12 b2 + 6 b1 + 3 b0  (b_i = bit i of l), j = 0..2.
+// The 78 Gram entries are formed in two passes over J (rows 0..3: 42 entries, rows 4..11: 36 entries) so that at
+// most NGH = 48 accumulators are live at a time (one pass over all 78 needed 255 registers and spilled).
+constexpr int NGH = 48;                 // accumulators per pass (42 and 36 used)
+constexpr int GRAM_SPLIT = 4;           // first row of the second pass
+static_assert(NGP == 2 * NGH, "two passes");
+
+// Halving butterfly over NGH values per lane: after the four halving levels lane l holds, in a[0..2], partial sums
+// of the entries  j + 24 b4 + 12 b3 + 6 b2 + 3 b1  (b_i = bit i of l), j = 0..2; the last level adds lanes l, l ^ 1.
 template <int HALF, int OFF>
-__device__ __forceinline__ void butterfly_level(double (&a)[NGP], int lane) {
+__device__ __forceinline__ void butterfly_level(double (&a)[NGH], int lane) {
   const bool up = lane & OFF;
 #pragma unroll
   for (int i = 0; i < HALF; ++i) {
@@ -334,16 +340,65 @@ __device__ __forceinline__ void butterfly_level(double (&a)[NGP], int lane) {
     a[i] = keep + __shfl_xor_sync(0xffffffffu, send, OFF);
   }
 }
-__host__ __device__ inline int butterfly_slot_index(int lane, int j) {
-  return j + 48 * ((lane >> 4) & 1) + 24 * ((lane >> 3) & 1) + 12 * ((lane >> 2) & 1) + 6 * ((lane >> 1) & 1) +
-         3 * (lane & 1);
+// slot (pass, l16 = lane >> 1, j) of the per-warp partials -> packed Gram index, or -1 for padding
+__host__ __device__ inline int butterfly_slot_index(int slot) {
+  const int pass = slot / NGH, r = slot % NGH, l16 = r / 3, j = r % 3;
+  const int li = j + 24 * ((l16 >> 3) & 1) + 12 * ((l16 >> 2) & 1) + 6 * ((l16 >> 1) & 1) + 3 * (l16 & 1);
+  const int base = pass == 0 ? 0 : gram_index(GRAM_SPLIT, GRAM_SPLIT);
+  const int count = pass == 0 ? gram_index(GRAM_SPLIT, GRAM_SPLIT) : NG - gram_index(GRAM_SPLIT, GRAM_SPLIT);
+  return li < count ? base + li : -1;
+}
+
+// Rows P0..P1-1 of the Gram matrix of a_0 = d - h, a_p = d_p h (p = 1..11) over the channels A, E, T for this
+// thread's bin, reduced over the warp and added to the warp's partials r[NGH] (slot order of butterfly_slot_index).
+template <int P0, int P1>
+__device__ __forceinline__ void gram_rows(const double* __restrict__ J, const double (&dr)[3], const double (&di)[3],
+                                          const double (&w)[3], double mDL, int lane, double* __restrict__ r) {
+  double a[NGH];
+#pragma unroll
+  for (int i = 0; i < NGH; ++i) a[i] = 0.0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double ar[NT], ai[NT];
+#pragma unroll
+    for (int pp = 0; pp < NT; ++pp) {
+      if (pp == 5) continue;                                  // D_L: from the value, below
+      if (pp < P0 && !(pp == 0 && P0 <= 5)) continue;         // not needed by this pass
+      const double* jp = J + pp * 6 * FBLOCK;
+      const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
+                   zi = jp[5 * FBLOCK];
+      if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
+      else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
+      else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
+    }
+    if (P0 <= 5) { ar[5] = mDL * ar[0]; ai[5] = mDL * ai[0]; }   // d h / d D_L = -h / D_L
+    if (P0 == 0) { ar[0] = dr[c] - ar[0]; ai[0] = di[c] - ai[0]; }
+#pragma unroll
+    for (int pp = P0; pp < P1; ++pp) {
+      const double wr = w[c] * ar[pp], wi = w[c] * ai[pp];
+#pragma unroll
+      for (int q = pp; q < NT; ++q) {
+        const int li = gram_index(pp, q) - gram_index(P0, P0);
+        a[li] = fma(wr, ar[q], fma(wi, ai[q], a[li]));
+      }
+    }
+  }
+  butterfly_level<24, 16>(a, lane);
+  butterfly_level<12, 8>(a, lane);
+  butterfly_level<6, 4>(a, lane);
+  butterfly_level<3, 2>(a, lane);
+#pragma unroll
+  for (int j = 0; j < 3; ++j) a[j] += __shfl_xor_sync(0xffffffffu, a[j], 1);
+  if (!(lane & 1)) {
+    double* rr = r + (lane >> 1) * 3;
+    rr[0] += a[0]; rr[1] += a[1]; rr[2] += a[2];
+  }
 }
 
 template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(FBLOCK, 2)
-fisher_kernel(const double* __restrict__ consts, long long B, const double2* __restrict__ data /* may be null */,
-              const double* __restrict__ psd, GridC G, DetC dc, int n_det, int det,
-              double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
+fisher_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ bins /* [n_det][NBF][N] */,
+              long long N, DetC dc, int n_det, int det, double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
   extern __shared__ double fsm[];
   double* Jsm = fsm;                                   // [NJ][FBLOCK]
   double* csm = Jsm + NJ * FBLOCK;                     // [FTILE][SMEM_STRIDE][DUW]
@@ -357,27 +412,18 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
   const int ns = (int)min((long long)FTILE, B - b0);
   for (int ch = 0; ch < FCHUNKS; ++ch) {
     const long long kbase = ((long long)blockIdx.x * FCHUNKS + ch) * FBLOCK;
-    if (kbase >= G.N) break;
+    if (kbase >= N) break;
     const long long k = kbase + threadIdx.x;
-    const bool live = k < G.N;
-    const long long kk = live ? k : G.N - 1;
-    const BinC bc = make_bin(fma((double)kk, G.df, G.f0), dc.Lbar);
-    double gr, gi;
-    tdi_prefactor(bc, dc.gen, gr, gi);
-    const double g2 = gr * gr + gi * gi;
-    const double nrm[3] = {1.4142135623730950488, 2.4494897427831780982, 1.7320508075688772935};
+    const bool live = k < N;
+    const double* bp = bins + (size_t)det * NBF * (size_t)N + (size_t)(live ? k : N - 1);
+    BinC bc;
+    bc.fT = bp[BF_FT * N]; bc.cf = bp[BF_CF * N]; bc.lnf3 = bp[BF_LNF3 * N]; bc.fm53 = bp[BF_FM53 * N];
+    bc.fm83 = bp[BF_FM83 * N]; bc.sth = bp[BF_STH * N]; bc.cth = bp[BF_CTH * N]; bc.fm76 = 0.0;
     double dr[3], di[3], w[3];
 #pragma unroll
     for (int c = 0; c < 3; ++c) {
-      const size_t idx = ((size_t)det * 3 + c) * (size_t)G.N + (size_t)kk;
-      double2 d = make_double2(0.0, 0.0);
-      if (data) d = data[idx];
-      const double Sn = psd[idx];
-      const bool use = live && isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
-      const double sc_ = use ? nrm[c] / g2 : 0.0;
-      dr[c] = (d.x * gr + d.y * gi) * sc_;
-      di[c] = (d.x * gi - d.y * gr) * sc_;
-      w[c] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+      dr[c] = bp[(BF_DR + c) * N]; di[c] = bp[(BF_DI + c) * N];
+      w[c] = live ? bp[(BF_W + c) * N] : 0.0;
     }
     for (int s = 0; s < ns; ++s) {
       const double* sc = csm + s * FS_STRIDE;
@@ -393,50 +439,17 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double2* __r
           first = false;
         }
       }
-      // Gram matrix of a_0 = d - h, a_p = d_p h (p = 1..11) over the channels A, E, T
-      const double mDL = cv(sc, W_MDL);      // d h / d D_L = -h / D_L
-      double a[NGP];
-#pragma unroll
-      for (int i = 0; i < NGP; ++i) a[i] = 0.0;
-#pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        double ar[NT], ai[NT];
-#pragma unroll
-        for (int pp = 0; pp < NT; ++pp) {
-          if (pp == 5) continue;
-          const double* jp = J + pp * 6 * FBLOCK;
-          const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
-                       zi = jp[5 * FBLOCK];
-          if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
-          else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
-          else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
-        }
-        ar[5] = mDL * ar[0]; ai[5] = mDL * ai[0];
-        ar[0] = dr[c] - ar[0]; ai[0] = di[c] - ai[0];
-#pragma unroll
-        for (int pp = 0; pp < NT; ++pp) {
-          const double wr = w[c] * ar[pp], wi = w[c] * ai[pp];
-#pragma unroll
-          for (int q = pp; q < NT; ++q) {
-            const int gi_ = gram_index(pp, q);
-            a[gi_] = fma(wr, ar[q], fma(wi, ai[q], a[gi_]));
-          }
-        }
-      }
-      butterfly_level<48, 16>(a, lane);
-      butterfly_level<24, 8>(a, lane);
-      butterfly_level<12, 4>(a, lane);
-      butterfly_level<6, 2>(a, lane);
-      butterfly_level<3, 1>(a, lane);
-      double* r = red + ((warp * FTILE + s) * NGP + lane * 3);
-      r[0] += a[0]; r[1] += a[1]; r[2] += a[2];
+      const double mDL = cv(sc, W_MDL);
+      double* r = red + (warp * FTILE + s) * NGP;
+      gram_rows<0, GRAM_SPLIT>(J, dr, di, w, mDL, lane, r);
+      gram_rows<GRAM_SPLIT, NT>(J, dr, di, w, mDL, lane, r + NGH);
     }
   }
   __syncthreads();
-  // cross-warp sum in fixed order; thread t < 96 owns slot (lane = t / 3, j = t % 3)
+  // cross-warp sum in fixed order; thread t < 96 owns slot t of the per-warp partials
   if (threadIdx.x < NGP) {
-    const int gidx = butterfly_slot_index(threadIdx.x / 3, threadIdx.x % 3);
-    if (gidx < NG) {
+    const int gidx = butterfly_slot_index(threadIdx.x);
+    if (gidx >= 0) {
       for (int s = 0; s < ns; ++s) {
         double t = 0.0;
 #pragma unroll
