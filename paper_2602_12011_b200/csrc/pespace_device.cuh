@@ -47,7 +47,7 @@ constexpr double kMagic = 6755399441055744.0;    // 1.5 * 2^52: x + kMagic round
 // ---- per-sample constant block (doubles)
 enum : int {
   W_A = 0,      // (pi Ms)^{1/3}
-  W_LNA,        // ln of it
+  W_LNA,        // ln of it (kept for reference: the kernels use the folded W_P5, W_P6, W_Q6 below)
   W_TC,         // t_c
   W_PH0,        // -(phi_c/pi + 1/8): constant phase of the (2,2) mode in turns
   W_P0, W_P2, W_P3, W_P4, W_P5, W_P5L, W_P6, W_P6L, W_P7,   // phase polynomial (turns * f'^{5/3})
@@ -280,7 +280,7 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
     const double uu = ul[l], vv = vl[l];
     const double v2_ = vv * vv;
     const double D = fma(uu, uu, v2_);
-    const double rD = (D > 0.0) ? rcp_pos(D) : 0.0;
+    const double rD = (__double2hiint(D) > 0) ? rcp_pos(D) : 0.0;   // D >= 0: sign/exponent test on the ALU pipe
     Wr[l] = (CKp * rD) * fma(uu, uu, -v2_);
     Wi[l] = (CKc * rD) * (uu * vv);
   }
@@ -328,7 +328,7 @@ __device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restric
   // kTurn f t_c in pu mod one turn, with the rounding error of the product recovered by fma
   const double p = bc.fT * tc;
   const double ftc = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
-  const double va = sc[W_A] * bc.cf, La = sc[W_LNA] + bc.lnf3;
+  const double va = sc[W_A] * bc.cf, La = bc.lnf3;     // ln (pi Ms)^{1/3} is folded into W_P5, W_P6, W_Q6
   constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
   if (c0) eval_class<KIND, 0, true, TAB>(bc, sc, dc, tab, va, La, ftc, S);
   if (c1) eval_class<KIND, 1, !c0, TAB>(bc, sc, dc, tab, va, La, ftc, S);
@@ -372,7 +372,8 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   const T mu1 = q / (1.0 + q), mu2 = 1.0 / (1.0 + q);
   const T Ds = DL * (kGpc / kC);
   const T a = p_cbrt(kPi * Ms);
-  put(W_A, a); put(W_LNA, p_log(a)); put(W_TC, tc);
+  const T lna = p_log(a);
+  put(W_A, a); put(W_LNA, lna); put(W_TC, tc);
   put(W_PH0, -kTurn * (phic / kPi + 0.125));            // pu, for m/2 = 1
   put(W_VALID, T(1.0));
   // TaylorF2 3.5PN coefficients, spin terms per G3
@@ -391,10 +392,14 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   const T a5 = 1.0 / (a * a * a * a * a);
   const T cP = kTurn * 3.0 / (256.0 * kPi * eta) * a5;  // kTurn Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
   put(W_P0, cP); put(W_P2, cP * ph2); put(W_P3, cP * ph3); put(W_P4, cP * ph4);
-  put(W_P5, cP * ph5a); put(W_P5L, cP * 3.0 * ph5a); put(W_P6, cP * ph6a); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
+  // ln v = ln (pi Ms)^{1/3} + ln f'^{1/3}: the sample part of the logarithm is folded into the constant terms, so
+  // the kernels multiply the *L coefficients by ln f'^{1/3} only (one add less per bin, no tangent on L)
+  put(W_P5, cP * ph5a + cP * 3.0 * ph5a * lna); put(W_P5L, cP * 3.0 * ph5a);
+  put(W_P6, cP * ph6a + cP * ph6l * lna); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
   const T cQ = cP / (3.0 * kYear);                       // kTurn (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
   put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
-  put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l)); put(W_Q6L, cQ * ph6l); put(W_Q7, 2.0 * cQ * ph7);
+  put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l) + cQ * ph6l * lna); put(W_Q6L, cQ * ph6l);
+  put(W_Q7, 2.0 * cQ * ph7);
   // amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
   const T amp0 = p_sqrt(2.0 * eta / 3.0) * 0.82630748711075811083 * (Ms * Ms / Ds) / (Ms * p_sqrt(p_cbrt(Ms)));
   const double s57 = sqrt(5.0 / 7.0);
@@ -557,7 +562,7 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
 }
 
 // K_main: grid (bin blocks, sample tiles); one launch per detector.
-constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1) + ((m >> 3) & 1); }
+__host__ __device__ constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1) + ((m >> 3) & 1); }
 
 template <int KIND, unsigned CMASK>
 #ifndef PESPACE_MINB1
@@ -590,7 +595,8 @@ loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ tr
 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ns = (int)min((long long)TILE, B - b0);
-  for (int s = 0; s < ns; ++s) {
+  // weighted |d - h|^2 of this thread's bin for sample s of the tile (S8)
+  auto term = [&](int s) {
     double S[6];
     eval_xyz<KIND, CMASK, true>(bc, smem + s * SMEM_STRIDE, dc, tab, S);
     const double Ar = S[4] - S[0], Ai = S[5] - S[1];                         // Z - X
@@ -601,10 +607,32 @@ loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ tr
     r0 = dr[1] - Er_; r1 = di[1] - Ei_;
     acc = fma(w[1], fma(r0, r0, r1 * r1), acc);
     r0 = dr[2] - Tr; r1 = di[2] - Ti;
-    acc = fma(w[2], fma(r0, r0, r1 * r1), acc);
+    return fma(w[2], fma(r0, r0, r1 * r1), acc);
+  };
+  if constexpr (popc4(CMASK) == 1) {
+    // S9, single-class kernels: four samples per trip, reduced over the warp by a halving butterfly (two halving
+    // levels, then three plain ones on ONE value: 6 shuffle-adds per 4 samples instead of 20).  After the halving
+    // levels the lanes with bits (4, 3) = (b4, b3) hold sample 2 b4 + b3 of the group.  The tile is staged with its
+    // tail clamped to sample B - 1 (stage_tile), so a ragged last group evaluates valid constants; only s < ns is kept.
+    for (int s0 = 0; s0 < ns; s0 += 4) {
+      double a[4];
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) red[warp][s] = acc;
+      for (int j = 0; j < 4; ++j) a[j] = term(s0 + j);
+      const bool up4 = lane & 16, up3 = lane & 8;
+      const double k0 = (up4 ? a[2] : a[0]) + __shfl_xor_sync(0xffffffffu, up4 ? a[0] : a[2], 16);
+      const double k1 = (up4 ? a[3] : a[1]) + __shfl_xor_sync(0xffffffffu, up4 ? a[1] : a[3], 16);
+      double acc = (up3 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, up3 ? k0 : k1, 8);
+#pragma unroll
+      for (int o = 4; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if ((lane & 7) == 0) red[warp][s0 + (lane >> 3)] = acc;     // s0 + j < TILE always; slots >= ns are never read
+    }
+  } else {
+    for (int s = 0; s < ns; ++s) {
+      double acc = term(s);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if (lane == 0) red[warp][s] = acc;
+    }
   }
   __syncthreads();
   if (threadIdx.x < ns) {

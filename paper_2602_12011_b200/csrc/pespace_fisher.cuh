@@ -91,17 +91,17 @@ __device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const dou
   const double* S83 = kClassS83;
   const double MHmc = 0.5 * (double)(MC + 1);
   const double sv = bc.cf * CB[MC];
-  Du<4> v(0.0), L(0.0);
+  Du<4> v(0.0);
   v.v = cv(sc, W_A) * sv; v.d[0] = ct(sc, W_A, 0) * sv;
-  L.v = cv(sc, W_LNA) + bc.lnf3 + LN3[MC]; L.d[0] = ct(sc, W_LNA, 0);
+  const double L = bc.lnf3 + LN3[MC];       // ln (pi Ms)^{1/3} and its tangent are folded into W_P5, W_P6, W_Q6
   const Du<4> v2 = v * v;
-  Du<4> P = dfma(c4(sc, W_P7), v, dfma(c4(sc, W_P6L), L, c4(sc, W_P6)));
-  P = dfma(P, v, dfma(c4(sc, W_P5L), L, c4(sc, W_P5)));
+  Du<4> P = dfma(c4(sc, W_P7), v, dfma(L, c4(sc, W_P6L), c4(sc, W_P6)));
+  P = dfma(P, v, dfma(L, c4(sc, W_P5L), c4(sc, W_P5)));
   P = dfma(P, v, c4(sc, W_P4));
   P = dfma(P, v, c4(sc, W_P3));
   P = dfma(P, v, c4(sc, W_P2));
   P = dfma(P, v2, c4(sc, W_P0));
-  Du<4> Q = dfma(c4(sc, W_Q7), v, dfma(c4(sc, W_Q6L), L, c4(sc, W_Q6)));
+  Du<4> Q = dfma(c4(sc, W_Q7), v, dfma(L, c4(sc, W_Q6L), c4(sc, W_Q6)));
   Q = dfma(Q, v, c4(sc, W_Q5));
   Q = dfma(Q, v, c4(sc, W_Q4));
   Q = dfma(Q, v, c4(sc, W_Q3));
@@ -204,7 +204,7 @@ __device__ __forceinline__ void fisher_class(int MC, bool FIRST, const BinC& bc,
     const G v2_ = vv * vv;
     const G D = dfma(uu, uu, v2_);
     G rD;
-    rD.v = (D.v > 0.0) ? rcp_pos(D.v) : 0.0;
+    rD.v = (__double2hiint(D.v) > 0) ? rcp_pos(D.v) : 0.0;
     const double m2 = -rD.v * rD.v;
 #pragma unroll
     for (int i = 0; i < 3; ++i) rD.d[i] = m2 * D.d[i];
