@@ -43,23 +43,25 @@ from paper_2602_12011_b200 import workloads as W         # noqa: E402
 # operands, the common case in this kernel) ~66 % (profiles/r01_fp64_operand_bandwidth.md).
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # FP64 operations of loglike_kernel per (sample, bin, detector), thread level, counted by ncu
-# (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / (B*N), profiles/r01_loglike_kernel_ncu.md).
+# (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / (B*N), profiles/r01_kernels_ncu.md).
 # They equal the operation list of the reduced formulas in DESIGN.md ("Algorithmic work") to <1 %; the
 # kernel has no redundant evaluation, so executed = algorithmic.  flop = 2*DFMA + DMUL + DADD.
 FP64_OPS_PER_UNIT = {
-    # (kernel, detector kind, mode-class mask): per (sample, bin, detector)
-    ("loglike", 0, 2): {"dfma": 169.17, "dmul": 59.88, "dadd": 35.27},      # kind 0, (2,2) only  -- config 2
-    ("loglike", 0, 15): {"dfma": 661.17, "dmul": 215.88, "dadd": 68.27},    # kind 0, five modes  -- configs 3, 4
-    ("loglike", 1, 15): None,                                               # kind 1, five modes  -- config 4
-    ("fisher", 0, 15): None,                                                # config 5
-    ("fisher", 1, 15): None,
+    # (kernel, detector kind, mode-class mask): per (sample, bin, detector); profiles/r01_kernels_ncu.md
+    ("loglike", 0, 2): {"dfma": 143.00, "dmul": 55.50, "dadd": 41.53},      # kind 0, (2,2) only  -- config 2
+    ("loglike", 0, 15): {"dfma": 563.00, "dmul": 198.03, "dadd": 104.05},   # kind 0, five modes  -- configs 3, 4
+    ("loglike", 1, 15): {"dfma": 535.00, "dmul": 234.03, "dadd": 113.05},   # kind 1, five modes  -- config 4
+    ("fisher", 0, 15): {"dfma": 3439.00, "dmul": 1435.25, "dadd": 829.15},  # config 5
+    ("fisher", 1, 15): {"dfma": 3275.00, "dmul": 1495.25, "dadd": 785.15},
 }
-# dram__bytes_read.sum + dram__bytes_write.sum of one loglike_kernel launch (same ncu capture)
-DRAM_TRAFFIC_PER_LAUNCH = {2: 21.03e6 + 0.86e6, 3: 21.54e6 + 33.45e6}
+# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (same ncu captures; config 4:
+# mean of the three launches of a step)
+DRAM_TRAFFIC_PER_LAUNCH = {2: 36.17e6 + 6.58e6, 3: 44.92e6 + 63.97e6, 4: (53.3e6 + 140.3e6 + 63.9e6 + 141.3e6 + 42.6e6 + 44.4e6) / 3,
+                           5: 35.2e6 + 3.8e6}
 # SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
 # kept for reference only -- the reduced algorithm needs less than half of it.
 SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0, 5: 100000.0}
-OPS_SOURCE = "profiles/r01_loglike_kernel_ncu.md"
+OPS_SOURCE = "profiles/r01_kernels_ncu.md"
 METRIC, UNIT = "lnL_evals_per_sec", "lnL/s"
 FISHER_METRIC, FISHER_UNIT = "fisher_evals_per_sec", "F/s"     # --config 5 only (S10: F and grad per sample)
 
