@@ -49,6 +49,11 @@ def lib():
         L.pespace_oracle_orbit.argtypes = [C.POINTER(_Det), C.c_double, dp]
         L.pespace_oracle_links.argtypes = [dp, C.c_int, C.c_int, C.c_double, C.POINTER(_Det), dp]
         L.pespace_oracle_tdi.argtypes = [dp, C.c_double, C.c_double, C.c_int, dp]
+        i64 = C.c_int64
+        L.pespace_oracle_response_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, i64, C.POINTER(_Model), dp]
+        L.pespace_oracle_loglike_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, dp, C.POINTER(_Grid),
+                                                 C.POINTER(_Model), dp]
+        L.pespace_oracle_tab_waveform.argtypes = [i64, dp, dp, dp, dp, dp, i64, dp, dp, dp]
         L.pespace_oracle_set_threads.argtypes = [C.c_int]
         L.pespace_oracle_set_threads.restype = None
         _lib = L
@@ -126,6 +131,53 @@ def fisher(params, data, psd, grid, model):
     _check(lib().pespace_oracle_fisher(_dp(p), B, _dp(d), _dp(s), C.byref(g), C.byref(m), _dp(F), _dp(grad)),
            "fisher")
     return F, grad
+
+
+def _table(table, B, model):
+    """table = (fnodes [K], amp, phase, tf each [B][n_modes][K]) -> contiguous float64 arrays, K"""
+    fn, a, ph, tf = (_f64(x) for x in table)
+    nm = bin(int(model.mode_mask)).count("1")
+    K = fn.shape[0]
+    for x in (a, ph, tf):
+        if x.shape != (B, nm, K):
+            raise ValueError(f"table arrays must be [B={B}][n_modes={nm}][K={K}], got {x.shape}")
+    return fn, a, ph, tf, K
+
+
+def response_tab(params, table, freqs, model) -> np.ndarray:
+    """T1: response from tabulated mode waveforms; complex128 [B][n_det][3][N]"""
+    p, f = _f64(np.atleast_2d(params)), _f64(freqs)
+    m, keep = _model(model)
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    fn, a, ph, tf, K = _table(table, B, model)
+    out = np.empty((B, nd, 3, N, 2), dtype=np.float64)
+    _check(lib().pespace_oracle_response_tab(_dp(p), B, K, _dp(fn), _dp(a), _dp(ph), _dp(tf), _dp(f), N, C.byref(m),
+                                             _dp(out)), "response_tab")
+    return out.view(np.complex128)[..., 0]
+
+
+def loglike_tab(params, table, data, psd, grid, model) -> np.ndarray:
+    """T1: lnL [B] from tabulated mode waveforms"""
+    p = _f64(np.atleast_2d(params))
+    d = np.ascontiguousarray(data, dtype=np.complex128).view(np.float64)
+    s = _f64(psd)
+    m, keep = _model(model)
+    g = _Grid(float(grid.f0), float(grid.df), int(grid.N))
+    B = p.shape[0]
+    fn, a, ph, tf, K = _table(table, B, model)
+    out = np.empty(B, dtype=np.float64)
+    _check(lib().pespace_oracle_loglike_tab(_dp(p), B, K, _dp(fn), _dp(a), _dp(ph), _dp(tf), _dp(d), _dp(s), C.byref(g),
+                                            C.byref(m), _dp(out)), "loglike_tab")
+    return out
+
+
+def tab_waveform(fnodes, amp, phase, tf, freqs):
+    """T1: the interpolants of one (sample, mode) table at freqs -> (A, Psi, t_f); NaN outside the table"""
+    fn, a, ph, t, f = (_f64(x) for x in (fnodes, amp, phase, tf, freqs))
+    oa, op, ot = (np.empty_like(f) for _ in range(3))
+    _check(lib().pespace_oracle_tab_waveform(fn.shape[0], _dp(fn), _dp(a), _dp(ph), _dp(t), _dp(f), f.shape[0], _dp(oa),
+                                             _dp(op), _dp(ot)), "tab_waveform")
+    return oa, op, ot
 
 
 def waveform(theta, l, m, freqs):

@@ -352,17 +352,23 @@ template <class T> void aet(const Cx<T> XYZ[3], Cx<T> AET[3]) {
 }
 
 // six links of one mode at one frequency for one detector
-template <class T> bool mode_links(const Source<T>& s, const Frame<T>& F, int l, int m, double f,
-                                   const pespace_oracle_detector& D, Cx<T> y[6]) {
-  T amp, psi, tf;
-  if (!mode_waveform(s, l, m, f, &amp, &psi, &tf)) return false;
+// six links of one mode from its amplitude, phase and time-frequency map at f
+template <class T> void links_from_waveform(const T& iota, const Frame<T>& F, int l, int m, double f, const T& amp,
+                                            const T& psi, const T& tf, const pespace_oracle_detector& D, Cx<T> y[6]) {
   const Cx<T> hlm = scale(expi(-psi), amp);                                // h_lm = A e^{-i Psi}
   Cx<T> Kp, Kc;
-  mode_polarisation(l, m, s.iota, &Kp, &Kc);
+  mode_polarisation(l, m, iota, &Kp, &Kc);
   V3<T> centre, off[3];
   orbit(D, tf, &centre, off);                                              // geometry at t = t_lm(f)
   const int R[6] = {0, 1, 0, 2, 1, 2}, S[6] = {1, 0, 2, 0, 2, 1};
   for (int i = 0; i < 6; ++i) y[i] = single_link(T(f), D.L_m, F, centre, off, R[i], S[i], Kp, Kc, hlm);
+}
+
+template <class T> bool mode_links(const Source<T>& s, const Frame<T>& F, int l, int m, double f,
+                                   const pespace_oracle_detector& D, Cx<T> y[6]) {
+  T amp, psi, tf;
+  if (!mode_waveform(s, l, m, f, &amp, &psi, &tf)) return false;
+  links_from_waveform(s.iota, F, l, m, f, amp, psi, tf, D, y);
   return true;
 }
 
@@ -435,6 +441,95 @@ int response_impl(const double* params, int64_t B, const double* freqs, int64_t 
   return 0;
 }
 
+// ---------------------------------------------------------------- T1: tabulated waveforms
+// The paper's pipeline hands per-mode amplitude, phase and t_f from the waveform generator to the response
+// (PAPER.md:151-157).  Here they arrive as tables on K shared nodes f_0 < ... < f_{K-1}, per sample and per mode of
+// the mask (bit order), for the reference extrinsic values t_c = 0, phi_c = 0, D_L = 1 Gpc (reading T1):
+//   Psi_lm(f) = Psi_tab(f) + 2 pi f t_c - m phi_c,   t_lm(f) = t_tab(f) + t_c,   A_lm(f) = A_tab(f) / D_L[Gpc].
+// Between nodes: Psi_tab is the cubic Hermite interpolant of the node values with node slopes 2 pi t_j (Eq. 4),
+// t_tab is (1/2pi) times the derivative of that interpolant, A_tab the cubic Lagrange polynomial through the four
+// nodes j-1..j+2 around the interval (stencil shifted to stay inside the table).  Outside [f_0, f_{K-1}] the mode is 0.
+struct WaveTable { int64_t K; const double *fn, *amp, *psi, *tf; int n_modes; };
+
+// interval index j with fn[j] <= f <= fn[j+1] (largest such j, at most K-2); -1 outside the table
+int64_t tab_interval(const WaveTable& W, double f) {
+  if (!(f >= W.fn[0]) || !(f <= W.fn[W.K - 1])) return -1;
+  int64_t lo = 0, hi = W.K - 1;                       // invariant: fn[lo] <= f, f <= fn[hi]
+  while (hi - lo > 1) {
+    const int64_t mid = (lo + hi) / 2;
+    if (W.fn[mid] <= f) lo = mid; else hi = mid;
+  }
+  return lo;
+}
+
+bool tab_waveform(const WaveTable& W, int64_t b, int imode, double f, double* amp, double* psi, double* tf) {
+  const int64_t j = tab_interval(W, f);
+  if (j < 0) return false;
+  const size_t base = ((size_t)b * W.n_modes + imode) * (size_t)W.K;
+  const double *P = W.psi + base, *Tt = W.tf + base, *A = W.amp + base;
+  const double h = W.fn[j + 1] - W.fn[j], s = (f - W.fn[j]) / h;
+  const double twopi = 2.0 * K<double>::pi();
+  // cubic Hermite basis and its derivative in s
+  const double h00 = (1.0 + 2.0 * s) * (1.0 - s) * (1.0 - s), h10 = s * (1.0 - s) * (1.0 - s);
+  const double h01 = s * s * (3.0 - 2.0 * s), h11 = s * s * (s - 1.0);
+  const double d00 = 6.0 * s * (s - 1.0), d10 = (1.0 - s) * (1.0 - 3.0 * s), d01 = -d00, d11 = s * (3.0 * s - 2.0);
+  *psi = h00 * P[j] + h01 * P[j + 1] + h * twopi * (h10 * Tt[j] + h11 * Tt[j + 1]);
+  *tf = (d00 * P[j] + d01 * P[j + 1]) / (h * twopi) + d10 * Tt[j] + d11 * Tt[j + 1];
+  int64_t j0 = j - 1;
+  if (j0 < 0) j0 = 0;
+  if (j0 > W.K - 4) j0 = W.K - 4;
+  double a = 0.0;
+  for (int i = 0; i < 4; ++i) {                       // Lagrange form
+    double w = 1.0;
+    for (int q = 0; q < 4; ++q)
+      if (q != i) w *= (f - W.fn[j0 + q]) / (W.fn[j0 + i] - W.fn[j0 + q]);
+    a += w * A[j0 + i];
+  }
+  *amp = a;
+  return true;
+}
+
+bool tab_sample_ok(const double* th) {                // M, q, chi1, chi2 are not used by the tabulated path
+  for (int i = 4; i < NPAR; ++i) if (!std::isfinite(th[i])) return false;
+  return th[4] > 0.0;
+}
+bool table_ok(const WaveTable& W) {
+  if (W.K < 4 || !W.fn || !W.amp || !W.psi || !W.tf) return false;
+  for (int64_t j = 0; j + 1 < W.K; ++j) if (!(W.fn[j + 1] > W.fn[j])) return false;
+  return W.fn[0] > 0.0;
+}
+
+// A, E, T of one detector at one frequency from the tables, summed over the modes of the mask
+void response_bin_tab(const WaveTable& W, int64_t b, const double* th, const Frame<double>& F, double f,
+                      uint32_t mode_mask, const pespace_oracle_detector& D, Cx<double> AET[3]) {
+  for (int c = 0; c < 3; ++c) AET[c] = cx<double>(0.0, 0.0);
+  const double DL = th[4], iota = th[5], phic = th[6], tc = th[10];
+  int imode = 0;
+  for (int im = 0; im < 5; ++im) {
+    if (!(mode_mask & (1u << im))) continue;
+    const int l = MODE_TABLE[im].l, m = MODE_TABLE[im].m;
+    double a, p, t;
+    if (tab_waveform(W, b, imode, f, &a, &p, &t)) {
+      const double amp = a / DL;
+      const double psi = p + 2.0 * K<double>::pi() * f * tc - (double)m * phic;
+      const double tf = t + tc;
+      Cx<double> y[6], XYZ[3], ch[3];
+      links_from_waveform(iota, F, l, m, f, amp, psi, tf, D, y);
+      tdi_xyz(y, f, D.L_m, D.tdi_gen, XYZ);
+      aet(XYZ, ch);
+      for (int c = 0; c < 3; ++c) AET[c] = AET[c] + ch[c];
+    }
+    ++imode;
+  }
+}
+
+Frame<double> tab_frame(const double* th) {
+  Source<double> s = Source<double>();
+  s.lam = th[7]; s.bet = th[8]; s.psi = th[9];
+  return make_frame(s);
+}
+int popcount5(uint32_t m) { int n = 0; for (int i = 0; i < 5; ++i) n += (m >> i) & 1u; return n; }
+
 }  // namespace
 
 // =================================================================== C ABI
@@ -456,6 +551,82 @@ int pespace_oracle_response(const double* params, int64_t B, const double* freqs
 int pespace_oracle_response_quad(const double* params, int64_t B, const double* freqs, int64_t N,
                                  const pespace_oracle_model* model, double* out_AET) {
   return response_impl<quad>(params, B, freqs, N, model, out_AET);
+}
+
+// T1: response and likelihood from tabulated mode waveforms (see the T1 block above)
+int pespace_oracle_response_tab(const double* params, int64_t B, int64_t K, const double* fnodes, const double* amp,
+                                const double* phase, const double* tf, const double* freqs, int64_t N,
+                                const pespace_oracle_model* model, double* out) {
+  if (!params || !freqs || !out || B <= 0 || N <= 0 || !model_ok(model)) return -1;
+  const WaveTable W = {K, fnodes, amp, phase, tf, popcount5(model->mode_mask)};
+  if (!table_ok(W)) return -1;
+  const int nd = model->n_det;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+#pragma omp parallel for schedule(dynamic, 1) num_threads(g_threads > 0 ? g_threads : omp_get_max_threads())
+  for (int64_t b = 0; b < B; ++b) {
+    double* ob = out + (size_t)b * nd * 3 * N * 2;
+    const double* th = params + b * NPAR;
+    if (!tab_sample_ok(th)) {
+      for (int64_t i = 0; i < (int64_t)nd * 3 * N * 2; ++i) ob[i] = nan;
+      continue;
+    }
+    const Frame<double> F = tab_frame(th);
+    for (int d = 0; d < nd; ++d)
+      for (int64_t k = 0; k < N; ++k) {
+        Cx<double> ch[3];
+        if (freqs[k] > 0.0) response_bin_tab(W, b, th, F, freqs[k], model->mode_mask, model->det[d], ch);
+        else for (int c = 0; c < 3; ++c) ch[c] = cx<double>(0.0, 0.0);
+        for (int c = 0; c < 3; ++c) {
+          ob[(((size_t)d * 3 + c) * N + k) * 2 + 0] = ch[c].re;
+          ob[(((size_t)d * 3 + c) * N + k) * 2 + 1] = ch[c].im;
+        }
+      }
+  }
+  return 0;
+}
+
+int pespace_oracle_loglike_tab(const double* params, int64_t B, int64_t K, const double* fnodes, const double* amp,
+                               const double* phase, const double* tf, const double* data, const double* psd,
+                               const pespace_oracle_grid* grid, const pespace_oracle_model* model, double* out_lnL) {
+  if (!params || !data || !psd || !out_lnL || B <= 0 || !grid_ok(grid) || !model_ok(model)) return -1;
+  const WaveTable W = {K, fnodes, amp, phase, tf, popcount5(model->mode_mask)};
+  if (!table_ok(W)) return -1;
+  const int nd = model->n_det;
+  const int64_t N = grid->N;
+#pragma omp parallel for schedule(dynamic, 1) num_threads(g_threads > 0 ? g_threads : omp_get_max_threads())
+  for (int64_t b = 0; b < B; ++b) {
+    const double* th = params + b * NPAR;
+    if (!tab_sample_ok(th)) { out_lnL[b] = -std::numeric_limits<double>::infinity(); continue; }
+    const Frame<double> F = tab_frame(th);
+    long double sum = 0.0L;
+    for (int d = 0; d < nd; ++d)
+      for (int64_t k = 0; k < N; ++k) {
+        const double f = std::fma((double)k, grid->df, grid->f0);          // G11
+        Cx<double> h[3];
+        response_bin_tab(W, b, th, F, f, model->mode_mask, model->det[d], h);
+        for (int c = 0; c < 3; ++c) {
+          const size_t idx = ((size_t)d * 3 + c) * N + k;
+          const double S = psd[idx];
+          if (!weight_ok(S)) continue;                                      // G9
+          const double rr = data[2 * idx] - h[c].re, ri = data[2 * idx + 1] - h[c].im;
+          sum += (long double)(rr * rr + ri * ri) / (long double)S;
+        }
+      }
+    out_lnL[b] = (double)(-0.5L * 4.0L * (long double)grid->df * sum);
+  }
+  return 0;
+}
+
+/* one mode's interpolated table values at the frequencies freqs (reference extrinsic values); out-of-table -> NaN */
+int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* amp, const double* phase,
+                                const double* tf, const double* freqs, int64_t N, double* out_amp, double* out_psi,
+                                double* out_tf) {
+  const WaveTable W = {K, fnodes, amp, phase, tf, 1};
+  if (!table_ok(W) || !freqs || !out_amp || !out_psi || !out_tf || N <= 0) return -1;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+  for (int64_t k = 0; k < N; ++k)
+    if (!tab_waveform(W, 0, 0, freqs[k], &out_amp[k], &out_psi[k], &out_tf[k])) out_amp[k] = out_psi[k] = out_tf[k] = nan;
+  return 0;
 }
 
 // O11: lnL = -1/2 sum_det sum_c 4 df sum_k |d - h|^2 / S   (Eq. 10, 11, 14 with T = 1/df)

@@ -60,6 +60,25 @@ int pespace_oracle_fisher(const double* params, int64_t B, const double* data_AE
                           const double* psd, const pespace_oracle_grid* grid,
                           const pespace_oracle_model* model, double* out_F, double* out_grad);
 
+/* ---- T1: tabulated mode waveforms (amplitude, phase and t_f per mode come
+ * from the waveform generator).  Tables on K >= 4 shared nodes fnodes[K] (strictly increasing, Hz): amp, phase, tf
+ * [B][n_modes][K], modes in bit order of the mask, for t_c = 0, phi_c = 0, D_L = 1 Gpc.  The call applies
+ * Psi += 2 pi f t_c - m phi_c, t_f += t_c, A /= D_L from theta; M, q, chi1, chi2 of theta are ignored.
+ * Interpolation: Psi cubic Hermite with node slopes 2 pi tf_j, t_f its derivative / 2 pi, A cubic Lagrange on
+ * 4 nodes; a mode is 0 outside [fnodes[0], fnodes[K-1]]. */
+int pespace_oracle_response_tab(const double* params, int64_t B, int64_t K, const double* fnodes,
+                                const double* amp, const double* phase, const double* tf,
+                                const double* freqs, int64_t N, const pespace_oracle_model* model,
+                                double* out_AET);
+int pespace_oracle_loglike_tab(const double* params, int64_t B, int64_t K, const double* fnodes,
+                               const double* amp, const double* phase, const double* tf,
+                               const double* data_AET, const double* psd, const pespace_oracle_grid* grid,
+                               const pespace_oracle_model* model, double* out_lnL);
+/* the interpolants of ONE (sample, mode) table at freqs[N]; NaN outside the table */
+int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* amp, const double* phase,
+                                const double* tf, const double* freqs, int64_t N, double* out_amp,
+                                double* out_psi, double* out_tf);
+
 /* ---- pieces, exported so that the pins can check them one at a time ---- */
 
 /* per-mode amplitude A_lm(f) [s], phase Psi_lm(f) [rad], t_lm(f) [s]   (O2-O5) */

@@ -242,3 +242,58 @@ def config(idx: int, B: Optional[int] = None, N: Optional[int] = None,
         return _jitter_workload("config5", 4, 104, B or 256, N or 262144, MODES_HM,
                                 [lisa_like(), taiji_like(), tianqin_like()], want_fisher=True)
     raise ValueError("config index must be 1..5")
+
+
+# ---------------------------------------------------------------- tabulated mode waveforms
+# Input recipes for the *_tab entry points: tables (fnodes [K], amp, phase, tf [B][n_modes][K]) for the reference
+# extrinsic values t_c = 0, phi_c = 0, D_L = 1 Gpc, modes in bit order of the mask.  Like the rest of this module
+# they hold none of the method's arithmetic: `table_from_waveform_fn` tabulates whatever per-mode waveform function
+# the caller passes in (the oracle's in the tests), `chirp_table` is a seeded-parameter synthetic input shaped like
+# an inspiral (power laws in f), used where no waveform generator may be called (bench.py).
+MODE_LM = ((2, 2), (2, 1), (3, 3), (3, 2), (4, 4))
+
+
+def log_nodes(f_lo: float, f_hi: float, K: int) -> np.ndarray:
+    """K log-spaced nodes covering [f_lo, f_hi] (end points widened by one part in 1e12)."""
+    return np.geomspace(f_lo * (1.0 - 1e-12), f_hi * (1.0 + 1e-12), K)
+
+
+def mask_modes(mode_mask: int):
+    return [lm for i, lm in enumerate(MODE_LM) if mode_mask & (1 << i)]
+
+
+def table_from_waveform_fn(params: np.ndarray, mode_mask: int, fnodes: np.ndarray,
+                           waveform_fn: Callable[[np.ndarray, int, int, np.ndarray], tuple]):
+    """waveform_fn(theta, l, m, freqs) -> (A, Psi, t_f); called with t_c = 0, phi_c = 0, D_L = 1 Gpc."""
+    params = np.atleast_2d(params)
+    modes = mask_modes(mode_mask)
+    B, K = params.shape[0], fnodes.shape[0]
+    amp, phase, tf = (np.empty((B, len(modes), K)) for _ in range(3))
+    for b in range(B):
+        th = params[b].copy()
+        th[4], th[6], th[10] = 1.0, 0.0, 0.0
+        for i, (l, m) in enumerate(modes):
+            amp[b, i], phase[b, i], tf[b, i] = waveform_fn(th, l, m, fnodes)
+    return fnodes, amp, phase, tf
+
+
+def chirp_table(params: np.ndarray, mode_mask: int, fnodes: np.ndarray):
+    """Synthetic smooth tables shaped like an inspiral: Psi = c0 (f')^(-5/3) (1 + c1 (f')^(2/3)) with f' = 2f/m,
+    t_f = (1/2pi) dPsi/df exactly, A = a0 (f')^(-7/6) / m, the scales set by theta's M and q."""
+    params = np.atleast_2d(params)
+    modes = mask_modes(mode_mask)
+    B, K = params.shape[0], fnodes.shape[0]
+    amp, phase, tf = (np.empty((B, len(modes), K)) for _ in range(3))
+    for b in range(B):
+        Ms = params[b, 0] * 4.925490947641267e-6
+        eta = params[b, 1] / (1.0 + params[b, 1]) ** 2
+        c0 = 3.0 / (128.0 * eta) * (np.pi * Ms) ** (-5.0 / 3.0)
+        c1 = (3715.0 / 756.0 + 55.0 * eta / 9.0) * (np.pi * Ms) ** (2.0 / 3.0)
+        a0 = np.sqrt(2.0 * eta / 3.0) * np.pi ** (-1.0 / 6.0) * Ms ** (5.0 / 6.0) * Ms / 1.0292712505433901e17
+        for i, (l, m) in enumerate(modes):
+            fp = 2.0 * fnodes / m
+            phase[b, i] = 0.5 * m * c0 * (fp ** (-5.0 / 3.0) + c1 / fp)
+            dpsi_dfp = c0 * (-5.0 / 3.0 * fp ** (-8.0 / 3.0) - c1 / fp ** 2)      # d/df' of the (2,2)-like phase
+            tf[b, i] = dpsi_dfp / (2.0 * np.pi)                                 # (m/2) (2/m) d/df' = d/df
+            amp[b, i] = a0 * fp ** (-7.0 / 6.0) / m
+    return fnodes, amp, phase, tf

@@ -573,3 +573,70 @@ def test_out_of_domain_samples_and_bad_arguments():
         oracle.response(THETA, f, W.Model(0, (LISA,)))
     with pytest.raises(ValueError):
         oracle.response(THETA, f, W.Model(1, (W.Detector("x", 2, 20, 1e9),)))
+
+
+# ------------------------------------------------------------------ T1: tabulated mode waveforms
+def test_T1_interpolants_are_exact_for_cubics_and_zero_outside():
+    """Cubic Hermite (phase, slopes 2 pi t_j), its derivative (t_f) and 4-node Lagrange (amplitude) reproduce
+    cubic polynomials exactly on non-uniform nodes; outside the table the interpolants are undefined (mode = 0)."""
+    rng = np.random.default_rng(5)
+    fn = np.sort(rng.uniform(1e-3, 2e-3, 40))
+    x = (fn - 1.5e-3) / 1e-3
+    cp, ca = rng.normal(size=4) * [50.0, 400.0, 30.0, 20.0], rng.normal(size=4)
+    P = lambda y: cp[0] + cp[1] * y + cp[2] * y ** 2 + cp[3] * y ** 3
+    dP = lambda y: (cp[1] + 2 * cp[2] * y + 3 * cp[3] * y ** 2) / 1e-3
+    A = lambda y: ca[0] + ca[1] * y + ca[2] * y ** 2 + ca[3] * y ** 3
+    f = np.concatenate([rng.uniform(fn[0], fn[-1], 500), fn[[0, 7, -1]]])
+    y = (f - 1.5e-3) / 1e-3
+    a, p, t = oracle.tab_waveform(fn, A(x), P(x), dP(x) / (2 * np.pi), f)
+    assert np.abs(p - P(y)).max() <= 1e-11 * np.abs(P(y)).max()
+    assert np.abs(t - dP(y) / (2 * np.pi)).max() <= 1e-10 * np.abs(dP(y)).max()
+    assert np.abs(a - A(y)).max() <= 1e-12 * np.abs(A(y)).max()
+    a, p, t = oracle.tab_waveform(fn, A(x), P(x), dP(x) / (2 * np.pi), np.array([fn[0] * 0.999, fn[-1] * 1.001]))
+    assert np.all(np.isnan(a)) and np.all(np.isnan(p)) and np.all(np.isnan(t))
+
+
+@pytest.mark.parametrize("mask,dets", [(1, (LISA,)), (31, (LISA, TQ))])
+def test_T1_tabulated_path_reproduces_the_analytic_path(mask, dets):
+    """Tables of the oracle's own analytic modes at t_c = 0, phi_c = 0, D_L = 1 Gpc, pushed through the tabulated
+    path with theta's t_c, phi_c, D_L, give the analytic response up to the interpolation error, which falls as
+    K^-4 (pins mode order, the signs of the t_c and phi_c terms, the 1/D_L scaling and the stencils)."""
+    model = W.Model(mask, dets)
+    f = np.geomspace(1.2e-4, 0.09, 400)
+    th = THETA.copy()
+    th[2], th[3] = 0.3, -0.2
+    want = oracle.response(th, f, model)[0]
+    errs = []
+    for K in (200, 400, 3000):
+        table = W.table_from_waveform_fn(th, mask, W.log_nodes(1e-4, 0.1, K), oracle.waveform)
+        got = oracle.response_tab(th, table, f, model)[0]
+        errs.append(max(np.abs(got[d] - want[d]).max() / np.abs(want[d]).max() for d in range(len(dets))))
+    assert errs[2] <= 2e-10, errs                    # floor: rounding of the 1e6 rad phase (1e-16 relative)
+    assert errs[0] / errs[1] > 10.0, errs            # fourth order: 16 per halving of the node spacing
+
+
+def test_T1_extrinsic_parameters_band_limits_and_likelihood():
+    model = W.Model(3, (LISA,))                                  # (2,2) and (2,1)
+    grid = W.Grid(1e-4, 2.5e-6, 600)
+    f = grid.freqs()
+    th = np.tile(THETA, (3, 1))
+    th[1, 4] *= 2.0                                              # D_L doubled
+    th[2, 6] += np.pi                                            # phi_c + pi: m = 2 unchanged, m = 1 flips sign
+    fn = W.log_nodes(1e-4, 1.2e-3, 900)                          # the table ends inside the grid
+    table = W.chirp_table(th, 3, fn)
+    r = oracle.response_tab(th, table, f, model)
+    inside = f <= fn[-1]
+    assert np.all(r[:, :, :, ~inside] == 0.0) and np.abs(r[0, 0, 0, inside]).min() > 0.0
+    assert np.allclose(r[1], 0.5 * r[0], rtol=1e-13, atol=0.0)
+    only22 = oracle.response_tab(th, tuple(x if x.ndim == 1 else x[:, :1] for x in table), f, W.Model(1, (LISA,)))
+    only21 = oracle.response_tab(th, tuple(x if x.ndim == 1 else x[:, 1:] for x in table), f, W.Model(2, (LISA,)))
+    scale = np.abs(r[0]).max()
+    assert np.abs(only22[0] + only21[0] - r[0]).max() <= 1e-13 * scale           # modes add, in bit order
+    assert np.abs(only22[2] - only22[0]).max() <= 1e-9 * scale
+    assert np.abs(only21[2] + only21[0]).max() <= 1e-9 * np.abs(only21[0]).max()
+    # noiseless data from sample 0: lnL = 0 there, negative elsewhere, and equal to the Whittle sum written out
+    psd = W.psd_aet(LISA, f)[None]
+    lnL = oracle.loglike_tab(th, table, r[0], psd, grid, model)
+    assert lnL[0] == 0.0 and lnL[1] < 0.0 and lnL[2] < 0.0
+    brute = -0.5 * 4.0 * grid.df * np.sum(np.abs(r[0] - r[1]) ** 2 / psd)
+    assert abs(lnL[1] - brute) <= 1e-12 * abs(brute)
