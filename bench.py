@@ -117,7 +117,7 @@ class ClockSampler:
 FISHER_REF_BINS = 8192   # the oracle's Fisher pass costs ~45 core-seconds per sample at N = 262144: time a bin subset
 
 
-def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0):
+def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0, tab_nodes: int = 0):
     """Time the oracle, as it stands, on a bounded sample of the workload: `n_samples` samples (None: sized from a
     one-sample-per-core calibration pass for ~target_s of wall time) x all N bins per step; for the Fisher path
     (config 5) x the first FISHER_REF_BINS bins, the rate scaled by FISHER_REF_BINS / N (the cost per bin is uniform).
@@ -128,9 +128,18 @@ def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0):
     wl = W.config(config, N=FISHER_REF_BINS) if fisher else full
     scale = wl.grid.N / full.grid.N
     psd = wl.psd()
-    data = wl.data(lambda p, fr, m: oracle.response(p, fr, m))
     cores = oracle.get_threads()
-    if fisher:
+    if tab_nodes:
+        f_all = wl.grid.freqs()
+        fnodes = W.log_nodes(f_all[0], f_all[-1], tab_nodes)
+        tab = lambda p: W.chirp_table(p, wl.model.mode_mask, fnodes)
+        data = wl.data(lambda p, fr, m: oracle.response_tab(p, tab(p), fr, m))
+        call = lambda p: oracle.loglike_tab(p, tab(p), data, psd, wl.grid, wl.model)
+    else:
+        data = wl.data(lambda p, fr, m: oracle.response(p, fr, m))
+    if tab_nodes:
+        pass
+    elif fisher:
         call = lambda p: oracle.fisher(p, data, psd, wl.grid, wl.model)
     else:
         call = lambda p: oracle.loglike(p, data, psd, wl.grid, wl.model)
@@ -158,7 +167,8 @@ def run_reference(args):
     fisher_mode = args.config == 5
     METRIC, UNIT = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (globals()["METRIC"], globals()["UNIT"])
     rate, sec_per_step, cores, sample = oracle_timed(args.config, args.ref_samples, args.steps,
-                                                     target_s=max(2.0, 60.0 / max(1, args.steps)))
+                                                     target_s=max(2.0, 60.0 / max(1, args.steps)),
+                                                     tab_nodes=args.tab_nodes if args.waveform == "tab" else 0)
     line = {
         "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3,
@@ -173,7 +183,8 @@ def run_reference(args):
 
 
 def workload_config(wl, args, l2):
-    return {"workload": f"config{args.config}: B={wl.B} x N={wl.grid.N}, {len(wl.model.detectors)} detector(s) "
+    tab = f" + tabulated mode waveforms (K={args.tab_nodes} log-spaced nodes)" if args.waveform == "tab" else ""
+    return {"workload": f"config{args.config}{tab}: B={wl.B} x N={wl.grid.N}, {len(wl.model.detectors)} detector(s) "
                         f"[{', '.join(d.name for d in wl.model.detectors)}], mode_mask={wl.model.mode_mask}, "
                         f"TDI {wl.model.detectors[0].tdi_gen / 10:.1f}, f0={wl.grid.f0} Hz, df=1/(30 d)",
             "B_per_gpu": wl.B, "N_bins": wl.grid.N, "n_det": len(wl.model.detectors),
@@ -194,7 +205,10 @@ def run_ours(args):
 
     # ---- inputs: synthetic, seeded; the injection comes from this library's own response call
     fisher_mode = args.config == 5
-    n_batches = 4
+    tab_mode = args.waveform == "tab"
+    if tab_mode and fisher_mode:
+        raise SystemExit("bench.py: --waveform tab applies to the likelihood configs 2-4")
+    n_batches = 2 if tab_mode else 4
     wls = [W.config(args.config, param_seed=pdist.rank_seed(1000 + i, rank)) for i in range(n_batches)]
     wl = wls[0]
     B, N = wl.B, wl.grid.N
@@ -202,6 +216,19 @@ def run_ours(args):
 
     def gpu_response(p, fr, m):
         return P.response(torch.from_numpy(np.ascontiguousarray(p)).to(device), freqs_d, m).cpu().numpy()
+
+    if tab_mode:
+        # synthetic tables (workloads.chirp_table: inspiral-shaped power laws) on K log-spaced nodes covering the grid
+        f_all = wl.grid.freqs()
+        fnodes = W.log_nodes(f_all[0], f_all[-1], args.tab_nodes)
+        tabs_h = [tuple(torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+                        for x in W.chirp_table(w.params, wl.model.mode_mask, fnodes)) for w in wls]
+        tabs_d = [P.WaveTable(*(x.to(device) for x in t)) for t in tabs_h]
+        inj_tab = P.WaveTable(*(torch.from_numpy(np.ascontiguousarray(x)).to(device)
+                                for x in W.chirp_table(wl.theta_inj[None], wl.model.mode_mask, fnodes)))
+
+        def gpu_response(p, fr, m):                                   # noqa: F811  (injection from the same tables)
+            return P.response_tab(torch.from_numpy(np.ascontiguousarray(p)).to(device), inj_tab, freqs_d, m).cpu().numpy()
 
     # host copies live in pinned memory: the e2e leg copies them to the device every step
     data_h = torch.from_numpy(np.ascontiguousarray(wl.data(gpu_response))).pin_memory()
@@ -212,6 +239,9 @@ def run_ours(args):
         fis = P.Fisher(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
         F_d = torch.empty((B, P.NPAR, P.NPAR), dtype=torch.float64, device=device)
         g_d = torch.empty((B, P.NPAR), dtype=torch.float64, device=device)
+    elif tab_mode:
+        lik = P.LikelihoodTab(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
+        out_d = torch.empty(B, dtype=torch.float64, device=device)
     else:
         lik = P.Likelihood(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
         out_d = torch.empty(B, dtype=torch.float64, device=device)
@@ -221,6 +251,8 @@ def run_ours(args):
         flush.zero_()
         if fisher_mode:
             fis(params_d[i % n_batches], F_d, g_d)
+        elif tab_mode:
+            lik(params_d[i % n_batches], tabs_d[i % n_batches], out_d)
         else:
             lik(params_d[i % n_batches], out_d)
 
@@ -259,17 +291,32 @@ def run_ours(args):
     # (theta, data set, PSD) from pinned host memory to the device and reads the result back, all inside
     # the timed region.  e2e_resident_data: the sampler-facing use, data set copied once, theta per step.
     e2e_steps = max(1, min(args.steps, 10))
-    ses = P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
-    res_h = torch.empty((B, P.NPAR, P.NPAR) if fisher_mode else (B,), dtype=torch.float64).pin_memory()
-    grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
+    if tab_mode:
+        # no host-buffer C entry point for tables yet: the e2e leg goes through the Python binding, copying theta and
+        # the step's tables (and, in the "full" variant, data and PSD) from pinned host memory with torch
+        res_h = torch.empty(B, dtype=torch.float64).pin_memory()
+        state = {"lik": lik}
 
-    def e2e_step(i, copy_data):
-        if copy_data:
-            ses.set_data(data_h, psd_h)
-        if fisher_mode:
-            ses.fisher(params_h[i % n_batches], True, res_h, grad_h)
-        else:
-            ses.loglike(params_h[i % n_batches], res_h)
+        def e2e_step(i, copy_data):
+            if copy_data:
+                state["lik"] = P.LikelihoodTab(data_h.to(device, non_blocking=True), psd_h.to(device, non_blocking=True),
+                                               wl.grid, wl.model, B)
+            t = P.WaveTable(*(x.to(device, non_blocking=True) for x in tabs_h[i % n_batches]))
+            state["lik"](params_h[i % n_batches].to(device, non_blocking=True), t, out_d)
+            res_h.copy_(out_d)
+            torch.cuda.synchronize()
+    ses = None if tab_mode else P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
+    grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
+    if not tab_mode:
+        res_h = torch.empty((B, P.NPAR, P.NPAR) if fisher_mode else (B,), dtype=torch.float64).pin_memory()
+
+        def e2e_step(i, copy_data):
+            if copy_data:
+                ses.set_data(data_h, psd_h)
+            if fisher_mode:
+                ses.fisher(params_h[i % n_batches], True, res_h, grad_h)
+            else:
+                ses.loglike(params_h[i % n_batches], res_h)
 
     e2e = {}
     for key, copy_data in (("full", True), ("resident", False)):
@@ -281,16 +328,17 @@ def run_ours(args):
         e2e_ms = (time.perf_counter() - t0) * 1e3                           # the calls are synchronous
         e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
         e2e[key] = e2e_units / (e2e_max_ms * 1e-3)
-    ses.close()
+    if ses is not None:
+        ses.close()
     nbytes = lambda t: t.numel() * t.element_size()
-    h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h)
+    h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h) + (sum(nbytes(x) for x in tabs_h[0]) if tab_mode else 0)
     d2h = nbytes(res_h) + (nbytes(grad_h) if fisher_mode else 0)
 
     if rank != 0:
         return
 
     # ---- roofline of the dominant kernel (per launch, timed live with CUDA events in the library)
-    kernel = "fisher" if fisher_mode else "loglike"
+    kernel = "fisher" if fisher_mode else ("loglike_tab" if tab_mode else "loglike")
     metric, unit = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (METRIC, UNIT)
     peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     dfma_tflops, _ = P.fp64_peak(8192, mode=0)
@@ -336,7 +384,8 @@ def run_ours(args):
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
-        rate, sec, cores, desc = oracle_timed(args.config, args.ref_samples, 1)
+        rate, sec, cores, desc = oracle_timed(args.config, args.ref_samples, 1,
+                                              tab_nodes=args.tab_nodes if tab_mode else 0)
         cpu_baseline = {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": desc}
 
     line = {
@@ -348,8 +397,10 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": e2e["full"], "unit": unit, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-                "api": "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
-                       " per step: theta, data set and PSD copied from pinned host memory, result read back",
+                "api": ("Python binding (LikelihoodTab): theta, the step's waveform tables, data set and PSD copied from "
+                        "pinned host memory with torch, lnL read back" if tab_mode else
+                        "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
+                        " per step: theta, data set and PSD copied from pinned host memory, result read back"),
                 "value_resident_data": e2e["resident"],
                 "resident_data_note": "same call with the data set copied once (sampler use): theta in, result out"},
         "gpu_launches": int(launches),
@@ -367,6 +418,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic",
+                    help="tab: pespace_loglike_tab on synthetic tabulated mode waveforms (SURVEY 8(f) N1)")
+    ap.add_argument("--tab-nodes", type=int, default=4096, help="nodes K of the waveform tables")
     ap.add_argument("--ref-samples", type=int, default=None,
                     help="samples per oracle pass (default: sized for ~15 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")

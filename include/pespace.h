@@ -98,6 +98,37 @@ int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, 
                    const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                    double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* ---- Tabulated mode waveforms.  In the paper the per-mode amplitude, phase and
+ * time-frequency map t_f come from the waveform generator (PhenomXAS / PhenomXHM) and the
+ * response is built on them (Eq. 4, 5).  These calls take them as tables, so that any externally generated
+ * waveform drives the same response / likelihood kernels; the analytic TaylorF2 modes of pespace_response /
+ * pespace_loglike are then not used.
+ *   d_fnodes [K]                 node frequencies (Hz), strictly increasing, K >= 4, shared by samples and modes
+ *   d_amp, d_phase, d_tf [B][n_modes][K]   A_lm (s), Psi_lm (rad), t_lm (s) at the nodes, h_lm = A e^{-i Psi},
+ *                                modes in bit order of mode_mask, for t_c = 0, phi_c = 0, D_L = 1 Gpc.
+ * From theta the calls use D_L, iota, phi_c, lambda, beta, psi, t_c:  Psi_lm(f) = Psi_tab(f) + 2 pi f t_c
+ * - m phi_c, t_lm(f) = t_tab(f) + t_c, A_lm = A_tab / D_L[Gpc];  M, q, chi1, chi2 are ignored (a sample is out
+ * of domain if one of the used entries is non-finite or D_L <= 0).  Between nodes Psi_tab is the cubic Hermite
+ * interpolant of the node phases with node slopes 2 pi t_j (Eq. 4), t_tab its derivative / 2 pi, A_tab the cubic
+ * Lagrange polynomial through the four nodes around the interval; a mode contributes 0 at frequencies outside
+ * [fnodes[0], fnodes[K-1]].  The node array is NOT checked for monotonicity (device memory). */
+typedef struct {
+  int64_t K;
+  const double* d_fnodes;
+  const double* d_amp;
+  const double* d_phase;
+  const double* d_tf;
+} pespace_wavetable;
+
+int pespace_response_tab(const double* d_params, int64_t B, const pespace_wavetable* table,
+                         const double* d_freqs, int64_t N, const pespace_model* model,
+                         double* d_out_AET, void* stream);
+size_t pespace_workspace_bytes_tab(int64_t B, const pespace_grid* grid, const pespace_model* model);
+int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetable* table,
+                        const double* d_data_AET, const double* d_psd, const pespace_grid* grid,
+                        const pespace_model* model, double* d_out_lnL, void* d_workspace,
+                        size_t workspace_bytes, void* stream);
+
 /* ---- Host-buffer entry points (a sampler evaluates many batches of theta against
  * ONE data set).  A session owns a stream and keeps the data set, the PSD, the workspace
  * and the result buffers resident on the device between calls; each call then moves only theta in

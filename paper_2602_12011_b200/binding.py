@@ -17,6 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
+           "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike",
            "pespace_session_fisher", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
@@ -41,6 +42,11 @@ class _Model(C.Structure):
     _fields_ = [("mode_mask", C.c_uint32), ("n_det", C.c_int32), ("det", C.POINTER(_Det))]
 
 
+class _WaveTable(C.Structure):
+    _fields_ = [("K", C.c_int64), ("d_fnodes", C.c_void_p), ("d_amp", C.c_void_p), ("d_phase", C.c_void_p),
+                ("d_tf", C.c_void_p)]
+
+
 def _load():
     if not os.path.exists(LIB_PATH):
         raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2602_12011_b200.build` "
@@ -53,6 +59,11 @@ def _load():
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
+    L.pespace_response_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, i64, C.POINTER(_Model), vp, vp]
+    L.pespace_workspace_bytes_tab.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
+    L.pespace_workspace_bytes_tab.restype = sz
+    L.pespace_loglike_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp,
+                                      vp, sz, vp]
     L.pespace_session_create.argtypes = [C.POINTER(_Grid), C.POINTER(_Model), i64, C.c_int, C.POINTER(vp)]
     L.pespace_session_set_data.argtypes = [vp, vp, vp]
     L.pespace_session_loglike.argtypes = [vp, vp, i64, vp]
@@ -158,6 +169,62 @@ class Likelihood:
 
 def loglike(params: torch.Tensor, data: torch.Tensor, psd: torch.Tensor, grid, model) -> torch.Tensor:
     return Likelihood(data, psd, grid, model, params.shape[0])(params)
+
+
+class WaveTable:
+    """Tabulated mode waveforms on the device (pespace_wavetable): fnodes [K], amp / phase / tf [B][n_modes][K]
+    for t_c = 0, phi_c = 0, D_L = 1 Gpc, modes in bit order of the model's mode_mask."""
+
+    def __init__(self, fnodes: torch.Tensor, amp: torch.Tensor, phase: torch.Tensor, tf: torch.Tensor):
+        self.fnodes, self.amp, self.phase, self.tf = (_dev(x, n) for x, n in
+                                                      ((fnodes, "fnodes"), (amp, "amp"), (phase, "phase"), (tf, "tf")))
+        K = self.fnodes.shape[0]
+        if self.amp.dim() != 3 or self.amp.shape[2] != K or self.phase.shape != self.amp.shape or \
+                self.tf.shape != self.amp.shape:
+            raise PespaceError("amp, phase and tf must be [B][n_modes][K] with K = len(fnodes)")
+        self.B, self.n_modes, self.K = int(self.amp.shape[0]), int(self.amp.shape[1]), int(K)
+        self.c = _WaveTable(self.K, self.fnodes.data_ptr(), self.amp.data_ptr(), self.phase.data_ptr(),
+                            self.tf.data_ptr())
+
+    def check(self, B: int, model) -> None:
+        if self.B != B or self.n_modes != bin(int(model.mode_mask)).count("1"):
+            raise PespaceError("table shape does not match the batch size / the number of modes of the mask")
+
+
+def response_tab(params: torch.Tensor, table: WaveTable, freqs: torch.Tensor, model,
+                 out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """Response from tabulated mode waveforms -> complex128 [B][n_det][3][N] (device)."""
+    p, f = _dev(params, "params"), _dev(freqs, "freqs")
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    table.check(B, model)
+    if out is None:
+        out = torch.empty((B, nd, 3, N, 2), dtype=torch.float64, device=p.device)
+    m, keep = _model(model)
+    _check(_lib.pespace_response_tab(p.data_ptr(), B, C.byref(table.c), f.data_ptr(), N, C.byref(m),
+                                     _dev(out, "out").data_ptr(), _stream_ptr()), "pespace_response_tab")
+    return torch.view_as_complex(out)
+
+
+class LikelihoodTab(Likelihood):
+    """pespace_loglike_tab with data, PSD and workspace resident on the device."""
+
+    def __init__(self, data: torch.Tensor, psd: torch.Tensor, grid, model, max_batch: int):
+        super().__init__(data, psd, grid, model, max_batch)
+        self.ws_bytes = int(_lib.pespace_workspace_bytes_tab(int(max_batch), C.byref(self._g), C.byref(self._m)))
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=self.data.device)
+
+    def __call__(self, params: torch.Tensor, table: WaveTable, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        p = _dev(params, "params")
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        table.check(B, self.model)
+        if out is None:
+            out = torch.empty(B, dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_loglike_tab(p.data_ptr(), B, C.byref(table.c), self.data.data_ptr(), self.psd.data_ptr(),
+                                        C.byref(self._g), C.byref(self._m), _dev(out, "out").data_ptr(),
+                                        self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_loglike_tab")
+        return out
 
 
 class Fisher:

@@ -170,7 +170,7 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
     // S0: per-bin table of this data set, once per call
     const PrepArgs A = make_prep_args(model);
     const dim3 gb((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det);
-    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, d_bins);
+    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
     LAUNCHED();
   }
   const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);

@@ -195,6 +195,11 @@ __device__ __forceinline__ void tdi_prefactor(const BinC& b, int gen, double& gr
   gi = (ar * zi + ai * zr) * b.fm76;
 }
 
+template <int KIND, bool FIRST, bool TAB>
+__device__ __forceinline__ void eval_geom(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
+                                          const double2* __restrict__ tab, double psi, double tau, double CKp,
+                                          double CKc, double (&S)[6]);
+
 // ---------------------------------------------------------------------------------------------
 // One mode class (m = MC + 1) of one (sample, bin, detector): adds its X, Y, Z (without the common
 // factor g z f^{-7/6}) to S.  All phases are carried in pu = 1/1024 turn (the prep kernel scales the
@@ -236,6 +241,16 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
   else if (MC == 3) { CKp = v2 * ka[0]; CKc = v2 * ka[2]; }
   else { CKp = v * ka[0]; CKc = v * ka[2]; }
 
+  eval_geom<KIND, FIRST, TAB>(bc, sc, dc, tab, psi, tau, CKp, CKc, S);
+}
+
+// S4-S7 of one mode (class) of one (sample, bin, detector) from its phase psi (pu, reduced), its time tau =
+// kTurn (t_lm - t_c) / yr and its amplitudes CKp, CKc (amplitude x polarisation content): adds X, Y, Z (without
+// the common per-bin factor) to S.  Shared by the analytic classes (eval_class) and the tabulated modes.
+template <int KIND, bool FIRST, bool TAB>
+__device__ __forceinline__ void eval_geom(const BinC& bc, const double* __restrict__ sc, const DetC& dc,
+                                          const double2* __restrict__ tab, double psi, double tau, double CKp,
+                                          double CKc, double (&S)[6]) {
   // ---- S4: orbit phase(s) and the two rotating combinations G1, G2 of each of k, u', v'
   double G1k, G2k, G1u, G2u, G1v, G2v, kR;
   if (KIND == 0) {
@@ -363,6 +378,58 @@ __device__ __forceinline__ bool sample_in_domain(const double* th) {
   return ok && th[0] > 0.0 && th[1] >= 1.0 && th[4] > 0.0;
 }
 
+// Frame and detector blocks of the per-sample constants (O7, O8): the sky basis with the polarisation angle
+// absorbed, projected on the orbit basis of every detector, and the orbital phases at t_c.
+template <class T, class Put>
+__device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc, const PrepArgs& A, Put put) {
+  // frame (O7) with the polarisation angle absorbed into the basis: u' = cos(psi) u + sin(psi) v, ...
+  const T cl = p_cos(lam), sl = p_sin(lam), cb = p_cos(bet), sb = p_sin(bet), cp = p_cos(pol), sp = p_sin(pol);
+  const T k[3] = {-(cb * cl), -(cb * sl), -sb};
+  const T u[3] = {sl, -cl, T(0.0)};
+  const T v[3] = {-(sb * cl), -(sb * sl), cb};
+  T up[3], vp[3];
+  for (int i = 0; i < 3; ++i) { up[i] = cp * u[i] + sp * v[i]; vp[i] = cp * v[i] - sp * u[i]; }
+  const double r43 = 1.0 / (4.0 * sqrt(3.0));
+  const T* W3[3] = {k, up, vp};
+  const int off[3] = {S_K - D_BASE, S_U - D_BASE, S_V - D_BASE};
+  const double tcv = p_val(tc);
+  for (int dI = 0; dI < A.n_det; ++dI) {
+    const DetC& D = A.det[dI];
+    const int base = D_BASE + D_STRIDE * dI;
+    for (int i = 0; i < D_STRIDE; ++i) put(base + i, T(0.0));
+    double a0 = tcv / kYear;
+    a0 -= rint(a0);
+    if (D.kind == 0) {
+      // orbital phase and sky basis in the frame rotated about z by lambda0 (see the layout note above)
+      put(base, T(kTurn * (a0 + (D.kappa - D.lambda0) / (2.0 * kPi))));
+      const double cL0 = cos(D.lambda0), sL0 = sin(D.lambda0);
+      for (int j = 0; j < 3; ++j) {
+        const T* w = W3[j];
+        const T wx = cL0 * w[0] + sL0 * w[1], wy = cL0 * w[1] - sL0 * w[0];
+        put(base + off[j] + 0, wx * r43); put(base + off[j] + 1, wy * r43); put(base + off[j] + 2, -0.5 * w[2]);
+        put(base + off[j] + 3, -3.0 * r43 * wx); put(base + off[j] + 4, -3.0 * r43 * wy);
+        if (j == 0) { put(base + (S_DX - D_BASE), (kAU / kC) * wx); put(base + (S_DY - D_BASE), (kAU / kC) * wy); }
+      }
+    } else {
+      put(base + (S_DX - D_BASE), (kAU / kC) * k[0]); put(base + (S_DY - D_BASE), (kAU / kC) * k[1]);
+      put(base, T(kTurn * a0));
+      double p0 = tcv / D.period_s;
+      p0 -= rint(p0);
+      put(base + 1, T(kTurn * (p0 + D.lambda0 / (2.0 * kPi))));
+      const double cL = cos(D.lon), sL = sin(D.lon), cB = cos(D.lat), sB = sin(D.lat);
+      const double nh[3] = {cB * cL, cB * sL, sB};
+      const double e1[3] = {-sL, cL, 0.0};
+      const double e2[3] = {nh[1] * e1[2] - nh[2] * e1[1], nh[2] * e1[0] - nh[0] * e1[2], nh[0] * e1[1] - nh[1] * e1[0]};
+      const double r3 = 1.0 / sqrt(3.0);
+      for (int j = 0; j < 3; ++j) {
+        const T* w = W3[j];
+        put(base + 2 + 2 * j, r3 * (w[0] * e1[0] + w[1] * e1[1] + w[2] * e1[2]));
+        put(base + 3 + 2 * j, r3 * (w[0] * e2[0] + w[1] * e2[1] + w[2] * e2[2]));
+      }
+    }
+  }
+}
+
 template <class T, class Put>
 __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   const T M = th[0], q = th[1], chi1 = th[2], chi2 = th[3], DL = th[4], iota = th[5], phic = th[6],
@@ -422,53 +489,8 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
     kam[4 * (m - 1) + 2 + slot] = 2.0 * Alm * Kc;      // factor 2 of n.e_x.n = 2 (n.u)(n.v)
   }
   for (int i = 0; i < 16; ++i) put(W_KA + i, kam[i]);
-  // frame (O7) with the polarisation angle absorbed into the basis: u' = cos(psi) u + sin(psi) v, ...
-  const T cl = p_cos(lam), sl = p_sin(lam), cb = p_cos(bet), sb = p_sin(bet), cp = p_cos(pol), sp = p_sin(pol);
-  const T k[3] = {-(cb * cl), -(cb * sl), -sb};
-  const T u[3] = {sl, -cl, T(0.0)};
-  const T v[3] = {-(sb * cl), -(sb * sl), cb};
-  T up[3], vp[3];
-  for (int i = 0; i < 3; ++i) { up[i] = cp * u[i] + sp * v[i]; vp[i] = cp * v[i] - sp * u[i]; }
-  const double r43 = 1.0 / (4.0 * sqrt(3.0));
-  const T* W3[3] = {k, up, vp};
-  const int off[3] = {S_K - D_BASE, S_U - D_BASE, S_V - D_BASE};
   put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
-  const double tcv = p_val(tc);
-  for (int dI = 0; dI < A.n_det; ++dI) {
-    const DetC& D = A.det[dI];
-    const int base = D_BASE + D_STRIDE * dI;
-    for (int i = 0; i < D_STRIDE; ++i) put(base + i, T(0.0));
-    double a0 = tcv / kYear;
-    a0 -= rint(a0);
-    if (D.kind == 0) {
-      // orbital phase and sky basis in the frame rotated about z by lambda0 (see the layout note above)
-      put(base, T(kTurn * (a0 + (D.kappa - D.lambda0) / (2.0 * kPi))));
-      const double cL0 = cos(D.lambda0), sL0 = sin(D.lambda0);
-      for (int j = 0; j < 3; ++j) {
-        const T* w = W3[j];
-        const T wx = cL0 * w[0] + sL0 * w[1], wy = cL0 * w[1] - sL0 * w[0];
-        put(base + off[j] + 0, wx * r43); put(base + off[j] + 1, wy * r43); put(base + off[j] + 2, -0.5 * w[2]);
-        put(base + off[j] + 3, -3.0 * r43 * wx); put(base + off[j] + 4, -3.0 * r43 * wy);
-        if (j == 0) { put(base + (S_DX - D_BASE), (kAU / kC) * wx); put(base + (S_DY - D_BASE), (kAU / kC) * wy); }
-      }
-    } else {
-      put(base + (S_DX - D_BASE), (kAU / kC) * k[0]); put(base + (S_DY - D_BASE), (kAU / kC) * k[1]);
-      put(base, T(kTurn * a0));
-      double p0 = tcv / D.period_s;
-      p0 -= rint(p0);
-      put(base + 1, T(kTurn * (p0 + D.lambda0 / (2.0 * kPi))));
-      const double cL = cos(D.lon), sL = sin(D.lon), cB = cos(D.lat), sB = sin(D.lat);
-      const double nh[3] = {cB * cL, cB * sL, sB};
-      const double e1[3] = {-sL, cL, 0.0};
-      const double e2[3] = {nh[1] * e1[2] - nh[2] * e1[1], nh[2] * e1[0] - nh[0] * e1[2], nh[0] * e1[1] - nh[1] * e1[0]};
-      const double r3 = 1.0 / sqrt(3.0);
-      for (int j = 0; j < 3; ++j) {
-        const T* w = W3[j];
-        put(base + 2 + 2 * j, r3 * (w[0] * e1[0] + w[1] * e1[1] + w[2] * e1[2]));
-        put(base + 3 + 2 * j, r3 * (w[0] * e2[0] + w[1] * e2[1] + w[2] * e2[2]));
-      }
-    }
-  }
+  prep_frame(lam, bet, pol, tc, A, put);
 }
 
 // sine/cosine table of sincos_tab: trig[j] = (sin, cos)(2 pi j / NTAB), |error| <= 1 ulp (sincospi)
@@ -534,12 +556,13 @@ enum : int { BF_FT = 0, BF_CF, BF_LNF3, BF_FM53, BF_FM83, BF_STH, BF_CTH, BF_DR,
 static_assert(NBF == 16, "bin record is 16 doubles");
 
 static __global__ void prep_bins_kernel(const double2* __restrict__ data, const double* __restrict__ psd, GridC G,
-                                        PrepArgs A, double* __restrict__ bins /* [n_det][NBF][N] */) {
+                                        PrepArgs A, int fold_f76, double* __restrict__ bins /* [n_det][NBF][N] */) {
   const long long k = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   const int det = blockIdx.y;
   if (k >= G.N) return;
   const DetC& dc = A.det[det];
-  const BinC bc = make_bin(fma((double)k, G.df, G.f0), dc.Lbar);
+  BinC bc = make_bin(fma((double)k, G.df, G.f0), dc.Lbar);
+  if (!fold_f76) bc.fm76 = 1.0;          // tabulated waveforms carry their own amplitude (pespace_tab.cuh)
   double gr, gi;
   tdi_prefactor(bc, dc.gen, gr, gi);
   const double g2 = gr * gr + gi * gi;

@@ -55,7 +55,7 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
   {
     // S0: per-bin table of this data set (d_data_AET == NULL: zeros, Fisher matrix only)
     const dim3 gb((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det);
-    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, d_bins);
+    prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
     LAUNCHED();
   }
   const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
