@@ -184,6 +184,8 @@ def run_reference(args):
 
 def workload_config(wl, args, l2):
     tab = f" + tabulated mode waveforms (K={args.tab_nodes} log-spaced nodes)" if args.waveform == "tab" else ""
+    if getattr(args, "grad_only", False) and args.config == 5:
+        tab += " (gradient only)"
     return {"workload": f"config{args.config}{tab}: B={wl.B} x N={wl.grid.N}, {len(wl.model.detectors)} detector(s) "
                         f"[{', '.join(d.name for d in wl.model.detectors)}], mode_mask={wl.model.mode_mask}, "
                         f"TDI {wl.model.detectors[0].tdi_gen / 10:.1f}, f0={wl.grid.f0} Hz, df=1/(30 d)",
@@ -250,7 +252,7 @@ def run_ours(args):
     def step(i):
         flush.zero_()
         if fisher_mode:
-            fis(params_d[i % n_batches], F_d, g_d)
+            fis(params_d[i % n_batches], F_d, g_d, grad_only=args.grad_only)
         elif tab_mode:
             lik(params_d[i % n_batches], tabs_d[i % n_batches], out_d)
         else:
@@ -280,7 +282,7 @@ def run_ours(args):
     main_ms, main_launches = P.profile_read()
     P.profile_enable(False)
     clocks = sampler.stop()
-    last = (F_d if fisher_mode else out_d).cpu().numpy()
+    last = ((g_d if args.grad_only else F_d) if fisher_mode else out_d).cpu().numpy()
     if not np.all(np.isfinite(last)):
         raise SystemExit("bench.py: non-finite result in the timed region")
 
@@ -314,7 +316,7 @@ def run_ours(args):
             if copy_data:
                 ses.set_data(data_h, psd_h)
             if fisher_mode:
-                ses.fisher(params_h[i % n_batches], True, res_h, grad_h)
+                ses.fisher(params_h[i % n_batches], True, res_h, grad_h, grad_only=args.grad_only)
             else:
                 ses.loglike(params_h[i % n_batches], res_h)
 
@@ -418,6 +420,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--grad-only", action="store_true",
+                    help="config 5: d lnL / d theta only (pespace_fisher with d_out_F = NULL)")
     ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic",
                     help="tab: pespace_loglike_tab on synthetic tabulated mode waveforms (SURVEY 8(f) N1)")
     ap.add_argument("--tab-nodes", type=int, default=4096, help="nodes K of the waveform tables")

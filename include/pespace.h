@@ -93,7 +93,9 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
 /* Forward-mode derivatives (Eq. 13, 14): F_ij = <d_i h | d_j h>, grad_i = d lnL / d theta_i
  * = <d - h | d_i h>, derivatives w.r.t. the 11 raw theta entries.
  *   d_out_F [B][11][11] symmetric, full storage; d_out_grad [B][11] or NULL;
- *   d_data_AET may be NULL: then the gradient is skipped. */
+ *   d_data_AET may be NULL: then the gradient is skipped (d_out_grad must be NULL);
+ *   d_out_F may be NULL when d_out_grad is not: gradient only (for gradient-based samplers),
+ *   which skips the 66 Fisher entries of the per-bin Gram matrix. */
 int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
                    const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                    double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
@@ -149,7 +151,7 @@ int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const
 /* h_params [B][11] -> h_out_lnL [B], B <= max_B.  PESPACE_EINVAL before data and PSD are set. */
 int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL);
 /* h_params [B][11] -> h_out_F [B][11][11] and, if h_out_grad != NULL, h_out_grad [B][11] (needs the
- * data set; the Fisher matrix alone needs only the PSD). */
+ * data set; the Fisher matrix alone needs only the PSD).  h_out_F may be NULL: gradient only. */
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
                            double* h_out_grad);
 /* Waits for the session's stream and frees everything the session owns. */

@@ -243,11 +243,21 @@ class Fisher:
         self.ws = torch.empty(max(self.ws_bytes, 16), dtype=torch.uint8, device=self.psd.device)
 
     def __call__(self, params: torch.Tensor, out_F: Optional[torch.Tensor] = None,
-                 out_grad: Optional[torch.Tensor] = None):
+                 out_grad: Optional[torch.Tensor] = None, grad_only: bool = False):
+        """-> (F, grad); grad_only=True skips the Fisher matrix (returns (None, grad): d lnL / d theta alone)."""
         p = _dev(params, "params")
         B = p.shape[0]
         if B > self.max_batch:
             raise PespaceError("batch larger than the workspace was sized for")
+        if grad_only:
+            if self.data is None:
+                raise PespaceError("the gradient needs the data set")
+            if out_grad is None:
+                out_grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+            _check(_lib.pespace_fisher(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g),
+                                       C.byref(self._m), None, _dev(out_grad, "out_grad").data_ptr(),
+                                       self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_fisher")
+            return None, out_grad
         if out_F is None:
             out_F = torch.empty((B, NPAR, NPAR), dtype=torch.float64, device=p.device)
         if self.data is not None and out_grad is None:
@@ -318,13 +328,17 @@ class Session:
         _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
         return out
 
-    def fisher(self, params, with_grad: bool = True, out_F=None, out_grad=None):
+    def fisher(self, params, with_grad: bool = True, out_F=None, out_grad=None, grad_only: bool = False):
         pp, p = _host_ptr(params, np.float64, "params")
         B = int(p.shape[0])
-        if out_F is None:
-            out_F = np.empty((B, NPAR, NPAR), dtype=np.float64)
         if with_grad and out_grad is None:
             out_grad = np.empty((B, NPAR), dtype=np.float64)
+        if grad_only:
+            gp, keep_g = _host_ptr(out_grad, np.float64, "out_grad")
+            _check(_lib.pespace_session_fisher(self._h, pp, B, None, gp), "pespace_session_fisher")
+            return None, out_grad
+        if out_F is None:
+            out_F = np.empty((B, NPAR, NPAR), dtype=np.float64)
         Fp, keep_F = _host_ptr(out_F, np.float64, "out_F")
         gp = None
         if with_grad:

@@ -35,8 +35,9 @@ size_t fisher_workspace_bytes(long long B, long long N, int n_det) {
 extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
                               const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                               double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream) {
-  if (!d_params || !d_psd || !d_out_F || !d_workspace || B <= 0 || !grid_ok(grid) || !model_ok(model))
+  if (!d_params || !d_psd || (!d_out_F && !d_out_grad) || !d_workspace || B <= 0 || !grid_ok(grid) || !model_ok(model))
     return PESPACE_EINVAL;
+  const int grad_only = d_out_F == nullptr;                   // d lnL / d theta alone: row 0 of the Gram matrix
   if (d_out_grad && !d_data_AET) return PESPACE_EINVAL;       // the gradient needs the data
   if (workspace_bytes < fisher_workspace_bytes(B, grid->N, model->n_det) || ((uintptr_t)d_workspace & 15u))
     return PESPACE_EINVAL;
@@ -63,7 +64,7 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc = prof_begin(ev, st); rc != PESPACE_OK) return rc;
-    CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, d_bins, G.N, dc, model->n_det, d, d_partial));
+    CU(fisher_launcher(dc.kind, cm)(g, st, d_consts, B, d_bins, G.N, dc, model->n_det, d, grad_only, d_partial));
     LAUNCHED();
     if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }

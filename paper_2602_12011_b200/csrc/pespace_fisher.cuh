@@ -395,10 +395,64 @@ __device__ __forceinline__ void gram_rows(const double* __restrict__ J, const do
   }
 }
 
+// Gradient only (pespace_fisher with d_out_F = NULL): row 0 of the Gram matrix, <d - h | d_p h> for p = 0..11, reduced
+// over the warp with two halving levels (12 -> 6 -> 3 values) and three plain ones; lanes 0, 8, 16, 24 add their
+// three sums to slots (lane >> 3) * 3 + j of r, i.e. Gram entries j + 6 b4 + 3 b3.
+__device__ __forceinline__ void gram_row0(const double* __restrict__ J, const double (&dr)[3], const double (&di)[3],
+                                          const double (&w)[3], double mDL, int lane, double* __restrict__ r) {
+  double a[NT];
+#pragma unroll
+  for (int i = 0; i < NT; ++i) a[i] = 0.0;
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    double ar[NT], ai[NT];
+#pragma unroll
+    for (int pp = 0; pp < NT; ++pp) {
+      if (pp == 5) continue;
+      const double* jp = J + pp * 6 * FBLOCK;
+      const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
+                   zi = jp[5 * FBLOCK];
+      if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
+      else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
+      else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
+    }
+    ar[5] = mDL * ar[0]; ai[5] = mDL * ai[0];
+    ar[0] = dr[c] - ar[0]; ai[0] = di[c] - ai[0];
+    const double wr = w[c] * ar[0], wi = w[c] * ai[0];
+#pragma unroll
+    for (int q = 0; q < NT; ++q) a[q] = fma(wr, ar[q], fma(wi, ai[q], a[q]));
+  }
+  {
+    const bool up = lane & 16;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      const double keep = up ? a[i + 6] : a[i], send = up ? a[i] : a[i + 6];
+      a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 16);
+    }
+  }
+  {
+    const bool up = lane & 8;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const double keep = up ? a[i + 3] : a[i], send = up ? a[i] : a[i + 3];
+      a[i] = keep + __shfl_xor_sync(0xffffffffu, send, 8);
+    }
+  }
+#pragma unroll
+  for (int o = 4; o > 0; o >>= 1)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) a[j] += __shfl_xor_sync(0xffffffffu, a[j], o);
+  if (!(lane & 7)) {
+    double* rr = r + (lane >> 3) * 3;
+    rr[0] += a[0]; rr[1] += a[1]; rr[2] += a[2];
+  }
+}
+
 template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(FBLOCK, 2)
 fisher_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ bins /* [n_det][NBF][N] */,
-              long long N, DetC dc, int n_det, int det, double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
+              long long N, DetC dc, int n_det, int det, int grad_only,
+              double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
   extern __shared__ double fsm[];
   double* Jsm = fsm;                                   // [NJ][FBLOCK]
   double* csm = Jsm + NJ * FBLOCK;                     // [FTILE][SMEM_STRIDE][DUW]
@@ -441,14 +495,19 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double* __re
       }
       const double mDL = cv(sc, W_MDL);
       double* r = red + (warp * FTILE + s) * NGP;
-      gram_rows<0, GRAM_SPLIT>(J, dr, di, w, mDL, lane, r);
-      gram_rows<GRAM_SPLIT, NT>(J, dr, di, w, mDL, lane, r + NGH);
+      if (grad_only) {
+        gram_row0(J, dr, di, w, mDL, lane, r);
+      } else {
+        gram_rows<0, GRAM_SPLIT>(J, dr, di, w, mDL, lane, r);
+        gram_rows<GRAM_SPLIT, NT>(J, dr, di, w, mDL, lane, r + NGH);
+      }
     }
   }
   __syncthreads();
   // cross-warp sum in fixed order; thread t < 96 owns slot t of the per-warp partials
   if (threadIdx.x < NGP) {
-    const int gidx = butterfly_slot_index(threadIdx.x);
+    // gradient only: slot t < 12 holds Gram entry (0, t) = packed index t
+    const int gidx = grad_only ? (threadIdx.x < NT ? (int)threadIdx.x : -1) : butterfly_slot_index(threadIdx.x);
     if (gidx >= 0) {
       for (int s = 0; s < ns; ++s) {
         double t = 0.0;
@@ -468,6 +527,7 @@ static __global__ void combine_fisher_kernel(const double* __restrict__ partial,
   if (t >= B * NG) return;
   const long long b = t / NG;
   const int idx = (int)(t % NG);
+  if (!outF && idx >= NT) return;          // gradient only: the kernel wrote row 0 of the Gram matrix only
   double sum = 0.0;
   for (int i = 0; i < n_slices; ++i) sum += partial[((size_t)i * (size_t)B + (size_t)b) * NG + idx];
   // W_A is 1 with all tangents 0 only for out-of-domain samples (prep_samples_du_kernel)

@@ -43,10 +43,10 @@ using Fn = ResponseFn;
 #else
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, long long B, const double* bins, long long N,
-                   const DetC& dc, int n_det, int det, double* partial) {
+                   const DetC& dc, int n_det, int det, int grad_only, double* partial) {
   static bool configured = false;
   if (cudaError_t e = opt_in_smem(fisher_kernel<KIND, CM>, fisher_smem_bytes(), configured); e != cudaSuccess) return e;
-  fisher_kernel<KIND, CM><<<g, FBLOCK, fisher_smem_bytes(), st>>>(consts, B, bins, N, dc, n_det, det, partial);
+  fisher_kernel<KIND, CM><<<g, FBLOCK, fisher_smem_bytes(), st>>>(consts, B, bins, N, dc, n_det, det, grad_only, partial);
   return cudaSuccess;
 }
 using Fn = FisherFn;

@@ -13,7 +13,7 @@ using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const doubl
 using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
                                    long long, const DetC&, int, int, double2*);
 using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&,
-                                 int, int, double*);
+                                 int, int, int, double*);
 
 // half 0: class masks 1..7, half 1: masks 8..15; each returns nullptr for a mask outside its half
 #define PESPACE_DECLARE_INST(FN, name) \

@@ -109,13 +109,15 @@ int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t 
 
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
                            double* h_out_grad) {
-  if (!s || !s->want_fisher || !h_params || !h_out_F || B <= 0 || B > s->max_B || !s->have_psd) return PESPACE_EINVAL;
+  if (!s || !s->want_fisher || !h_params || (!h_out_F && !h_out_grad) || B <= 0 || B > s->max_B || !s->have_psd)
+    return PESPACE_EINVAL;
   if (h_out_grad && !s->have_data) return PESPACE_EINVAL;
   CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
   const int rc = pespace_fisher(s->d_params, B, h_out_grad ? s->d_data : nullptr, s->d_psd, &s->grid, &s->model,
-                                s->d_F, h_out_grad ? s->d_grad : nullptr, s->d_ws_f, s->ws_f_bytes, s->st);
+                                h_out_F ? s->d_F : nullptr, h_out_grad ? s->d_grad : nullptr, s->d_ws_f, s->ws_f_bytes,
+                                s->st);
   if (rc != PESPACE_OK) return rc;
-  CU(cudaMemcpyAsync(h_out_F, s->d_F, (size_t)B * NPAR * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
+  if (h_out_F) CU(cudaMemcpyAsync(h_out_F, s->d_F, (size_t)B * NPAR * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
   if (h_out_grad) CU(cudaMemcpyAsync(h_out_grad, s->d_grad, (size_t)B * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
   CU(cudaStreamSynchronize(s->st));
   return PESPACE_OK;

@@ -338,6 +338,28 @@ def test_fisher_edge_cases_and_determinism(P):
     assert (np.abs(F[ok] - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
 
 
+def test_fisher_gradient_only_mode(P):
+    """pespace_fisher with d_out_F = NULL returns d lnL / d theta alone: within tolerance of the oracle and of the
+    full call (the reduction tree differs, so not bit-identical), deterministic, also through a session."""
+    wl = W.config(5, B=13, N=2500)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    fis = P.Fisher(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    none, g = fis(dev(wl.params), grad_only=True)
+    assert none is None
+    g = g.cpu().numpy()
+    Fo, go = oracle.fisher(wl.params, data, psd, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    rr = -2.0 * oracle.loglike(wl.params, data, psd, wl.grid, wl.model)
+    assert (np.abs(g - go) / (d * np.sqrt(rr)[:, None])).max() <= TOL_F
+    assert np.array_equal(g, fis(dev(wl.params), grad_only=True)[1].cpu().numpy())
+    ses = P.Session(wl.grid, wl.model, wl.B, want_fisher=True)
+    ses.set_data(data, psd)
+    assert np.array_equal(ses.fisher(wl.params, grad_only=True)[1], g)
+    ses.close()
+    with pytest.raises(P.PespaceError):
+        P.Fisher(None, dev(psd), wl.grid, wl.model, wl.B)(dev(wl.params), grad_only=True)
+
+
 def test_fisher_gradient_is_the_derivative_of_loglike(P):
     """d lnL / d theta_i from pespace_fisher against a central difference of pespace_loglike (GPU only):
     ties the two entry points together at a size where the oracle would take minutes."""
