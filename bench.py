@@ -293,21 +293,14 @@ def run_ours(args):
     # (theta, data set, PSD) from pinned host memory to the device and reads the result back, all inside
     # the timed region.  e2e_resident_data: the sampler-facing use, data set copied once, theta per step.
     e2e_steps = max(1, min(args.steps, 10))
+    ses = P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
     if tab_mode:
-        # no host-buffer C entry point for tables yet: the e2e leg goes through the Python binding, copying theta and
-        # the step's tables (and, in the "full" variant, data and PSD) from pinned host memory with torch
         res_h = torch.empty(B, dtype=torch.float64).pin_memory()
-        state = {"lik": lik}
 
         def e2e_step(i, copy_data):
             if copy_data:
-                state["lik"] = P.LikelihoodTab(data_h.to(device, non_blocking=True), psd_h.to(device, non_blocking=True),
-                                               wl.grid, wl.model, B)
-            t = P.WaveTable(*(x.to(device, non_blocking=True) for x in tabs_h[i % n_batches]))
-            state["lik"](params_h[i % n_batches].to(device, non_blocking=True), t, out_d)
-            res_h.copy_(out_d)
-            torch.cuda.synchronize()
-    ses = None if tab_mode else P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
+                ses.set_data(data_h, psd_h)
+            ses.loglike_tab(params_h[i % n_batches], tabs_h[i % n_batches], res_h)
     grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
     if not tab_mode:
         res_h = torch.empty((B, P.NPAR, P.NPAR) if fisher_mode else (B,), dtype=torch.float64).pin_memory()
@@ -330,8 +323,7 @@ def run_ours(args):
         e2e_ms = (time.perf_counter() - t0) * 1e3                           # the calls are synchronous
         e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
         e2e[key] = e2e_units / (e2e_max_ms * 1e-3)
-    if ses is not None:
-        ses.close()
+    ses.close()
     nbytes = lambda t: t.numel() * t.element_size()
     h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h) + (sum(nbytes(x) for x in tabs_h[0]) if tab_mode else 0)
     d2h = nbytes(res_h) + (nbytes(grad_h) if fisher_mode else 0)
@@ -399,8 +391,8 @@ def run_ours(args):
         "clocks": clocks,
         "e2e": {"value": e2e["full"], "unit": unit, "h2d_bytes_per_step": int(h2d),
                 "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-                "api": ("Python binding (LikelihoodTab): theta, the step's waveform tables, data set and PSD copied from "
-                        "pinned host memory with torch, lnL read back" if tab_mode else
+                "api": ("pespace_session_set_data + pespace_session_loglike_tab per step: theta, the step's waveform "
+                        "tables, data set and PSD copied from pinned host memory, lnL read back" if tab_mode else
                         "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
                         " per step: theta, data set and PSD copied from pinned host memory, result read back"),
                 "value_resident_data": e2e["resident"],

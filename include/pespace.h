@@ -154,6 +154,12 @@ int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t 
  * data set; the Fisher matrix alone needs only the PSD).  h_out_F may be NULL: gradient only. */
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
                            double* h_out_grad);
+/* Tabulated mode waveforms through a session: h_fnodes [K] (checked here for strictly increasing order),
+ * h_amp, h_phase, h_tf [B][n_modes][K] as in pespace_wavetable but in HOST memory; they are copied to the device
+ * with theta on every call (the tables belong to the batch).  Device buffers are allocated on first use. */
+int pespace_session_loglike_tab(pespace_session* s, const double* h_params, int64_t B, int64_t K,
+                                const double* h_fnodes, const double* h_amp, const double* h_phase,
+                                const double* h_tf, double* h_out_lnL);
 /* Waits for the session's stream and frees everything the session owns. */
 int pespace_session_destroy(pespace_session* s);
 

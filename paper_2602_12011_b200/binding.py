@@ -19,7 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike",
-           "pespace_session_fisher", "pespace_session_destroy",
+           "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
            "pespace_launch_count", "pespace_strerror",
            "pespace_version")
@@ -68,6 +68,7 @@ def _load():
     L.pespace_session_set_data.argtypes = [vp, vp, vp]
     L.pespace_session_loglike.argtypes = [vp, vp, i64, vp]
     L.pespace_session_fisher.argtypes = [vp, vp, i64, vp, vp]
+    L.pespace_session_loglike_tab.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp]
     L.pespace_session_destroy.argtypes = [vp]
     L.pespace_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
     L.pespace_profile_enable.argtypes = [C.c_int]
@@ -326,6 +327,23 @@ class Session:
             out = np.empty(p.shape[0], dtype=np.float64)
         op, o = _host_ptr(out, np.float64, "out")
         _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
+        return out
+
+    def loglike_tab(self, params, table, out=None):
+        """table = (fnodes [K], amp, phase, tf [B][n_modes][K]) as host arrays / CPU tensors"""
+        pp, p = _host_ptr(params, np.float64, "params")
+        B = int(p.shape[0])
+        (fp, fn), (ap, a), (hp, ph), (tp, tf) = (_host_ptr(x, np.float64, n) for x, n in
+                                                 zip(table, ("fnodes", "amp", "phase", "tf")))
+        K = int(fn.shape[0])
+        nm = bin(int(self.model.mode_mask)).count("1")
+        for x in (a, ph, tf):
+            if tuple(x.shape) != (B, nm, K):
+                raise PespaceError(f"table arrays must be [B={B}][n_modes={nm}][K={K}]")
+        if out is None:
+            out = np.empty(B, dtype=np.float64)
+        op, o = _host_ptr(out, np.float64, "out")
+        _check(_lib.pespace_session_loglike_tab(self._h, pp, B, K, fp, ap, hp, tp, op), "pespace_session_loglike_tab")
         return out
 
     def fisher(self, params, with_grad: bool = True, out_F=None, out_grad=None, grad_only: bool = False):

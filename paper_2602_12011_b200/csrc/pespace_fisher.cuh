@@ -23,9 +23,21 @@
 
 namespace pespace {
 
-constexpr int FBLOCK = 128;   // threads = bins per chunk
-constexpr int FTILE = 4;      // samples per block
-constexpr int FCHUNKS = 16;   // chunks per block
+#ifndef PESPACE_FBLOCK
+#define PESPACE_FBLOCK 128
+#endif
+#ifndef PESPACE_FMINB
+#define PESPACE_FMINB 2
+#endif
+constexpr int FBLOCK = PESPACE_FBLOCK;   // threads = bins per chunk
+#ifndef PESPACE_FTILE
+#define PESPACE_FTILE 4
+#endif
+#ifndef PESPACE_FCHUNKS
+#define PESPACE_FCHUNKS 16
+#endif
+constexpr int FTILE = PESPACE_FTILE;      // samples per block
+constexpr int FCHUNKS = PESPACE_FCHUNKS;  // chunks per block
 constexpr int NT = 12;        // value + 11 tangents
 constexpr int NJ = NT * 6;    // x (X, Y, Z) x (re, im)
 constexpr int NG = 78;        // upper triangle of the 12 x 12 Gram matrix
@@ -449,7 +461,7 @@ __device__ __forceinline__ void gram_row0(const double* __restrict__ J, const do
 }
 
 template <int KIND, unsigned CMASK>
-__global__ void __launch_bounds__(FBLOCK, 2)
+__global__ void __launch_bounds__(FBLOCK, PESPACE_FMINB)
 fisher_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ bins /* [n_det][NBF][N] */,
               long long N, DetC dc, int n_det, int det, int grad_only,
               double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {

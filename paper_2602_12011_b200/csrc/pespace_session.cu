@@ -20,8 +20,10 @@ struct pespace_session {
   bool have_data = false, have_psd = false;
   cudaStream_t st = nullptr;
   double *d_params = nullptr, *d_data = nullptr, *d_psd = nullptr, *d_lnL = nullptr, *d_F = nullptr, *d_grad = nullptr;
-  void *d_ws = nullptr, *d_ws_f = nullptr;
-  size_t ws_bytes = 0, ws_f_bytes = 0;
+  void *d_ws = nullptr, *d_ws_f = nullptr, *d_ws_t = nullptr;
+  size_t ws_bytes = 0, ws_f_bytes = 0, ws_t_bytes = 0;
+  double* d_tab = nullptr;          // [fnodes K | amp | phase | tf], grown on demand (pespace_session_loglike_tab)
+  size_t tab_doubles = 0;
   size_t n_series() const { return (size_t)model.n_det * 3 * (size_t)grid.N; }
 };
 
@@ -30,7 +32,7 @@ namespace {
 void release(pespace_session* s) {
   if (!s) return;
   cudaFree(s->d_params); cudaFree(s->d_data); cudaFree(s->d_psd); cudaFree(s->d_lnL); cudaFree(s->d_F);
-  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f);
+  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab);
   if (s->st) cudaStreamDestroy(s->st);
   delete s;
 }
@@ -119,6 +121,43 @@ int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B
   if (rc != PESPACE_OK) return rc;
   if (h_out_F) CU(cudaMemcpyAsync(h_out_F, s->d_F, (size_t)B * NPAR * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
   if (h_out_grad) CU(cudaMemcpyAsync(h_out_grad, s->d_grad, (size_t)B * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
+  CU(cudaStreamSynchronize(s->st));
+  return PESPACE_OK;
+}
+
+int pespace_session_loglike_tab(pespace_session* s, const double* h_params, int64_t B, int64_t K,
+                                const double* h_fnodes, const double* h_amp, const double* h_phase, const double* h_tf,
+                                double* h_out_lnL) {
+  if (!s || !h_params || !h_out_lnL || !h_fnodes || !h_amp || !h_phase || !h_tf || B <= 0 || B > s->max_B || K < 4 ||
+      !s->have_data || !s->have_psd)
+    return PESPACE_EINVAL;
+  for (int64_t j = 0; j + 1 < K; ++j)
+    if (!(h_fnodes[j + 1] > h_fnodes[j])) return PESPACE_EINVAL;      // host memory: the node order can be checked
+  int n_modes = 0;
+  for (int i = 0; i < 5; ++i) n_modes += (s->model.mode_mask >> i) & 1u;
+  const size_t per = (size_t)B * n_modes * (size_t)K, need = (size_t)K + 3 * per;
+  if (need > s->tab_doubles) {
+    CU(cudaStreamSynchronize(s->st));
+    cudaFree(s->d_tab);
+    s->d_tab = nullptr; s->tab_doubles = 0;
+    if (cudaMalloc((void**)&s->d_tab, need * 8) != cudaSuccess) { cudaGetLastError(); return PESPACE_ENOMEM; }
+    s->tab_doubles = need;
+  }
+  if (!s->d_ws_t) {
+    s->ws_t_bytes = pespace_workspace_bytes_tab(s->max_B, &s->grid, &s->model);
+    if (cudaMalloc(&s->d_ws_t, s->ws_t_bytes) != cudaSuccess) { cudaGetLastError(); return PESPACE_ENOMEM; }
+  }
+  double *d_fn = s->d_tab, *d_amp = d_fn + K, *d_ph = d_amp + per, *d_tf = d_ph + per;
+  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  CU(cudaMemcpyAsync(d_fn, h_fnodes, (size_t)K * 8, cudaMemcpyHostToDevice, s->st));
+  CU(cudaMemcpyAsync(d_amp, h_amp, per * 8, cudaMemcpyHostToDevice, s->st));
+  CU(cudaMemcpyAsync(d_ph, h_phase, per * 8, cudaMemcpyHostToDevice, s->st));
+  CU(cudaMemcpyAsync(d_tf, h_tf, per * 8, cudaMemcpyHostToDevice, s->st));
+  const pespace_wavetable T = {K, d_fn, d_amp, d_ph, d_tf};
+  const int rc = pespace_loglike_tab(s->d_params, B, &T, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL, s->d_ws_t,
+                                     s->ws_t_bytes, s->st);
+  if (rc != PESPACE_OK) return rc;
+  CU(cudaMemcpyAsync(h_out_lnL, s->d_lnL, (size_t)B * 8, cudaMemcpyDeviceToHost, s->st));
   CU(cudaStreamSynchronize(s->st));
   return PESPACE_OK;
 }

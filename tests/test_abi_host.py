@@ -109,5 +109,30 @@ def test_session_argument_validation_without_a_device():
     assert L.pespace_session_set_data(None, None, None) == EINVAL
     assert L.pespace_session_loglike(None, None, 4, None) == EINVAL
     assert L.pespace_session_fisher(None, None, 4, None, None) == EINVAL
+    assert L.pespace_session_loglike_tab(None, None, 4, 8, None, None, None, None, None) == EINVAL
     assert L.pespace_session_destroy(None) == EINVAL
     assert L.pespace_loglike_host(None, 4, None, None, C.byref(g), C.byref(m), None) == EINVAL
+
+
+def test_tab_argument_validation_without_a_device():
+    """pespace_*_tab reject bad arguments before any CUDA call (include/pespace.h, tabulated mode waveforms)."""
+    from paper_2602_12011_b200 import binding as P
+    L = P.lib()
+    wl = W.config(2, B=4, N=64)
+    m, keep = P._model(wl.model)
+    g = P._grid(wl.grid)
+    EINVAL = -1
+    fake = 0x1000
+    good = P._WaveTable(16, fake, fake, fake, fake)
+    assert L.pespace_response_tab(fake, 4, None, fake, 64, C.byref(m), fake, None) == EINVAL
+    assert L.pespace_response_tab(fake, 4, C.byref(P._WaveTable(3, fake, fake, fake, fake)), fake, 64, C.byref(m), fake,
+                                  None) == EINVAL                               # K < 4
+    assert L.pespace_response_tab(fake, 4, C.byref(P._WaveTable(16, fake, None, fake, fake)), fake, 64, C.byref(m), fake,
+                                  None) == EINVAL                               # missing table array
+    assert L.pespace_response_tab(None, 4, C.byref(good), fake, 64, C.byref(m), fake, None) == EINVAL
+    assert L.pespace_loglike_tab(fake, 4, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 8, None) == EINVAL
+    assert L.pespace_loglike_tab(fake, 0, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 1 << 30,
+                                 None) == EINVAL
+    assert L.pespace_workspace_bytes_tab(0, C.byref(g), C.byref(m)) == 0
+    ws_tab, ws = L.pespace_workspace_bytes_tab(4, C.byref(g), C.byref(m)), L.pespace_workspace_bytes(4, C.byref(g), C.byref(m), 0)
+    assert ws_tab > ws > 0

@@ -162,3 +162,20 @@ def test_tab_full_size_sampled_parity(P):
     want = oracle.loglike_tab(wl.params[idx], sub, data, psd, wl.grid, wl.model)
     assert np.all(np.isfinite(got))
     assert np.all(np.abs(got[idx] - want) <= TOL_LNL * np.abs(want)), np.abs(got[idx] - want) / np.abs(want)
+
+
+def test_tab_session_matches_device_call(P):
+    """pespace_session_loglike_tab (host tables) is bit-identical to pespace_loglike_tab; unordered nodes rejected."""
+    wl = W.config(3, B=9, N=900)
+    f = wl.grid.freqs()
+    table = W.chirp_table(wl.params, wl.model.mode_mask, W.log_nodes(f[0], f[-1], 200))
+    data, psd = noisy_data(wl, table)
+    want = P.LikelihoodTab(dev(data), dev(psd), wl.grid, wl.model, wl.B)(dev(wl.params), dev_table(P, table)).cpu().numpy()
+    ses = P.Session(wl.grid, wl.model, 16)
+    ses.set_data(data, psd)
+    assert np.array_equal(ses.loglike_tab(wl.params, table), want)
+    assert np.array_equal(ses.loglike_tab(wl.params[:5], tuple(x if x.ndim == 1 else x[:5] for x in table)), want[:5])
+    bad = (table[0][::-1].copy(),) + table[1:]
+    with pytest.raises(P.PespaceError):
+        ses.loglike_tab(wl.params, bad)
+    ses.close()
