@@ -94,6 +94,13 @@ struct BinC { double fT, cf, lnf3, fm53, fm83, fm76, sth, cth; };   // fT = kTur
 
 // round to nearest integer without FRND/F2I (quarter-rate conversion unit): two full-rate DADDs
 __device__ __forceinline__ double rint_magic(double x) { return (x + kMagic) - kMagic; }
+// nearest multiple of one turn (kTurn = 2^10 pu) the same way: 1.5 * 2^62 has ulp 2^10 (|x| < 2^61)
+constexpr double kMagicTurn = 6917529027641081856.0;
+static_assert(kTurn == 1024.0, "kMagicTurn rounds to multiples of 2^10");
+__device__ __forceinline__ double whole_turns(double x) { return (x + kMagicTurn) - kMagicTurn; }
+// x * y modulo one turn with a single rounding: the multiple of kTurn nearest to the rounded product is removed
+// inside an fma (the exact product minus that multiple is at most ~kTurn/2 in magnitude)
+__device__ __forceinline__ double mul_mod_turn(double x, double y) { return fma(x, y, -whole_turns(x * y)); }
 
 // sin and cos of (pi/2) x, x in QUARTER TURNS, |x| < 2^30.  Octant reduction y = x - rint(x),
 // then near-minimax polynomials in y^2 on |y| <= 1/2 (max abs error 1.2e-16 / 1.8e-16,
@@ -230,7 +237,7 @@ __device__ __forceinline__ void eval_class(const BinC& bc, const double* __restr
   Q = fma(Q, v, sc[W_Q2]);
   Q = fma(Q, v2, sc[W_Q0]);
   double psi = ((MC == 1) ? bc.fm53 : S83[MC] * bc.fm53) * P;     // PN phase, pu (up to ~1e8 and beyond)
-  psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);         // mod one turn, exact
+  psi -= whole_turns(psi);                                         // mod one turn, exact
   psi += fma(MH[MC], sc[W_PH0], ftc);                              // + kTurn [f t_c - (m/2)(phi_c/pi + 1/8)]
   const double tau = ((MC == 1) ? bc.fm83 : S83[MC] * bc.fm83) * Q;   // kTurn (t_lm - t_c) / yr
 
@@ -304,10 +311,12 @@ __device__ __forceinline__ void eval_geom(const BinC& bc, const double* __restri
   double Er[3], Ei[3];
   {
     const double nun[3] = {nu0, nu1, nu2};
+    const double fTL = bc.fT * dc.Lbar;              // per bin: hoisted out of the sample loop
+    const double base = fma(bc.fT, kR, psi);         // phase at the guiding centre
 #pragma unroll
     for (int n = 0; n < 3; ++n) {
       double s, c;
-      sincos_pu<TAB>(fma(bc.fT, fma(dc.Lbar, nun[n], kR), psi), tab, s, c);
+      sincos_pu<TAB>(fma(fTL, nun[n], base), tab, s, c);
       Er[n] = c; Ei[n] = s;          // note: Ei holds +sin; the minus sign is carried below
     }
   }
@@ -341,8 +350,7 @@ __device__ __forceinline__ void eval_xyz(const BinC& bc, const double* __restric
                                          const double2* __restrict__ tab, double (&S)[6]) {
   const double tc = sc[W_TC];
   // kTurn f t_c in pu mod one turn, with the rounding error of the product recovered by fma
-  const double p = bc.fT * tc;
-  const double ftc = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
+  const double ftc = mul_mod_turn(bc.fT, tc);
   const double va = sc[W_A] * bc.cf, La = bc.lnf3;     // ln (pi Ms)^{1/3} is folded into W_P5, W_P6, W_Q6
   constexpr bool c0 = CMASK & 1u, c1 = CMASK & 2u, c2 = CMASK & 4u, c3 = CMASK & 8u;
   if (c0) eval_class<KIND, 0, true, TAB>(bc, sc, dc, tab, va, La, ftc, S);

@@ -121,7 +121,7 @@ __device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const dou
   Q = dfma(Q, v2, c4(sc, W_Q0));
   const double sp = S83[MC] * bc.fm53, sq = S83[MC] * bc.fm83;
   double psi = sp * P.v;
-  psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);
+  psi -= whole_turns(psi);
   o.psi = psi + fma(MHmc, cv(sc, W_PH0), ftc4);
   o.tau = sq * Q.v;
 #pragma unroll
@@ -494,8 +494,7 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double* __re
     for (int s = 0; s < ns; ++s) {
       const double* sc = csm + s * FS_STRIDE;
       const double tc = cv(sc, W_TC);
-      const double p = bc.fT * tc;
-      const double ftc4 = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
+      const double ftc4 = mul_mod_turn(bc.fT, tc);
       {
         bool first = true;
 #pragma unroll 1

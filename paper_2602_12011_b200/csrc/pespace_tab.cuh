@@ -112,8 +112,7 @@ __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[N
                                              const DetC& dc, const double2* __restrict__ tab, const TabC& T,
                                              long long b, double (&S)[6]) {
   const double tc = sc[W_TC];
-  const double p = bc.fT * tc;
-  const double ftc = fma(rint_magic(p * (1.0 / kTurn)), -kTurn, p) + fma(bc.fT, tc, -p);
+  const double ftc = mul_mod_turn(bc.fT, tc);
   const long long j = (long long)w[WT_J], j0 = (long long)w[WT_J0];
 #pragma unroll
   for (int i = 0; i < 6; ++i) S[i] = 0.0;
@@ -125,7 +124,7 @@ __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[N
     const double* A = T.amp + base + j0;
     const double P0 = P[0], dP = P[1] - P0, t0 = Tt[0], t1 = Tt[1];
     double psi = fma(w[WT_H01], dP, P0) * (kTurn / (2.0 * kPi));     // node part of Psi_tab, pu (up to ~1e8)
-    psi = fma(rint_magic(psi * (1.0 / kTurn)), -kTurn, psi);         // mod one turn, exact
+    psi -= whole_turns(psi);                                         // mod one turn, exact
     psi += fma(w[WT_C10], t0, w[WT_C11] * t1);                       // slope part (small)
     psi += fma((double)T.m[i], sc[W_PH0], ftc);                      // + kTurn [f t_c - m phi_c / 2 pi]
     const double tau = fma(w[WT_Q01], dP, fma(w[WT_Q10], t0, w[WT_Q11] * t1));   // kTurn t_tab / yr
