@@ -328,6 +328,27 @@ def run_ours(args):
     h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h) + (sum(nbytes(x) for x in tabs_h[0]) if tab_mode else 0)
     d2h = nbytes(res_h) + (nbytes(grad_h) if fisher_mode else 0)
 
+    # ---- optional: pespace_response on a slice of the batch (48 B written per (sample, bin, detector))
+    response_info = None
+    if args.response and not tab_mode:
+        Br = min(B, args.response_batch)
+        out_r = torch.empty((Br, len(wl.model.detectors), 3, N, 2), dtype=torch.float64, device=device)
+        pr = params_d[0][:Br].contiguous()
+        for _ in range(2):
+            P.response(pr, freqs_d, wl.model, out_r)
+        torch.cuda.synchronize()
+        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        r0.record()
+        for _ in range(5):
+            P.response(pr, freqs_d, wl.model, out_r)
+        r1.record()
+        torch.cuda.synchronize()
+        r_ms = r0.elapsed_time(r1) / 5
+        response_info = {"batch": Br, "ms_per_call": r_ms, "bin_evals_per_sec": Br * N / (r_ms * 1e-3),
+                         "bytes_written_per_call": out_r.numel() * 8,
+                         "write_gbs": out_r.numel() * 8 / (r_ms * 1e-3) / 1e9}
+        del out_r
+
     if rank != 0:
         return
 
@@ -401,6 +422,7 @@ def run_ours(args):
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
         "result_check": {"min": float(last.min()), "max": float(last.max())},
+        "response": response_info,
     }
     print(json.dumps(line), flush=True)
 
@@ -412,6 +434,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--response", action="store_true", help="also time pespace_response on a slice of the batch")
+    ap.add_argument("--response-batch", type=int, default=256)
     ap.add_argument("--grad-only", action="store_true",
                     help="config 5: d lnL / d theta only (pespace_fisher with d_out_F = NULL)")
     ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic",
