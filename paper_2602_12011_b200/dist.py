@@ -77,3 +77,34 @@ def gather_lnL(local: "np.ndarray", device=None) -> "np.ndarray":
     out = [torch.empty_like(x) for _ in range(dist.get_world_size())]
     dist.all_gather(out, x)
     return torch.cat(out).cpu().numpy()
+
+
+class ShardedLikelihood:
+    """Strong scaling over samples: every rank holds the same data set and the same batch of theta,
+    evaluates the samples [lo, hi) of `shard_bounds` with `local_eval` (e.g. a `binding.Likelihood`: tensor of
+    theta [b][11] -> tensor of lnL [b]) and one all-gather of ceil(B / G) doubles per rank restores the full lnL
+    vector on every rank, in sample order.  No other collective touches the data path; the result of each sample is
+    bit-identical to the single-GPU one (the reduction of a sample never crosses ranks)."""
+
+    def __init__(self, local_eval):
+        self.local_eval = local_eval
+
+    def __call__(self, params: "torch.Tensor") -> "torch.Tensor":
+        import torch
+        import torch.distributed as dist
+        B = params.shape[0]
+        if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
+            return self.local_eval(params)
+        rank, world = dist.get_rank(), dist.get_world_size()
+        lo, hi = shard_bounds(B, rank, world)
+        per = -(-B // world)
+        mine = torch.full((per,), float("nan"), dtype=torch.float64, device=params.device)
+        if hi > lo:
+            mine[:hi - lo] = self.local_eval(params[lo:hi].contiguous())
+        parts = [torch.empty_like(mine) for _ in range(world)]
+        dist.all_gather(parts, mine)
+        out = torch.empty(B, dtype=torch.float64, device=params.device)
+        for r, part in enumerate(parts):
+            rlo, rhi = shard_bounds(B, r, world)
+            out[rlo:rhi] = part[:rhi - rlo]
+        return out

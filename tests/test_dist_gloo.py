@@ -36,7 +36,12 @@ def _worker(rank: int, world: int, port: int, B: int, out_dir: str) -> None:
     t_max, units = pdist.aggregate(10.0 + rank, hi - lo)
     # weak scaling: every rank draws its own batch
     mine = W.config(2, B=4, N=8, param_seed=pdist.rank_seed(1000, rank)).params
-    np.savez(os.path.join(out_dir, f"r{rank}.npz"), full=full, t_max=t_max, units=units, mine=mine, lo=lo, hi=hi)
+    import torch
+    sharded = pdist.ShardedLikelihood(lambda p: torch.from_numpy(_stand_in_lnL(p.numpy())))
+    strong = sharded(torch.from_numpy(wl.params)).numpy()          # same batch on every rank, split and gathered
+    tiny = sharded(torch.from_numpy(wl.params[:1])).numpy()        # fewer samples than ranks: one rank idles
+    np.savez(os.path.join(out_dir, f"r{rank}.npz"), full=full, t_max=t_max, units=units, mine=mine, lo=lo, hi=hi,
+             strong=strong, tiny=tiny)
     import torch.distributed as dist
     dist.destroy_process_group()
 
@@ -53,6 +58,7 @@ def test_sample_sharding_world_size_2(tmp_path):
         got = np.concatenate([full[i * per:i * per + (res[i]["hi"] - res[i]["lo"])] for i in range(world)])
         assert np.array_equal(got, want)                        # gather restores sample order, bit for bit
         assert float(r["t_max"]) == 11.0 and float(r["units"]) == B      # MAX of times, SUM of units
+        assert np.array_equal(r["strong"], want) and np.array_equal(r["tiny"], want[:1])   # ShardedLikelihood
     assert int(res[0]["lo"]) == 0 and int(res[0]["hi"]) == int(res[1]["lo"]) and int(res[1]["hi"]) == B
     assert not np.array_equal(res[0]["mine"], res[1]["mine"])    # different batches per rank
     assert np.array_equal(res[0]["mine"], W.config(2, B=4, N=8, param_seed=1000).params)   # rank 0 keeps the seed
