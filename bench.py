@@ -208,6 +208,9 @@ def run_ours(args):
     # ---- inputs: synthetic, seeded; the injection comes from this library's own response call
     fisher_mode = args.config == 5
     tab_mode = args.waveform == "tab"
+    mixed_mode = args.precision == "mixed"
+    if mixed_mode and (fisher_mode or tab_mode):
+        raise SystemExit("bench.py: --precision mixed applies to the analytic likelihood configs 2-4")
     if tab_mode and fisher_mode:
         raise SystemExit("bench.py: --waveform tab applies to the likelihood configs 2-4")
     n_batches = 2 if tab_mode else 4
@@ -256,7 +259,7 @@ def run_ours(args):
         elif tab_mode:
             lik(params_d[i % n_batches], tabs_d[i % n_batches], out_d)
         else:
-            lik(params_d[i % n_batches], out_d)
+            lik(params_d[i % n_batches], out_d, mixed=mixed_mode)
 
     for i in range(args.warmup):
         step(i)
@@ -353,7 +356,7 @@ def run_ours(args):
         return
 
     # ---- roofline of the dominant kernel (per launch, timed live with CUDA events in the library)
-    kernel = "fisher" if fisher_mode else ("loglike_tab" if tab_mode else "loglike")
+    kernel = "fisher" if fisher_mode else ("loglike_tab" if tab_mode else ("loglike_mixed" if mixed_mode else "loglike"))
     metric, unit = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (METRIC, UNIT)
     peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
     dfma_tflops, _ = P.fp64_peak(8192, mode=0)
@@ -406,7 +409,7 @@ def run_ours(args):
     line = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64", "data": "synthetic",
+        "dtype": "f64+f32 (mixed: FP64 phases, FP32 geometry)" if mixed_mode else "f64", "data": "synthetic",
         "bin_evals_per_sec": value * N,
         "config": workload_config(wl, args, l2="256 MiB buffer rewritten before every step, inside the timed region"),
         "clocks": clocks,
@@ -434,6 +437,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
+    ap.add_argument("--precision", choices=["f64", "mixed"], default="f64",
+                    help="mixed: pespace_loglike_mixed (FP64 phases, FP32 geometry; SURVEY 8(f) N2) in the device-timed leg")
     ap.add_argument("--response", action="store_true", help="also time pespace_response on a slice of the batch")
     ap.add_argument("--response-batch", type=int, default=256)
     ap.add_argument("--grad-only", action="store_true",

@@ -100,6 +100,17 @@ int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, 
                    const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                    double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* Mixed-precision twin of pespace_loglike (the paper's float32 mode for searches and coarse
+ * maximisation).  Same arguments, same workspace size.  Every phase that enters an exponential
+ * (PN phase, 2 pi f t_c, Doppler phases, their sum and its reduction modulo one turn) stays FP64; the t_lm polynomial,
+ * orbit, projections, arm weights, sines / cosines of the reduced phases, TDI sums and the whitened residual run in
+ * FP32.  Accuracy ~1e-6 relative on the response, a few 1e-6 of max(|lnL|, <h|h>/2) on lnL (tests/test_gpu_mixed.py):
+ * NOT a substitute for pespace_loglike where |delta lnL| << 1 matters.  Inputs must be detector-like in magnitude:
+ * sqrt(4 df / S_n) |h| x 2^-64 and x 2^64 must both be representable in FP32 (not checked). */
+int pespace_loglike_mixed(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                          const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                          void* d_workspace, size_t workspace_bytes, void* stream);
+
 /* ---- Tabulated mode waveforms.  In the paper the per-mode amplitude, phase and
  * time-frequency map t_f come from the waveform generator (PhenomXAS / PhenomXHM) and the
  * response is built on them (Eq. 4, 5).  These calls take them as tables, so that any externally generated

@@ -17,7 +17,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
-           "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
+           "pespace_loglike_mixed", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike",
            "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
@@ -57,6 +57,7 @@ def _load():
     L.pespace_workspace_bytes.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model), C.c_int]
     L.pespace_workspace_bytes.restype = sz
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
+    L.pespace_loglike_mixed.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
     L.pespace_response_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, i64, C.POINTER(_Model), vp, vp]
@@ -155,16 +156,18 @@ class Likelihood:
         self.ws_bytes = workspace_bytes(max_batch, grid, model)
         self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=self.data.device)
 
-    def __call__(self, params: torch.Tensor, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    def __call__(self, params: torch.Tensor, out: Optional[torch.Tensor] = None, mixed: bool = False) -> torch.Tensor:
+        """mixed=True: pespace_loglike_mixed (FP64 phases, FP32 geometry; ~1e-6 relative accuracy)."""
         p = _dev(params, "params")
         B = p.shape[0]
         if B > self.max_batch:
             raise PespaceError("batch larger than the workspace was sized for")
         if out is None:
             out = torch.empty(B, dtype=torch.float64, device=p.device)
-        _check(_lib.pespace_loglike(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g),
-                                    C.byref(self._m), _dev(out, "out").data_ptr(), self.ws.data_ptr(),
-                                    self.ws_bytes, _stream_ptr()), "pespace_loglike")
+        fn, name = (_lib.pespace_loglike_mixed, "pespace_loglike_mixed") if mixed else \
+            (_lib.pespace_loglike, "pespace_loglike")
+        _check(fn(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g), C.byref(self._m),
+                  _dev(out, "out").data_ptr(), self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), name)
         return out
 
 

@@ -570,7 +570,7 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
   if (k >= G.N) return;
   const DetC& dc = A.det[det];
   BinC bc = make_bin(fma((double)k, G.df, G.f0), dc.Lbar);
-  if (!fold_f76) bc.fm76 = 1.0;          // tabulated waveforms carry their own amplitude (pespace_tab.cuh)
+  if (!fold_f76) bc.fm76 = 1.0;          // 0: tabulated waveforms carry their own amplitude (pespace_tab.cuh)
   double gr, gi;
   tdi_prefactor(bc, dc.gen, gr, gi);
   const double g2 = gr * gr + gi * gi;
@@ -586,9 +586,16 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
     const double Sn = psd[idx];
     const bool use = isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
     const double sc_ = use ? nrm[c] / g2 : 0.0;
-    o[(BF_DR + c) * N] = (d.x * gr + d.y * gi) * sc_;          // d * conj(g) / |g|^2 * nrm
-    o[(BF_DI + c) * N] = (d.x * gi - d.y * gr) * sc_;          // MINUS the imaginary part: eval_xyz returns (Re, -Im)
-    o[(BF_W + c) * N] = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+    double vr = (d.x * gr + d.y * gi) * sc_;                    // d * conj(g) / |g|^2 * nrm
+    double vi = (d.x * gi - d.y * gr) * sc_;                    // MINUS the imaginary part: eval_xyz returns (Re, -Im)
+    double vw = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+    if (fold_f76 == 2) {           // mixed-precision kernel (pespace_mixed.cuh): whitened data, sqrt(w) / 2^64
+      const double sq = sqrt(vw);
+      vr *= sq; vi *= sq; vw = sq * (1.0 / 18446744073709551616.0);
+    }
+    o[(BF_DR + c) * N] = vr;
+    o[(BF_DI + c) * N] = vi;
+    o[(BF_W + c) * N] = vw;
   }
 }
 
