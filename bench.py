@@ -369,6 +369,8 @@ def run_ours(args):
     per_det = [FP64_OPS_PER_UNIT.get((kernel, d.kind, cmask)) for d in wl.model.detectors]
     known = [o for o in per_det if o]
     ops = {k: sum(o[k] for o in known) / len(known) for k in ("dfma", "dmul", "dadd")} if len(known) == n_det else None
+    if fisher_mode and args.grad_only:
+        ops = None                    # no ncu op counts for the gradient-only variant
     roofline = {"bound": "alu", "kernel": f"{kernel}_kernel", "achieved": None, "peak": peak_tflops,
                 "unit": "TFLOP/s", "frac": None, "traffic": DRAM_TRAFFIC_PER_LAUNCH.get(args.config)}
     if ops:
@@ -420,6 +422,8 @@ def run_ours(args):
                         "tables, data set and PSD copied from pinned host memory, lnL read back" if tab_mode else
                         "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
                         " per step: theta, data set and PSD copied from pinned host memory, result read back"),
+                "precision_note": ("the host-buffer session calls run the FP64 kernel; --precision mixed applies to the "
+                                   "device-timed leg only") if mixed_mode else None,
                 "value_resident_data": e2e["resident"],
                 "resident_data_note": "same call with the data set copied once (sampler use): theta in, result out"},
         "gpu_launches": int(launches),
