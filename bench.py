@@ -154,6 +154,13 @@ def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0, tab
     for _ in range(steps):
         call(wl.params[idx])
     dt = time.perf_counter() - t0
+    # one-thread figure (the paper's own CPU protocol is one core): two samples on one thread
+    oracle.set_threads(1)
+    t1 = time.perf_counter()
+    call(wl.params[idx[:2]])
+    one_thread = 2 / (time.perf_counter() - t1) * scale
+    oracle.set_threads(0)
+    oracle_timed.one_thread = one_thread
     bins = f"all {wl.grid.N} bins" if not fisher else f"the first {wl.grid.N} of {full.grid.N} bins (rate scaled by {scale:.5f})"
     desc = (f"{n_samples} of {full.B} samples (evenly spaced) x {bins} per pass, {steps} pass(es), "
             f"{dt / steps:.1f} s per pass, OpenMP over samples")
@@ -176,7 +183,8 @@ def run_reference(args):
         "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "bin_evals_per_sec": rate * wl.grid.N,
         "config": workload_config(wl, args, l2="n/a (CPU)"),
-        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+                         "value_one_thread": oracle_timed.one_thread},
         "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
@@ -407,7 +415,8 @@ def run_ours(args):
     if not args.no_cpu_baseline and world == 1:
         rate, sec, cores, desc = oracle_timed(args.config, args.ref_samples, 1,
                                               tab_nodes=args.tab_nodes if tab_mode else 0)
-        cpu_baseline = {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": desc}
+        cpu_baseline = {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": desc,
+                        "value_one_thread": oracle_timed.one_thread}
 
     line = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
