@@ -11,6 +11,11 @@
 // One source, three scalar types: double (the oracle), Dual<11> (forward-mode
 // derivatives, O12) and __float128 (pin P14: is double enough?).
 //
+// Tabulated mode waveforms (T1 block below, reading T1 of DESIGN.md): the interpolation is an
+// approximation of the caller's waveform, so it follows its definition step by step (binary search, cubic Hermite
+// with slopes 2 pi t_j, its derivative, 4-node Lagrange); pinned by the T1 tests (exactness on cubics, reproduction
+// of the analytic path at fourth order, extrinsic scalings, band limits, brute-force Whittle sum).
+//
 // Pins (tests/test_oracle_pins.py): P1-P16 of SURVEY.md 8(c).  "Parity
 // unpinned": absolute values of the Taiji-/TianQin-like results (G8, G13 are
 // proposals, not in the paper) and the spin terms of G3 beyond "vanish at
