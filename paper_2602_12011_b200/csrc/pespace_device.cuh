@@ -531,7 +531,10 @@ static __global__ void prep_samples_kernel(const double* __restrict__ params, lo
 }
 
 // ---------------------------------------------------------------------------------------------
-constexpr int BLOCK = 256;      // threads = bins per block
+#ifndef PESPACE_BLOCK
+#define PESPACE_BLOCK 256
+#endif
+constexpr int BLOCK = PESPACE_BLOCK;      // threads = bins per block
 constexpr int TILE = 64;        // samples staged in shared memory per block
 
 // dynamic shared memory of the likelihood / response kernels: [trig table | sample constants | warp partials]
@@ -606,7 +609,12 @@ template <int KIND, unsigned CMASK>
 #ifndef PESPACE_MINB1
 #define PESPACE_MINB1 3
 #endif
-__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? PESPACE_MINB1 : 2)
+// multi-class kernels: ONE resident block per SM (255 registers, no spills) beats two at 128 registers with 58
+// spill instructions per unit (config 3: 59.5 vs 63.9 ms); 8 warps per SM keep the FP64 issue port busy
+#ifndef PESPACE_MINBM
+#define PESPACE_MINBM 1
+#endif
+__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? PESPACE_MINB1 : PESPACE_MINBM)
 loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
                const double* __restrict__ bins /* [n_det][NBF][N] */, long long N, DetC dc, int n_det, int det,
                double* __restrict__ partial /* [n_det][gridDim.x][B] */) {

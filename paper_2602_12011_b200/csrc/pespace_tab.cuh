@@ -150,8 +150,11 @@ __device__ __forceinline__ void stage_tile_n(double* smem, const double* __restr
 }
 
 // likelihood from tables: grid (bin blocks, sample tiles of TAB_TILE); one launch per detector
+#ifndef PESPACE_MINBT
+#define PESPACE_MINBT 2
+#endif
 template <int KIND>
-__global__ void __launch_bounds__(BLOCK, 2)
+__global__ void __launch_bounds__(BLOCK, PESPACE_MINBT)
 loglike_tab_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, TabC T,
                    const double* __restrict__ bins /* [n_det][NBF][N] */, const double* __restrict__ wt /* [NWT][N] */,
                    long long N, DetC dc, int n_det, int det, double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
