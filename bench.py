@@ -48,7 +48,7 @@ SM_COUNT, FP64_LANES_PER_SM = 148, 64
 # kernel has no redundant evaluation, so executed = algorithmic.  flop = 2*DFMA + DMUL + DADD.
 FP64_OPS_PER_UNIT = {
     # (kernel, detector kind, mode-class mask): per (sample, bin, detector); profiles/r01_kernels_ncu.md
-    ("loglike", 0, 2): {"dfma": 140.00, "dmul": 53.75, "dadd": 40.53},      # kind 0, (2,2) only  -- config 2
+    ("loglike", 0, 2): {"dfma": 140.00, "dmul": 53.02, "dadd": 40.53},      # kind 0, (2,2) only  -- config 2
     ("loglike", 0, 15): {"dfma": 554.00, "dmul": 188.11, "dadd": 101.08},   # kind 0, five modes  -- configs 3, 4
     ("loglike", 1, 15): {"dfma": 526.00, "dmul": 224.11, "dadd": 109.08},   # kind 1, five modes  -- config 4
     ("fisher", 0, 15): {"dfma": 3438.00, "dmul": 1430.25, "dadd": 828.15},  # config 5
@@ -57,7 +57,7 @@ FP64_OPS_PER_UNIT = {
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (same ncu captures; config 4:
 # mean of the three launches of a step)
-DRAM_TRAFFIC_PER_LAUNCH = {2: 36.00e6 + 7.51e6, 3: 36.18e6 + 5.39e6, 4: (40.4e6 + 36.6e6 + 42.1e6 + 37.2e6 + 41.3e6 + 37.9e6) / 3,
+DRAM_TRAFFIC_PER_LAUNCH = {2: 35.91e6 + 5.18e6, 3: 36.18e6 + 5.39e6, 4: (40.4e6 + 36.6e6 + 42.1e6 + 37.2e6 + 41.3e6 + 37.9e6) / 3,
                            5: 35.8e6 + 6.8e6}
 # SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
 # kept for reference only -- the reduced algorithm needs less than half of it.

@@ -606,8 +606,10 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
 __host__ __device__ constexpr int popc4(unsigned m) { return (m & 1) + ((m >> 1) & 1) + ((m >> 2) & 1) + ((m >> 3) & 1); }
 
 template <int KIND, unsigned CMASK>
+// single-class kernels: two resident blocks per SM (128 registers) run 1.7 % faster than three (80 registers, with
+// re-materialised constants and a spill), and 5 % faster than one
 #ifndef PESPACE_MINB1
-#define PESPACE_MINB1 3
+#define PESPACE_MINB1 2
 #endif
 // multi-class kernels: ONE resident block per SM (255 registers, no spills) beats two at 128 registers with 58
 // spill instructions per unit (config 3: 59.5 vs 63.9 ms); 8 warps per SM keep the FP64 issue port busy
