@@ -172,8 +172,11 @@ constexpr size_t mixed_smem_bytes() {
          sizeof(float) * (size_t)MIX_TILE * SMEM_STRIDE + sizeof(double) * (size_t)(BLOCK / 32) * MIX_TILE;
 }
 
+#ifndef PESPACE_MINBX
+#define PESPACE_MINBX 2
+#endif
 template <int KIND>
-__global__ void __launch_bounds__(BLOCK, 3)
+__global__ void __launch_bounds__(BLOCK, PESPACE_MINBX)
 loglike_mixed_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, unsigned cmask,
                      const double* __restrict__ bins /* [n_det][NBF][N], built with fold mode 2 */, long long N, DetC dc,
                      int n_det, int det, double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
