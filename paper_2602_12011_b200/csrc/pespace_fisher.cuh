@@ -96,6 +96,17 @@ __constant__ double kClassCB[4] = {1.2599210498948731648, 1.0, 0.873580464736298
 __constant__ double kClassLN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
 __constant__ double kClassS83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
 
+// Horner step a * x + c on (value; M, q, chi1, chi2) where x depends on M only (x = (xv; xd, 0, 0, 0)): the products
+// with the structural zeros of x are not formed (6 instead of 9 instructions)
+__device__ __forceinline__ Du<4> horner_m(const Du<4>& a, double xv, double xd, const Du<4>& c) {
+  Du<4> r;
+  r.v = fma(a.v, xv, c.v);
+  r.d[0] = fma(a.v, xd, fma(a.d[0], xv, c.d[0]));
+#pragma unroll
+  for (int i = 1; i < 4; ++i) r.d[i] = fma(a.d[i], xv, c.d[i]);
+  return r;
+}
+
 __device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const double* __restrict__ sc, double ftc4,
                                                ClassScal& o) {
   const double* CB = kClassCB;
@@ -106,19 +117,19 @@ __device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const dou
   Du<4> v(0.0);
   v.v = cv(sc, W_A) * sv; v.d[0] = ct(sc, W_A, 0) * sv;
   const double L = bc.lnf3 + LN3[MC];       // ln (pi Ms)^{1/3} and its tangent are folded into W_P5, W_P6, W_Q6
-  const Du<4> v2 = v * v;
-  Du<4> P = dfma(c4(sc, W_P7), v, dfma(L, c4(sc, W_P6L), c4(sc, W_P6)));
-  P = dfma(P, v, dfma(L, c4(sc, W_P5L), c4(sc, W_P5)));
-  P = dfma(P, v, c4(sc, W_P4));
-  P = dfma(P, v, c4(sc, W_P3));
-  P = dfma(P, v, c4(sc, W_P2));
-  P = dfma(P, v2, c4(sc, W_P0));
-  Du<4> Q = dfma(c4(sc, W_Q7), v, dfma(L, c4(sc, W_Q6L), c4(sc, W_Q6)));
-  Q = dfma(Q, v, c4(sc, W_Q5));
-  Q = dfma(Q, v, c4(sc, W_Q4));
-  Q = dfma(Q, v, c4(sc, W_Q3));
-  Q = dfma(Q, v, c4(sc, W_Q2));
-  Q = dfma(Q, v2, c4(sc, W_Q0));
+  const double vv = v.v, vd = v.d[0], v2v = vv * vv, v2d = 2.0 * vv * vd;      // v^2 and its M tangent
+  Du<4> P = horner_m(c4(sc, W_P7), vv, vd, dfma(L, c4(sc, W_P6L), c4(sc, W_P6)));
+  P = horner_m(P, vv, vd, dfma(L, c4(sc, W_P5L), c4(sc, W_P5)));
+  P = horner_m(P, vv, vd, c4(sc, W_P4));
+  P = horner_m(P, vv, vd, c4(sc, W_P3));
+  P = horner_m(P, vv, vd, c4(sc, W_P2));
+  P = horner_m(P, v2v, v2d, c4(sc, W_P0));
+  Du<4> Q = horner_m(c4(sc, W_Q7), vv, vd, dfma(L, c4(sc, W_Q6L), c4(sc, W_Q6)));
+  Q = horner_m(Q, vv, vd, c4(sc, W_Q5));
+  Q = horner_m(Q, vv, vd, c4(sc, W_Q4));
+  Q = horner_m(Q, vv, vd, c4(sc, W_Q3));
+  Q = horner_m(Q, vv, vd, c4(sc, W_Q2));
+  Q = horner_m(Q, v2v, v2d, c4(sc, W_Q0));
   const double sp = S83[MC] * bc.fm53, sq = S83[MC] * bc.fm83;
   double psi = sp * P.v;
   psi -= whole_turns(psi);
