@@ -81,6 +81,15 @@ __device__ __forceinline__ Du<3> ang(double v, double d0) {
   return r;
 }
 
+// a b - c d on 3-tangent duals with the subtraction fused into the products (14 instead of 18 instructions)
+__device__ __forceinline__ Du<3> prod_diff(const Du<3>& a, const Du<3>& b, const Du<3>& c, const Du<3>& d) {
+  Du<3> r;
+  r.v = fma(a.v, b.v, -(c.v * d.v));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) r.d[i] = fma(a.v, b.d[i], fma(a.d[i], b.v, -fma(c.v, d.d[i], c.d[i] * d.v)));
+  return r;
+}
+
 // phase-like scalars of one class handed from stage A to stage C
 struct ClassScal {
   double psi;        // phase, pu (reduced)
@@ -290,8 +299,8 @@ __device__ __forceinline__ void fisher_class(int MC, bool FIRST, const BinC& bc,
     G b1r, b1i, b2r, b2i;
     bracket(r, s1, k1, b1r, b1i);
     bracket(r, s2, k2, b2r, b2i);
-    const G Hpr = Wp[l1] * b1r - Wp[l2] * b2r, Hpi = Wp[l1] * b1i - Wp[l2] * b2i;
-    const G Hcr = Wc[l1] * b1r - Wc[l2] * b2r, Hci = Wc[l1] * b1i - Wc[l2] * b2i;
+    const G Hpr = prod_diff(Wp[l1], b1r, Wp[l2], b2r), Hpi = prod_diff(Wp[l1], b1i, Wp[l2], b2i);
+    const G Hcr = prod_diff(Wc[l1], b1r, Wc[l2], b2r), Hci = prod_diff(Wc[l1], b1i, Wc[l2], b2i);
     const double kp = cs.CKp.v, kc = cs.CKc.v;
     const double hr = fma(kp, Hpr.v, -kc * Hci.v), hi = fma(kp, Hpi.v, kc * Hcr.v);      // CKp Hp + i CKc Hc
     double Tr[3], Ti[3];
