@@ -57,7 +57,7 @@ extern "C" int pespace_loglike_mixed(const double* d_params, int64_t B, const do
     LAUNCHED();
     if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }
-  combine_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_partial, d_consts, B, (int)(n_det * nbb), stride, d_out_lnL);
+  combine_kernel<<<PESPACE_COMBINE_GRID(B), 0, st>>>(d_partial, d_consts, B, (int)(n_det * nbb), stride, d_out_lnL);
   LAUNCHED();
   return PESPACE_OK;
 }

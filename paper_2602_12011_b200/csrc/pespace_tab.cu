@@ -151,8 +151,7 @@ int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetab
     LAUNCHED();
     if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
   }
-  const int th = 128;
-  combine_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_partial, d_consts, B, (int)(model->n_det * p.nbb),
+  combine_kernel<<<PESPACE_COMBINE_GRID(B), 0, st>>>(d_partial, d_consts, B, (int)(model->n_det * p.nbb),
                                                                 p.stride, d_out_lnL);
   LAUNCHED();
   return PESPACE_OK;
