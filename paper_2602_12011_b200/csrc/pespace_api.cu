@@ -27,8 +27,8 @@ struct Plan {
   int n_det, stride;
   long long nbb;          // bin blocks
   long long ntile;        // sample tiles
-  size_t trig_bytes, consts_bytes, partial_bytes, bins_bytes;   // workspace: [trig table | sample constants | block
-                                                                // partials | per-bin table (likelihood only)]
+  size_t trig_bytes, consts_bytes, partial_bytes, bins_bytes;   // workspace: [trig table | per-bin table (likelihood
+                                                                // only) | sample constants | block partials]
 };
 Plan make_plan(long long B, long long N, int n_det) {
   Plan p;
@@ -151,6 +151,17 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
 int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
                     const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
                     void* d_workspace, size_t workspace_bytes, void* stream) {
+  return pespace::host::loglike_impl(d_params, B, d_data_AET, d_psd, grid, model, d_out_lnL, d_workspace, workspace_bytes,
+                                     stream, false);
+}
+
+}  // extern "C"
+
+// pespace_loglike with one extra switch for the session calls: bins_ready = the per-bin table (S0) at the head of the
+// workspace was written by an earlier call for the same data set, PSD, grid and model and is reused
+int pespace::host::loglike_impl(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                                const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                                void* d_workspace, size_t workspace_bytes, void* stream, bool bins_ready) {
   if (!d_params || !d_data_AET || !d_psd || !d_out_lnL || !d_workspace || B <= 0 || !grid_ok(grid) ||
       !model_ok(model))
     return PESPACE_EINVAL;
@@ -159,15 +170,15 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
   cudaStream_t st = (cudaStream_t)stream;
   const Plan p = make_plan(B, grid->N, model->n_det);
   double2* d_trig = (double2*)d_workspace;
-  double* d_consts = (double*)((char*)d_workspace + p.trig_bytes);
-  double* d_partial = (double*)((char*)d_workspace + p.trig_bytes + p.consts_bytes);
-  double* d_bins = (double*)((char*)d_workspace + p.trig_bytes + p.consts_bytes + p.partial_bytes);
+  double* d_bins = (double*)((char*)d_workspace + p.trig_bytes);           // B-independent offset: reusable across calls
+  double* d_consts = (double*)((char*)d_workspace + p.trig_bytes + p.bins_bytes);
+  double* d_partial = (double*)((char*)d_workspace + p.trig_bytes + p.bins_bytes + p.consts_bytes);
   int rc = run_prep(d_params, B, model, d_consts, d_trig, st);
   if (rc != PESPACE_OK) return rc;
   const unsigned cm = class_mask(model->mode_mask);
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
-  {
-    // S0: per-bin table of this data set, once per call
+  if (!bins_ready) {
+    // S0: per-bin table of this data set, once per call (once per data set through a session)
     const PrepArgs A = make_prep_args(model);
     const dim3 gb((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det);
     prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
@@ -187,6 +198,8 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
   LAUNCHED();
   return PESPACE_OK;
 }
+
+extern "C" {
 
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms) {
   if (iters <= 0 || !h_out_tflops || (mode != 0 && mode != 1)) return PESPACE_EINVAL;

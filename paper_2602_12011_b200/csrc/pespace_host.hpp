@@ -74,6 +74,12 @@ struct EvPair { cudaEvent_t a = nullptr, b = nullptr; };
 int prof_begin(EvPair& ev, cudaStream_t st);   // no-op unless profiling is enabled
 int prof_end(EvPair& ev, cudaStream_t st);
 
+// pespace_loglike with a switch for callers that keep the workspace between calls (pespace_session.cu): bins_ready =
+// the per-bin table at the head of the workspace is still valid for this data set, PSD, grid and model
+int loglike_impl(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                 const pespace_grid* grid, const pespace_model* model, double* d_out_lnL, void* d_workspace,
+                 size_t workspace_bytes, void* stream, bool bins_ready);
+
 // Fisher path (pespace_fisher.cu)
 size_t fisher_workspace_bytes(long long B, long long N, int n_det);
 

@@ -18,6 +18,7 @@ struct pespace_session {
   long long max_B = 0;
   int want_fisher = 0;
   bool have_data = false, have_psd = false;
+  bool bins_ready = false;          // the per-bin table in d_ws matches the current data set and PSD
   cudaStream_t st = nullptr;
   double *d_params = nullptr, *d_data = nullptr, *d_psd = nullptr, *d_lnL = nullptr, *d_F = nullptr, *d_grad = nullptr;
   void *d_ws = nullptr, *d_ws_f = nullptr, *d_ws_t = nullptr;
@@ -94,6 +95,7 @@ int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const
     CU(cudaMemcpyAsync(s->d_psd, h_psd, nS * 8, cudaMemcpyHostToDevice, s->st));
     s->have_psd = true;
   }
+  s->bins_ready = false;
   CU(cudaStreamSynchronize(s->st));   // the caller may reuse its buffers on return
   return PESPACE_OK;
 }
@@ -101,9 +103,10 @@ int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const
 int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL) {
   if (!s || !h_params || !h_out_lnL || B <= 0 || B > s->max_B || !s->have_data || !s->have_psd) return PESPACE_EINVAL;
   CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
-  const int rc = pespace_loglike(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL, s->d_ws,
-                                 s->ws_bytes, s->st);
-  if (rc != PESPACE_OK) return rc;
+  const int rc = loglike_impl(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL, s->d_ws, s->ws_bytes,
+                              s->st, s->bins_ready);      // the S0 table is built once per data set
+  if (rc != PESPACE_OK) { s->bins_ready = false; return rc; }
+  s->bins_ready = true;
   CU(cudaMemcpyAsync(h_out_lnL, s->d_lnL, (size_t)B * 8, cudaMemcpyDeviceToHost, s->st));
   CU(cudaStreamSynchronize(s->st));
   return PESPACE_OK;

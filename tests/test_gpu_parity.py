@@ -236,6 +236,12 @@ def test_session_matches_device_calls_and_oracle(P):
     Fd, gd = P.fisher(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model)
     assert np.array_equal(F, Fd.cpu().numpy()) and np.array_equal(g, gd.cpu().numpy())
     assert np.array_equal(F0, F)
+    # the per-bin table is cached per data set: a new data set must invalidate it
+    ses.set_data(np.zeros_like(data), None)
+    z = ses.loglike(wl.params)
+    assert np.array_equal(z, P.loglike(dev(wl.params), dev(np.zeros_like(data)), dev(psd), wl.grid, wl.model).cpu().numpy())
+    ses.set_data(data, None)
+    assert np.array_equal(ses.loglike(wl.params), a)
     with pytest.raises(P.PespaceError):
         ses.loglike(np.tile(wl.params, (2, 1)))                  # batch larger than max_B
     ses.close()
