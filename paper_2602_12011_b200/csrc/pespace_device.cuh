@@ -668,9 +668,10 @@ loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ tr
   if constexpr (popc4(CMASK) == 1) {
     // S9, single-class kernels: four samples per trip, reduced over the warp by a halving butterfly (two halving
     // levels, then three plain ones on ONE value: 6 shuffle-adds per 4 samples instead of 20).  After the halving
-    // levels the lanes with bits (4, 3) = (b4, b3) hold sample 2 b4 + b3 of the group.  The tile is staged with its
-    // tail clamped to sample B - 1 (stage_tile), so a ragged last group evaluates valid constants; only s < ns is kept.
-    for (int s0 = 0; s0 < ns; s0 += 4) {
+    // levels the lanes with bits (4, 3) = (b4, b3) hold sample 2 b4 + b3 of the group.  The ragged tail of a tile
+    // (fewer than four samples left) takes the plain five-level tree below.
+    const int ns4 = ns & ~3;
+    for (int s0 = 0; s0 < ns4; s0 += 4) {
       double a[4];
 #pragma unroll
       for (int j = 0; j < 4; ++j) a[j] = term(s0 + j);
@@ -680,7 +681,13 @@ loglike_kernel(const double* __restrict__ consts, const double2* __restrict__ tr
       double acc = (up3 ? k1 : k0) + __shfl_xor_sync(0xffffffffu, up3 ? k0 : k1, 8);
 #pragma unroll
       for (int o = 4; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-      if ((lane & 7) == 0) red[warp][s0 + (lane >> 3)] = acc;     // s0 + j < TILE always; slots >= ns are never read
+      if ((lane & 7) == 0) red[warp][s0 + (lane >> 3)] = acc;
+    }
+    for (int s = ns4; s < ns; ++s) {        // ragged tail of the tile (and batches of fewer than four samples)
+      double acc = term(s);
+#pragma unroll
+      for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+      if (lane == 0) red[warp][s] = acc;
     }
   } else {
     for (int s = 0; s < ns; ++s) {
