@@ -100,7 +100,7 @@ struct ClassScal {
 };
 
 // class constants, indexed by m - 1 at run time (the class loop of the Fisher kernel is NOT unrolled: the unrolled
-// body was 154 KB of code per kernel and stalled on instruction fetch, profiles/r01_fisher_kernel_ncu.md)
+// body was 154 KB of code per kernel and stalled on instruction fetch, profiles/r01_kernels_ncu.md)
 __constant__ double kClassCB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886905, 0.79370052598409973738};
 __constant__ double kClassLN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
 __constant__ double kClassS83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
