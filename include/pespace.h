@@ -159,7 +159,9 @@ int pespace_session_create(const pespace_grid* grid, const pespace_model* model,
 /* Copies the data set h_data_AET [n_det][3][N][2] and / or the PSD h_psd [n_det][3][N] to the
  * device (either pointer may be NULL: that array is left as it is). */
 int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const double* h_psd);
-/* h_params [B][11] -> h_out_lnL [B], B <= max_B.  PESPACE_EINVAL before data and PSD are set. */
+/* h_params [B][11] -> h_out_lnL [B], B <= max_B.  PESPACE_EINVAL before data and PSD are set.  The per-bin
+ * table of the data set (S0) is built by the first call after pespace_session_set_data and reused afterwards;
+ * lnL (and theta of batches up to 256 samples) travel through mapped pinned memory owned by the session. */
 int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL);
 /* h_params [B][11] -> h_out_F [B][11][11] and, if h_out_grad != NULL, h_out_grad [B][11] (needs the
  * data set; the Fisher matrix alone needs only the PSD).  h_out_F may be NULL: gradient only. */

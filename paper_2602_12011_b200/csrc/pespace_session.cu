@@ -23,6 +23,9 @@ struct pespace_session {
   double *d_params = nullptr, *d_data = nullptr, *d_psd = nullptr, *d_lnL = nullptr, *d_F = nullptr, *d_grad = nullptr;
   void *d_ws = nullptr, *d_ws_f = nullptr, *d_ws_t = nullptr;
   size_t ws_bytes = 0, ws_f_bytes = 0, ws_t_bytes = 0;
+  // zero-copy result path of pespace_session_loglike: combine_kernel writes lnL straight into mapped pinned host
+  // memory (no device-to-host copy call; theta of small batches goes the same way in the other direction)
+  double *h_lnL_pin = nullptr, *d_lnL_map = nullptr, *h_par_pin = nullptr, *d_par_map = nullptr;
   double* d_tab = nullptr;          // [fnodes K | amp | phase | tf], grown on demand (pespace_session_loglike_tab)
   size_t tab_doubles = 0;
   size_t n_series() const { return (size_t)model.n_det * 3 * (size_t)grid.N; }
@@ -34,6 +37,8 @@ void release(pespace_session* s) {
   if (!s) return;
   cudaFree(s->d_params); cudaFree(s->d_data); cudaFree(s->d_psd); cudaFree(s->d_lnL); cudaFree(s->d_F);
   cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab);
+  if (s->h_lnL_pin) cudaFreeHost(s->h_lnL_pin);
+  if (s->h_par_pin) cudaFreeHost(s->h_par_pin);
   if (s->st) cudaStreamDestroy(s->st);
   delete s;
 }
@@ -64,6 +69,11 @@ int pespace_session_create(const pespace_grid* grid, const pespace_model* model,
             cudaMalloc((void**)&s->d_psd, nS * 8) == cudaSuccess &&
             cudaMalloc((void**)&s->d_lnL, (size_t)max_B * 8) == cudaSuccess &&
             cudaMalloc(&s->d_ws, s->ws_bytes) == cudaSuccess;
+  constexpr int64_t kMappedThetaMax = 256;       // samples whose theta is read over the bus by the prep kernel
+  ok = ok && cudaHostAlloc((void**)&s->h_lnL_pin, (size_t)max_B * 8, cudaHostAllocMapped) == cudaSuccess &&
+       cudaHostGetDevicePointer((void**)&s->d_lnL_map, s->h_lnL_pin, 0) == cudaSuccess &&
+       cudaHostAlloc((void**)&s->h_par_pin, (size_t)kMappedThetaMax * NPAR * 8, cudaHostAllocMapped) == cudaSuccess &&
+       cudaHostGetDevicePointer((void**)&s->d_par_map, s->h_par_pin, 0) == cudaSuccess;
   if (ok && want_fisher)
     ok = cudaMalloc((void**)&s->d_F, (size_t)max_B * NPAR * NPAR * 8) == cudaSuccess &&
          cudaMalloc((void**)&s->d_grad, (size_t)max_B * NPAR * 8) == cudaSuccess &&
@@ -102,13 +112,19 @@ int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const
 
 int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL) {
   if (!s || !h_params || !h_out_lnL || B <= 0 || B > s->max_B || !s->have_data || !s->have_psd) return PESPACE_EINVAL;
-  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
-  const int rc = loglike_impl(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL, s->d_ws, s->ws_bytes,
+  const double* d_theta = s->d_params;
+  if (B <= 256) {                                       // small batch: theta through mapped pinned memory, no copy call
+    std::memcpy(s->h_par_pin, h_params, (size_t)B * NPAR * 8);
+    d_theta = s->d_par_map;
+  } else {
+    CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  }
+  const int rc = loglike_impl(d_theta, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL_map, s->d_ws, s->ws_bytes,
                               s->st, s->bins_ready);      // the S0 table is built once per data set
   if (rc != PESPACE_OK) { s->bins_ready = false; return rc; }
   s->bins_ready = true;
-  CU(cudaMemcpyAsync(h_out_lnL, s->d_lnL, (size_t)B * 8, cudaMemcpyDeviceToHost, s->st));
   CU(cudaStreamSynchronize(s->st));
+  std::memcpy(h_out_lnL, s->h_lnL_pin, (size_t)B * 8);
   return PESPACE_OK;
 }
 
