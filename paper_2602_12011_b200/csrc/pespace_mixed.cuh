@@ -167,10 +167,11 @@ __device__ __forceinline__ void eval_class_mixed(int MC, bool first, double fT, 
 // dynamic shared memory: [float2 (sin, cos) table | float2 (sin, cos - 1) table | FP64 sample constants | FP32 copy |
 // warp partials]
 constexpr int MIX_TILE = 64;
-constexpr size_t mixed_smem_bytes() {
+constexpr size_t mixed_smem_used() {
   return 2 * sizeof(float2) * NTAB + sizeof(double) * (size_t)MIX_TILE * SMEM_STRIDE +
          sizeof(float) * (size_t)MIX_TILE * SMEM_STRIDE + sizeof(double) * (size_t)(BLOCK / 32) * MIX_TILE;
 }
+constexpr size_t mixed_smem_bytes() { return mixed_smem_used(); }
 
 #ifndef PESPACE_MINBX
 #define PESPACE_MINBX 2
