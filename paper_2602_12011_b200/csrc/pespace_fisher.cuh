@@ -13,7 +13,7 @@
 // so the per-bin geometry runs on a 3-tangent dual number (orbit angle, lambda, beta), the phase and
 // time polynomials on a 4-tangent one (M, q, chi1, chi2), and everything else is closed form.
 //
-// Launch geometry: block = 128 threads = 128 consecutive bins ("chunk"); a block walks FCHUNKS chunks and a
+// Launch geometry: block = 128 threads = 128 consecutive bins ("chunk"); a block walks FCHUNKS (4) chunks and a
 // tile of FTILE samples.  The 12 x 3 complex numbers (value + 11 tangents of X, Y, Z) of one (sample, bin)
 // are accumulated over the mode classes in shared memory (thread-private columns), then the upper triangle
 // of the 12 x 12 Gram matrix of (residual, d_1 h, ..., d_11 h) -- 78 numbers -- is formed per thread and
@@ -34,7 +34,7 @@ constexpr int FBLOCK = PESPACE_FBLOCK;   // threads = bins per chunk
 #define PESPACE_FTILE 4
 #endif
 #ifndef PESPACE_FCHUNKS
-#define PESPACE_FCHUNKS 16
+#define PESPACE_FCHUNKS 4
 #endif
 constexpr int FTILE = PESPACE_FTILE;      // samples per block
 constexpr int FCHUNKS = PESPACE_FCHUNKS;  // chunks per block
