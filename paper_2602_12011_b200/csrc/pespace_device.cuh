@@ -535,7 +535,10 @@ static __global__ void prep_samples_kernel(const double* __restrict__ params, lo
 #define PESPACE_BLOCK 256
 #endif
 constexpr int BLOCK = PESPACE_BLOCK;      // threads = bins per block
-constexpr int TILE = 64;        // samples staged in shared memory per block
+#ifndef PESPACE_TILE
+#define PESPACE_TILE 64
+#endif
+constexpr int TILE = PESPACE_TILE;        // samples staged in shared memory per block
 
 // dynamic shared memory of the likelihood / response kernels: [trig table | sample constants | warp partials]
 extern __shared__ __align__(16) unsigned char pespace_dyn_smem[];
