@@ -133,7 +133,10 @@ __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[N
   }
 }
 
-constexpr int TAB_TILE = 32;     // samples per block
+#ifndef PESPACE_TAB_TILE
+#define PESPACE_TAB_TILE 64
+#endif
+constexpr int TAB_TILE = PESPACE_TAB_TILE;     // samples per block
 constexpr size_t tab_smem_bytes() {
   return sizeof(double) * ((size_t)2 * NTAB + (size_t)TAB_TILE * SMEM_STRIDE + (size_t)(BLOCK / 32) * TAB_TILE);
 }
