@@ -172,6 +172,30 @@ def test_source_along_an_arm_is_regular(P):
     check_response(P, th[None, :], f, W.Model(1, (det,)))
 
 
+def test_special_angles_and_equal_masses(P):
+    """Face-on / face-off (iota = 0, pi), ecliptic poles (beta = +-pi/2), equal masses (q = 1: the odd-m amplitudes
+    vanish), psi = 0, phi_c = 0, t_c at the edges of the data."""
+    wl = W.config(4, B=8, N=900)
+    th = np.tile(wl.theta_inj, (8, 1))
+    th[0, 5] = 0.0
+    th[1, 5] = np.pi
+    th[2, 8] = 0.5 * np.pi
+    th[3, 8] = -0.5 * np.pi
+    th[4, 1] = 1.0
+    th[5, 9] = 0.0; th[5, 6] = 0.0
+    th[6, 10] = 0.0
+    th[7, 10] = 1.0 / wl.grid.df
+    wl.params = th
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    check_loglike(P, wl, data, psd)
+    check_response(P, th, wl.grid.freqs()[::4], wl.model)
+    F, g = P.fisher(dev(th), dev(data), dev(psd), wl.grid, wl.model)
+    Fo, go = oracle.fisher(th, data, psd, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    d = np.where(d > 0, d, 1.0)                       # q = 1: d/dq of the odd-m modes is the only content of that row
+    assert (np.abs(F.cpu().numpy() - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
+
+
 def test_bitwise_determinism(P):
     wl = W.config(3, B=130, N=2000)
     data, psd = wl.data(oracle_response_fn), wl.psd()
