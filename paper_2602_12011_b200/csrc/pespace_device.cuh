@@ -14,8 +14,9 @@
 //          E_n = exp(-2 pi i f k.x_n), W_l = (n_l.P.n_l)/(1-(k.n_l)^2), which is Eq. 5
 //           inserted into Eq. 6 -- derivation in DESIGN.md
 //   S8     residual against data, weighted by 1/S_n         [Eq. 10, PAPER.md:124]
-// The per-bin factors g z f^{-7/6} are folded into the data and weights once per
-// thread, so the inner loop never touches them.
+// The per-bin factors (f^{1/3}, ln f, f^{-5/3}, f^{-8/3}, sin/cos 2 pi f L) and the data and
+// weights with g z f^{-7/6} folded in are written once per call by prep_bins_kernel (S0), so the
+// inner loop never touches a transcendental or a division of the library.
 #pragma once
 #include <cstdint>
 #include <cuda_runtime.h>
