@@ -323,7 +323,7 @@ def run_ours(args):
             if fisher_mode:
                 ses.fisher(params_h[i % n_batches], True, res_h, grad_h, grad_only=args.grad_only)
             else:
-                ses.loglike(params_h[i % n_batches], res_h)
+                ses.loglike(params_h[i % n_batches], res_h, mixed=mixed_mode)
 
     e2e = {}
     for key, copy_data in (("full", True), ("resident", False)):
@@ -431,8 +431,7 @@ def run_ours(args):
                         "tables, data set and PSD copied from pinned host memory, lnL read back" if tab_mode else
                         "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
                         " per step: theta, data set and PSD copied from pinned host memory, result read back"),
-                "precision_note": ("the host-buffer session calls run the FP64 kernel; --precision mixed applies to the "
-                                   "device-timed leg only") if mixed_mode else None,
+                "precision_note": "pespace_session_loglike_mixed" if mixed_mode else None,
                 "value_resident_data": e2e["resident"],
                 "resident_data_note": "same call with the data set copied once (sampler use): theta in, result out"},
         "gpu_launches": int(launches),

@@ -163,6 +163,8 @@ int pespace_session_set_data(pespace_session* s, const double* h_data_AET, const
  * table of the data set (S0) is built by the first call after pespace_session_set_data and reused afterwards;
  * lnL (and theta of batches up to 256 samples) travel through mapped pinned memory owned by the session. */
 int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL);
+/* Same through pespace_loglike_mixed (FP64 phases, FP32 geometry; see there for the accuracy). */
+int pespace_session_loglike_mixed(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL);
 /* h_params [B][11] -> h_out_F [B][11][11] and, if h_out_grad != NULL, h_out_grad [B][11] (needs the
  * data set; the Fisher matrix alone needs only the PSD).  h_out_F may be NULL: gradient only. */
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,

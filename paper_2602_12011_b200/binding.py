@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_loglike_mixed", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
-           "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike",
+           "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
            "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
            "pespace_launch_count", "pespace_strerror",
@@ -68,6 +68,7 @@ def _load():
     L.pespace_session_create.argtypes = [C.POINTER(_Grid), C.POINTER(_Model), i64, C.c_int, C.POINTER(vp)]
     L.pespace_session_set_data.argtypes = [vp, vp, vp]
     L.pespace_session_loglike.argtypes = [vp, vp, i64, vp]
+    L.pespace_session_loglike_mixed.argtypes = [vp, vp, i64, vp]
     L.pespace_session_fisher.argtypes = [vp, vp, i64, vp, vp]
     L.pespace_session_loglike_tab.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp]
     L.pespace_session_destroy.argtypes = [vp]
@@ -324,12 +325,15 @@ class Session:
             sp, keep_s = _host_ptr(psd, np.float64, "psd")
         _check(_lib.pespace_session_set_data(self._h, dp, sp), "pespace_session_set_data")
 
-    def loglike(self, params, out=None):
+    def loglike(self, params, out=None, mixed: bool = False):
         pp, p = _host_ptr(params, np.float64, "params")
         if out is None:
             out = np.empty(p.shape[0], dtype=np.float64)
         op, o = _host_ptr(out, np.float64, "out")
-        _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
+        if mixed:
+            _check(_lib.pespace_session_loglike_mixed(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike_mixed")
+        else:
+            _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
         return out
 
     def loglike_tab(self, params, table, out=None):

@@ -128,6 +128,18 @@ int pespace_session_loglike(pespace_session* s, const double* h_params, int64_t 
   return PESPACE_OK;
 }
 
+int pespace_session_loglike_mixed(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL) {
+  if (!s || !h_params || !h_out_lnL || B <= 0 || B > s->max_B || !s->have_data || !s->have_psd) return PESPACE_EINVAL;
+  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  s->bins_ready = false;            // the mixed kernel keeps its own (whitened) per-bin table in the same workspace
+  const int rc = pespace_loglike_mixed(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model, s->d_lnL_map, s->d_ws,
+                                       s->ws_bytes, s->st);
+  if (rc != PESPACE_OK) return rc;
+  CU(cudaStreamSynchronize(s->st));
+  std::memcpy(h_out_lnL, s->h_lnL_pin, (size_t)B * 8);
+  return PESPACE_OK;
+}
+
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
                            double* h_out_grad) {
   if (!s || !s->want_fisher || !h_params || (!h_out_F && !h_out_grad) || B <= 0 || B > s->max_B || !s->have_psd)

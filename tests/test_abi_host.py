@@ -108,6 +108,7 @@ def test_session_argument_validation_without_a_device():
     assert L.pespace_session_create(C.byref(g), C.byref(m), 4, 0, None) == EINVAL
     assert L.pespace_session_set_data(None, None, None) == EINVAL
     assert L.pespace_session_loglike(None, None, 4, None) == EINVAL
+    assert L.pespace_session_loglike_mixed(None, None, 4, None) == EINVAL
     assert L.pespace_session_fisher(None, None, 4, None, None) == EINVAL
     assert L.pespace_session_loglike_tab(None, None, 4, 8, None, None, None, None, None) == EINVAL
     assert L.pespace_session_destroy(None) == EINVAL

@@ -80,6 +80,19 @@ def test_mixed_edge_cases_and_determinism(P):
     assert np.all(np.abs(a[ok] - want) <= TOL_MIXED * np.abs(want))
 
 
+def test_mixed_session_matches_device_call(P):
+    wl = W.config(3, B=21, N=800)
+    data = wl.data(lambda p, f, m: oracle.response(p, f, m))
+    psd = wl.psd()
+    want = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, wl.B)(dev(wl.params), mixed=True).cpu().numpy()
+    ses = P.Session(wl.grid, wl.model, 32)
+    ses.set_data(data, psd)
+    full = ses.loglike(wl.params)                              # FP64 first: fills the cached per-bin table
+    assert np.array_equal(ses.loglike(wl.params, mixed=True), want)
+    assert np.array_equal(ses.loglike(wl.params), full)        # and the FP64 table is rebuilt after a mixed call
+    ses.close()
+
+
 def test_mixed_full_size_sampled(P):
     wl = W.config(2)
     data = wl.data(lambda p, f, m: oracle.response(p, f, m))
