@@ -49,8 +49,14 @@ class _WaveTable(C.Structure):
 
 def _load():
     if not os.path.exists(LIB_PATH):
-        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2602_12011_b200.build` "
-                          "(there is no CPU fallback)")
+        # not built yet (a fresh checkout: the library is not under version control): compile it in-tree with nvcc.
+        # There is no CPU fallback: if the build fails, importing this module fails.
+        try:
+            from . import build as _build
+            _build.build()
+        except Exception as exc:
+            raise ImportError(f"{LIB_PATH} is missing and could not be built ({exc}); run "
+                              "`python -m paper_2602_12011_b200.build` (there is no CPU fallback)") from exc
     L = C.CDLL(LIB_PATH)
     vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
     L.pespace_response.argtypes = [vp, i64, vp, i64, C.POINTER(_Model), vp, vp]
