@@ -137,3 +137,13 @@ def test_tab_argument_validation_without_a_device():
     assert L.pespace_workspace_bytes_tab(0, C.byref(g), C.byref(m)) == 0
     ws_tab, ws = L.pespace_workspace_bytes_tab(4, C.byref(g), C.byref(m)), L.pespace_workspace_bytes(4, C.byref(g), C.byref(m), 0)
     assert ws_tab > ws > 0
+
+
+def test_header_is_plain_c():
+    """include/pespace.h is a C ABI: it must compile as C99 and as C++ with no other header of this repository."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "pespace.h")
+    for cmd in (["gcc", "-x", "c", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", hdr],
+                ["g++", "-x", "c++", "-Wall", "-Werror", "-fsyntax-only", hdr]):
+        res = subprocess.run(cmd, capture_output=True, text=True)
+        assert res.returncode == 0, res.stderr
