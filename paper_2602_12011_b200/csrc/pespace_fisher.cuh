@@ -261,14 +261,21 @@ __device__ __forceinline__ void fisher_class(int MC, bool FIRST, const BinC& bc,
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
     const G uu = ul[l], vv = vl[l];
-    const G v2_ = vv * vv;
-    const G D = dfma(uu, uu, v2_);
+    G u2_, v2_, D, xi;                        // squares written out: (x^2)' = (2 x) x'
+    {
+      const double tu2 = uu.v + uu.v, tv2 = vv.v + vv.v;
+      u2_.v = uu.v * uu.v; v2_.v = vv.v * vv.v;
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { u2_.d[i] = tu2 * uu.d[i]; v2_.d[i] = tv2 * vv.d[i]; }
+      D = u2_ + v2_;
+      xi = u2_ - v2_;
+    }
     G rD;
     rD.v = (__double2hiint(D.v) > 0) ? rcp_pos(D.v) : 0.0;
     const double m2 = -rD.v * rD.v;
 #pragma unroll
     for (int i = 0; i < 3; ++i) rD.d[i] = m2 * D.d[i];
-    Wp[l] = rD * (uu * uu - v2_);
+    Wp[l] = rD * xi;
     Wc[l] = rD * (uu * vv);
   }
 
