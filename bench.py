@@ -51,14 +51,14 @@ FP64_OPS_PER_UNIT = {
     ("loglike", 0, 2): {"dfma": 140.00, "dmul": 53.02, "dadd": 40.53},      # kind 0, (2,2) only  -- config 2
     ("loglike", 0, 15): {"dfma": 554.00, "dmul": 188.11, "dadd": 101.08},   # kind 0, five modes  -- configs 3, 4
     ("loglike", 1, 15): {"dfma": 526.00, "dmul": 224.11, "dadd": 109.08},   # kind 1, five modes  -- config 4
-    ("fisher", 0, 15): {"dfma": 3222.00, "dmul": 1282.25, "dadd": 652.15},  # config 5
-    ("fisher", 1, 15): {"dfma": 3102.00, "dmul": 1366.25, "dadd": 644.15},
+    ("fisher", 0, 15): {"dfma": 3150.00, "dmul": 1246.25, "dadd": 640.61},  # config 5
+    ("fisher", 1, 15): {"dfma": 3030.00, "dmul": 1330.25, "dadd": 632.61},
     ("loglike_tab", 0, 2): {"dfma": 136.00, "dmul": 52.03, "dadd": 46.03},   # --waveform tab, config 2 (one mode)
 }
 # dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (same ncu captures; config 4:
 # mean of the three launches of a step)
 DRAM_TRAFFIC_PER_LAUNCH = {2: 35.91e6 + 5.18e6, 3: 36.18e6 + 5.39e6, 4: (40.4e6 + 36.6e6 + 42.1e6 + 37.2e6 + 41.3e6 + 37.9e6) / 3,
-                           5: 35.2e6 + 3.9e6}
+                           5: 36.9e6 + 57.6e6}
 # SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
 # kept for reference only -- the reduced algorithm needs less than half of it.
 SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0, 5: 100000.0}
