@@ -69,7 +69,7 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
     if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }
   const long long nt = (long long)B * NG;
-  combine_fisher_kernel<<<(unsigned)((nt + 127) / 128), 128, 0, st>>>(
+  combine_fisher_kernel<<<(unsigned)((nt + 31) / 32), dim3(32, CGROUPS), 0, st>>>(
       d_partial, d_consts, B, (int)(model->n_det * p.nbx), fisher_const_stride(model->n_det), d_out_F, d_out_grad);
   LAUNCHED();
   return PESPACE_OK;

@@ -589,13 +589,23 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double* __re
 static __global__ void combine_fisher_kernel(const double* __restrict__ partial, const double* __restrict__ consts,
                                       long long B, int n_slices, int const_stride, double* __restrict__ outF,
                                       double* __restrict__ out_grad) {
-  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (t >= B * NG) return;
-  const long long b = t / NG;
-  const int idx = (int)(t % NG);
-  if (!outF && idx >= NT) return;          // gradient only: the kernel wrote row 0 of the Gram matrix only
+  // block = 32 consecutive (sample, Gram entry) pairs x CGROUPS slice groups, added in the order of the groups
+  __shared__ double part[CGROUPS][33];
+  const int x = threadIdx.x, g = threadIdx.y;
+  const long long t = (long long)blockIdx.x * 32 + x;
+  const bool live = t < B * NG;
+  const long long b = live ? t / NG : 0;
+  const int idx = live ? (int)(t % NG) : 0;
+  const bool wanted = live && (outF || idx < NT);          // gradient only: the kernel wrote row 0 of the Gram matrix only
+  double acc = 0.0;
+  if (wanted)
+    for (int i = g; i < n_slices; i += CGROUPS) acc += partial[((size_t)i * (size_t)B + (size_t)b) * NG + idx];
+  part[g][x] = acc;
+  __syncthreads();
+  if (g != 0 || !wanted) return;
   double sum = 0.0;
-  for (int i = 0; i < n_slices; ++i) sum += partial[((size_t)i * (size_t)B + (size_t)b) * NG + idx];
+#pragma unroll
+  for (int k = 0; k < CGROUPS; ++k) sum += part[k][x];
   // W_A is 1 with all tangents 0 only for out-of-domain samples (prep_samples_du_kernel)
   const bool valid = consts[(size_t)b * const_stride + W_A * DUW + 1] != 0.0;
   if (!valid) sum = CUDART_NAN;
