@@ -342,8 +342,12 @@ template <class T> void tdi_xyz(const Cx<T> y[6], const T& f, double L_m, int ge
   const Cx<T> z = expi(-(T(2.0) * K<T>::pi() * f * Lbar));
   const Cx<T> one = cx<T>(T(1.0), T(0.0));
   const Cx<T> z2 = z * z;
+  // g(z) = 1 - z^2 (generation 1.5) or (1 - z^2)(1 - z^4) = 1 - z^2 - z^4 + z^6 (2.0): Eq. 6 as SURVEY O10 states it.
+  // The PRODUCT form is evaluated: where z^2 = 1 (f = n c / 2L, inside the band of configs 2-5, G9) both factors
+  // vanish and the expanded sum of four O(1) terms keeps only ~1e-16 / |g| relative digits -- 3e-7 one bin from
+  // the null against this definition's own binary128 evaluation (pin P14 extended to the nulls), the product 1e-11.
   Cx<T> g = one - z2;
-  if (gen == 20) { const Cx<T> z4 = z2 * z2; g = one - z2 - z4 + z4 * z2; }
+  if (gen == 20) g = g * (one - z2 * z2);
   const Cx<T>&y12 = y[0], &y21 = y[1], &y13 = y[2], &y31 = y[3], &y23 = y[4], &y32 = y[5];
   XYZ[0] = g * (y13 - y12 + z * (y31 - y21));
   XYZ[1] = g * (y21 - y23 + z * (y12 - y32));

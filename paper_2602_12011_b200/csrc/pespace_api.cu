@@ -126,6 +126,7 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
   if (!d_params || !d_freqs || !d_out_AET || B <= 0 || N <= 0 || !model_ok(model)) return PESPACE_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   const Plan p = make_plan(B, N, model->n_det);
+  if (p.ntile > 65535) return PESPACE_EINVAL;                 // gridDim.y
   char* d_scratch = nullptr;
   CU(cudaMallocAsync((void**)&d_scratch, p.trig_bytes + p.consts_bytes, st));
   double2* d_trig = (double2*)d_scratch;
@@ -169,6 +170,7 @@ int pespace::host::loglike_impl(const double* d_params, int64_t B, const double*
     return PESPACE_EINVAL;
   cudaStream_t st = (cudaStream_t)stream;
   const Plan p = make_plan(B, grid->N, model->n_det);
+  if (p.ntile > 65535) return PESPACE_EINVAL;                 // gridDim.y
   double2* d_trig = (double2*)d_workspace;
   double* d_bins = (double*)((char*)d_workspace + p.trig_bytes);           // B-independent offset: reusable across calls
   double* d_consts = (double*)((char*)d_workspace + p.trig_bytes + p.bins_bytes);

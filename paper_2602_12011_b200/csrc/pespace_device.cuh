@@ -588,7 +588,12 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
   if (!fold_f76) bc.fm76 = 1.0;          // 0: tabulated waveforms carry their own amplitude (pespace_tab.cuh)
   double gr, gi;
   tdi_prefactor(bc, dc.gen, gr, gi);
-  const double g2 = gr * gr + gi * gi;
+  double g2 = gr * gr + gi * gi;
+  // Reading G9: the weight of a bin depends on the PSD alone.  Where g(z) is EXACTLY 0 (2 f L / c an exact integer:
+  // the template vanishes identically) the bin keeps its theta-independent term |d|^2 4 df / S of Eq. 10: a stand-in
+  // prefactor of 1e-100 makes the folded data d / g huge against the (then negligible) folded template while
+  // w |g|^2 |d / g|^2 = w |d|^2 stays exact; nothing over- or underflows for |d|, 1/S of detector-like magnitude.
+  if (!(g2 > 0.0)) { gr = 1e-100; gi = 0.0; g2 = 1e-200; }
   double* o = bins + (size_t)det * NBF * (size_t)G.N + (size_t)k;
   const size_t N = (size_t)G.N;
   o[BF_FT * N] = bc.fT; o[BF_CF * N] = bc.cf; o[BF_LNF3 * N] = bc.lnf3; o[BF_FM53 * N] = bc.fm53;
@@ -597,13 +602,18 @@ static __global__ void prep_bins_kernel(const double2* __restrict__ data, const 
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     const size_t idx = ((size_t)det * 3 + c) * N + (size_t)k;
-    const double2 d = data ? data[idx] : make_double2(0.0, 0.0);     // no data set: Fisher matrix only
     const double Sn = psd[idx];
-    const bool use = isfinite(Sn) && Sn > 0.0 && g2 > 0.0;
-    const double sc_ = use ? nrm[c] / g2 : 0.0;
-    double vr = (d.x * gr + d.y * gi) * sc_;                    // d * conj(g) / |g|^2 * nrm
-    double vi = (d.x * gi - d.y * gr) * sc_;                    // MINUS the imaginary part: eval_xyz returns (Re, -Im)
-    double vw = use ? (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]) : 0.0;
+    const bool use = isfinite(Sn) && Sn > 0.0;
+    // a masked bin (PSD 0, negative or non-finite) is skipped WITHOUT looking at its data: NaN / Inf there must not
+    // reach the sums (0 * NaN = NaN)
+    double vr = 0.0, vi = 0.0, vw = 0.0;
+    if (use) {
+      const double2 d = data ? data[idx] : make_double2(0.0, 0.0);   // no data set: Fisher matrix only
+      const double sc_ = nrm[c] / g2;
+      vr = (d.x * gr + d.y * gi) * sc_;                    // d * conj(g) / |g|^2 * nrm
+      vi = (d.x * gi - d.y * gr) * sc_;                    // MINUS the imaginary part: eval_xyz returns (Re, -Im)
+      vw = (4.0 * G.df / Sn) * g2 / (nrm[c] * nrm[c]);
+    }
     if (fold_f76 == 2) {           // mixed-precision kernel (pespace_mixed.cuh): whitened data, sqrt(w) / 2^64
       const double sq = sqrt(vw);
       vr *= sq; vi *= sq; vw = sq * (1.0 / 18446744073709551616.0);

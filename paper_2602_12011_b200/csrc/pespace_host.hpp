@@ -69,6 +69,20 @@ inline unsigned class_mask(unsigned mode_mask) {
 
 inline size_t align_up(size_t x, size_t a) { return (x + a - 1) / a * a; }
 
+// Dynamic shared memory beyond 48 KB is an opt-in attribute of a kernel PER DEVICE: one flag per device ordinal
+// (atomic: host threads may race to set it, setting it twice is harmless); ordinals >= 64 set it on every launch.
+struct SmemOptIn { std::atomic<unsigned long long> done{0}; };
+template <class K>
+inline cudaError_t opt_in_smem(K kernel, size_t bytes, SmemOptIn& flag) {
+  int dev = 0;
+  if (cudaError_t e = cudaGetDevice(&dev); e != cudaSuccess) return e;
+  const unsigned long long bit = (dev >= 0 && dev < 64) ? (1ull << dev) : 0ull;
+  if (flag.done.load(std::memory_order_acquire) & bit) return cudaSuccess;
+  const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
+  if (e == cudaSuccess) flag.done.fetch_or(bit, std::memory_order_release);
+  return e;
+}
+
 // optional event timing of the dominant kernels (pespace_profile_enable / _read); defined in pespace_api.cu
 struct EvPair { cudaEvent_t a = nullptr, b = nullptr; };
 int prof_begin(EvPair& ev, cudaStream_t st);   // no-op unless profiling is enabled

@@ -11,20 +11,13 @@ namespace pespace {
 namespace host {
 namespace {
 
-// the kernels use dynamic shared memory beyond 48 KB: opt in once per instantiation
-template <class K>
-cudaError_t opt_in_smem(K kernel, size_t bytes, bool& done) {
-  if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes);
-  done = e == cudaSuccess;
-  return e;
-}
+// the kernels use dynamic shared memory beyond 48 KB: opt in once per instantiation and device (opt_in_smem)
 
 #if PESPACE_INST_WHAT == 0
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
                    const double* bins, long long N, const DetC& dc, int n_det, int det, double* partial) {
-  static bool configured = false;
+  static SmemOptIn configured;
   if (cudaError_t e = opt_in_smem(loglike_kernel<KIND, CM>, kernel_smem_bytes(), configured); e != cudaSuccess) return e;
   loglike_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, bins, N, dc, n_det, det, partial);
   return cudaSuccess;
@@ -34,7 +27,7 @@ using Fn = LoglikeFn;
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
                    const double* freqs, long long N, const DetC& dc, int n_det, int det, double2* out) {
-  static bool configured = false;
+  static SmemOptIn configured;
   if (cudaError_t e = opt_in_smem(response_kernel<KIND, CM>, kernel_smem_bytes(), configured); e != cudaSuccess) return e;
   response_kernel<KIND, CM><<<g, BLOCK, kernel_smem_bytes(), st>>>(consts, trig, B, freqs, N, dc, n_det, det, out);
   return cudaSuccess;
@@ -44,7 +37,7 @@ using Fn = ResponseFn;
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, long long B, const double* bins, long long N,
                    const DetC& dc, int n_det, int det, int grad_only, double* partial) {
-  static bool configured = false;
+  static SmemOptIn configured;
   if (cudaError_t e = opt_in_smem(fisher_kernel<KIND, CM>, fisher_smem_bytes(), configured); e != cudaSuccess) return e;
   fisher_kernel<KIND, CM><<<g, FBLOCK, fisher_smem_bytes(), st>>>(consts, B, bins, N, dc, n_det, det, grad_only, partial);
   return cudaSuccess;

@@ -36,22 +36,16 @@ extern "C" int pespace_loglike_mixed(const double* d_params, int64_t B, const do
   LAUNCHED();
   const unsigned cm = class_mask(model->mode_mask);
   const dim3 g((unsigned)nbb, (unsigned)ntile);
-  static bool cfg0 = false, cfg1 = false;
+  static SmemOptIn cfg0, cfg1;
   for (int d = 0; d < n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc = prof_begin(ev, st); rc != PESPACE_OK) return rc;
     if (dc.kind == 0) {
-      if (!cfg0) {
-        CU(cudaFuncSetAttribute(loglike_mixed_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mixed_smem_bytes()));
-        cfg0 = true;
-      }
+      CU(opt_in_smem(loglike_mixed_kernel<0>, mixed_smem_bytes(), cfg0));
       loglike_mixed_kernel<0><<<g, BLOCK, mixed_smem_bytes(), st>>>(d_consts, d_trig, B, cm, d_bins, N, dc, n_det, d, d_partial);
     } else {
-      if (!cfg1) {
-        CU(cudaFuncSetAttribute(loglike_mixed_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)mixed_smem_bytes()));
-        cfg1 = true;
-      }
+      CU(opt_in_smem(loglike_mixed_kernel<1>, mixed_smem_bytes(), cfg1));
       loglike_mixed_kernel<1><<<g, BLOCK, mixed_smem_bytes(), st>>>(d_consts, d_trig, B, cm, d_bins, N, dc, n_det, d, d_partial);
     }
     LAUNCHED();

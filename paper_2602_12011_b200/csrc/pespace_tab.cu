@@ -42,12 +42,7 @@ TabC make_tab(const pespace_wavetable* t, unsigned mode_mask) {
 }
 
 template <class K>
-cudaError_t opt_in(K kernel, bool& done) {
-  if (done) return cudaSuccess;
-  cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tab_smem_bytes());
-  done = e == cudaSuccess;
-  return e;
-}
+cudaError_t opt_in(K kernel, SmemOptIn& done) { return opt_in_smem(kernel, tab_smem_bytes(), done); }
 
 int run_prep_tab(const double* d_params, long long B, const pespace_model* model, double* d_consts, double2* d_trig,
                  cudaStream_t st) {
@@ -82,7 +77,7 @@ int pespace_response_tab(const double* d_params, int64_t B, const pespace_waveta
   int rc = run_prep_tab(d_params, B, model, d_consts, d_trig, st);
   const TabC T = make_tab(table, model->mode_mask);
   const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
-  static bool cfg0 = false, cfg1 = false;
+  static SmemOptIn cfg0, cfg1;
   for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
     const DetC dc = make_det(model->det[d]);
     cudaError_t e;
@@ -134,7 +129,7 @@ int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetab
   LAUNCHED();
   const TabC T = make_tab(table, model->mode_mask);
   const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
-  static bool cfg0 = false, cfg1 = false;
+  static SmemOptIn cfg0, cfg1;
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
     EvPair ev;

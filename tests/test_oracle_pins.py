@@ -170,6 +170,109 @@ def test_higher_mode_maps_follow_the_22_mode():
         assert np.allclose(a, math.sqrt(2 / m) * c * vm ** p * a2, rtol=1e-13, atol=0)
 
 
+def test_spin_terms_against_the_poisson_will_forms():
+    """G3 / O2: the 1.5PN spin-orbit and 2PN spin-spin terms, pinned against the forms printed by Poisson & Will,
+    Phys. Rev. D 52, 848 (1995), Eqs. (1.3)-(1.5) [also Cutler & Flanagan 1994 for beta; Kidder 1995 for sigma],
+    restated here from the individual masses and NOT taken from the oracle:
+        beta  = (1/12) sum_i [113 (m_i/M)^2 + 75 eta] (L.chi_i),
+        sigma = (eta/48) [-247 chi_1.chi_2 + 721 (L.chi_1)(L.chi_2)]      (aligned spins: both products chi_1 chi_2),
+        Psi(f) = 2 pi f t_c - phi_c - pi/4 + (3/128)(pi Mc f)^{-5/3} [1 + ... - 4 (4 pi - beta) x^{3/2}
+                                                                          + 10 (3058673/1016064 + ... - sigma) x^2],
+        t(f)   = t_c - (5/256) Mc (pi Mc f)^{-8/3} [1 + ... - (8/5)(4 pi - beta) x^{3/2} + 2 (... - sigma) x^2],
+    with x = (pi M f)^{2/3}.  Only the spin-dependent differences are compared, so the non-spinning part (pins P1, P2)
+    drops out: the phase AND the time-frequency map, each against its own printed series."""
+    for M, q, chi1, chi2 in ((2e6, 3.0, 0.6, -0.3), (4e5, 1.0, -0.9, 0.7), (7e6, 7.5, 0.25, 0.8), (1e6, 2.0, 0.5, 0.0)):
+        th = THETA.copy(); th[0], th[1] = M, q
+        m1, m2 = q / (1 + q), 1 / (1 + q)                      # m_i / M
+        eta = m1 * m2
+        beta = ((113 * m1 ** 2 + 75 * eta) * chi1 + (113 * m2 ** 2 + 75 * eta) * chi2) / 12
+        sigma = eta / 48 * (-247 + 721) * chi1 * chi2
+        Ms = M * TSUN
+        Mc = eta ** 0.6 * Ms
+        f = np.array([1.3e-4, 7e-4, 3e-3, 1.1e-2])
+        x = (math.pi * Ms * f) ** (2.0 / 3.0)
+        th0, ths = th.copy(), th.copy()
+        ths[2], ths[3] = chi1, chi2
+        _, p0, t0 = oracle.waveform(th0, 2, 2, f)
+        _, ps, ts = oracle.waveform(ths, 2, 2, f)
+        dpsi = 3 / 128 * (math.pi * Mc * f) ** (-5.0 / 3.0) * (4 * beta * x ** 1.5 - 10 * sigma * x ** 2)
+        dt = -5 / 256 * Mc * (math.pi * Mc * f) ** (-8.0 / 3.0) * (8 / 5 * beta * x ** 1.5 - 2 * sigma * x ** 2)
+        assert np.allclose(ps - p0, dpsi, rtol=1e-9, atol=1e-9 * np.abs(p0).max() * 1e-3)
+        assert np.allclose(ts - t0, dt, rtol=1e-9, atol=1e-12 * np.abs(t0 - th[10]).max())
+        assert np.abs(dpsi).min() > 1e-2                       # the spin terms are not negligible in the comparison
+    # each spin separately, equal spins, and the antisymmetric combination at q = 1 (beta keeps only 75 eta terms)
+    th = THETA.copy(); th[1] = 1.0; th[2], th[3] = 0.4, -0.4
+    _, ps, _ = oracle.waveform(th, 2, 2, np.array([1e-3]))
+    th[2] = th[3] = 0.0
+    _, p0, _ = oracle.waveform(th, 2, 2, np.array([1e-3]))
+    x = (math.pi * th[0] * TSUN * 1e-3) ** (2.0 / 3.0)
+    want = 3 / 128 * 4 * (math.pi * th[0] * TSUN * 1e-3) ** (-5.0 / 3.0) * (-10 * (0.25 / 48 * 474 * -0.16) * x ** 2)
+    assert ps[0] - p0[0] == pytest.approx(want, rel=1e-8)     # beta = 0 by symmetry, sigma < 0
+
+
+def _point_mass_moment(q, l, current):
+    """Newtonian radiative multipole of two point masses on a circular orbit, mass-ratio dependence only: the mass
+    moment of order l is sum_A m_A r_A^l e^{-i m phi_A}, the current moment carries one more power of r_A (r x v);
+    body 2 sits opposite body 1 (phi_2 = phi_1 + pi), r_1 = (m_2/M) r, r_2 = (m_1/M) r.  Returned in units of
+    mu r^l (mu r^{l+1} Omega), with the sign (-1)^power for body 2."""
+    m1, m2 = q / (1 + q), 1 / (1 + q)
+    p = l + 1 if current else l
+    return (m1 * m2 ** p + m2 * (-m1) ** p) / (m1 * m2)
+
+
+def test_mode_amplitude_ratios_against_multipole_moments_and_test_mass_fluxes():
+    """O5: the c_lm v^{p_lm} table, pinned WITHOUT restating it.
+    (a) Mass-ratio dependence: a mode with l + m even is a mass multipole of order l, with l + m odd a current
+        multipole of order l; for two point masses these are sum_A m_A (+-r_A)^l and sum_A m_A (+-r_A)^{l+1}
+        (`_point_mass_moment`), so A_lm(q) / A_lm(q_ref) at equal M, f must follow them (this is where delta and
+        1 - 3 eta come from; equal masses kill the odd-m modes).
+    (b) Numbers and powers of v: in the test-mass limit the energy flux carried by mode (l,m) relative to (2,2)
+        at the same ORBITAL frequency is, at leading order, the black-hole-perturbation result of Poisson,
+        Phys. Rev. D 47, 1497 (1993), Eq. (5.12)-(5.13) [eta_21 = v^2/36, eta_33 = (1215/896) v^2, eta_32 = (5/63) v^4,
+        eta_44 = (1280/567) v^4, v = (M Omega)^{1/3}].  Flux ~ (m Omega)^2 |h_lm(t)|^2 and the stationary-phase
+        transform gives |h~_lm(f = m F)|^2 = |h_lm|^2 pi / (m dOmega/dt), hence
+        flux_lm / flux_22 = (m^2/4) (m/2) |h~_lm(m F)|^2 / |h~_22(2 F)|^2."""
+    th = THETA.copy()
+    F = np.array([2e-5, 1e-4, 7e-4])                        # orbital frequencies
+    # (b) test-mass limit
+    th[1] = 1e7
+    poisson = {(2, 1): (1 / 36, 2), (3, 3): (1215 / 896, 2), (3, 2): (5 / 63, 4), (4, 4): (1280 / 567, 4)}
+    a22, _, _ = oracle.waveform(th, 2, 2, 2 * F)
+    v = (2 * math.pi * th[0] * TSUN * F) ** (1.0 / 3.0)     # (M Omega)^{1/3}
+    for (l, m), (coef, power) in poisson.items():
+        alm, _, _ = oracle.waveform(th, l, m, m * F)
+        flux_ratio = (m * m / 4) * (m / 2) * (alm / a22) ** 2
+        assert np.allclose(flux_ratio, coef * v ** power, rtol=3e-6, atol=0), (l, m)   # q = 1e7: delta, 1 - 3 eta to 1e-6
+    # (a) mass-ratio dependence against the point-mass moments, normalised to the (2,2) mode (mu r^2: moment 1)
+    qref = 5.0
+    for q in (1.0, 1.3, 3.0, 8.0):
+        for (l, m) in ((2, 1), (3, 3), (3, 2), (4, 4)):
+            ratio = []
+            for qq in (q, qref):
+                th[1] = qq
+                alm, _, _ = oracle.waveform(th, l, m, m * F)
+                a22, _, _ = oracle.waveform(th, 2, 2, 2 * F)
+                ratio.append(alm / a22)
+            want = abs(_point_mass_moment(q, l, (l + m) % 2 == 1)) / abs(_point_mass_moment(qref, l, (l + m) % 2 == 1))
+            assert np.allclose(ratio[0] / ratio[1], want, rtol=1e-12, atol=1e-15), (q, l, m)
+    assert _point_mass_moment(1.0, 3, False) == 0.0 and _point_mass_moment(1.0, 2, True) == 0.0
+
+
+def test_mode_constant_phase_reading_G5():
+    """G5 is a READING, not a pin: BASELINE.json writes Psi_lm = (m/2) Psi_22 without argument; applied to the whole
+    of Psi_22(2f/m) this gives the constant -(m/2)(pi/4) = -m pi/8 per mode (a stricter stationary-phase treatment
+    would give -pi/4 for every m).  The paper fixes neither; DESIGN.md lists it as "reading, unpinned".  This test
+    only makes the reading explicit: with t_c = phi_c = 0, Psi_lm(f) + m pi/8 is (m/2) x the PN part of Psi_22(2f/m),
+    the PN part being pinned by P1/P2 through t_22."""
+    th = THETA.copy(); th[6] = 0.0; th[10] = 0.0
+    f = np.array([3e-4, 2e-3])
+    for (l, m) in ((2, 1), (3, 3), (3, 2), (4, 4)):
+        _, plm, _ = oracle.waveform(th, l, m, f)
+        _, p22, _ = oracle.waveform(th, 2, 2, 2 * f / m)
+        pn22 = p22 + math.pi / 4
+        assert np.allclose(plm + m * math.pi / 8, m / 2 * pn22, rtol=1e-14, atol=0)
+
+
 def test_amplitude_is_textbook_restricted_pn():
     """O4: A_22 * (Y_22 + Y_2-2)/2 equals (1+cos^2 i)/2 sqrt(5/24) pi^{-2/3} Mc^{5/6} f^{-7/6} / D."""
     th = THETA.copy()
@@ -538,6 +641,39 @@ def test_P14_double_vs_binary128_on_config1_bins():
             # tolerance: |Psi| * 2^-53 with |Psi| up to ~3e5 rad for the lightest systems -> 3e-11;
             # measured worst case is ~1e-11 (SURVEY's 1e-12 holds for M >= 1e6 only)
             assert np.abs(r[b, 0, c] - rq[b, 0, c]).max() <= 1e-10 * np.abs(rq[b, 0, c]).max()
+
+
+def test_P14_double_vs_binary128_over_the_full_band_and_at_the_nulls():
+    """P14 over the band of configs 2-5 (0.1 ... 101 mHz) and in the neighbourhood of every in-band zero of g(z)
+    (Eq. 6; G9): bin by bin, the double oracle must agree with its own binary128 evaluation to 2e-9 of the bin's
+    largest channel (2 pi f t_c reaches 1.3e6 rad: one ulp of that phase is 2.3e-10 rad; measured 6e-10), and
+    also within +-3 bins of the zeros, where the expanded form 1 - z^2 - z^4 + z^6 lost up to 3e-7 (the oracle
+    evaluates the product (1 - z^2)(1 - z^4) of SURVEY O10 for that reason)."""
+    grid = W.config(2).grid
+    fgrid = grid.freqs()
+    th = W.config(4, B=2).params
+    for gen in (20, 15):
+        for det in (W.lisa_like(gen), W.taiji_like(gen), W.tianqin_like(gen)):
+            idx = set(range(0, grid.N, 4099))
+            step = C_SI / ((4.0 if gen == 20 else 2.0) * det.L_m)
+            nulls = [n * step for n in range(1, int(fgrid[-1] / step) + 1)]
+            for fn in nulls:
+                k0 = int(round((fn - grid.f0) / grid.df))
+                idx |= {k for k in range(k0 - 3, k0 + 4) if 0 <= k < grid.N}
+            f = fgrid[np.array(sorted(idx))]
+            model = W.Model(W.MODES_HM, (det,))
+            r = oracle.response(th, f, model)[:, 0]
+            rq = oracle.response(th, f, model, quad=True)[:, 0]
+            s = np.abs(rq).max(axis=1, keepdims=True)
+            err = (np.abs(r - rq) / s).max(axis=(0, 1))
+            # the bin NEAREST a zero may sit arbitrarily close to it (LISA-like 29.979 mHz: 0.005 bin, |g| 5e-7 of
+            # its typical size): there the double rounding of the argument 2 pi f L shows as 3e-9; tolerance 1e-8
+            nearest = np.zeros(f.size, dtype=bool)
+            for fn in nulls:
+                nearest[np.argmin(np.abs(f - fn))] = True
+            assert err[~nearest].max() <= 2e-9 and err.max() <= 1e-8, (gen, det.name, err.max())
+            if det.kind == 0:
+                assert len(nulls) >= (3 if gen == 20 else 1)
 
 
 # ------------------------------------------------------------------ P16: SNR sanity on the full config-2 grid
