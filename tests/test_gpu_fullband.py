@@ -7,12 +7,17 @@ in-band null of the TDI prefactor g(z) of Eq. 6 (n 
 turns.  Tolerance PER BIN (not per array, so that a frequency-local error cannot hide behind the large low-frequency
 amplitudes): with s_k = max_c |h_c(f_k)| of the oracle,
 
-    |got_c(f_k) - want_c(f_k)| <= 1e-8 |want_c(f_k)| + FLOOR(f_k) s_k,    FLOOR = 4e-15 (1 + 1/x_k) / |1 - z^2|...
+    |got_c(f_k) - want_c(f_k)| <= 1e-8 |want_c(f_k)| + FLOOR(f_k) s_k,
+    FLOOR(f) = 16 eps (1 + 1/x) + 4 eps 2 pi f / df,     x = 2 pi f L / c,  eps = 2^-52
 
-see `bin_floor`: both sides form X, Y, Z from six single links of relative rounding error eps = 2.2e-16 whose sum
-cancels to O(x) of a link (x = 2 pi f L / c; the long-wavelength limit, pin P7) and, for T = (X+Y+Z)/sqrt3, to
-O(x^3) (pin P8): the absolute rounding noise of ANY double evaluation is ~ eps |y| ~ (eps / x) s_k per bin, the
-oracle's included.
+(`bin_floor`).  First term: both sides form X, Y, Z from six single links of relative rounding error eps whose sum
+cancels to O(x) of a link (the long-wavelength limit, pin P7) and, for T = (X+Y+Z)/sqrt3, to O(x^3) (pin P8): the
+absolute rounding noise of ANY double evaluation is ~ eps |y| ~ (eps / x) s_k per bin, the oracle's included.
+Second term: the oracle adds 2 pi f t_c (up to 2 pi f / df = 1.6e6 rad at the top of the band) to the PN phase in
+double, i.e. it carries an absolute phase error of a few eps |phase| (pin P14 over the band: the double oracle is
+6e-10 from its own binary128 evaluation at 0.1 Hz; the CUDA path, which reduces the two phases separately, 5e-13).
+A channel therefore agrees to 1e-8 of ITSELF or, where it is small against its neighbours (T at low f, a channel
+passing through zero), to better than 1e-9 of the bin's largest channel.
 
 The per-bin analogue for the derivatives (S10) runs pespace_fisher on ONE-bin grids: F_ij is then
 4 df sum_c Re[conj(d_i h_c) d_j h_c] / S_c of that bin alone, compared entry by entry on the Cauchy-Schwarz scale.
@@ -72,25 +77,30 @@ def band_indices(grid, dets, stride=257, around=3):
     return np.array(sorted(idx)), n_null
 
 
-def bin_floor(det, f):
-    """rounding-noise floor of one bin relative to the bin's largest channel (module docstring): 16 eps (1 + 1/x)"""
+def cancel_floor(det, f):
+    """rounding noise of the link sums relative to the bin's largest channel: 16 eps (1 + 1/x) (module docstring)"""
     x = 2.0 * np.pi * f * det.L_m / C_SI
     return 16.0 * EPS * (1.0 + 1.0 / x)
 
 
-def check_response_per_bin(got, want, f, dets, what=""):
+def bin_floor(det, f, df):
+    """cancellation noise + the oracle's phase rounding, 4 eps 2 pi f / df (t_c <= T = 1/df)"""
+    return cancel_floor(det, f) + 4.0 * EPS * 2.0 * np.pi * f / df
+
+
+def check_response_per_bin(got, want, f, dets, what="", df=W.MONTH_DF):
     worst = 0.0
     for b in range(want.shape[0]):
         for d, det in enumerate(dets):
             s = np.abs(want[b, d]).max(axis=0)                     # [N]: largest channel of the bin
             assert np.all(s > 0.0)
-            floor = bin_floor(det, f) * s
+            floor = bin_floor(det, f, df) * s
             for c in range(3):
                 err = np.abs(got[b, d, c] - want[b, d, c])
                 tol = TOL_RESP * np.abs(want[b, d, c]) + floor
                 bad = np.nonzero(err > tol)[0]
                 assert bad.size == 0, (what, b, d, c, f[bad[:5]], (err[bad[:5]] / s[bad[:5]]))
-                worst = max(worst, float((err / (np.abs(want[b, d, c]) + floor / TOL_RESP)).max()))
+                worst = max(worst, float((err / tol).max()))
     return worst
 
 
@@ -135,6 +145,23 @@ def test_response_near_nulls_dense(P):
             assert np.abs(want[0, 0, 0]).min() < 0.05 * np.abs(want[0, 0, 0]).max()
 
 
+@pytest.mark.parametrize("gen", [20, 15])
+def test_response_tab_full_band_per_bin(P, gen):
+    """pespace_response_tab (tabulated mode waveforms, reading T1) over the full band, same sample of bins and the same
+    per-bin tolerance: tables of the oracle's analytic modes on 2000 log-spaced nodes, five modes, three detectors"""
+    grid = W.config(2).grid
+    dets = (W.lisa_like(gen), W.taiji_like(gen), W.tianqin_like(gen))
+    model = W.Model(W.MODES_HM, dets)
+    idx, _ = band_indices(grid, dets)
+    fgrid = grid.freqs()
+    f = fgrid[idx]
+    th = W.config(4, B=4).params
+    table = W.table_from_waveform_fn(th, model.mode_mask, W.log_nodes(fgrid[0], fgrid[-1], 2000), oracle.waveform)
+    got = P.response_tab(dev(th), P.WaveTable(*(dev(x) for x in table)), dev(f), model).cpu().numpy()
+    want = oracle.response_tab(th, table, f, model)
+    check_response_per_bin(got, want, f, dets, f"tab gen {gen}")
+
+
 def _window_workload(det_list, k0, n, B, mask, seed):
     """an n-bin stretch of the config-2 lattice starting at bin k0: same df, f0 moved"""
     base = W.config(2).grid
@@ -154,7 +181,7 @@ def test_loglike_noisy_window_straddling_a_null(P, gen):
             k0 = int(round((fn - base.f0) / base.df)) - 200
             wl = _window_workload([det], k0, 401, 9, W.MODES_HM, 7)
             data, psd = wl.data(oracle_response_fn), wl.psd()
-            assert psd[0, 0].min() < 1e-6 * np.median(psd[0, 0])
+            assert psd[0, 0].min() < 1e-3 * np.median(psd[0, 0])
             got = P.loglike(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model).cpu().numpy()
             want = oracle.loglike(wl.params, data, psd, wl.grid, wl.model)
             hh = -2.0 * oracle.loglike(wl.params, np.zeros_like(data), psd, wl.grid, wl.model)
@@ -176,10 +203,17 @@ def test_loglike_high_band_windows_three_detectors(P):
 
 
 # --------------------------------------------------------------------------------------------------------------- S10
+def phase_floor(f, df):
+    """the double oracle's phase rounding, 4 eps 2 pi f / df (module docstring; pin P14 over the band)"""
+    return 4.0 * EPS * 2.0 * np.pi * f / df
+
+
 def test_fisher_single_bin_grids_over_the_band(P):
     """per-bin derivative parity: pespace_fisher on ONE-bin grids placed over the band (incl. +-2 bins of the nulls and
     v > 1): every F_ij of the bin against the oracle's 11-tangent dual number on the Cauchy-Schwarz scale, and the
-    gradient with noisy data."""
+    gradient with noisy data.  Tolerance of a single bin: 1e-9 + 8 x the double oracle's phase rounding (the modes
+    carry independent roundings of phases up to 1.6e6 rad, which moves their interference terms; measured against
+    binary128 finite differences in the next test: oracle 2.2e-9 at 63 mHz, CUDA path 4e-11)."""
     base = W.config(2).grid
     fgrid = base.freqs()
     dets = (W.lisa_like(), W.taiji_like(), W.tianqin_like())
@@ -202,9 +236,55 @@ def test_fisher_single_bin_grids_over_the_band(P):
         eF = (np.abs(F.cpu().numpy() - Fo) / (d[:, :, None] * d[:, None, :])).max()
         rr = -2.0 * oracle.loglike(th, data, psd, wl.grid, wl.model)
         eg = (np.abs(g.cpu().numpy() - go) / (d * np.sqrt(rr)[:, None])).max()
-        assert eF <= TOL_F and eg <= TOL_F, (k, fgrid[k], eF, eg)
-        worstF, worstg = max(worstF, eF), max(worstg, eg)
-    print(f"single-bin Fisher over the band: {len(ks)} bins, worst F {worstF:.2e}, worst grad {worstg:.2e}")
+        tol_F = TOL_F + 8.0 * phase_floor(fgrid[k], base.df)
+        # gradient of ONE bin: the rounding noise of d_i h_c (cancel_floor, relative to the largest channel) enters
+        # <d - h | d_i h> through every channel with weight sqrt(w_c); on the scale sqrt(F_ii <r|r>) >= sqrt(w_A) ...
+        # that is cancel_floor x sqrt(S_max / S_min) -- at low f the T channel of a short-arm detector is pure
+        # rounding noise (pin P8) whitened by a PSD (x^2/3) S_A.  (F itself is insensitive: the noise is multiplied by
+        # the small d_j h_T.)  In sums over many bins the term averages out; here it is the whole result.
+        tol_g = tol_F + max(cancel_floor(det, fgrid[k]) * np.sqrt(psd[i].max() / psd[i].min()) for i, det in enumerate(dets))
+        assert eF <= tol_F and eg <= tol_g, (k, fgrid[k], eF, eg, tol_F, tol_g)
+        worstF, worstg = max(worstF, eF / tol_F), max(worstg, eg / tol_g)
+    print(f"single-bin Fisher over the band: {len(ks)} bins, worst F / tolerance {worstF:.2f}, worst grad / tolerance {worstg:.2f}")
+
+
+def test_fisher_single_bins_against_binary128_finite_differences(P):
+    """the extrinsic 6 x 6 block (D_L, iota, phi_c, lambda, beta, psi) of single-bin Fisher matrices against
+    Richardson-extrapolated central differences of the oracle's response evaluated in IEEE BINARY128 (steps chosen so
+    that the phase moves by 2e-3 and 1e-3 rad: truncation 1e-12, resolution of the double output 1e-13): the exact
+    definition to 1e-11, at 1e-9.  (The mass and spin columns would need steps too small for the double output.)"""
+    base = W.config(2).grid
+    fgrid = base.freqs()
+    dets = (W.lisa_like(), W.taiji_like(), W.tianqin_like())
+    th = W.config(5, B=2).params
+    th[1, 2] = 0.5; th[1, 3] = -0.3
+    sub = [4, 5, 6, 7, 8, 9]
+    for k in (20000, 77448, 130000, 163830, 233200, 261000):        # 7.8 ... 100.8 mHz; 77448: LISA-like 30 mHz null + 1
+        wl = _window_workload(dets, k, 1, 2, W.MODES_HM, 13)
+        wl.params = th
+        psd = wl.psd()
+        F, _ = P.fisher(dev(th), None, dev(psd), wl.grid, wl.model)
+        f = wl.grid.freqs()
+        dopp = 2.0 * np.pi * f[0] * 499.005 + 2.0                     # rad of phase per rad of sky angle (AU/c) + pattern
+        sens = {4: 1.0, 5: 1.0, 6: 4.0, 7: dopp, 8: dopp, 9: 4.0}
+        J = np.zeros((2, 11, 3, 3), dtype=complex)
+        for i in sub:
+            for b in range(2):
+                est = []
+                for hs in (2e-3, 1e-3):
+                    h = hs / sens[i] * (abs(th[b, i]) if i == 4 else 1.0)
+                    tp, tm = th[b:b + 1].copy(), th[b:b + 1].copy()
+                    tp[0, i] += h; tm[0, i] -= h
+                    rp = oracle.response(tp, f, wl.model, quad=True)[0, :, :, 0]
+                    rm = oracle.response(tm, f, wl.model, quad=True)[0, :, :, 0]
+                    est.append((rp - rm) / (tp[0, i] - tm[0, i]))
+                J[b, i] = (4.0 * est[1] - est[0]) / 3.0
+        w = 4.0 * wl.grid.df / psd[:, :, 0]
+        Fq = np.einsum("bidc,bjdc,dc->bij", np.conj(J), J, w).real
+        ix = np.ix_(range(2), sub, sub)
+        d = np.sqrt(np.einsum("bii->bi", Fq[ix]))
+        err = (np.abs(F.cpu().numpy()[ix] - Fq[ix]) / (d[:, :, None] * d[:, None, :])).max()
+        assert err <= TOL_F, (k, fgrid[k], err)
 
 
 def test_fisher_windows_at_the_nulls(P):
@@ -267,7 +347,7 @@ def test_masked_bins_ignore_the_data_and_exact_nulls_keep_their_weight(P):
     assert (np.abs(F.cpu().numpy() - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
     rr = -2.0 * want2
     assert (np.abs(g.cpu().numpy() - go) / (d * np.sqrt(rr)[:, None])).max() <= TOL_F
-    lm = P.loglike_mixed(dev(th), dev(data2), dev(psd2), grid, model).cpu().numpy()
+    lm = P.Likelihood(dev(data2), dev(psd2), grid, model, th.shape[0])(dev(th), mixed=True).cpu().numpy()
     assert np.abs(lm - want2).max() <= 5e-6 * np.abs(want2).min()
 
 
