@@ -100,6 +100,20 @@ int pespace_fisher(const double* d_params, int64_t B, const double* d_data_AET, 
                    const pespace_grid* grid, const pespace_model* model, double* d_out_F,
                    double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* lnL AND its gradient d lnL / d theta [B][11] in one pass by REVERSE mode ("The
+ * backward mode ... is more suitable for cases of large inputs and small output such as computing the gradients of
+ * the likelihood function"; :163, :171 gradient-based samplers).  The kernel evaluates the response as
+ * pespace_loglike does, seeds the adjoint of (X, Y, Z) with the weighted residual (Eq. 10) and sweeps back through
+ * Eq. 6, 5, the orbit, Eq. 4 and the waveform of every mode to the per-sample constants; no tangent is carried per
+ * bin.  grad_i = <d - h | d_i h> of Eq. 13/14, the quantity pespace_fisher returns in d_out_grad (derivatives
+ * w.r.t. the raw theta entries), at about 2.5-3x the cost of pespace_loglike instead of 6x.  Either output pointer
+ * may be NULL (not both).  Out-of-domain samples: lnL = -INFINITY, NaN gradient row.  Workspace:
+ * pespace_workspace_bytes_grad.  Same inputs, bit-identical outputs.  B <= 65535 x 32 per call. */
+size_t pespace_workspace_bytes_grad(int64_t B, const pespace_grid* grid, const pespace_model* model);
+int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                         const pespace_grid* grid, const pespace_model* model, double* d_out_lnL /* [B] */,
+                         double* d_out_grad /* [B][11] */, void* d_workspace, size_t workspace_bytes, void* stream);
+
 /* Mixed-precision twin of pespace_loglike (the paper's float32 mode for searches and coarse
  * maximisation).  Same arguments, same workspace size.  Every phase that enters an exponential
  * (PN phase, 2 pi f t_c, Doppler phases, their sum and its reduction modulo one turn) stays FP64; the t_lm polynomial,

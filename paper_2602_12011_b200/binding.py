@@ -65,6 +65,9 @@ def _load():
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_loglike_mixed.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
     L.pespace_fisher.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
+    L.pespace_workspace_bytes_grad.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
+    L.pespace_workspace_bytes_grad.restype = sz
+    L.pespace_loglike_grad.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
     L.pespace_response_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, i64, C.POINTER(_Model), vp, vp]
     L.pespace_workspace_bytes_tab.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
@@ -284,6 +287,39 @@ class Fisher:
 def fisher(params: torch.Tensor, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):
     """-> (F [B][11][11], grad [B][11] or None)."""
     return Fisher(data, psd, grid, model, params.shape[0])(params)
+
+
+class LikelihoodGrad(Likelihood):
+    """pespace_loglike_grad: lnL and d lnL / d theta in one reverse-mode pass (data, PSD, workspace resident)."""
+
+    def __init__(self, data: torch.Tensor, psd: torch.Tensor, grid, model, max_batch: int):
+        super().__init__(data, psd, grid, model, max_batch)
+        self.ws_bytes = int(_lib.pespace_workspace_bytes_grad(max_batch, C.byref(self._g), C.byref(self._m)))
+        if self.ws_bytes == 0:
+            raise PespaceError("pespace_workspace_bytes_grad rejected the arguments")
+        self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=self.data.device)
+
+    def __call__(self, params: torch.Tensor, out_lnL: Optional[torch.Tensor] = None,
+                 out_grad: Optional[torch.Tensor] = None):
+        """-> (lnL [B], grad [B][11])"""
+        p = _dev(params, "params")
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        if out_lnL is None:
+            out_lnL = torch.empty(B, dtype=torch.float64, device=p.device)
+        if out_grad is None:
+            out_grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_loglike_grad(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g),
+                                         C.byref(self._m), _dev(out_lnL, "out_lnL").data_ptr(),
+                                         _dev(out_grad, "out_grad").data_ptr(), self.ws.data_ptr(), self.ws_bytes,
+                                         _stream_ptr()), "pespace_loglike_grad")
+        return out_lnL, out_grad
+
+
+def loglike_grad(params: torch.Tensor, data: torch.Tensor, psd: torch.Tensor, grid, model):
+    """-> (lnL [B], d lnL / d theta [B][11]) by reverse mode"""
+    return LikelihoodGrad(data, psd, grid, model, params.shape[0])(params)
 
 
 def loglike_host(params: np.ndarray, data: np.ndarray, psd: np.ndarray, grid, model) -> np.ndarray:

@@ -66,6 +66,9 @@ enum : int {
   S_DY,
 };
 constexpr int D_STRIDE = 24;
+// [19..22] (both kinds): (AU/c) u'_x, u'_y, v'_x, v'_y in the frame of S_DX, S_DY -- the Doppler part of the sky
+// "torques" of the adjoint gradient (pespace_grad.cuh); unused by the other kernels
+enum : int { S_UX = D_BASE + 19, S_UY, S_VX, S_VY };
 // kind 0: [0] alpha0 - lambda0 (pu), [2..16] S_K, S_U, S_V, [17..18] S_DX, S_DY.  The constellation with rotation
 //         phase lambda0 is the lambda0 = 0 constellation at orbital phase alpha - lambda0, rotated about z by lambda0:
 //         the rotation is applied to k, u', v' here, so the kernels only ever see spacecraft at 0, 120, 240 degrees.
@@ -418,9 +421,13 @@ __device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc
         put(base + off[j] + 0, wx * r43); put(base + off[j] + 1, wy * r43); put(base + off[j] + 2, -0.5 * w[2]);
         put(base + off[j] + 3, -3.0 * r43 * wx); put(base + off[j] + 4, -3.0 * r43 * wy);
         if (j == 0) { put(base + (S_DX - D_BASE), (kAU / kC) * wx); put(base + (S_DY - D_BASE), (kAU / kC) * wy); }
+        if (j == 1) { put(base + (S_UX - D_BASE), (kAU / kC) * wx); put(base + (S_UY - D_BASE), (kAU / kC) * wy); }
+        if (j == 2) { put(base + (S_VX - D_BASE), (kAU / kC) * wx); put(base + (S_VY - D_BASE), (kAU / kC) * wy); }
       }
     } else {
       put(base + (S_DX - D_BASE), (kAU / kC) * k[0]); put(base + (S_DY - D_BASE), (kAU / kC) * k[1]);
+      put(base + (S_UX - D_BASE), (kAU / kC) * up[0]); put(base + (S_UY - D_BASE), (kAU / kC) * up[1]);
+      put(base + (S_VX - D_BASE), (kAU / kC) * vp[0]); put(base + (S_VY - D_BASE), (kAU / kC) * vp[1]);
       put(base, T(kTurn * a0));
       double p0 = tcv / D.period_s;
       p0 -= rint(p0);

@@ -1,10 +1,13 @@
 // pespace_inst.cuh -- body of the pespace_inst_*.cu translation units.  The including file defines
-//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher
+//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher, 3 adjoint gradient
 //   PESPACE_INST_KIND  0 heliocentric, 1 geocentric
 //   PESPACE_INST_HALF  0 class masks 1..7, 1 class masks 8..15
 #include "pespace_launch.hpp"
 #if PESPACE_INST_WHAT == 2
 #include "pespace_fisher.cuh"
+#endif
+#if PESPACE_INST_WHAT == 3
+#include "pespace_grad.cuh"
 #endif
 
 namespace pespace {
@@ -33,6 +36,16 @@ cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2*
   return cudaSuccess;
 }
 using Fn = ResponseFn;
+#elif PESPACE_INST_WHAT == 3
+template <int KIND, unsigned CM>
+cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
+                   const double* bins, long long N, const DetC& dc, int n_det, int det, double* partial) {
+  static SmemOptIn configured;
+  if (cudaError_t e = opt_in_smem(loglike_grad_kernel<KIND, CM>, grad_smem_bytes(), configured); e != cudaSuccess) return e;
+  loglike_grad_kernel<KIND, CM><<<g, BLOCK, grad_smem_bytes(), st>>>(consts, trig, B, bins, N, dc, n_det, det, partial);
+  return cudaSuccess;
+}
+using Fn = GradFn;
 #else
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, long long B, const double* bins, long long N,
@@ -64,6 +77,8 @@ constexpr unsigned kBase = 8;
 #define PESPACE_INST_NAME PESPACE_CAT(loglike_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
 #elif PESPACE_INST_WHAT == 1
 #define PESPACE_INST_NAME PESPACE_CAT(response_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
+#elif PESPACE_INST_WHAT == 3
+#define PESPACE_INST_NAME PESPACE_CAT(grad_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
 #else
 #define PESPACE_INST_NAME PESPACE_CAT(fisher_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
 #endif

@@ -12,6 +12,8 @@ using LoglikeFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const doubl
                                   long long, const DetC&, int, int, double*);
 using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
                                    long long, const DetC&, int, int, double2*);
+using GradFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*, long long,
+                               const DetC&, int, int, double*);
 using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&,
                                  int, int, int, double*);
 
@@ -27,6 +29,7 @@ using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, c
 PESPACE_DECLARE_INST(LoglikeFn, loglike_launcher)
 PESPACE_DECLARE_INST(ResponseFn, response_launcher)
 PESPACE_DECLARE_INST(FisherFn, fisher_launcher)
+PESPACE_DECLARE_INST(GradFn, grad_launcher)
 #undef PESPACE_DECLARE_INST
 
 }  // namespace host
