@@ -12,10 +12,10 @@ struct GradPlan {
   long long nbx, ntile;
   size_t trig_bytes, bins_bytes, consts_bytes, du_bytes, partial_bytes;   // workspace, in this order
 };
-GradPlan make_grad_plan(long long B, long long N, int n_det) {
+GradPlan make_grad_plan(long long B, long long N, int n_det, unsigned cmask) {
   GradPlan p;
   p.nbx = (N + (long long)BLOCK * GCHUNKS - 1) / ((long long)BLOCK * GCHUNKS);
-  p.ntile = (B + GTILE - 1) / GTILE;
+  p.ntile = (B + grad_tile(cmask) - 1) / grad_tile(cmask);
   p.trig_bytes = align_up((size_t)NTAB * sizeof(double2), 256);
   p.bins_bytes = align_up((size_t)n_det * NBF * (size_t)N * sizeof(double), 256);
   p.consts_bytes = align_up((size_t)B * sample_stride(n_det) * sizeof(double), 256);
@@ -30,7 +30,7 @@ extern "C" {
 
 size_t pespace_workspace_bytes_grad(int64_t B, const pespace_grid* grid, const pespace_model* model) {
   if (B <= 0 || !grid_ok(grid) || !model_ok(model)) return 0;
-  const GradPlan p = make_grad_plan(B, grid->N, model->n_det);
+  const GradPlan p = make_grad_plan(B, grid->N, model->n_det, class_mask(model->mode_mask));
   return p.trig_bytes + p.bins_bytes + p.consts_bytes + p.du_bytes + p.partial_bytes;
 }
 
@@ -42,7 +42,7 @@ int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data
     return PESPACE_EINVAL;
   if (workspace_bytes < pespace_workspace_bytes_grad(B, grid, model) || ((uintptr_t)d_workspace & 15u))
     return PESPACE_EINVAL;
-  const GradPlan p = make_grad_plan(B, grid->N, model->n_det);
+  const GradPlan p = make_grad_plan(B, grid->N, model->n_det, class_mask(model->mode_mask));
   if (p.ntile > 65535) return PESPACE_EINVAL;                 // gridDim.y
   cudaStream_t st = (cudaStream_t)stream;
   char* ws = (char*)d_workspace;

@@ -31,9 +31,11 @@
 //                        three numbers per (sample, bin) whatever the detector or class; omega for lambda is z^ and
 //                        for beta is u, in triad components (-sin b, sin p cos b, cos p cos b) and (0, cos p, -sin p).
 //
-// Cost: single-class kernels run forward once and backward once; multi-class kernels need the total response before
-// any adjoint exists, so they run the forward pass twice (pass 1: all classes -> residual; pass 2: per class
-// forward + backward).  No tangent is carried per bin.
+// Cost: single-class kernels run forward once and backward once with the forward state in registers.  Multi-class
+// kernels need the total response before any adjoint exists: pass 1 runs the classes forward and parks the expensive
+// part of each class's state (the six G's, sin / cos of the orbit angle, three reciprocals, three exponentials: NST =
+// 17 doubles) in a thread-private shared-memory column; pass 2 reloads it, re-derives the cheap rest and sweeps
+// back (run-time class loop).  No tangent is carried per bin.
 #pragma once
 #include "pespace_device.cuh"
 #include "pespace_fisher.cuh"
@@ -46,8 +48,11 @@ namespace pespace {
 #ifndef PESPACE_GCHUNKS
 #define PESPACE_GCHUNKS 4
 #endif
-constexpr int GTILE = PESPACE_GTILE;       // samples per block
+constexpr int GTILE = PESPACE_GTILE;       // samples per block, single-class kernels
+constexpr int GTILE_M = 16;                // samples per block, multi-class kernels (shared memory holds the state stash)
 constexpr int GCHUNKS = PESPACE_GCHUNKS;   // chunks of BLOCK bins per block
+constexpr int NST = 17;                    // stashed doubles per class (multi-class kernels)
+__host__ __device__ constexpr int grad_tile(unsigned cmask) { return popc4(cmask) == 1 ? GTILE : GTILE_M; }
 
 // reduced vector of one (sample, block)
 enum : int {
@@ -69,10 +74,16 @@ __host__ __device__ constexpr int grad_ka_slot(int mc, int j /* 0 a+, 1 b+, 2 ax
 // number of leading slots a kernel with class mask CMASK can touch
 __host__ __device__ constexpr int grad_nv(unsigned cmask) { return (cmask & 8u) ? 34 : (cmask & 4u) ? 32 : (cmask & 1u) ? 30 : 28; }
 
-constexpr size_t grad_smem_bytes() {
-  return sizeof(double) * ((size_t)2 * NTAB + (size_t)GTILE * SMEM_STRIDE + (size_t)(BLOCK / 32) * GTILE * NVP);
+// per-warp scratch region (doubles): the state stash of the multi-class kernels ([class][NST][32 lanes]) and the
+// transpose buffer of the reduction ([32 values][33]) share it -- the stash is dead once pass 2 of a sample is done
+__host__ __device__ constexpr int grad_region(unsigned cmask) {
+  return (popc4(cmask) > 1 && popc4(cmask) * NST * 32 > 32 * 33) ? popc4(cmask) * NST * 32 : 32 * 33;
 }
-
+__host__ __device__ constexpr size_t grad_smem_bytes(unsigned cmask) {
+  return sizeof(double) * ((size_t)2 * NTAB + (size_t)grad_tile(cmask) * SMEM_STRIDE +
+                           (size_t)(BLOCK / 32) * grad_tile(cmask) * NVP + (size_t)(BLOCK / 32) * grad_region(cmask));
+}
+static_assert(grad_smem_bytes(15u) <= 227u * 1024u && grad_smem_bytes(2u) <= 227u * 1024u, "one block per SM");
 static_assert(S_VY < D_BASE + D_STRIDE, "detector block holds the torque constants S_UX ... S_VY");
 
 // forward state of one mode class that the backward sweep needs
@@ -186,43 +197,87 @@ __device__ __forceinline__ void grad_fwd_class(int mc, bool first, const BinC& b
   add(S[4], S[5], 2, 0, st.kb_, -Wr[1], -Wi[1], false);
 }
 
-// backward sweep of one class: Sb = adjoint of S (Re, -Im parts of X, Y, Z); adds to acc
+// multi-class kernels: park / reload the expensive part of a class's forward state (col = this lane's column in the
+// warp's region, stride 32)
+template <int KIND>
+__device__ __forceinline__ void grad_store_state(const ClassState<KIND>& st, double* __restrict__ col) {
+  col[0 * 32] = st.G1k; col[1 * 32] = st.G2k; col[2 * 32] = st.G1u; col[3 * 32] = st.G2u;
+  col[4 * 32] = st.G1v; col[5 * 32] = st.G2v; col[6 * 32] = st.s1; col[7 * 32] = st.c1;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    col[(8 + i) * 32] = st.rD[i]; col[(11 + i) * 32] = st.Er[i]; col[(14 + i) * 32] = st.Ei[i];
+  }
+}
+template <int KIND>
+__device__ __forceinline__ void grad_restore_state(int mc, const BinC& bc, const double* __restrict__ sc, double va,
+                                                   double La, const double* __restrict__ col, ClassState<KIND>& st) {
+  const double v = va * kClassCB[mc], v2 = v * v;
+  st.v = v; st.v2 = v2; st.L = La + kClassLN3[mc];
+  st.sp = kClassS83[mc] * bc.fm53;
+  st.sq = kClassS83[mc] * bc.fm83;
+  const double* ka = sc + W_KA + 4 * mc;
+  if (mc == 1) { st.CKp = fma(ka[1], v2, ka[0]); st.CKc = fma(ka[3], v2, ka[2]); }
+  else { const double vp = (mc == 3) ? v2 : v; st.CKp = vp * ka[0]; st.CKc = vp * ka[2]; }
+  st.G1k = col[0 * 32]; st.G2k = col[1 * 32]; st.G1u = col[2 * 32]; st.G2u = col[3 * 32];
+  st.G1v = col[4 * 32]; st.G2v = col[5 * 32]; st.s1 = col[6 * 32]; st.c1 = col[7 * 32];
+  if (KIND == 0) { st.c2 = fma(2.0 * st.c1, st.c1, -1.0); st.s2 = 2.0 * st.s1 * st.c1; }
+  else { st.c2 = 0.0; st.s2 = 0.0; }                       // kind 1: the backward sweep does not use them
+  constexpr double R3H = 0.86602540378443864676;
+  const double tk = R3H * st.G2k, tu = R3H * st.G2u, tv = R3H * st.G2v;
+  st.ka_ = tk + tk; st.kb_ = fma(-1.5, st.G1k, -tk); st.kc_ = fma(1.5, st.G1k, -tk);
+  st.uu[0] = tu + tu; st.uu[1] = fma(-1.5, st.G1u, -tu); st.uu[2] = fma(1.5, st.G1u, -tu);
+  st.vv[0] = tv + tv; st.vv[1] = fma(-1.5, st.G1v, -tv); st.vv[2] = fma(1.5, st.G1v, -tv);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    st.rD[i] = col[(8 + i) * 32]; st.Er[i] = col[(11 + i) * 32]; st.Ei[i] = col[(14 + i) * 32];
+    st.pl[i] = st.rD[i] * fma(st.uu[i], st.uu[i], -st.vv[i] * st.vv[i]);
+    st.ql[i] = st.rD[i] * (st.uu[i] * st.vv[i]);
+  }
+}
+
+// backward sweep of one class: Sb = adjoint of S (Re, -Im parts of X, Y, Z); adds to acc.  Written as FMA chains
+// (accumulators as addends, signs on the small factors): every DADD / DMUL saved is two issue cycles of the FP64 pipe.
 template <int KIND>
 __device__ __forceinline__ void grad_bwd_class(int mc, const BinC& bc, const double* __restrict__ sc, const DetC& dc,
                                                const ClassState<KIND>& st, const double (&Sb)[6], double (&acc)[NV]) {
   const double MH = 0.5 * (double)(mc + 1);
   double Wrb[3] = {0.0, 0.0, 0.0}, Wib[3] = {0.0, 0.0, 0.0}, Erb[3] = {0.0, 0.0, 0.0}, Eib[3] = {0.0, 0.0, 0.0};
   double kab = 0.0, kbb = 0.0, kcb = 0.0;
-  // adjoint of  S += sg W_l B(r, s, kap),  B = kap (E_s - cth E_r) -/+ i sth E_r   (see `add` of the forward pass)
-  auto back = [&](double Sbr, double Sbi, int r, int s_, double kap, double& kapb, double ksg, int l, double sg) {
-    const double wr = sg * (st.CKp * st.pl[l]), wi = sg * (st.CKc * st.ql[l]);
+  const double Wr[3] = {st.CKp * st.pl[0], st.CKp * st.pl[1], st.CKp * st.pl[2]};
+  const double Wi[3] = {st.CKc * st.ql[0], st.CKc * st.ql[1], st.CKc * st.ql[2]};
+  const double sEr[3] = {bc.sth * st.Er[0], bc.sth * st.Er[1], bc.sth * st.Er[2]};
+  const double sEi[3] = {bc.sth * st.Ei[0], bc.sth * st.Ei[1], bc.sth * st.Ei[2]};
+  const double kac = st.ka_ * bc.cth, kbc = st.kb_ * bc.cth, kcc = st.kc_ * bc.cth;
+  // adjoint of  S += sg W_l B(r, s, kap),  B = kap (E_s - cth E_r) -/+ i sth E_r,  kap = ks k  (see `add` of the
+  // forward pass).  (tr, ti) = sg (Sbr, Sbi); k = |kap| factor with sign ks; kc = k cth
+  auto back = [&](double tr, double ti, int r, int s_, double k, double kc, double ks, double& kb_adj, int l) {
     const double er = fma(-bc.cth, st.Er[r], st.Er[s_]), ei = fma(-bc.cth, st.Ei[r], st.Ei[s_]);
-    const double br = fma(kap, er, -bc.sth * st.Ei[r]);
-    const double bi = fma(kap, ei, bc.sth * st.Er[r]);
-    Wrb[l] = fma(sg, fma(Sbr, br, Sbi * bi), Wrb[l]);
-    Wib[l] = fma(sg, fma(Sbi, br, -Sbr * bi), Wib[l]);
-    const double brb = fma(Sbr, wr, Sbi * wi), bib = fma(Sbi, wr, -Sbr * wi);
-    kapb = fma(ksg, fma(brb, er, bib * ei), kapb);
-    const double erb = kap * brb, eib = kap * bib;
-    Erb[s_] += erb; Eib[s_] += eib;
-    Erb[r] += fma(-bc.cth, erb, bc.sth * bib);
-    Eib[r] += fma(-bc.cth, eib, -bc.sth * brb);
+    const double br = fma(ks * k, er, -sEi[r]);
+    const double bi = fma(ks * k, ei, sEr[r]);
+    Wrb[l] = fma(tr, br, fma(ti, bi, Wrb[l]));
+    Wib[l] = fma(ti, br, fma(-tr, bi, Wib[l]));
+    const double brb = fma(tr, Wr[l], ti * Wi[l]), bib = fma(ti, Wr[l], -tr * Wi[l]);
+    kb_adj = fma(ks * brb, er, fma(ks * bib, ei, kb_adj));
+    Erb[s_] = fma(ks * k, brb, Erb[s_]);
+    Eib[s_] = fma(ks * k, bib, Eib[s_]);
+    Erb[r] = fma(-ks * kc, brb, fma(bc.sth, bib, Erb[r]));
+    Eib[r] = fma(-ks * kc, bib, fma(-bc.sth, brb, Eib[r]));
   };
-  back(Sb[0], Sb[1], 0, 2, -st.kb_, kbb, -1.0, 1, 1.0);
-  back(Sb[0], Sb[1], 0, 1, st.kc_, kcb, 1.0, 2, -1.0);
-  back(Sb[2], Sb[3], 1, 0, -st.kc_, kcb, -1.0, 2, 1.0);
-  back(Sb[2], Sb[3], 1, 2, st.ka_, kab, 1.0, 0, -1.0);
-  back(Sb[4], Sb[5], 2, 1, -st.ka_, kab, -1.0, 0, 1.0);
-  back(Sb[4], Sb[5], 2, 0, st.kb_, kbb, 1.0, 1, -1.0);
+  back(Sb[0], Sb[1], 0, 2, st.kb_, kbc, -1.0, kbb, 1);        // X: + W_b B(1,3,-kb)
+  back(-Sb[0], -Sb[1], 0, 1, st.kc_, kcc, 1.0, kcb, 2);       //    - W_c B(1,2, kc)
+  back(Sb[2], Sb[3], 1, 0, st.kc_, kcc, -1.0, kcb, 2);        // Y: + W_c B(2,1,-kc)
+  back(-Sb[2], -Sb[3], 1, 2, st.ka_, kac, 1.0, kab, 0);       //    - W_a B(2,3, ka)
+  back(Sb[4], Sb[5], 2, 1, st.ka_, kac, -1.0, kab, 0);        // Z: + W_a B(3,2,-ka)
+  back(-Sb[4], -Sb[5], 2, 0, st.kb_, kbc, 1.0, kbb, 1);       //    - W_b B(3,1, kb)
 
   // ---- exponentials: phase_n [rad] = kappa (fTL nu_n + fT kR + psi),  E_n = (cos, sin)
   const double pb0 = fma(st.Er[0], Eib[0], -st.Ei[0] * Erb[0]);
   const double pb1 = fma(st.Er[1], Eib[1], -st.Ei[1] * Erb[1]);
   const double pb2 = fma(st.Er[2], Eib[2], -st.Ei[2] * Erb[2]);
   const double psib = (pb0 + pb1) + pb2;                    // per radian of the class phase
-  const double kfTL = kRadPerPu * bc.fT * dc.Lbar;
-  const double nub0 = kfTL * pb0, nub1 = kfTL * pb1, nub2 = kfTL * pb2;
-  const double kRb = (kRadPerPu * bc.fT) * psib;
+  const double kfT = kRadPerPu * bc.fT;
+  const double kfTL = kfT * dc.Lbar;
+  const double kRb = kfT * psib;
 
   // ---- arm weights: Wr = CKp pl, Wi = CKc ql, pl = rD (uu^2 - vv^2), ql = rD uu vv, rD = 1 / (uu^2 + vv^2)
   double CKpb = 0.0, CKcb = 0.0, uub[3], vvb[3];
@@ -231,24 +286,24 @@ __device__ __forceinline__ void grad_bwd_class(int mc, const BinC& bc, const dou
     CKpb = fma(Wrb[l], st.pl[l], CKpb);
     CKcb = fma(Wib[l], st.ql[l], CKcb);
     const double plb = Wrb[l] * st.CKp, qlb = Wib[l] * st.CKc;
-    const double xib = plb * st.rD[l], chb = qlb * st.rD[l];
-    const double Db = -st.rD[l] * fma(plb, st.pl[l], qlb * st.ql[l]);
-    uub[l] = fma(st.vv[l], chb, 2.0 * st.uu[l] * (Db + xib));
-    vvb[l] = fma(st.uu[l], chb, 2.0 * st.vv[l] * (Db - xib));
+    const double rD2 = st.rD[l] + st.rD[l];
+    const double xib2 = plb * rD2, chb = qlb * st.rD[l];                   // 2 xi_bar, chi_bar
+    const double Db2 = -rD2 * fma(plb, st.pl[l], qlb * st.ql[l]);           // 2 D_bar
+    uub[l] = fma(st.vv[l], chb, st.uu[l] * (Db2 + xib2));
+    vvb[l] = fma(st.uu[l], chb, st.vv[l] * (Db2 - xib2));
   }
-  // ---- projections on the arms and the spacecraft
+  // ---- projections on the arms and the spacecraft (nu_n_bar = kfTL pb_n folded in)
   constexpr double R3H = 0.86602540378443864676;
-  const double G1ub = 1.5 * (uub[2] - uub[1]), G2ub = R3H * (2.0 * uub[0] - uub[1] - uub[2]);
-  const double G1vb = 1.5 * (vvb[2] - vvb[1]), G2vb = R3H * (2.0 * vvb[0] - vvb[1] - vvb[2]);
-  const double G1kb = fma(1.5, kcb - kbb, fma(-0.5, nub1 + nub2, nub0));
-  const double G2kb = R3H * (2.0 * kab - kbb - kcb + nub1 - nub2);
+  const double G1ub = 1.5 * (uub[2] - uub[1]), G2ub = R3H * (fma(2.0, uub[0], -uub[1]) - uub[2]);
+  const double G1vb = 1.5 * (vvb[2] - vvb[1]), G2vb = R3H * (fma(2.0, vvb[0], -vvb[1]) - vvb[2]);
+  const double G1kb = fma(1.5, kcb - kbb, kfTL * fma(-0.5, pb1 + pb2, pb0));
+  const double G2kb = R3H * fma(kfTL, pb1 - pb2, fma(2.0, kab, -kbb) - kcb);
 
   // ---- torques and orbit angle(s)
   double alphab;                     // per radian of the orbit angle (kind 1: alpha_E + (yr / P) phi)
-  double uR, vR;
+  const double uR = fma(sc[S_UX], st.c1, sc[S_UY] * st.s1);
+  const double vR = fma(sc[S_VX], st.c1, sc[S_VY] * st.s1);
   if (KIND == 0) {
-    uR = fma(sc[S_UX], st.c1, sc[S_UY] * st.s1);
-    vR = fma(sc[S_VX], st.c1, sc[S_VY] * st.s1);
     const double* wk = sc + S_K; const double* wu = sc + S_U; const double* wv = sc + S_V;
     const double c2b = fma(G1kb, wk[0], fma(-G2kb, wk[1], fma(G1ub, wu[0], fma(-G2ub, wu[1], fma(G1vb, wv[0], -G2vb * wv[1])))));
     const double s2b = fma(G1kb, wk[1], fma(G2kb, wk[0], fma(G1ub, wu[1], fma(G2ub, wu[0], fma(G1vb, wv[1], G2vb * wv[0])))));
@@ -256,18 +311,16 @@ __device__ __forceinline__ void grad_bwd_class(int mc, const BinC& bc, const dou
     const double sab = fma(G2kb, wk[2], fma(G2ub, wu[2], fma(G2vb, wv[2], kRb * sc[S_DY])));
     alphab = fma(-2.0 * st.s2, c2b, fma(2.0 * st.c2, s2b, fma(-st.s1, cab, st.c1 * sab)));
   } else {
-    uR = fma(sc[S_UX], st.c1, sc[S_UY] * st.s1);
-    vR = fma(sc[S_VX], st.c1, sc[S_VY] * st.s1);
     const double phib = fma(G1kb, st.G2k, fma(-G2kb, st.G1k, fma(G1ub, st.G2u, fma(-G2ub, st.G1u, fma(G1vb, st.G2v, -G2vb * st.G1v)))));
     const double aEb = kRb * fma(sc[S_DY], st.c1, -sc[S_DX] * st.s1);
     alphab = fma(dc.yr_over_p, phib, aEb);
   }
-  acc[GV_TK] += fma(G1ub, st.G1v, fma(-G1vb, st.G1u, fma(G2ub, st.G2v, -G2vb * st.G2u)));
-  acc[GV_TU] += fma(-G1kb, st.G1v, fma(G1vb, st.G1k, fma(-G2kb, st.G2v, fma(G2vb, st.G2k, -kRb * vR))));
-  acc[GV_TV] += fma(G1kb, st.G1u, fma(-G1ub, st.G1k, fma(G2kb, st.G2u, fma(-G2ub, st.G2k, kRb * uR))));
+  acc[GV_TK] = fma(G1ub, st.G1v, fma(-G1vb, st.G1u, fma(G2ub, st.G2v, fma(-G2vb, st.G2u, acc[GV_TK]))));
+  acc[GV_TU] = fma(-G1kb, st.G1v, fma(G1vb, st.G1k, fma(-G2kb, st.G2v, fma(G2vb, st.G2k, fma(-kRb, vR, acc[GV_TU])))));
+  acc[GV_TV] = fma(G1kb, st.G1u, fma(-G1ub, st.G1k, fma(G2kb, st.G2u, fma(-G2ub, st.G2k, fma(kRb, uR, acc[GV_TV])))));
 
   // ---- phase and time polynomials: moments of the basis
-  const double pm = kRadPerPu * st.sp * psib, qm = kRadPerPu * st.sq * alphab;
+  const double pm = (kRadPerPu * st.sp) * psib, qm = (kRadPerPu * st.sq) * alphab;
   const double v = st.v, v2 = st.v2, v3 = v2 * v, v4 = v2 * v2, v5 = v4 * v, v6 = v5 * v, v7 = v6 * v;
   const double v5L = v5 * st.L, v6L = v6 * st.L;
   acc[GV_PM + 0] += pm;
@@ -288,7 +341,7 @@ __device__ __forceinline__ void grad_bwd_class(int mc, const BinC& bc, const dou
   acc[GV_QM + 6] = fma(qm, v6L, acc[GV_QM + 6]);
   acc[GV_QM + 7] = fma(qm, v7, acc[GV_QM + 7]);
   acc[GV_PHIC] = fma(MH, psib, acc[GV_PHIC]);
-  acc[GV_TCP] = fma(kRadPerPu * bc.fT, psib, acc[GV_TCP]);
+  acc[GV_TCP] = fma(kfT, psib, acc[GV_TCP]);
   acc[GV_ALPHA] = fma(kRadPerPu, alphab, acc[GV_ALPHA]);
   // ---- amplitudes
   if (mc == 1) {
@@ -308,10 +361,13 @@ __device__ __forceinline__ void grad_bwd_class(int mc, const BinC& bc, const dou
   }
 }
 
-// Sum over the warp of NVL <= NV values per lane: a halving butterfly over the first 32 (31 shuffle-adds; lane l ends
-// with the total of value l) and a plain tree for the rest.  Adds into the warp's row r[NVP].  Fixed order.
+// Sum over the warp of NVL <= NV values per lane, added into the warp's row r[NVP]; fixed order.  Values 0..31 go
+// through a shared-memory transpose (scr: [32][33] doubles, conflict-free both ways): every lane stores its values,
+// lane j then adds up row j -- 32 STS + 32 LDS + 31 DADD per thread instead of the 31 shuffle-adds and 124 selects of a
+// halving butterfly on 64-bit values.  Values 32, 33 (kernels with the m = 4 class) take a plain shuffle tree.
 template <int NVL>
-__device__ __forceinline__ void grad_warp_reduce(double (&a)[NV], int lane, double* __restrict__ r) {
+__device__ __forceinline__ void grad_warp_reduce(double (&a)[NV], int lane, double* __restrict__ scr,
+                                                 double* __restrict__ r) {
 #pragma unroll
   for (int j = 32; j < NVL; ++j) {
     double x = a[j];
@@ -319,17 +375,19 @@ __device__ __forceinline__ void grad_warp_reduce(double (&a)[NV], int lane, doub
     for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(0xffffffffu, x, o);
     if (lane == j - 32) r[j] += x;
   }
+  constexpr int NR = NVL < 32 ? NVL : 32;
+  __syncwarp();                                   // every lane is done with the stash that shares this region
 #pragma unroll
-  for (int half = 16; half > 0; half >>= 1) {
-    const bool up = lane & half;
+  for (int j = 0; j < NR; ++j) scr[j * 33 + lane] = a[j];
+  __syncwarp();
+  if (lane < NR) {
+    const double* row = scr + lane * 33;
+    double t0 = row[0], t1 = row[1], t2 = row[2], t3 = row[3];
 #pragma unroll
-    for (int i = 0; i < half; ++i) {
-      const double lo = (i < NVL) ? a[i] : 0.0, hi = (i + half < NVL) ? a[i + half] : 0.0;
-      const double keep = up ? hi : lo, send = up ? lo : hi;
-      a[i] = keep + __shfl_xor_sync(0xffffffffu, send, half);
-    }
+    for (int i = 4; i < 32; i += 4) { t0 += row[i]; t1 += row[i + 1]; t2 += row[i + 2]; t3 += row[i + 3]; }
+    r[lane] += (t0 + t1) + (t2 + t3);
   }
-  r[lane] += a[0];
+  __syncwarp();                                   // before the next sample's stash / transpose overwrites the region
 }
 
 template <int KIND, unsigned CMASK>
@@ -337,14 +395,19 @@ __global__ void __launch_bounds__(BLOCK, 1)
 loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
                     const double* __restrict__ bins /* [n_det][NBF][N] */, long long N, DetC dc, int n_det, int det,
                     double* __restrict__ partial /* [n_det][gridDim.x][B][NVP] */) {
+  constexpr int NCLS = popc4(CMASK);
+  constexpr int NVL = grad_nv(CMASK);
+  constexpr int TILE_G = grad_tile(CMASK);
   double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
   double* smem = reinterpret_cast<double*>(tab + NTAB);
-  double* red = smem + GTILE * SMEM_STRIDE;            // [warps][GTILE][NVP]
-  const long long b0 = (long long)blockIdx.y * GTILE;
+  double* red = smem + TILE_G * SMEM_STRIDE;                     // [warps][TILE_G][NVP]
+  double* region = red + (BLOCK / 32) * TILE_G * NVP + (threadIdx.x >> 5) * grad_region(CMASK);   // this warp's scratch
+  double* stash = region + (threadIdx.x & 31);                   // [class][NST][32]: this lane's column
+  const long long b0 = (long long)blockIdx.y * TILE_G;
   stage_trig(tab, trig);
   {
     const int stride = sample_stride(n_det);
-    for (int i = threadIdx.x; i < GTILE * SMEM_STRIDE; i += BLOCK) {
+    for (int i = threadIdx.x; i < TILE_G * SMEM_STRIDE; i += BLOCK) {
       const int s = i / SMEM_STRIDE, j = i % SMEM_STRIDE;
       long long b = b0 + s;
       if (b >= B) b = B - 1;
@@ -352,12 +415,10 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
       smem[i] = consts[b * stride + src];
     }
   }
-  for (int i = threadIdx.x; i < (BLOCK / 32) * GTILE * NVP; i += BLOCK) red[i] = 0.0;
+  for (int i = threadIdx.x; i < (BLOCK / 32) * TILE_G * NVP; i += BLOCK) red[i] = 0.0;
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  const int ns = (int)min((long long)GTILE, B - b0);
-  constexpr int NCLS = popc4(CMASK);
-  constexpr int NVL = grad_nv(CMASK);
+  const int ns = (int)min((long long)TILE_G, B - b0);
   for (int ch = 0; ch < GCHUNKS; ++ch) {
     const long long kbase = ((long long)blockIdx.x * GCHUNKS + ch) * BLOCK;
     if (kbase >= N) break;
@@ -383,7 +444,19 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
         constexpr int MC0 = (CMASK & 1u) ? 0 : (CMASK & 2u) ? 1 : (CMASK & 4u) ? 2 : 3;
         grad_fwd_class<KIND>(MC0, true, bc, sc, dc, tab, va, La, ftc, st, S);
       } else {
-        eval_xyz<KIND, CMASK, true>(bc, sc, dc, tab, S);     // pass 1: the total response
+        // pass 1: every class forward, the expensive part of its state parked in shared memory.  The class loop is NOT
+        // unrolled: unrolled, the four bodies were scheduled across each other with 1.6 KB of spills per thread and the
+        // kernel ran 1.7x slower
+        bool first = true;
+        int slot = 0;
+#pragma unroll 1
+        for (int mc = 0; mc < 4; ++mc) {
+          if (!((CMASK >> mc) & 1u)) continue;
+          grad_fwd_class<KIND>(mc, first, bc, sc, dc, tab, va, La, ftc, st, S);
+          grad_store_state<KIND>(st, stash + slot * (NST * 32));
+          first = false;
+          ++slot;
+        }
       }
       double acc[NV];
 #pragma unroll
@@ -391,16 +464,11 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
       double Sb[6];
       {
         // residual and its weight: adjoint seeds of A = Z - X, E = X - 2Y + Z, T = X + Y + Z (unnormalised, as folded)
-        const double a0 = w[0] * (dr[0] - (S[4] - S[0])), a1 = w[0] * (di[0] - (S[5] - S[1]));
-        const double e0 = w[1] * (dr[1] - (S[0] - 2.0 * S[2] + S[4])), e1 = w[1] * (di[1] - (S[1] - 2.0 * S[3] + S[5]));
-        const double t0 = w[2] * (dr[2] - (S[0] + S[2] + S[4])), t1 = w[2] * (di[2] - (S[1] + S[3] + S[5]));
-        double q = a0 * (dr[0] - (S[4] - S[0]));
-        q = fma(a1, di[0] - (S[5] - S[1]), q);
-        q = fma(e0, dr[1] - (S[0] - 2.0 * S[2] + S[4]), q);
-        q = fma(e1, di[1] - (S[1] - 2.0 * S[3] + S[5]), q);
-        q = fma(t0, dr[2] - (S[0] + S[2] + S[4]), q);
-        q = fma(t1, di[2] - (S[1] + S[3] + S[5]), q);
-        acc[GV_LNL] = q;
+        const double ra0 = dr[0] - (S[4] - S[0]), ra1 = di[0] - (S[5] - S[1]);
+        const double re0 = dr[1] - (S[0] - 2.0 * S[2] + S[4]), re1 = di[1] - (S[1] - 2.0 * S[3] + S[5]);
+        const double rt0 = dr[2] - (S[0] + S[2] + S[4]), rt1 = di[2] - (S[1] + S[3] + S[5]);
+        const double a0 = w[0] * ra0, a1 = w[0] * ra1, e0 = w[1] * re0, e1 = w[1] * re1, t0 = w[2] * rt0, t1 = w[2] * rt1;
+        acc[GV_LNL] = fma(t1, rt1, fma(t0, rt0, fma(e1, re1, fma(e0, re0, fma(a1, ra1, a0 * ra0)))));
         Sb[0] = (e0 + t0) - a0; Sb[1] = (e1 + t1) - a1;
         Sb[2] = fma(-2.0, e0, t0); Sb[3] = fma(-2.0, e1, t1);
         Sb[4] = (e0 + t0) + a0; Sb[5] = (e1 + t1) + a1;
@@ -409,15 +477,16 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
         constexpr int MC0 = (CMASK & 1u) ? 0 : (CMASK & 2u) ? 1 : (CMASK & 4u) ? 2 : 3;
         grad_bwd_class<KIND>(MC0, bc, sc, dc, st, Sb, acc);
       } else {
+        int slot = 0;
 #pragma unroll 1
         for (int mc = 0; mc < 4; ++mc) {
           if (!((CMASK >> mc) & 1u)) continue;
-          double S2[6];
-          grad_fwd_class<KIND>(mc, true, bc, sc, dc, tab, va, La, ftc, st, S2);   // pass 2: the class again, state kept
+          grad_restore_state<KIND>(mc, bc, sc, va, La, stash + slot * (NST * 32), st);   // pass 2
           grad_bwd_class<KIND>(mc, bc, sc, dc, st, Sb, acc);
+          ++slot;
         }
       }
-      grad_warp_reduce<NVL>(acc, lane, red + (warp * GTILE + s) * NVP);
+      grad_warp_reduce<NVL>(acc, lane, region, red + (warp * TILE_G + s) * NVP);
     }
   }
   __syncthreads();
@@ -426,7 +495,7 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
     const int s = i / NVP, j = i % NVP;
     double t = 0.0;
 #pragma unroll
-    for (int wv = 0; wv < BLOCK / 32; ++wv) t += red[(wv * GTILE + s) * NVP + j];
+    for (int wv = 0; wv < BLOCK / 32; ++wv) t += red[(wv * TILE_G + s) * NVP + j];
     partial[(((size_t)det * gridDim.x + blockIdx.x) * (size_t)B + (size_t)(b0 + s)) * NVP + j] = t;
   }
 }

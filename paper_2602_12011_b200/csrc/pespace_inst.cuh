@@ -41,8 +41,8 @@ template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
                    const double* bins, long long N, const DetC& dc, int n_det, int det, double* partial) {
   static SmemOptIn configured;
-  if (cudaError_t e = opt_in_smem(loglike_grad_kernel<KIND, CM>, grad_smem_bytes(), configured); e != cudaSuccess) return e;
-  loglike_grad_kernel<KIND, CM><<<g, BLOCK, grad_smem_bytes(), st>>>(consts, trig, B, bins, N, dc, n_det, det, partial);
+  if (cudaError_t e = opt_in_smem(loglike_grad_kernel<KIND, CM>, grad_smem_bytes(CM), configured); e != cudaSuccess) return e;
+  loglike_grad_kernel<KIND, CM><<<g, BLOCK, grad_smem_bytes(CM), st>>>(consts, trig, B, bins, N, dc, n_det, det, partial);
   return cudaSuccess;
 }
 using Fn = GradFn;
