@@ -398,6 +398,7 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
   constexpr int NCLS = popc4(CMASK);
   constexpr int NVL = grad_nv(CMASK);
   constexpr int TILE_G = grad_tile(CMASK);
+  constexpr int MCL = (CMASK & 8u) ? 3 : (CMASK & 4u) ? 2 : (CMASK & 2u) ? 1 : 0;   // the last class of the mask
   double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
   double* smem = reinterpret_cast<double*>(tab + NTAB);
   double* red = smem + TILE_G * SMEM_STRIDE;                     // [warps][TILE_G][NVP]
@@ -453,7 +454,7 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
         for (int mc = 0; mc < 4; ++mc) {
           if (!((CMASK >> mc) & 1u)) continue;
           grad_fwd_class<KIND>(mc, first, bc, sc, dc, tab, va, La, ftc, st, S);
-          grad_store_state<KIND>(st, stash + slot * (NST * 32));
+          if (mc != MCL) grad_store_state<KIND>(st, stash + slot * (NST * 32));   // the last class stays in registers
           first = false;
           ++slot;
         }
@@ -477,11 +478,12 @@ loglike_grad_kernel(const double* __restrict__ consts, const double2* __restrict
         constexpr int MC0 = (CMASK & 1u) ? 0 : (CMASK & 2u) ? 1 : (CMASK & 4u) ? 2 : 3;
         grad_bwd_class<KIND>(MC0, bc, sc, dc, st, Sb, acc);
       } else {
+        grad_bwd_class<KIND>(MCL, bc, sc, dc, st, Sb, acc);       // pass 2: the last class first, its state is still live
         int slot = 0;
 #pragma unroll 1
-        for (int mc = 0; mc < 4; ++mc) {
+        for (int mc = 0; mc < MCL; ++mc) {
           if (!((CMASK >> mc) & 1u)) continue;
-          grad_restore_state<KIND>(mc, bc, sc, va, La, stash + slot * (NST * 32), st);   // pass 2
+          grad_restore_state<KIND>(mc, bc, sc, va, La, stash + slot * (NST * 32), st);
           grad_bwd_class<KIND>(mc, bc, sc, dc, st, Sb, acc);
           ++slot;
         }
