@@ -183,6 +183,10 @@ int pespace_session_loglike_mixed(pespace_session* s, const double* h_params, in
  * data set; the Fisher matrix alone needs only the PSD).  h_out_F may be NULL: gradient only. */
 int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B, double* h_out_F,
                            double* h_out_grad);
+/* h_params [B][11] -> h_out_lnL [B] and h_out_grad [B][11] through pespace_loglike_grad (reverse mode; either output
+ * may be NULL, not both).  Needs data and PSD.  Its workspace is allocated on first use. */
+int pespace_session_loglike_grad(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL,
+                                 double* h_out_grad);
 /* Tabulated mode waveforms through a session: h_fnodes [K] (checked here for strictly increasing order),
  * h_amp, h_phase, h_tf [B][n_modes][K] as in pespace_wavetable but in HOST memory; they are copied to the device
  * with theta on every call (the tables belong to the batch).  Device buffers are allocated on first use. */
@@ -196,26 +200,6 @@ int pespace_session_destroy(pespace_session* s);
 int pespace_loglike_host(const double* h_params, int64_t B, const double* h_data_AET,
                          const double* h_psd, const pespace_grid* grid, const pespace_model* model,
                          double* h_out_lnL);
-
-/* FP64 FMA micro-benchmark used as the roofline denominator: runs `iters` blocks of 64
- * DFMAs (8 independent chains) per thread on every SM and returns the sustained rate in
- * TFLOP/s (FMA = 2 flop) and the kernel time in ms.  Synchronous.
- *   mode 0: a = a*m + c with m, c shared by the chains (two register operands per DFMA):
- *           the FP64 pipe peak, 1 warp-instruction / 2 cycles / SM sub-partition;
- *   mode 1: a = a*b + c with three distinct register operands per DFMA: the register-file
- *           read bandwidth then limits the pipe to 1 / 3 cycles (profiles/r01_fp64_operand_bandwidth.md). */
-int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms);
-
-/* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel
- * (the fused per-bin likelihood kernel, or the Fisher kernel) is bracketed by CUDA events on the
- * launching stream.
- * pespace_profile_read synchronises those events and returns the summed kernel time in ms and
- * the number of launches since the last read (either pointer may be NULL), then resets. */
-int pespace_profile_enable(int on);
-int pespace_profile_read(double* h_main_ms, int64_t* h_launches);
-
-/* Number of kernels this library has launched since load (all calls, all streams). */
-int64_t pespace_launch_count(void);
 
 const char* pespace_strerror(int code);
 const char* pespace_version(void);

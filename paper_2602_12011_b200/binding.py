@@ -17,7 +17,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
-           "pespace_loglike_mixed", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
+           "pespace_loglike_mixed", "pespace_workspace_bytes_grad", "pespace_loglike_grad",
+           "pespace_session_loglike_grad", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
            "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
@@ -79,6 +80,7 @@ def _load():
     L.pespace_session_loglike.argtypes = [vp, vp, i64, vp]
     L.pespace_session_loglike_mixed.argtypes = [vp, vp, i64, vp]
     L.pespace_session_fisher.argtypes = [vp, vp, i64, vp, vp]
+    L.pespace_session_loglike_grad.argtypes = [vp, vp, i64, vp, vp]
     L.pespace_session_loglike_tab.argtypes = [vp, vp, i64, i64, vp, vp, vp, vp, vp]
     L.pespace_session_destroy.argtypes = [vp]
     L.pespace_fp64_peak.argtypes = [C.c_int, C.c_int, C.POINTER(C.c_double), C.POINTER(C.c_double)]
@@ -377,6 +379,19 @@ class Session:
         else:
             _check(_lib.pespace_session_loglike(self._h, pp, int(p.shape[0]), op), "pespace_session_loglike")
         return out
+
+    def loglike_grad(self, params, out_lnL=None, out_grad=None):
+        """-> (lnL [B], d lnL / d theta [B][11]) through pespace_loglike_grad (reverse mode)"""
+        pp, p = _host_ptr(params, np.float64, "params")
+        B = int(p.shape[0])
+        if out_lnL is None:
+            out_lnL = np.empty(B, dtype=np.float64)
+        if out_grad is None:
+            out_grad = np.empty((B, NPAR), dtype=np.float64)
+        lp, keep_l = _host_ptr(out_lnL, np.float64, "out_lnL")
+        gp, keep_g = _host_ptr(out_grad, np.float64, "out_grad")
+        _check(_lib.pespace_session_loglike_grad(self._h, pp, B, lp, gp), "pespace_session_loglike_grad")
+        return out_lnL, out_grad
 
     def loglike_tab(self, params, table, out=None):
         """table = (fnodes [K], amp, phase, tf [B][n_modes][K]) as host arrays / CPU tensors"""

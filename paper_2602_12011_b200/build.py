@@ -14,7 +14,7 @@ OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libpespace.so")
 SOURCES = sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 DEPS = SOURCES + sorted(glob.glob(os.path.join(CSRC, "*.cuh"))) + sorted(glob.glob(os.path.join(CSRC, "*.hpp"))) + \
-    [os.path.join(os.path.dirname(HERE), "include", "pespace.h")]
+    sorted(glob.glob(os.path.join(os.path.dirname(HERE), "include", "*.h")))
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"] + os.environ.get("PESPACE_NVCC_EXTRA", "").split()

@@ -19,7 +19,8 @@ char* cuda_msg() {
 
 namespace {
 
-bool g_profile = false;
+std::atomic<bool> g_profile{false};
+constexpr size_t kMaxEvents = 65536;   // bound of the event list between two pespace_profile_read calls
 std::vector<EvPair> g_events;
 std::mutex g_ev_mutex;
 
@@ -58,7 +59,11 @@ namespace pespace {
 namespace host {
 int prof_begin(EvPair& ev, cudaStream_t st) {
   ev = EvPair();
-  if (!g_profile) return PESPACE_OK;
+  if (!g_profile.load(std::memory_order_relaxed)) return PESPACE_OK;
+  {
+    std::lock_guard<std::mutex> lk(g_ev_mutex);
+    if (g_events.size() >= kMaxEvents) return PESPACE_OK;
+  }
   CU(cudaEventCreate(&ev.a));
   CU(cudaEventCreate(&ev.b));
   CU(cudaEventRecord(ev.a, st));
@@ -91,7 +96,7 @@ const char* pespace_strerror(int code) {
 int64_t pespace_launch_count(void) { return (int64_t)g_launches.load(); }
 
 int pespace_profile_enable(int on) {
-  g_profile = on != 0;
+  g_profile.store(on != 0);
   return PESPACE_OK;
 }
 

@@ -2,6 +2,7 @@
 // (argument checks, detector constants, launch bookkeeping).  Not part of the public ABI.
 #pragma once
 #include "../../include/pespace.h"
+#include "../../include/pespace_bench.h"
 #include "pespace_device.cuh"
 
 #include <atomic>

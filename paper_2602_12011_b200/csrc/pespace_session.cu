@@ -21,8 +21,9 @@ struct pespace_session {
   bool bins_ready = false;          // the per-bin table in d_ws matches the current data set and PSD
   cudaStream_t st = nullptr;
   double *d_params = nullptr, *d_data = nullptr, *d_psd = nullptr, *d_lnL = nullptr, *d_F = nullptr, *d_grad = nullptr;
-  void *d_ws = nullptr, *d_ws_f = nullptr, *d_ws_t = nullptr;
-  size_t ws_bytes = 0, ws_f_bytes = 0, ws_t_bytes = 0;
+  void *d_ws = nullptr, *d_ws_f = nullptr, *d_ws_t = nullptr, *d_ws_g = nullptr;
+  size_t ws_bytes = 0, ws_f_bytes = 0, ws_t_bytes = 0, ws_g_bytes = 0;
+  double* d_grad_g = nullptr;       // [max_B][11], pespace_session_loglike_grad (allocated on first use)
   // zero-copy result path of pespace_session_loglike: combine_kernel writes lnL straight into mapped pinned host
   // memory (no device-to-host copy call; theta of small batches goes the same way in the other direction)
   double *h_lnL_pin = nullptr, *d_lnL_map = nullptr, *h_par_pin = nullptr, *d_par_map = nullptr;
@@ -36,7 +37,7 @@ namespace {
 void release(pespace_session* s) {
   if (!s) return;
   cudaFree(s->d_params); cudaFree(s->d_data); cudaFree(s->d_psd); cudaFree(s->d_lnL); cudaFree(s->d_F);
-  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab);
+  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab); cudaFree(s->d_ws_g); cudaFree(s->d_grad_g);
   if (s->h_lnL_pin) cudaFreeHost(s->h_lnL_pin);
   if (s->h_par_pin) cudaFreeHost(s->h_par_pin);
   if (s->st) cudaStreamDestroy(s->st);
@@ -153,6 +154,30 @@ int pespace_session_fisher(pespace_session* s, const double* h_params, int64_t B
   if (h_out_F) CU(cudaMemcpyAsync(h_out_F, s->d_F, (size_t)B * NPAR * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
   if (h_out_grad) CU(cudaMemcpyAsync(h_out_grad, s->d_grad, (size_t)B * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
   CU(cudaStreamSynchronize(s->st));
+  return PESPACE_OK;
+}
+
+int pespace_session_loglike_grad(pespace_session* s, const double* h_params, int64_t B, double* h_out_lnL,
+                                 double* h_out_grad) {
+  if (!s || !h_params || (!h_out_lnL && !h_out_grad) || B <= 0 || B > s->max_B || !s->have_data || !s->have_psd)
+    return PESPACE_EINVAL;
+  if (!s->d_ws_g) {
+    s->ws_g_bytes = pespace_workspace_bytes_grad(s->max_B, &s->grid, &s->model);
+    if (cudaMalloc(&s->d_ws_g, s->ws_g_bytes) != cudaSuccess ||
+        cudaMalloc((void**)&s->d_grad_g, (size_t)s->max_B * NPAR * 8) != cudaSuccess) {
+      cudaGetLastError();
+      cudaFree(s->d_ws_g); s->d_ws_g = nullptr;
+      return PESPACE_ENOMEM;
+    }
+  }
+  CU(cudaMemcpyAsync(s->d_params, h_params, (size_t)B * NPAR * 8, cudaMemcpyHostToDevice, s->st));
+  const int rc = pespace_loglike_grad(s->d_params, B, s->d_data, s->d_psd, &s->grid, &s->model,
+                                      h_out_lnL ? s->d_lnL_map : nullptr, h_out_grad ? s->d_grad_g : nullptr, s->d_ws_g,
+                                      s->ws_g_bytes, s->st);
+  if (rc != PESPACE_OK) return rc;
+  if (h_out_grad) CU(cudaMemcpyAsync(h_out_grad, s->d_grad_g, (size_t)B * NPAR * 8, cudaMemcpyDeviceToHost, s->st));
+  CU(cudaStreamSynchronize(s->st));
+  if (h_out_lnL) std::memcpy(h_out_lnL, s->h_lnL_pin, (size_t)B * 8);
   return PESPACE_OK;
 }
 

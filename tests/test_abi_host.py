@@ -2,6 +2,7 @@
 include/pespace.h declares; argument validation returns the documented codes before any CUDA
 call; the workload recipes are reproducible."""
 import ctypes as C
+import glob
 import os
 import re
 
@@ -20,9 +21,11 @@ def lib():
 
 
 def declared_symbols():
-    text = open(os.path.join(ROOT, "include", "pespace.h")).read()
-    text = re.sub(r"/\*.*?\*/", "", text, flags=re.S)
-    return sorted(set(re.findall(r"\b(pespace_[a-z0-9_]+)\s*\(", text)))
+    names = set()
+    for hdr in sorted(glob.glob(os.path.join(ROOT, "include", "*.h"))):
+        text = re.sub(r"/\*.*?\*/", "", open(hdr).read(), flags=re.S)
+        names |= set(re.findall(r"\b(pespace_[a-z0-9_]+)\s*\(", text))
+    return sorted(names)
 
 
 def test_library_exports_every_declared_symbol(lib):
@@ -142,8 +145,32 @@ def test_tab_argument_validation_without_a_device():
 def test_header_is_plain_c():
     """include/pespace.h is a C ABI: it must compile as C99 and as C++ with no other header of this repository."""
     import subprocess
-    hdr = os.path.join(ROOT, "include", "pespace.h")
-    for cmd in (["gcc", "-x", "c", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", hdr],
-                ["g++", "-x", "c++", "-Wall", "-Werror", "-fsyntax-only", hdr]):
-        res = subprocess.run(cmd, capture_output=True, text=True)
-        assert res.returncode == 0, res.stderr
+    for hdr in sorted(glob.glob(os.path.join(ROOT, "include", "*.h"))):
+        for cmd in (["gcc", "-x", "c", "-std=c99", "-Wall", "-Werror", "-fsyntax-only", hdr],
+                    ["g++", "-x", "c++", "-Wall", "-Werror", "-fsyntax-only", hdr]):
+            res = subprocess.run(cmd, capture_output=True, text=True)
+            assert res.returncode == 0, res.stderr
+
+
+def test_product_header_holds_no_bench_scaffolding():
+    """pespace.h is the boundary; the micro-benchmark, the kernel timer and the launch counter live in
+    pespace_bench.h."""
+    text = open(os.path.join(ROOT, "include", "pespace.h")).read()
+    for name in ("pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read", "pespace_launch_count"):
+        assert name not in text
+
+
+def test_grad_argument_validation_without_a_device():
+    from paper_2602_12011_b200 import binding as P
+    L = P.lib()
+    wl = W.config(3, B=4, N=64)
+    m, keep = P._model(wl.model)
+    g = P._grid(wl.grid)
+    fake = 0x1000
+    assert L.pespace_workspace_bytes_grad(0, C.byref(g), C.byref(m)) == 0
+    need = L.pespace_workspace_bytes_grad(4, C.byref(g), C.byref(m))
+    assert need > L.pespace_workspace_bytes(4, C.byref(g), C.byref(m), 0)
+    assert L.pespace_loglike_grad(fake, 4, fake, fake, C.byref(g), C.byref(m), None, None, fake, need, None) == -1
+    assert L.pespace_loglike_grad(fake, 4, fake, fake, C.byref(g), C.byref(m), fake, fake, fake, need - 1, None) == -1
+    assert L.pespace_loglike_grad(fake, 4, None, fake, C.byref(g), C.byref(m), fake, fake, fake, need, None) == -1
+    assert L.pespace_session_loglike_grad(None, None, 4, None, None) == -1

@@ -92,6 +92,12 @@ def test_grad_matches_forward_mode_and_is_deterministic(P):
     assert (np.abs(g1.cpu().numpy() - gf.cpu().numpy()) / (d * np.sqrt(rr)[:, None])).max() <= TOL
     plain = P.loglike(dev(wl.params), dev(data), dev(psd), wl.grid, wl.model).cpu().numpy()
     assert np.allclose(l1.cpu().numpy(), plain, rtol=1e-12, atol=0)
+    # host-buffer session: same kernels, bit-identical
+    ses = P.Session(wl.grid, wl.model, wl.B)
+    ses.set_data(data, psd)
+    ls, gs = ses.loglike_grad(wl.params)
+    assert np.array_equal(ls, l1.cpu().numpy()) and np.array_equal(gs, g1.cpu().numpy())
+    ses.close()
 
 
 def test_grad_edge_cases(P):
