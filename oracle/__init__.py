@@ -54,6 +54,11 @@ def lib():
         L.pespace_oracle_loglike_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, dp, C.POINTER(_Grid),
                                                  C.POINTER(_Model), dp]
         L.pespace_oracle_tab_waveform.argtypes = [i64, dp, dp, dp, dp, dp, i64, dp, dp, dp]
+        dbl = C.c_double
+        L.pespace_oracle_response_orb.argtypes = [dp, i64, i64, dbl, dbl, dp, dp, dp, i64, C.POINTER(_Model), dp]
+        L.pespace_oracle_loglike_orb.argtypes = [dp, i64, i64, dbl, dbl, dp, dp, dp, dp, C.POINTER(_Grid),
+                                                 C.POINTER(_Model), dp]
+        L.pespace_oracle_orbit_tab.argtypes = [i64, dbl, dbl, dp, dp, dbl, dp]
         L.pespace_oracle_set_threads.argtypes = [C.c_int]
         L.pespace_oracle_set_threads.restype = None
         _lib = L
@@ -178,6 +183,52 @@ def tab_waveform(fnodes, amp, phase, tf, freqs):
     _check(lib().pespace_oracle_tab_waveform(fn.shape[0], _dp(fn), _dp(a), _dp(ph), _dp(t), _dp(f), f.shape[0], _dp(oa),
                                              _dp(op), _dp(ot)), "tab_waveform")
     return oa, op, ot
+
+
+def _orbit(orbit, nd):
+    """orbit = (t0, dt, pos [n_det][K][3][3], vel [n_det][K][3][3]) -> (t0, dt, pos, vel, K)"""
+    t0, dt, pos, vel = orbit
+    pos, vel = _f64(pos), _f64(vel)
+    if pos.ndim != 4 or pos.shape[0] != nd or pos.shape[2:] != (3, 3) or vel.shape != pos.shape:
+        raise ValueError(f"orbit tables must be [n_det={nd}][K][3][3], got {pos.shape} and {vel.shape}")
+    return float(t0), float(dt), pos, vel, pos.shape[1]
+
+
+def response_orb(params, orbit, freqs, model) -> np.ndarray:
+    """T2: response with tabulated orbits; complex128 [B][n_det][3][N]"""
+    p, f = _f64(np.atleast_2d(params)), _f64(freqs)
+    m, keep = _model(model)
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    t0, dt, pos, vel, K = _orbit(orbit, nd)
+    out = np.empty((B, nd, 3, N, 2), dtype=np.float64)
+    _check(lib().pespace_oracle_response_orb(_dp(p), B, K, t0, dt, _dp(pos), _dp(vel), _dp(f), N, C.byref(m), _dp(out)),
+           "response_orb")
+    return out.view(np.complex128)[..., 0]
+
+
+def loglike_orb(params, orbit, data, psd, grid, model) -> np.ndarray:
+    """T2: lnL [B] with tabulated orbits"""
+    p = _f64(np.atleast_2d(params))
+    d = np.ascontiguousarray(data, dtype=np.complex128).view(np.float64)
+    s = _f64(psd)
+    m, keep = _model(model)
+    g = _Grid(float(grid.f0), float(grid.df), int(grid.N))
+    t0, dt, pos, vel, K = _orbit(orbit, len(model.detectors))
+    out = np.empty(p.shape[0], dtype=np.float64)
+    _check(lib().pespace_oracle_loglike_orb(_dp(p), p.shape[0], K, t0, dt, _dp(pos), _dp(vel), _dp(d), _dp(s),
+                                            C.byref(g), C.byref(m), _dp(out)), "loglike_orb")
+    return out
+
+
+def orbit_tab(t0, dt, pos, vel, t):
+    """T2: interpolated positions [3][3] of one detector's table (pos, vel [K][3][3]) at t; None outside the table"""
+    pos, vel = _f64(pos), _f64(vel)
+    out = np.empty((3, 3), dtype=np.float64)
+    rc = lib().pespace_oracle_orbit_tab(pos.shape[0], float(t0), float(dt), _dp(pos), _dp(vel), float(t), _dp(out))
+    if rc == 1:
+        return None
+    _check(rc, "orbit_tab")
+    return out
 
 
 def waveform(theta, l, m, freqs):

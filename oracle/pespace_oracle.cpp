@@ -16,6 +16,10 @@
 // with slopes 2 pi t_j, its derivative, 4-node Lagrange); pinned by the T1 tests (exactness on cubics, reproduction
 // of the analytic path at fourth order, extrinsic scalings, band limits, brute-force Whittle sum).
 //
+// Tabulated orbits (T2 block, reading T2 of DESIGN.md): cubic Hermite in time on the caller's
+// position / velocity tables; pinned by the T2 tests (exact on cubic trajectories, reproduces the analytic orbit and
+// its response when fed dense samples of it, rigid arms between nodes, zero outside the table).
+//
 // Pins (tests/test_oracle_pins.py): P1-P16 of SURVEY.md 8(c).  "Parity
 // unpinned": absolute values of the Taiji-/TianQin-like results (G8, G13 are
 // proposals, not in the paper) and the spin terms of G3 beyond "vanish at
@@ -311,6 +315,43 @@ template <class T> void orbit(const pespace_oracle_detector& D, const T& t, V3<T
   }
 }
 
+// ---------------------------------------------------------------- T2: tabulated numerical orbits
+// "Support for high-precision numerical orbits will be extended in future work".  Reading T2 of
+// the spacecraft positions arrive as tables on a uniform time grid t_j = t0 + j dt, j = 0..K-1 (SSB time,
+// same origin as t_c): pos [K][3 spacecraft][3] in metres and vel [K][3][3] in m/s.  Between nodes every coordinate
+// is the cubic Hermite interpolant with the node velocities as slopes,
+//   x(t) = h00(u) x_j + h10(u) dt v_j + h01(u) x_{j+1} + h11(u) dt v_{j+1},  u = (t - t_j) / dt,
+//   h00 = 2u^3 - 3u^2 + 1, h10 = u^3 - 2u^2 + u, h01 = -2u^3 + 3u^2, h11 = u^3 - u^2.
+// Eq. 5 / Eq. 6 keep the constant nominal arm length L of the detector description (the paper's formalism is the
+// rigid equal-arm one): n_rs = (x_r - x_s) / L and k.(x_r + x_s) are taken from the table.  A mode
+// whose t_lm(f) falls outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.
+struct OrbitTab { int64_t K; double t0, dt; const double *pos, *vel; };
+
+template <class T> bool orbit_tab(const OrbitTab& O, const T& t, V3<T>* centre, V3<T> off[3]) {
+  const double tv = o_val(t);
+  const double t_end = O.t0 + (double)(O.K - 1) * O.dt;
+  if (!(tv >= O.t0) || !(tv <= t_end)) return false;
+  int64_t j = (int64_t)std::floor((tv - O.t0) / O.dt);
+  if (j < 0) j = 0;
+  if (j > O.K - 2) j = O.K - 2;
+  const T u = (t - T(O.t0 + (double)j * O.dt)) / T(O.dt);
+  const T u2 = u * u, u3 = u2 * u;
+  const T h00 = T(2.0) * u3 - T(3.0) * u2 + T(1.0), h10 = u3 - T(2.0) * u2 + u;
+  const T h01 = T(3.0) * u2 - T(2.0) * u3, h11 = u3 - u2;
+  const double *p0 = O.pos + (size_t)j * 9, *p1 = p0 + 9, *v0 = O.vel + (size_t)j * 9, *v1 = v0 + 9;
+  centre->x = T(0.0); centre->y = T(0.0); centre->z = T(0.0);
+  for (int n = 0; n < 3; ++n) {
+    T c[3];
+    for (int a = 0; a < 3; ++a)
+      c[a] = h00 * T(p0[3 * n + a]) + h10 * T(O.dt * v0[3 * n + a]) + h01 * T(p1[3 * n + a]) + h11 * T(O.dt * v1[3 * n + a]);
+    off[n].x = c[0]; off[n].y = c[1]; off[n].z = c[2];
+  }
+  return true;
+}
+bool orbit_tab_ok(const OrbitTab& O) {
+  return O.K >= 2 && O.pos && O.vel && O.dt > 0.0 && std::isfinite(O.dt) && std::isfinite(O.t0);
+}
+
 // ---------------------------------------------------------------- O9: single link, Eq. 5
 template <class T> T sinc(const T& x) {
   const double ax = std::fabs(o_val(x));
@@ -363,33 +404,41 @@ template <class T> void aet(const Cx<T> XYZ[3], Cx<T> AET[3]) {
 // six links of one mode at one frequency for one detector
 // six links of one mode from its amplitude, phase and time-frequency map at f
 template <class T> void links_from_waveform(const T& iota, const Frame<T>& F, int l, int m, double f, const T& amp,
-                                            const T& psi, const T& tf, const pespace_oracle_detector& D, Cx<T> y[6]) {
+                                            const T& psi, const T& tf, const pespace_oracle_detector& D, Cx<T> y[6],
+                                            const OrbitTab* ot = nullptr) {
   const Cx<T> hlm = scale(expi(-psi), amp);                                // h_lm = A e^{-i Psi}
   Cx<T> Kp, Kc;
   mode_polarisation(l, m, iota, &Kp, &Kc);
   V3<T> centre, off[3];
-  orbit(D, tf, &centre, off);                                              // geometry at t = t_lm(f)
+  if (ot) {                                                                // T2: positions from the orbit table
+    if (!orbit_tab(*ot, tf, &centre, off)) {
+      for (int i = 0; i < 6; ++i) y[i] = cx<T>(T(0.0), T(0.0));
+      return;
+    }
+  } else {
+    orbit(D, tf, &centre, off);                                            // geometry at t = t_lm(f)
+  }
   const int R[6] = {0, 1, 0, 2, 1, 2}, S[6] = {1, 0, 2, 0, 2, 1};
   for (int i = 0; i < 6; ++i) y[i] = single_link(T(f), D.L_m, F, centre, off, R[i], S[i], Kp, Kc, hlm);
 }
 
 template <class T> bool mode_links(const Source<T>& s, const Frame<T>& F, int l, int m, double f,
-                                   const pespace_oracle_detector& D, Cx<T> y[6]) {
+                                   const pespace_oracle_detector& D, Cx<T> y[6], const OrbitTab* ot = nullptr) {
   T amp, psi, tf;
   if (!mode_waveform(s, l, m, f, &amp, &psi, &tf)) return false;
-  links_from_waveform(s.iota, F, l, m, f, amp, psi, tf, D, y);
+  links_from_waveform(s.iota, F, l, m, f, amp, psi, tf, D, y, ot);
   return true;
 }
 
 // A,E,T of one detector at one frequency, summed over the modes of the mask
 template <class T> void response_bin(const Source<T>& s, const Frame<T>& F, double f, uint32_t mode_mask,
-                                     const pespace_oracle_detector& D, Cx<T> AET[3]) {
+                                     const pespace_oracle_detector& D, Cx<T> AET[3], const OrbitTab* ot = nullptr) {
   Cx<T> sum[3];
   for (int c = 0; c < 3; ++c) sum[c] = cx<T>(T(0.0), T(0.0));
   for (int im = 0; im < 5; ++im) {
     if (!(mode_mask & (1u << im))) continue;
     Cx<T> y[6], XYZ[3], ch[3];
-    mode_links(s, F, MODE_TABLE[im].l, MODE_TABLE[im].m, f, D, y);
+    mode_links(s, F, MODE_TABLE[im].l, MODE_TABLE[im].m, f, D, y, ot);
     tdi_xyz(y, T(f), D.L_m, D.tdi_gen, XYZ);
     aet(XYZ, ch);
     for (int c = 0; c < 3; ++c) sum[c] = sum[c] + ch[c];
@@ -421,7 +470,7 @@ int g_threads = 0;
 
 template <class T>
 int response_impl(const double* params, int64_t B, const double* freqs, int64_t N,
-                  const pespace_oracle_model* model, double* out) {
+                  const pespace_oracle_model* model, double* out, const OrbitTab* tabs = nullptr) {
   if (!params || !freqs || !out || B <= 0 || N <= 0 || !model_ok(model)) return -1;
   const int nd = model->n_det;
   const double nan = std::numeric_limits<double>::quiet_NaN();
@@ -439,7 +488,7 @@ int response_impl(const double* params, int64_t B, const double* freqs, int64_t 
     for (int d = 0; d < nd; ++d)
       for (int64_t k = 0; k < N; ++k) {
         Cx<T> ch[3];
-        if (freqs[k] > 0.0) response_bin(s, F, freqs[k], model->mode_mask, model->det[d], ch);
+        if (freqs[k] > 0.0) response_bin(s, F, freqs[k], model->mode_mask, model->det[d], ch, tabs ? tabs + d : nullptr);
         else for (int c = 0; c < 3; ++c) ch[c] = cx<T>(T(0.0), T(0.0));
         for (int c = 0; c < 3; ++c) {
           ob[(((size_t)d * 3 + c) * N + k) * 2 + 0] = o_val(ch[c].re);
@@ -639,9 +688,9 @@ int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* a
 }
 
 // O11: lnL = -1/2 sum_det sum_c 4 df sum_k |d - h|^2 / S   (Eq. 10, 11, 14 with T = 1/df)
-int pespace_oracle_loglike(const double* params, int64_t B, const double* data, const double* psd,
-                           const pespace_oracle_grid* grid, const pespace_oracle_model* model,
-                           double* out_lnL) {
+static int loglike_impl(const double* params, int64_t B, const double* data, const double* psd,
+                        const pespace_oracle_grid* grid, const pespace_oracle_model* model, double* out_lnL,
+                        const OrbitTab* tabs) {
   if (!params || !data || !psd || !out_lnL || B <= 0 || !grid_ok(grid) || !model_ok(model)) return -1;
   const int nd = model->n_det;
   const int64_t N = grid->N;
@@ -656,7 +705,7 @@ int pespace_oracle_loglike(const double* params, int64_t B, const double* data, 
       for (int64_t k = 0; k < N; ++k) {
         const double f = std::fma((double)k, grid->df, grid->f0);          // G11
         Cx<double> h[3];
-        response_bin(s, F, f, model->mode_mask, model->det[d], h);
+        response_bin(s, F, f, model->mode_mask, model->det[d], h, tabs ? tabs + d : nullptr);
         for (int c = 0; c < 3; ++c) {
           const size_t idx = ((size_t)d * 3 + c) * N + k;
           const double S = psd[idx];
@@ -667,6 +716,47 @@ int pespace_oracle_loglike(const double* params, int64_t B, const double* data, 
       }
     out_lnL[b] = (double)(-0.5L * 4.0L * (long double)grid->df * sum);
   }
+  return 0;
+}
+int pespace_oracle_loglike(const double* params, int64_t B, const double* data, const double* psd,
+                           const pespace_oracle_grid* grid, const pespace_oracle_model* model,
+                           double* out_lnL) {
+  return loglike_impl(params, B, data, psd, grid, model, out_lnL, nullptr);
+}
+
+// T2: response and likelihood with tabulated orbits; pos, vel [n_det][K][3][3]
+static bool make_orbit_tabs(const pespace_oracle_model* model, int64_t K, double t0, double dt, const double* pos,
+                            const double* vel, std::vector<OrbitTab>* out) {
+  if (!model_ok(model)) return false;
+  for (int d = 0; d < model->n_det; ++d) {
+    const OrbitTab O = {K, t0, dt, pos ? pos + (size_t)d * K * 9 : nullptr, vel ? vel + (size_t)d * K * 9 : nullptr};
+    if (!orbit_tab_ok(O)) return false;
+    out->push_back(O);
+  }
+  return true;
+}
+int pespace_oracle_response_orb(const double* params, int64_t B, int64_t K, double t0, double dt, const double* pos,
+                                const double* vel, const double* freqs, int64_t N, const pespace_oracle_model* model,
+                                double* out_AET) {
+  std::vector<OrbitTab> tabs;
+  if (!make_orbit_tabs(model, K, t0, dt, pos, vel, &tabs)) return -1;
+  return response_impl<double>(params, B, freqs, N, model, out_AET, tabs.data());
+}
+int pespace_oracle_loglike_orb(const double* params, int64_t B, int64_t K, double t0, double dt, const double* pos,
+                               const double* vel, const double* data, const double* psd,
+                               const pespace_oracle_grid* grid, const pespace_oracle_model* model, double* out_lnL) {
+  std::vector<OrbitTab> tabs;
+  if (!make_orbit_tabs(model, K, t0, dt, pos, vel, &tabs)) return -1;
+  return loglike_impl(params, B, data, psd, grid, model, out_lnL, tabs.data());
+}
+/* the interpolated positions [3][3] (metres) of ONE detector's table at time t; returns 1 outside the table */
+int pespace_oracle_orbit_tab(int64_t K, double t0, double dt, const double* pos, const double* vel, double t,
+                             double* out_xyz) {
+  const OrbitTab O = {K, t0, dt, pos, vel};
+  if (!orbit_tab_ok(O) || !out_xyz) return -1;
+  V3<double> c, off[3];
+  if (!orbit_tab<double>(O, t, &c, off)) return 1;
+  for (int n = 0; n < 3; ++n) { out_xyz[3 * n] = off[n].x; out_xyz[3 * n + 1] = off[n].y; out_xyz[3 * n + 2] = off[n].z; }
   return 0;
 }
 

@@ -79,6 +79,20 @@ int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* a
                                 const double* tf, const double* freqs, int64_t N, double* out_amp,
                                 double* out_psi, double* out_tf);
 
+/* ---- T2: tabulated numerical orbits.  Positions pos [n_det][K][3 spacecraft][3]
+ * (metres) and velocities vel [n_det][K][3][3] (m/s) on the uniform time grid t0 + j dt (SSB seconds, origin of t_c);
+ * cubic Hermite in time; Eq. 5 / 6 keep the nominal L of the detector description; a mode whose t_lm(f) lies outside
+ * the table contributes 0.  The detector's kind / kappa / lambda0 / period / pointing are ignored. */
+int pespace_oracle_response_orb(const double* params, int64_t B, int64_t K, double t0, double dt, const double* pos,
+                                const double* vel, const double* freqs, int64_t N, const pespace_oracle_model* model,
+                                double* out_AET);
+int pespace_oracle_loglike_orb(const double* params, int64_t B, int64_t K, double t0, double dt, const double* pos,
+                               const double* vel, const double* data_AET, const double* psd,
+                               const pespace_oracle_grid* grid, const pespace_oracle_model* model, double* out_lnL);
+/* interpolated positions [3][3] of ONE detector's table (pos, vel [K][3][3]) at time t; returns 1 outside the table */
+int pespace_oracle_orbit_tab(int64_t K, double t0, double dt, const double* pos, const double* vel, double t,
+                             double* out_xyz);
+
 /* ---- pieces, exported so that the pins can check them one at a time ---- */
 
 /* per-mode amplitude A_lm(f) [s], phase Psi_lm(f) [rad], t_lm(f) [s]   (O2-O5) */

@@ -297,3 +297,70 @@ def chirp_table(params: np.ndarray, mode_mask: int, fnodes: np.ndarray):
             tf[b, i] = dpsi_dfp / (2.0 * np.pi)                                 # (m/2) (2/m) d/df' = d/df
             amp[b, i] = a0 * fp ** (-7.0 / 6.0) / m
     return fnodes, amp, phase, tf
+
+
+# ---------------------------------------------------------------- tabulated numerical orbits
+# Input recipes for the *_orb entry points: (t0, dt, pos [n_det][K][3][3] m, vel [n_det][K][3][3] m/s) on a uniform
+# time grid.  `orbit_table_from_fn` samples whatever position function the caller passes in (the oracle's analytic
+# orbit in the tests) and differentiates it numerically; `synthetic_orbit_table` is a seeded toy ephemeris shaped like
+# a numerical orbit product (a cartwheeling triangle on a one-year circle plus small smooth perturbations), used where
+# no orbit code may be called (bench.py).  Neither evaluates anything the method computes.
+def orbit_table_from_fn(dets, t0: float, dt: float, K: int, orbit_fn: Callable[[Detector, float], np.ndarray],
+                        h: float = 64.0):
+    """orbit_fn(det, t) -> positions [3][3] in metres.  Velocities: five-point central differences with step h."""
+    t = t0 + dt * np.arange(K)
+    pos = np.empty((len(dets), K, 3, 3))
+    vel = np.empty_like(pos)
+    for d, det in enumerate(dets):
+        for j, tj in enumerate(t):
+            pos[d, j] = orbit_fn(det, tj)
+            vel[d, j] = (-orbit_fn(det, tj + 2 * h) + 8.0 * orbit_fn(det, tj + h) - 8.0 * orbit_fn(det, tj - h)
+                         + orbit_fn(det, tj - 2 * h)) / (12.0 * h)
+    return float(t0), float(dt), pos, vel
+
+
+def synthetic_orbit_table(dets, t0: float, dt: float, K: int, seed: int = 0, rel_pert: float = 2e-3):
+    """Seeded toy ephemeris: per detector an equilateral triangle of side L_m whose centre moves on a circle of 1 au
+    (one turn per 31558150 s, phase kappa; kind 1: on Earth's circle) and which turns in its own plane (heliocentric:
+    once per orbit in a plane tilted by 60 degrees; geocentric: once per period_s in the plane normal to (lon, lat)),
+    plus smooth perturbations of relative size rel_pert of the arm length (three harmonics per coordinate, seeded)
+    standing in for the arm breathing of real numerical orbits.  Velocities are the exact time derivatives."""
+    AU, YR = 149597870700.0, 31558149.763545603
+    rng = np.random.default_rng(seed)
+    t = t0 + dt * np.arange(K)
+    pos = np.empty((len(dets), K, 3, 3))
+    vel = np.empty_like(pos)
+    for d, det in enumerate(dets):
+        w0 = 2.0 * np.pi / YR
+        a = w0 * t + (det.kappa if det.kind == 0 else 0.0)
+        cen = AU * np.stack([np.cos(a), np.sin(a), np.zeros_like(a)], axis=-1)
+        dcen = AU * w0 * np.stack([-np.sin(a), np.cos(a), np.zeros_like(a)], axis=-1)
+        r = det.L_m / np.sqrt(3.0)
+        if det.kind == 0:
+            wr = w0
+            e1 = np.stack([np.cos(a) * 0.5, np.sin(a) * 0.5, -np.sqrt(0.75) * np.ones_like(a)], axis=-1)   # tilted radial
+            e2 = np.stack([-np.sin(a), np.cos(a), np.zeros_like(a)], axis=-1)
+            de1 = w0 * np.stack([-np.sin(a) * 0.5, np.cos(a) * 0.5, np.zeros_like(a)], axis=-1)
+            de2 = w0 * np.stack([-np.cos(a), -np.sin(a), np.zeros_like(a)], axis=-1)
+        else:
+            wr = 2.0 * np.pi / det.period_s
+            n = np.array([np.cos(det.lat) * np.cos(det.lon), np.cos(det.lat) * np.sin(det.lon), np.sin(det.lat)])
+            b1 = np.array([-np.sin(det.lon), np.cos(det.lon), 0.0])
+            b2 = np.cross(n, b1)
+            e1, e2 = np.tile(b1, (K, 1)), np.tile(b2, (K, 1))
+            de1 = de2 = np.zeros((K, 3))
+        for sc in range(3):
+            ph = -wr * t + 2.0 * np.pi * sc / 3.0 + det.lambda0 if det.kind == 0 else wr * t + 2.0 * np.pi * sc / 3.0 + det.lambda0
+            dph = -wr if det.kind == 0 else wr
+            c, s_ = np.cos(ph)[:, None], np.sin(ph)[:, None]
+            x = cen + r * (c * e1 + s_ * e2)
+            v = dcen + r * (c * de1 + s_ * de2) + r * dph * (-s_ * e1 + c * e2)
+            for ax in range(3):
+                for _ in range(3):
+                    amp = rel_pert * det.L_m * rng.uniform(-1.0, 1.0)
+                    om = 2.0 * np.pi / (YR / rng.integers(1, 6))
+                    p0 = rng.uniform(0.0, 2.0 * np.pi)
+                    x[:, ax] += amp * np.sin(om * t + p0)
+                    v[:, ax] += amp * om * np.cos(om * t + p0)
+            pos[d, :, sc], vel[d, :, sc] = x, v
+    return float(t0), float(dt), pos, vel

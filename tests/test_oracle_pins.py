@@ -776,3 +776,70 @@ def test_T1_extrinsic_parameters_band_limits_and_likelihood():
     assert lnL[0] == 0.0 and lnL[1] < 0.0 and lnL[2] < 0.0
     brute = -0.5 * 4.0 * grid.df * np.sum(np.abs(r[0] - r[1]) ** 2 / psd)
     assert abs(lnL[1] - brute) <= 1e-12 * abs(brute)
+
+
+# ------------------------------------------------------------------ T2: tabulated numerical orbits
+def test_T2_hermite_is_exact_on_cubic_trajectories_and_empty_outside():
+    rng = np.random.default_rng(8)
+    t0, dt, K = -1000.0, 3600.0, 9
+    t = t0 + dt * np.arange(K)
+    co = rng.normal(size=(4, 3, 3)) * np.array([1e11, 1e4, 1e-3, 1e-10])[:, None, None]     # x = a + b t + c t^2 + d t^3
+    pos = sum(co[i] * t[:, None, None] ** i for i in range(4))
+    vel = sum(i * co[i] * t[:, None, None] ** (i - 1) for i in range(1, 4))
+    for tt in (t0, t0 + 0.37 * dt, t0 + 4.5 * dt, t0 + 7.999 * dt, t[-1]):
+        want = sum(co[i] * tt ** i for i in range(4))
+        got = oracle.orbit_tab(t0, dt, pos, vel, tt)
+        assert np.allclose(got, want, rtol=1e-13, atol=1e-3)
+    assert oracle.orbit_tab(t0, dt, pos, vel, t0 - 1.0) is None and oracle.orbit_tab(t0, dt, pos, vel, t[-1] + 1.0) is None
+    # the nodes themselves are reproduced exactly
+    assert np.array_equal(oracle.orbit_tab(t0, dt, pos, vel, t[3]), pos[3])
+
+
+@pytest.mark.parametrize("det,dt", [(LISA, 3600.0), (TAIJI, 3600.0), (TQ, 300.0)])
+def test_T2_dense_table_reproduces_the_analytic_orbit_and_rigid_arms(det, dt):
+    t0, K = 1.0e6, 200
+    tab = W.orbit_table_from_fn([det], t0, dt, K, oracle.orbit)
+    rng = np.random.default_rng(2)
+    for tt in t0 + dt * (K - 1) * rng.uniform(0.0, 1.0, 25):
+        x = oracle.orbit_tab(tab[0], tab[1], tab[2][0], tab[3][0], tt)
+        assert np.allclose(x, oracle.orbit(det, tt), rtol=0, atol=2e-3)                   # metres, at 1.5e11 m
+        for r, s_ in ((0, 1), (0, 2), (1, 2)):
+            assert np.linalg.norm(x[r] - x[s_]) / det.L_m == pytest.approx(1.0, abs=1e-9)   # P3 on the interpolant
+
+
+def test_T2_response_and_likelihood_with_dense_tables_match_the_analytic_path():
+    """fed dense samples of the analytic orbits, the tabulated-orbit path reproduces O8-O11; a table that starts late
+    leaves the low frequencies (early t_lm) empty; the Whittle sum is the brute-force one"""
+    th = np.array([THETA, THETA * (1 + 0.01 * np.array([1, -1, 0, 0, 2, 1, -1, 1, 1, -1, 0.5]))])
+    dets = (LISA, TAIJI, TQ)
+    model = W.Model(W.MODES_HM, dets)
+    f = np.geomspace(2e-4, 9e-2, 60)
+    tl = np.array([oracle.waveform(t_, l, m, f)[2] for t_ in th for (l, m) in MODES])     # every t_lm(f) of the test
+    t_lo, t_hi = tl.min() - 10.0, tl.max() + 10.0           # (t_lm is not monotonic beyond v ~ 1, G2)
+    dt = 300.0
+    K = int((t_hi - t_lo) / dt) + 2
+    # one table per detector on the same grid; the short-period detector sets dt
+    tab = W.orbit_table_from_fn(dets, t_lo, dt, K, oracle.orbit)
+    got = oracle.response_orb(th, tab, f, model)
+    want = oracle.response(th, f, model)
+    for d in range(3):
+        assert np.abs(got[:, d] - want[:, d]).max() <= 1e-9 * np.abs(want[:, d]).max()
+    # late table: modes whose t_lm(f) precedes the first node vanish
+    _, _, t22 = oracle.waveform(th[0], 2, 2, f)
+    cut = 12                                     # still on the monotonic branch of t_22(f)
+    t_start = 0.5 * (t22[cut - 1] + t22[cut])
+    K2 = int((t_hi - t_start) / dt) + 2
+    late = W.orbit_table_from_fn(dets[:1], t_start, dt, K2, oracle.orbit)
+    m22 = W.Model(W.MODES_22_ONLY, dets[:1])
+    r = oracle.response_orb(th[:1], late, f, m22)[0, 0]
+    assert np.all(np.diff(t22[:cut + 8]) > 0)
+    assert np.all(r[:, :cut] == 0) and np.all(np.abs(r[0, cut:cut + 8]) > 0)
+    # Whittle sum by brute force
+    grid = W.Grid(1e-3, 2e-5, 50)
+    fg = grid.freqs()
+    rng = np.random.default_rng(4)
+    psd = np.stack([W.psd_aet(dd, fg) for dd in dets])
+    data = W.coloured_noise(psd, grid.df, rng) + oracle.response_orb(th[:1], tab, fg, model)[0]
+    h = oracle.response_orb(th, tab, fg, model)
+    brute = -0.5 * 4.0 * grid.df * (np.abs(data[None] - h) ** 2 / psd[None]).sum(axis=(1, 2, 3))
+    assert np.allclose(oracle.loglike_orb(th, tab, data, psd, grid, model), brute, rtol=1e-12, atol=0)
