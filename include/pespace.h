@@ -156,6 +156,29 @@ int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetab
                         const pespace_model* model, double* d_out_lnL, void* d_workspace,
                         size_t workspace_bytes, void* stream);
 
+/* ---- Tabulated numerical orbits ("Support for high-precision numerical orbits will
+ * be extended in future work").  The spacecraft positions at t_lm(f) (Eq. 4, 5) are read from tables instead of the
+ * analytic Keplerian orbits: d_pos [n_det][K][3 spacecraft][3] in metres and d_vel [n_det][K][3][3] in m/s on the
+ * uniform time grid t0 + j dt, j = 0..K-1 (SSB seconds, same origin as t_c), K >= 2.  Between nodes every coordinate
+ * is the cubic Hermite interpolant with the node velocities as slopes.  Eq. 5 / Eq. 6 keep the nominal constant arm
+ * length L_m of the detector description in the delays (the paper's formalism assumes rigid equal arms, PAPER.md:55,
+ * :61); the link directions n_rs = (x_r - x_s) / |x_r - x_s| (unit vectors: the arms of a numerical orbit breathe) and
+ * k.(x_r + x_s) come from the table; kind, kappa, lambda0, period_s, lon, lat of the description are ignored.  A mode whose t_lm(f) lies outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.  Waveform:
+ * the analytic TaylorF2 modes of pespace_loglike.  Workspace of pespace_loglike_orb: pespace_workspace_bytes(B, grid,
+ * model, 0).  Errors and per-sample domain as pespace_loglike. */
+typedef struct {
+  int64_t K;
+  double t0, dt;
+  const double* d_pos;
+  const double* d_vel;
+} pespace_orbittable;
+
+int pespace_response_orb(const double* d_params, int64_t B, const pespace_orbittable* orbit, const double* d_freqs,
+                         int64_t N, const pespace_model* model, double* d_out_AET, void* stream);
+int pespace_loglike_orb(const double* d_params, int64_t B, const pespace_orbittable* orbit, const double* d_data_AET,
+                        const double* d_psd, const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                        void* d_workspace, size_t workspace_bytes, void* stream);
+
 /* ---- Host-buffer entry points (a sampler evaluates many batches of theta against
  * ONE data set).  A session owns a stream and keeps the data set, the PSD, the workspace
  * and the result buffers resident on the device between calls; each call then moves only theta in

@@ -322,9 +322,10 @@ template <class T> void orbit(const pespace_oracle_detector& D, const T& t, V3<T
 // is the cubic Hermite interpolant with the node velocities as slopes,
 //   x(t) = h00(u) x_j + h10(u) dt v_j + h01(u) x_{j+1} + h11(u) dt v_{j+1},  u = (t - t_j) / dt,
 //   h00 = 2u^3 - 3u^2 + 1, h10 = u^3 - 2u^2 + u, h01 = -2u^3 + 3u^2, h11 = u^3 - u^2.
-// Eq. 5 / Eq. 6 keep the constant nominal arm length L of the detector description (the paper's formalism is the
-// rigid equal-arm one): n_rs = (x_r - x_s) / L and k.(x_r + x_s) are taken from the table.  A mode
-// whose t_lm(f) falls outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.
+// The delays keep the constant nominal arm length L of the detector description (the paper's formalism is the rigid
+// equal-arm one); the single link is the transform of Eq. 1 with the positions and the unit link
+// vectors n_rs = (x_r - x_s) / |x_r - x_s| from the table (see single_link), Eq. 6 is unchanged.  A mode whose
+// t_lm(f) falls outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.
 struct OrbitTab { int64_t K; double t0, dt; const double *pos, *vel; };
 
 template <class T> bool orbit_tab(const OrbitTab& O, const T& t, V3<T>* centre, V3<T> off[3]) {
@@ -361,15 +362,33 @@ template <class T> T sinc(const T& x) {
 // y_rs for receiver r, sender s (0-based), one mode.  Times in seconds.
 template <class T> Cx<T> single_link(const T& f, double L_m, const Frame<T>& F, const V3<T>& centre,
                                      const V3<T> off[3], int r, int s, const Cx<T>& Kp, const Cx<T>& Kc,
-                                     const Cx<T>& hlm) {
+                                     const Cx<T>& hlm, bool unit_arms = false) {
   const T pi = K<T>::pi();
   const T Lbar = T(L_m) / T(C_SI);
-  const V3<T> n = smul(off[r] - off[s], T(1.0) / T(L_m));                  // n_rs = (x_r - x_s)/L
+  const V3<T> dx = off[r] - off[s];
   const V3<T> xr = centre + off[r], xs = centre + off[s];
+  const Cx<T> minus_i = cx<T>(T(0.0), T(-1.0));
+  if (unit_arms) {
+    // T2, tabulated orbits: the arms breathe, so k.(x_r - x_s) = L k.n_rs no longer holds and Eq. 5 is not the
+    // transform of Eq. 1 any more.  Eq. 1 is the definition; its transform at frozen geometry is
+    //   y_rs = [ e^{-2 pi i f (L + k.x_s)} - e^{-2 pi i f k.x_r} ] / (2 (1 - k.n_rs)) n_rs.h.n_rs
+    // with the UNIT link vector n_rs = (x_r - x_s) / |x_r - x_s| and the nominal L (pin P5: equal to Eq. 5 for
+    // rigid arms).  The pole at k.n_rs = 1 is cancelled by n.P.n = O(1 - (k.n)^2); no special case is made for it.
+    const V3<T> n = smul(dx, T(1.0) / o_sqrt(dot(dx, dx)));
+    const T kn = dot(F.k, n);
+    // the difference of the two exponentials is written as -2 i sin(a) e^{-i pi f [L + k.(x_r + x_s)]} with
+    // a = pi f [L - k.(x_r - x_s)] (= the sinc argument of Eq. 5 when the arms are rigid): same number, no cancellation
+    const T a = pi * f * (Lbar - dot(F.k, dx) / T(C_SI));
+    const T kxx = dot(F.k, xr + xs) / T(C_SI);
+    const Cx<T> pref = scale(minus_i, o_sin(a) / (T(1.0) - kn));
+    const Cx<T> ph = expi(-(pi * f * (Lbar + kxx)));
+    const Cx<T> nPn = arm_projection(F, n, Kp, Kc);
+    return pref * ph * nPn * hlm;
+  }
+  const V3<T> n = smul(dx, T(1.0) / T(L_m));                               // n_rs = (x_r - x_s)/L
   const T kn = dot(F.k, n);
   const T kxx = dot(F.k, xr + xs) / T(C_SI);                               // k.(x_r + x_s)/c
   const T x = pi * f * Lbar * (T(1.0) - kn);
-  const Cx<T> minus_i = cx<T>(T(0.0), T(-1.0));
   const Cx<T> pref = scale(minus_i, pi * f * Lbar * sinc(x));              // -i pi f L sinc[...]
   const Cx<T> ph = expi(-(pi * f * (Lbar + kxx)));                         // exp{-i pi f [L + k.(x_r+x_s)]}
   const Cx<T> nPn = arm_projection(F, n, Kp, Kc);                          // n.P^{lm}.n
@@ -419,7 +438,7 @@ template <class T> void links_from_waveform(const T& iota, const Frame<T>& F, in
     orbit(D, tf, &centre, off);                                            // geometry at t = t_lm(f)
   }
   const int R[6] = {0, 1, 0, 2, 1, 2}, S[6] = {1, 0, 2, 0, 2, 1};
-  for (int i = 0; i < 6; ++i) y[i] = single_link(T(f), D.L_m, F, centre, off, R[i], S[i], Kp, Kc, hlm);
+  for (int i = 0; i < 6; ++i) y[i] = single_link(T(f), D.L_m, F, centre, off, R[i], S[i], Kp, Kc, hlm, ot != nullptr);
 }
 
 template <class T> bool mode_links(const Source<T>& s, const Frame<T>& F, int l, int m, double f,

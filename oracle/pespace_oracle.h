@@ -81,8 +81,8 @@ int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* a
 
 /* ---- T2: tabulated numerical orbits.  Positions pos [n_det][K][3 spacecraft][3]
  * (metres) and velocities vel [n_det][K][3][3] (m/s) on the uniform time grid t0 + j dt (SSB seconds, origin of t_c);
- * cubic Hermite in time; Eq. 5 / 6 keep the nominal L of the detector description; a mode whose t_lm(f) lies outside
- * the table contributes 0.  The detector's kind / kappa / lambda0 / period / pointing are ignored. */
+ * cubic Hermite in time; Eq. 5 / 6 keep the nominal L of the detector description, the link directions are the unit
+ * vectors (x_r - x_s) / |x_r - x_s|; a mode whose t_lm(f) lies outside the table contributes 0.  The detector's kind / kappa / lambda0 / period / pointing are ignored. */
 int pespace_oracle_response_orb(const double* params, int64_t B, int64_t K, double t0, double dt, const double* pos,
                                 const double* vel, const double* freqs, int64_t N, const pespace_oracle_model* model,
                                 double* out_AET);

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_loglike_mixed", "pespace_workspace_bytes_grad", "pespace_loglike_grad",
-           "pespace_session_loglike_grad", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
+           "pespace_session_loglike_grad", "pespace_response_orb", "pespace_loglike_orb", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
            "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
@@ -41,6 +41,10 @@ class _Grid(C.Structure):
 
 class _Model(C.Structure):
     _fields_ = [("mode_mask", C.c_uint32), ("n_det", C.c_int32), ("det", C.POINTER(_Det))]
+
+
+class _OrbitTable(C.Structure):
+    _fields_ = [("K", C.c_int64), ("t0", C.c_double), ("dt", C.c_double), ("d_pos", C.c_void_p), ("d_vel", C.c_void_p)]
 
 
 class _WaveTable(C.Structure):
@@ -69,6 +73,9 @@ def _load():
     L.pespace_workspace_bytes_grad.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
     L.pespace_workspace_bytes_grad.restype = sz
     L.pespace_loglike_grad.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
+    L.pespace_response_orb.argtypes = [vp, i64, C.POINTER(_OrbitTable), vp, i64, C.POINTER(_Model), vp, vp]
+    L.pespace_loglike_orb.argtypes = [vp, i64, C.POINTER(_OrbitTable), vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp,
+                                      vp, sz, vp]
     L.pespace_loglike_host.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp]
     L.pespace_response_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, i64, C.POINTER(_Model), vp, vp]
     L.pespace_workspace_bytes_tab.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
@@ -289,6 +296,53 @@ class Fisher:
 def fisher(params: torch.Tensor, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):
     """-> (F [B][11][11], grad [B][11] or None)."""
     return Fisher(data, psd, grid, model, params.shape[0])(params)
+
+
+class OrbitTable:
+    """Device-resident orbit tables: pos, vel [n_det][K][3][3] on the time grid t0 + j dt."""
+
+    def __init__(self, t0: float, dt: float, pos: torch.Tensor, vel: torch.Tensor):
+        self.t0, self.dt = float(t0), float(dt)
+        self.pos, self.vel = _dev(pos.contiguous(), "pos"), _dev(vel.contiguous(), "vel")
+        if self.pos.dim() != 4 or tuple(self.pos.shape[2:]) != (3, 3) or self.vel.shape != self.pos.shape:
+            raise PespaceError("orbit tables must be [n_det][K][3][3]")
+        self.K = int(self.pos.shape[1])
+        self.c = _OrbitTable(self.K, self.t0, self.dt, self.pos.data_ptr(), self.vel.data_ptr())
+
+    def check(self, model) -> None:
+        if self.pos.shape[0] != len(model.detectors):
+            raise PespaceError(f"orbit tables hold {self.pos.shape[0]} detector(s), the model {len(model.detectors)}")
+
+
+def response_orb(params: torch.Tensor, orbit: OrbitTable, freqs: torch.Tensor, model,
+                 out: Optional[torch.Tensor] = None) -> torch.Tensor:
+    """complex128 [B][n_det][3][N] with the spacecraft positions from `orbit`"""
+    p, f = _dev(params, "params"), _dev(freqs, "freqs")
+    orbit.check(model)
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    if out is None:
+        out = torch.empty((B, nd, 3, N, 2), dtype=torch.float64, device=p.device)
+    m, keep = _model(model)
+    _check(_lib.pespace_response_orb(p.data_ptr(), B, C.byref(orbit.c), f.data_ptr(), N, C.byref(m),
+                                     _dev(out, "out").data_ptr(), _stream_ptr()), "pespace_response_orb")
+    return torch.view_as_complex(out)
+
+
+class LikelihoodOrb(Likelihood):
+    """pespace_loglike_orb: likelihood with tabulated orbits; data, PSD and workspace resident."""
+
+    def __call__(self, params: torch.Tensor, orbit: OrbitTable, out: Optional[torch.Tensor] = None) -> torch.Tensor:
+        p = _dev(params, "params")
+        orbit.check(self.model)
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        if out is None:
+            out = torch.empty(B, dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_loglike_orb(p.data_ptr(), B, C.byref(orbit.c), self.data.data_ptr(), self.psd.data_ptr(),
+                                        C.byref(self._g), C.byref(self._m), _dev(out, "out").data_ptr(),
+                                        self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_loglike_orb")
+        return out
 
 
 class LikelihoodGrad(Likelihood):

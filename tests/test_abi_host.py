@@ -174,3 +174,23 @@ def test_grad_argument_validation_without_a_device():
     assert L.pespace_loglike_grad(fake, 4, fake, fake, C.byref(g), C.byref(m), fake, fake, fake, need - 1, None) == -1
     assert L.pespace_loglike_grad(fake, 4, None, fake, C.byref(g), C.byref(m), fake, fake, fake, need, None) == -1
     assert L.pespace_session_loglike_grad(None, None, 4, None, None) == -1
+
+
+def test_orb_argument_validation_without_a_device():
+    from paper_2602_12011_b200 import binding as P
+    L = P.lib()
+    wl = W.config(3, B=4, N=64)
+    m, keep = P._model(wl.model)
+    g = P._grid(wl.grid)
+    fake = 0x1000
+    good = P._OrbitTable(16, 0.0, 100.0, fake, fake)
+    assert L.pespace_response_orb(fake, 4, None, fake, 64, C.byref(m), fake, None) == -1
+    assert L.pespace_response_orb(fake, 4, C.byref(P._OrbitTable(1, 0.0, 100.0, fake, fake)), fake, 64, C.byref(m), fake,
+                                  None) == -1                                   # K < 2
+    assert L.pespace_response_orb(fake, 4, C.byref(P._OrbitTable(16, 0.0, 0.0, fake, fake)), fake, 64, C.byref(m), fake,
+                                  None) == -1                                   # dt <= 0
+    assert L.pespace_response_orb(fake, 4, C.byref(P._OrbitTable(16, 0.0, 1.0, fake, None)), fake, 64, C.byref(m), fake,
+                                  None) == -1
+    assert L.pespace_loglike_orb(fake, 4, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 8, None) == -1
+    assert L.pespace_loglike_orb(fake, 0, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 1 << 30,
+                                 None) == -1
