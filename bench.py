@@ -1,20 +1,26 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the batched likelihood hot path on B200 (one JSON line on stdout).
 
-  python bench.py --gpus N --steps K --warmup W [--config 2|3|4] [--impl reference]
+  python bench.py --gpus N --steps K --warmup W [--config 2|3|4|5] [--path ...] [--impl reference]
 
-A "step" is one pass of the whole hot path (per-sample constants ->
-fused per-bin kernel -> fixed-order combine) over one batch of B synthetic samples: one
-pespace_loglike call.  The workload at N=1 is BASELINE.json configs[1] ("config 2":
-B=4096 x N=262144, one LISA-like detector, (2,2) mode), the one the metric is quoted on.
-With N>1 GPUs (torchrun) every rank evaluates its own batch of B samples on replicated
-data -- no data-path collective -- so scaling is "weak" and `value` is the whole-job rate.
+A "step" is one pass of the whole hot path (per-bin table -> per-sample constants ->
+fused per-bin kernel -> fixed-order combine) over one batch of B synthetic samples: one pespace_loglike call.  The
+workload at N=1 is BASELINE.json configs[1] ("config 2": B=4096 x N=262144, one LISA-like detector, (2,2) mode), the
+one the metric is quoted on.  With N>1 GPUs (torchrun) every rank evaluates its own batch of B samples on replicated
+data -- no data-path collective -- so scaling is "weak" and `value` is the whole-job rate; `--scaling strong` splits
+ONE global batch over the ranks (dist.ShardedLikelihood: all-gather of lnL inside the timed region).
 
-value     device-timed lnL evaluations/s, inputs resident in HBM (CUDA events, max over ranks)
-e2e       the same metric through the C ABI with HOST buffers (pespace_loglike_host):
-          H2D of params + data + psd and D2H of lnL inside the timed region
-roofline  the dominant kernel (loglike_kernel) against the FP64 ALU peak
+value          device-timed evaluations/s, inputs resident in HBM (CUDA events, max over ranks)
+e2e            the same metric through the C ABI with HOST buffers (pespace_session_*): H2D of theta + data + PSD and
+               D2H of the result inside the timed region
+roofline       the dominant kernel against the FP64 ALU peak; operation counts from profiles/r02_ops.json (ncu),
+               marked stale when the kernel sources have changed since they were counted
+other_configs  (default run only) short device-timed runs of configs 3, 4, 5 (Fisher), the adjoint gradient and
+               pespace_response, so that every BASELINE.json config and every north-star call is in the driver's line
 cpu_baseline / --impl reference   the oracle, as it stands, on the box's host cores
+
+--path selects the entry point that is timed: loglike (default; config 5: fisher), mixed, tab, orb, grad (adjoint
+lnL + gradient), fisher-grad (forward-mode gradient, pespace_fisher with d_out_F = NULL).
 """
 from __future__ import annotations
 
@@ -24,7 +30,6 @@ import os
 import subprocess
 import sys
 import tempfile
-import threading
 import time
 
 import numpy as np
@@ -33,38 +38,33 @@ ROOT = os.path.dirname(os.path.abspath(__file__))
 if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
+from paper_2602_12011_b200 import build as pbuild        # noqa: E402
 from paper_2602_12011_b200 import dist as pdist          # noqa: E402
 from paper_2602_12011_b200 import workloads as W         # noqa: E402
 
 # ---- roofline constants
-# FP64 ALU peak: 148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (1965 MHz) = 37.22 TFLOP/s.  The
-# library's own DFMA micro-benchmark (pespace_fp64_peak) is run in the same process and reported next
-# to it: mode 0 (two register operands) reaches ~98 % of that figure, mode 1 (three distinct register
-# operands, the common case in this kernel) ~66 % (profiles/r01_fp64_operand_bandwidth.md).
+# FP64 ALU peak: 148 SMs x 64 FP64 lanes x 2 flop x clocks.max.sm (1965 MHz) = 37.22 TFLOP/s; MEASURED_PEAKS.json has no
+# FP64 entry, so the library's own DFMA micro-benchmark (pespace_fp64_peak) is run in the same process and reported
+# beside it.  The operation counts per unit of work come from profiles/r02_ops.json (written from ncu CSVs by
+# paper_2602_12011_b200/ops_from_ncu.py and stamped with the content hash of the kernel sources).
 SM_COUNT, FP64_LANES_PER_SM = 148, 64
-# FP64 operations of loglike_kernel per (sample, bin, detector), thread level, counted by ncu
-# (smsp__sass_thread_inst_executed_op_{dfma,dmul,dadd}_pred_on.sum / (B*N), profiles/r01_kernels_ncu.md).
-# They equal the operation list of the reduced formulas in DESIGN.md ("Algorithmic work") to <1 %; the
-# kernel has no redundant evaluation, so executed = algorithmic.  flop = 2*DFMA + DMUL + DADD.
-FP64_OPS_PER_UNIT = {
-    # (kernel, detector kind, mode-class mask): per (sample, bin, detector); profiles/r01_kernels_ncu.md
-    ("loglike", 0, 2): {"dfma": 140.00, "dmul": 53.02, "dadd": 40.53},      # kind 0, (2,2) only  -- config 2
-    ("loglike", 0, 15): {"dfma": 554.00, "dmul": 188.11, "dadd": 101.08},   # kind 0, five modes  -- configs 3, 4
-    ("loglike", 1, 15): {"dfma": 526.00, "dmul": 224.11, "dadd": 109.08},   # kind 1, five modes  -- config 4
-    ("fisher", 0, 15): {"dfma": 3150.00, "dmul": 1246.25, "dadd": 640.61},  # config 5
-    ("fisher", 1, 15): {"dfma": 3030.00, "dmul": 1330.25, "dadd": 632.61},
-    ("loglike_tab", 0, 2): {"dfma": 136.00, "dmul": 52.03, "dadd": 46.03},   # --waveform tab, config 2 (one mode)
-}
-# dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel (same ncu captures; config 4:
-# mean of the three launches of a step)
-DRAM_TRAFFIC_PER_LAUNCH = {2: 35.91e6 + 5.18e6, 3: 36.18e6 + 5.39e6, 4: (40.4e6 + 36.6e6 + 42.1e6 + 37.2e6 + 41.3e6 + 37.9e6) / 3,
-                           5: 36.9e6 + 57.6e6}
-# SURVEY.md 8(d) survey-time estimate (library-cost transcendentals: sincos 40, cbrt 30, log 35, ...);
-# kept for reference only -- the reduced algorithm needs less than half of it.
+OPS_FILE = os.path.join(ROOT, "profiles", "r02_ops.json")
+# SURVEY.md 8(d) survey-time estimate (library-cost transcendentals); kept for reference only
 SURVEY_FLOP_PER_BIN_EVAL = {2: 970.0, 3: 4500.0, 4: 11200.0, 5: 100000.0}
-OPS_SOURCE = "profiles/r01_kernels_ncu.md"
-METRIC, UNIT = "lnL_evals_per_sec", "lnL/s"
-FISHER_METRIC, FISHER_UNIT = "fisher_evals_per_sec", "F/s"     # --config 5 only (S10: F and grad per sample)
+UNITS = {"loglike": ("lnL_evals_per_sec", "lnL/s"), "mixed": ("lnL_evals_per_sec", "lnL/s"),
+         "tab": ("lnL_evals_per_sec", "lnL/s"), "orb": ("lnL_evals_per_sec", "lnL/s"),
+         "fisher": ("fisher_evals_per_sec", "F/s"), "fisher-grad": ("grad_evals_per_sec", "grad/s"),
+         "grad": ("lnL_and_grad_evals_per_sec", "(lnL+grad)/s")}
+KERNEL_OF = {"loglike": "loglike", "mixed": "loglike_mixed", "tab": "loglike_tab", "orb": "loglike_orb",
+             "fisher": "fisher", "fisher-grad": "fisher", "grad": "loglike_grad"}
+
+
+def load_ops():
+    try:
+        doc = json.load(open(OPS_FILE))
+    except (OSError, ValueError):
+        return {"kernels": {}, "csrc_hash": None}
+    return doc
 
 
 class ClockSampler:
@@ -118,32 +118,34 @@ class ClockSampler:
 FISHER_REF_BINS = 8192   # the oracle's Fisher pass costs ~45 core-seconds per sample at N = 262144: time a bin subset
 
 
-def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0, tab_nodes: int = 0):
+def oracle_timed(config: int, path: str, n_samples, steps: int, target_s: float = 12.0, tab_nodes: int = 0):
     """Time the oracle, as it stands, on a bounded sample of the workload: `n_samples` samples (None: sized from a
-    one-sample-per-core calibration pass for ~target_s of wall time) x all N bins per step; for the Fisher path
-    (config 5) x the first FISHER_REF_BINS bins, the rate scaled by FISHER_REF_BINS / N (the cost per bin is uniform).
+    one-sample-per-core calibration pass for ~target_s of wall time) x all N bins per step; for the derivative paths
+    x the first FISHER_REF_BINS bins, the rate scaled by FISHER_REF_BINS / N (the cost per bin is uniform).
     -> (rate in full-N evaluations/s, seconds per step, cores, description of the sample)."""
     import oracle
-    fisher = config == 5
+    deriv = path in ("fisher", "fisher-grad", "grad")
     full = W.config(config)
-    wl = W.config(config, N=FISHER_REF_BINS) if fisher else full
+    wl = W.config(config, N=FISHER_REF_BINS) if deriv else full
     scale = wl.grid.N / full.grid.N
     psd = wl.psd()
     cores = oracle.get_threads()
-    if tab_nodes:
+    if path == "tab":
         f_all = wl.grid.freqs()
         fnodes = W.log_nodes(f_all[0], f_all[-1], tab_nodes)
         tab = lambda p: W.chirp_table(p, wl.model.mode_mask, fnodes)
         data = wl.data(lambda p, fr, m: oracle.response_tab(p, tab(p), fr, m))
         call = lambda p: oracle.loglike_tab(p, tab(p), data, psd, wl.grid, wl.model)
+    elif path == "orb":
+        otab = orbit_table_for(wl)
+        data = wl.data(lambda p, fr, m: oracle.response_orb(p, otab, fr, m))
+        call = lambda p: oracle.loglike_orb(p, otab, data, psd, wl.grid, wl.model)
     else:
         data = wl.data(lambda p, fr, m: oracle.response(p, fr, m))
-    if tab_nodes:
-        pass
-    elif fisher:
-        call = lambda p: oracle.fisher(p, data, psd, wl.grid, wl.model)
-    else:
-        call = lambda p: oracle.loglike(p, data, psd, wl.grid, wl.model)
+        if deriv:
+            call = lambda p: oracle.fisher(p, data, psd, wl.grid, wl.model)
+        else:
+            call = lambda p: oracle.loglike(p, data, psd, wl.grid, wl.model)
     t0 = time.perf_counter()
     call(wl.params[:cores])                                                  # warm-up + calibration
     t_cal = time.perf_counter() - t0
@@ -161,46 +163,208 @@ def oracle_timed(config: int, n_samples, steps: int, target_s: float = 12.0, tab
     one_thread = 2 / (time.perf_counter() - t1) * scale
     oracle.set_threads(0)
     oracle_timed.one_thread = one_thread
-    bins = f"all {wl.grid.N} bins" if not fisher else f"the first {wl.grid.N} of {full.grid.N} bins (rate scaled by {scale:.5f})"
+    bins = f"all {wl.grid.N} bins" if not deriv else f"the first {wl.grid.N} of {full.grid.N} bins (rate scaled by {scale:.5f})"
+    what = " (the oracle's forward-mode F + gradient pass)" if deriv else ""
     desc = (f"{n_samples} of {full.B} samples (evenly spaced) x {bins} per pass, {steps} pass(es), "
-            f"{dt / steps:.1f} s per pass, OpenMP over samples")
+            f"{dt / steps:.1f} s per pass, OpenMP over samples{what}")
     return n_samples * steps / dt * scale, dt / steps, cores, desc
+
+
+def orbit_table_for(wl, dt: float = 1800.0):
+    """seeded toy ephemeris covering every t_lm of the workload with margin (input recipe only: workloads.py)"""
+    T = 1.0 / wl.grid.df                 # t_44(1e-4 Hz) = t_22(5e-5 Hz) lies 12.5 T before t_c for the config masses
+    t_lo, t_hi = -16.0 * T, 2.2 * T
+    return W.synthetic_orbit_table(wl.model.detectors, t_lo, dt, int((t_hi - t_lo) / dt) + 2, seed=17)
+
+
+def default_path(args) -> str:
+    if args.path:
+        return args.path
+    return "fisher" if args.config == 5 else "loglike"
+
+
+def workload_config(wl, args, path, l2):
+    extra = {"tab": f" + tabulated mode waveforms (K={args.tab_nodes} log-spaced nodes)", "orb": " + tabulated orbits",
+             "grad": " (lnL + adjoint gradient)", "fisher-grad": " (forward-mode gradient only)",
+             "mixed": " (mixed precision)"}.get(path, "")
+    return {"workload": f"config{args.config}{extra}: B={wl.B} x N={wl.grid.N}, {len(wl.model.detectors)} detector(s) "
+                        f"[{', '.join(d.name for d in wl.model.detectors)}], mode_mask={wl.model.mode_mask}, "
+                        f"TDI {wl.model.detectors[0].tdi_gen / 10:.1f}, f0={wl.grid.f0} Hz, df=1/(30 d)",
+            "path": path, "B_per_gpu": wl.B, "N_bins": wl.grid.N, "n_det": len(wl.model.detectors),
+            "mode_mask": wl.model.mode_mask,
+            "parallelism": (f"one global batch split over {args.gpus} rank(s), all-gather of lnL" if args.scaling == "strong"
+                            else f"sample-sharded x{args.gpus} (no data-path collective)"),
+            "l2": l2}
 
 
 def run_reference(args):
     rank, _, world = pdist.env_world()
     if rank != 0:
         return
+    path = default_path(args)
     wl = W.config(args.config)
-    fisher_mode = args.config == 5
-    METRIC, UNIT = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (globals()["METRIC"], globals()["UNIT"])
-    rate, sec_per_step, cores, sample = oracle_timed(args.config, args.ref_samples, args.steps,
+    metric, unit = UNITS[path]
+    rate, sec_per_step, cores, sample = oracle_timed(args.config, path, args.ref_samples, args.steps,
                                                      target_s=max(2.0, 60.0 / max(1, args.steps)),
-                                                     tab_nodes=args.tab_nodes if args.waveform == "tab" else 0)
+                                                     tab_nodes=args.tab_nodes)
     line = {
-        "impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+        "impl": "reference", "metric": metric, "value": rate, "unit": unit, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3,
-        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "higher_is_better": True, "scaling": args.scaling, "vs_baseline": None, "dtype": "f64", "data": "synthetic",
         "bin_evals_per_sec": rate * wl.grid.N,
-        "config": workload_config(wl, args, l2="n/a (CPU)"),
-        "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample,
+        "config": workload_config(wl, args, path, l2="n/a (CPU)"),
+        "cpu_baseline": {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": sample,
                          "value_one_thread": oracle_timed.one_thread},
-        "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "e2e": {"value": rate, "unit": unit, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
         "gpu_launches": 0,
     }
     print(json.dumps(line), flush=True)
 
 
-def workload_config(wl, args, l2):
-    tab = f" + tabulated mode waveforms (K={args.tab_nodes} log-spaced nodes)" if args.waveform == "tab" else ""
-    if getattr(args, "grad_only", False) and args.config == 5:
-        tab += " (gradient only)"
-    return {"workload": f"config{args.config}{tab}: B={wl.B} x N={wl.grid.N}, {len(wl.model.detectors)} detector(s) "
-                        f"[{', '.join(d.name for d in wl.model.detectors)}], mode_mask={wl.model.mode_mask}, "
-                        f"TDI {wl.model.detectors[0].tdi_gen / 10:.1f}, f0={wl.grid.f0} Hz, df=1/(30 d)",
-            "B_per_gpu": wl.B, "N_bins": wl.grid.N, "n_det": len(wl.model.detectors),
-            "mode_mask": wl.model.mode_mask, "parallelism": f"sample-sharded x{args.gpus} (no data-path collective)",
-            "l2": l2}
+# ------------------------------------------------------------------------------------------------ device side
+class Bench:
+    """One (config, path) workload resident on the device: builds the inputs, exposes step(i)."""
+
+    def __init__(self, P, torch, device, rank, config, path, args, B=None, world=1):
+        self.P, self.torch, self.device, self.path = P, torch, device, path
+        n_batches = 2 if path == "tab" else 4
+        strong = args.scaling == "strong" and world > 1
+        seed_rank = 0 if strong else rank                 # strong scaling: every rank holds the SAME global batch
+        self.wls = [W.config(config, B=B, param_seed=pdist.rank_seed(1000 + i, seed_rank)) for i in range(n_batches)]
+        wl = self.wl = self.wls[0]
+        self.B, self.N, self.n_batches = wl.B, wl.grid.N, n_batches
+        dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).to(device)
+        self.freqs_d = dev(wl.grid.freqs())
+        self.tabs_h = self.tabs_d = self.orbit = None
+        if path == "tab":
+            f_all = wl.grid.freqs()
+            fnodes = W.log_nodes(f_all[0], f_all[-1], args.tab_nodes)
+            self.tabs_h = [tuple(torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
+                                 for x in W.chirp_table(w.params, wl.model.mode_mask, fnodes)) for w in self.wls]
+            self.tabs_d = [P.WaveTable(*(x.to(device) for x in t)) for t in self.tabs_h]
+            inj_tab = P.WaveTable(*(dev(x) for x in W.chirp_table(wl.theta_inj[None], wl.model.mode_mask, fnodes)))
+            resp = lambda p, fr, m: P.response_tab(dev(p), inj_tab, self.freqs_d, m).cpu().numpy()
+        elif path == "orb":
+            ot = orbit_table_for(wl)
+            self.orbit = P.OrbitTable(ot[0], ot[1], dev(ot[2]), dev(ot[3]))
+            resp = lambda p, fr, m: P.response_orb(dev(p), self.orbit, self.freqs_d, m).cpu().numpy()
+        else:
+            resp = lambda p, fr, m: P.response(dev(p), self.freqs_d, m).cpu().numpy()
+        # the injection comes from this library's own response call; host copies live in pinned memory
+        self.data_h = torch.from_numpy(np.ascontiguousarray(wl.data(resp))).pin_memory()
+        self.psd_h = torch.from_numpy(np.ascontiguousarray(wl.psd())).pin_memory()
+        self.params_h = [torch.from_numpy(np.ascontiguousarray(w.params)).pin_memory() for w in self.wls]
+        self.params_d = [p.to(device) for p in self.params_h]
+        data_d, psd_d = self.data_h.to(device), self.psd_h.to(device)
+        B = self.B
+        f64 = dict(dtype=torch.float64, device=device)
+        self.out_d = torch.empty(B, **f64)
+        self.F_d = self.g_d = None
+        if path in ("fisher", "fisher-grad"):
+            self.obj = P.Fisher(data_d, psd_d, wl.grid, wl.model, B)
+            self.F_d, self.g_d = torch.empty((B, P.NPAR, P.NPAR), **f64), torch.empty((B, P.NPAR), **f64)
+        elif path == "grad":
+            self.obj = P.LikelihoodGrad(data_d, psd_d, wl.grid, wl.model, B)
+            self.g_d = torch.empty((B, P.NPAR), **f64)
+        elif path == "tab":
+            self.obj = P.LikelihoodTab(data_d, psd_d, wl.grid, wl.model, B)
+        elif path == "orb":
+            self.obj = P.LikelihoodOrb(data_d, psd_d, wl.grid, wl.model, B)
+        else:
+            self.obj = P.Likelihood(data_d, psd_d, wl.grid, wl.model, B)
+        self.sharded = None
+        if strong and path in ("loglike", "mixed"):
+            self.sharded = pdist.ShardedLikelihood(lambda p: self.obj(p, mixed=(path == "mixed")))
+
+    def step(self, i):
+        p = self.params_d[i % self.n_batches]
+        if self.path == "fisher":
+            self.obj(p, self.F_d, self.g_d)
+        elif self.path == "fisher-grad":
+            self.obj(p, None, self.g_d, grad_only=True)
+        elif self.path == "grad":
+            self.obj(p, self.out_d, self.g_d)
+        elif self.path == "tab":
+            self.obj(p, self.tabs_d[i % self.n_batches], self.out_d)
+        elif self.path == "orb":
+            self.obj(p, self.orbit, self.out_d)
+        elif self.sharded is not None:
+            self.out_d = self.sharded(p)
+        else:
+            self.obj(p, self.out_d, mixed=(self.path == "mixed"))
+
+    def result(self):
+        t = {"fisher": self.F_d, "fisher-grad": self.g_d, "grad": self.g_d}.get(self.path, self.out_d)
+        return t.cpu().numpy()
+
+
+def timed_run(b: Bench, steps: int, warmup: int, flush, device):
+    """-> dict(elapsed_ms, launches, kernel_ms_total, kernel_launches); exactly `steps` steps, device events, barrier +
+    synchronize on both sides; the L2 flush (a 256 MiB buffer rewritten) sits inside the timed region"""
+    P, torch = b.P, b.torch
+    for i in range(warmup):
+        flush.zero_()
+        b.step(i)
+    torch.cuda.synchronize()
+    P.profile_enable(True)
+    P.profile_read()
+    launches0 = P.launch_count()
+    pdist.barrier(device)
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for i in range(steps):
+        flush.zero_()
+        b.step(i)
+    e1.record()
+    torch.cuda.synchronize()
+    pdist.barrier(device)
+    main_ms, main_launches = P.profile_read()
+    P.profile_enable(False)
+    return {"elapsed_ms": e0.elapsed_time(e1), "launches": P.launch_count() - launches0, "kernel_ms_total": main_ms,
+            "kernel_launches": main_launches}
+
+
+def class_mask(mode_mask: int) -> int:
+    return (2 if mode_mask & 9 else 0) | (1 if mode_mask & 2 else 0) | (4 if mode_mask & 4 else 0) | \
+           (8 if mode_mask & 16 else 0)
+
+
+def roofline_of(path, wl, B, N, kern_ms, ops_doc, peak_tflops, sm_max_mhz, stale):
+    """roofline object of the dominant kernel of `path` from the ncu operation table (None entries when the table has
+    no row for one of the kernels involved)"""
+    kernel = KERNEL_OF[path]
+    cm = class_mask(wl.model.mode_mask)
+    rows = []
+    for d in wl.model.detectors:
+        key_mask = 0 if kernel in ("loglike_tab", "loglike_mixed", "loglike_orb") else cm
+        key_kind = 0 if kernel == "loglike_orb" else d.kind
+        rows.append(ops_doc["kernels"].get(f"{kernel}|{key_kind}|{key_mask}"))
+    out = {"bound": "alu", "kernel": f"{kernel}_kernel", "achieved": None, "peak": peak_tflops, "unit": "TFLOP/s",
+           "frac": None, "traffic": None, "kernel_ms": kern_ms, "stale": stale,
+           "ops_source": os.path.relpath(OPS_FILE, ROOT), "ops_csrc_hash": ops_doc.get("csrc_hash")}
+    if path == "fisher-grad" or not all(rows):
+        return out                                         # no ncu counts for this variant
+    n = len(rows)
+    ops = {k: sum(r[k] for r in rows) / n for k in ("dfma", "dmul", "dadd", "dram_bytes_per_launch")}
+    flop_per_unit = 2.0 * ops["dfma"] + ops["dmul"] + ops["dadd"]
+    inst_per_unit = ops["dfma"] + ops["dmul"] + ops["dadd"]
+    achieved = flop_per_unit * B * N / (kern_ms * 1e-3) / 1e12
+    # issue cost on the FP64 pipe (profiles/r01_fp64_operand_bandwidth.md): one 64-bit register operand per cycle and
+    # SM sub-partition, at least 2 cycles per instruction -> a DFMA with three distinct registers takes 3 cycles
+    cyc = 3.0 * ops["dfma"] + 2.0 * (ops["dmul"] + ops["dadd"])
+    t_operand = cyc * (B * N / 32.0) / (SM_COUNT * 4) / (sm_max_mhz * 1e6)
+    out.update({
+        "achieved": achieved, "frac": achieved / peak_tflops, "traffic": ops["dram_bytes_per_launch"],
+        "flop_per_unit": flop_per_unit, "unit_of_work": "(sample, bin, detector)",
+        "flop_per_launch": flop_per_unit * B * N,
+        "fma_share_of_fp64_instructions": ops["dfma"] / inst_per_unit,
+        "fp64_pipe_frac": inst_per_unit * B * N / (kern_ms * 1e-3) / (peak_tflops * 1e12 / 2.0),
+        "operand_bandwidth_bound_ms": t_operand * 1e3,
+        "frac_of_operand_bandwidth_bound": t_operand * 1e3 / kern_ms,
+        "hbm_gbs_achieved": ops["dram_bytes_per_launch"] / (kern_ms * 1e-3) / 1e9,
+    })
+    return out
 
 
 def run_ours(args):
@@ -213,231 +377,169 @@ def run_ours(args):
     rank, local_rank, world = pdist.init("nccl")
     torch.cuda.set_device(local_rank)
     device = torch.device("cuda", local_rank)
+    path = default_path(args)
+    if path in ("fisher", "fisher-grad") and args.config != 5:
+        pass                                            # any config may run the derivative paths
+    metric, unit = UNITS[path]
+    ops_doc = load_ops()
+    stale = ops_doc.get("csrc_hash") != pbuild.csrc_hash()
 
-    # ---- inputs: synthetic, seeded; the injection comes from this library's own response call
-    fisher_mode = args.config == 5
-    tab_mode = args.waveform == "tab"
-    mixed_mode = args.precision == "mixed"
-    if mixed_mode and (fisher_mode or tab_mode):
-        raise SystemExit("bench.py: --precision mixed applies to the analytic likelihood configs 2-4")
-    if tab_mode and fisher_mode:
-        raise SystemExit("bench.py: --waveform tab applies to the likelihood configs 2-4")
-    n_batches = 2 if tab_mode else 4
-    wls = [W.config(args.config, param_seed=pdist.rank_seed(1000 + i, rank)) for i in range(n_batches)]
-    wl = wls[0]
-    B, N = wl.B, wl.grid.N
-    freqs_d = torch.from_numpy(wl.grid.freqs()).to(device)
-
-    def gpu_response(p, fr, m):
-        return P.response(torch.from_numpy(np.ascontiguousarray(p)).to(device), freqs_d, m).cpu().numpy()
-
-    if tab_mode:
-        # synthetic tables (workloads.chirp_table: inspiral-shaped power laws) on K log-spaced nodes covering the grid
-        f_all = wl.grid.freqs()
-        fnodes = W.log_nodes(f_all[0], f_all[-1], args.tab_nodes)
-        tabs_h = [tuple(torch.from_numpy(np.ascontiguousarray(x)).pin_memory()
-                        for x in W.chirp_table(w.params, wl.model.mode_mask, fnodes)) for w in wls]
-        tabs_d = [P.WaveTable(*(x.to(device) for x in t)) for t in tabs_h]
-        inj_tab = P.WaveTable(*(torch.from_numpy(np.ascontiguousarray(x)).to(device)
-                                for x in W.chirp_table(wl.theta_inj[None], wl.model.mode_mask, fnodes)))
-
-        def gpu_response(p, fr, m):                                   # noqa: F811  (injection from the same tables)
-            return P.response_tab(torch.from_numpy(np.ascontiguousarray(p)).to(device), inj_tab, freqs_d, m).cpu().numpy()
-
-    # host copies live in pinned memory: the e2e leg copies them to the device every step
-    data_h = torch.from_numpy(np.ascontiguousarray(wl.data(gpu_response))).pin_memory()
-    psd_h = torch.from_numpy(np.ascontiguousarray(wl.psd())).pin_memory()
-    params_h = [torch.from_numpy(np.ascontiguousarray(w.params)).pin_memory() for w in wls]
-    params_d = [p.to(device) for p in params_h]
-    if fisher_mode:
-        fis = P.Fisher(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
-        F_d = torch.empty((B, P.NPAR, P.NPAR), dtype=torch.float64, device=device)
-        g_d = torch.empty((B, P.NPAR), dtype=torch.float64, device=device)
-    elif tab_mode:
-        lik = P.LikelihoodTab(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
-        out_d = torch.empty(B, dtype=torch.float64, device=device)
-    else:
-        lik = P.Likelihood(data_h.to(device), psd_h.to(device), wl.grid, wl.model, B)
-        out_d = torch.empty(B, dtype=torch.float64, device=device)
+    main = Bench(P, torch, device, rank, args.config, path, args, world=world)
+    wl, B, N = main.wl, main.B, main.N
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=device)   # > 126 MB L2
 
-    def step(i):
-        flush.zero_()
-        if fisher_mode:
-            fis(params_d[i % n_batches], F_d, g_d, grad_only=args.grad_only)
-        elif tab_mode:
-            lik(params_d[i % n_batches], tabs_d[i % n_batches], out_d)
-        else:
-            lik(params_d[i % n_batches], out_d, mixed=mixed_mode)
-
-    for i in range(args.warmup):
-        step(i)
-    torch.cuda.synchronize()
-
-    # ---- timed region: exactly K steps, device events, barrier + sync on both sides
     sampler = ClockSampler(local_rank)
     sampler.start()
-    P.profile_enable(True)
-    P.profile_read()
-    launches0 = P.launch_count()
-    pdist.barrier(device)
-    torch.cuda.synchronize()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
-    for i in range(args.steps):
-        step(i)
-    e1.record()
-    torch.cuda.synchronize()
-    pdist.barrier(device)
-    elapsed_ms = e0.elapsed_time(e1)
-    launches = P.launch_count() - launches0
-    main_ms, main_launches = P.profile_read()
-    P.profile_enable(False)
+    t = timed_run(main, args.steps, args.warmup, flush, device)
     clocks = sampler.stop()
-    last = ((g_d if args.grad_only else F_d) if fisher_mode else out_d).cpu().numpy()
+    last = main.result()
     if not np.all(np.isfinite(last)):
         raise SystemExit("bench.py: non-finite result in the timed region")
-
-    max_ms, total_units = pdist.aggregate(elapsed_ms, B * args.steps, device)
+    strong = args.scaling == "strong" and world > 1
+    units_here = (B / world if strong else B) * args.steps
+    max_ms, total_units = pdist.aggregate(t["elapsed_ms"], units_here, device)
     value = total_units / (max_ms * 1e-3)
 
-    # ---- e2e: HOST buffers through the C ABI (pespace_session_*): every step copies that step's inputs
-    # (theta, data set, PSD) from pinned host memory to the device and reads the result back, all inside
-    # the timed region.  e2e_resident_data: the sampler-facing use, data set copied once, theta per step.
+    # ---- e2e: HOST buffers through the C ABI (pespace_session_*): every step copies that step's inputs (theta, data
+    # set, PSD) from pinned host memory to the device and reads the result back, all inside the timed region.
+    # value_resident_data: the sampler-facing use, data set copied once, theta per step.
     e2e_steps = max(1, min(args.steps, 10))
-    ses = P.Session(wl.grid, wl.model, B, want_fisher=fisher_mode)
-    if tab_mode:
-        res_h = torch.empty(B, dtype=torch.float64).pin_memory()
+    e2e, h2d, d2h, e2e_api = {"full": None, "resident": None}, 0, 0, None
+    nbytes = lambda x: x.numel() * x.element_size()
+    if path != "orb":
+        ses = P.Session(wl.grid, wl.model, B, want_fisher=path in ("fisher", "fisher-grad"))
+        grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
+        res_h = torch.empty((B, P.NPAR, P.NPAR) if path == "fisher" else (B,), dtype=torch.float64).pin_memory()
+        nb = main.n_batches
 
         def e2e_step(i, copy_data):
             if copy_data:
-                ses.set_data(data_h, psd_h)
-            ses.loglike_tab(params_h[i % n_batches], tabs_h[i % n_batches], res_h)
-    grad_h = torch.empty((B, P.NPAR), dtype=torch.float64).pin_memory()
-    if not tab_mode:
-        res_h = torch.empty((B, P.NPAR, P.NPAR) if fisher_mode else (B,), dtype=torch.float64).pin_memory()
-
-        def e2e_step(i, copy_data):
-            if copy_data:
-                ses.set_data(data_h, psd_h)
-            if fisher_mode:
-                ses.fisher(params_h[i % n_batches], True, res_h, grad_h, grad_only=args.grad_only)
+                ses.set_data(main.data_h, main.psd_h)
+            p = main.params_h[i % nb]
+            if path == "tab":
+                ses.loglike_tab(p, main.tabs_h[i % nb], res_h)
+            elif path == "fisher":
+                ses.fisher(p, True, res_h, grad_h)
+            elif path == "fisher-grad":
+                ses.fisher(p, True, None, grad_h, grad_only=True)
+            elif path == "grad":
+                ses.loglike_grad(p, res_h, grad_h)
             else:
-                ses.loglike(params_h[i % n_batches], res_h, mixed=mixed_mode)
+                ses.loglike(p, res_h, mixed=(path == "mixed"))
 
-    e2e = {}
-    for key, copy_data in (("full", True), ("resident", False)):
-        e2e_step(0, True)                                                   # warm-up
-        pdist.barrier(device)
-        t0 = time.perf_counter()
-        for i in range(e2e_steps):
-            e2e_step(i, copy_data)
-        e2e_ms = (time.perf_counter() - t0) * 1e3                           # the calls are synchronous
-        e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
-        e2e[key] = e2e_units / (e2e_max_ms * 1e-3)
-    ses.close()
-    nbytes = lambda t: t.numel() * t.element_size()
-    h2d = nbytes(params_h[0]) + nbytes(data_h) + nbytes(psd_h) + (sum(nbytes(x) for x in tabs_h[0]) if tab_mode else 0)
-    d2h = nbytes(res_h) + (nbytes(grad_h) if fisher_mode else 0)
+        for key, copy_data in (("full", True), ("resident", False)):
+            e2e_step(0, True)                                                   # warm-up
+            pdist.barrier(device)
+            t0 = time.perf_counter()
+            for i in range(e2e_steps):
+                e2e_step(i, copy_data)
+            e2e_ms = (time.perf_counter() - t0) * 1e3                           # the calls are synchronous
+            e2e_max_ms, e2e_units = pdist.aggregate(e2e_ms, B * e2e_steps, device)
+            e2e[key] = e2e_units / (e2e_max_ms * 1e-3)
+        ses.close()
+        h2d = nbytes(main.params_h[0]) + nbytes(main.data_h) + nbytes(main.psd_h) + \
+            (sum(nbytes(x) for x in main.tabs_h[0]) if path == "tab" else 0)
+        d2h = (nbytes(res_h) if path != "fisher-grad" else 0) + (nbytes(grad_h) if path in ("fisher", "fisher-grad", "grad") else 0)
+        call = {"tab": "loglike_tab", "fisher": "fisher", "fisher-grad": "fisher", "grad": "loglike_grad",
+                "mixed": "loglike_mixed"}.get(path, "loglike")
+        e2e_api = (f"pespace_session_set_data + pespace_session_{call} per step: theta, data set and PSD"
+                   f"{' and the waveform tables' if path == 'tab' else ''} copied from pinned host memory, result read back")
 
-    # ---- optional: pespace_response on a slice of the batch (48 B written per (sample, bin, detector))
+    # ---- the other configs and calls, device-timed only (3 steps each after 3 warm-ups)
+    others = None
+    if args.others and world == 1:
+        others = []
+        peak0 = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+        for cfg, pth in ((3, "loglike"), (4, "loglike"), (5, "fisher"), (5, "grad"), (2, "grad")):
+            if cfg == args.config and pth == path:
+                continue
+            oargs = argparse.Namespace(**vars(args))
+            oargs.config = cfg
+            ob = Bench(P, torch, device, rank, cfg, pth, oargs)
+            ot = timed_run(ob, 3, 3, flush, device)
+            if not np.all(np.isfinite(ob.result())):
+                raise SystemExit(f"bench.py: non-finite result in config {cfg} / {pth}")
+            km = ot["kernel_ms_total"] / max(1, ot["kernel_launches"])
+            rf = roofline_of(pth, ob.wl, ob.B, ob.N, km, ops_doc, peak0, clocks.get("sm_max_mhz") or 1965.0, stale)
+            m_, u_ = UNITS[pth]
+            others.append({"config": cfg, "path": pth, "metric": m_, "unit": u_,
+                           "value": ob.B * 3 / (ot["elapsed_ms"] * 1e-3), "ms_per_step": ot["elapsed_ms"] / 3,
+                           "B": ob.B, "N": ob.N, "n_det": len(ob.wl.model.detectors), "mode_mask": ob.wl.model.mode_mask,
+                           "kernel_ms": km, "kernel_launches_per_step": ot["kernel_launches"] / 3,
+                           "gpu_launches": int(ot["launches"]), "frac": rf["frac"], "achieved_tflops": rf["achieved"],
+                           "flop_per_unit": rf.get("flop_per_unit")})
+            del ob
+            torch.cuda.empty_cache()
+
+    # ---- pespace_response on a slice of the batch (48 B written per (sample, bin, detector))
     response_info = None
-    if args.response and not tab_mode:
-        Br = min(B, args.response_batch)
-        out_r = torch.empty((Br, len(wl.model.detectors), 3, N, 2), dtype=torch.float64, device=device)
-        pr = params_d[0][:Br].contiguous()
-        for _ in range(2):
-            P.response(pr, freqs_d, wl.model, out_r)
-        torch.cuda.synchronize()
-        r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        r0.record()
-        for _ in range(5):
-            P.response(pr, freqs_d, wl.model, out_r)
-        r1.record()
-        torch.cuda.synchronize()
-        r_ms = r0.elapsed_time(r1) / 5
-        response_info = {"batch": Br, "ms_per_call": r_ms, "bin_evals_per_sec": Br * N / (r_ms * 1e-3),
-                         "bytes_written_per_call": out_r.numel() * 8,
-                         "write_gbs": out_r.numel() * 8 / (r_ms * 1e-3) / 1e9}
-        del out_r
+    if (args.response or args.others) and world == 1:
+        response_info = []
+        for cfg in (2, 3):
+            wr = W.config(cfg, B=args.response_batch)
+            pr = torch.from_numpy(np.ascontiguousarray(wr.params)).to(device)
+            out_r = torch.empty((wr.B, len(wr.model.detectors), 3, N, 2), dtype=torch.float64, device=device)
+            for _ in range(2):
+                P.response(pr, main.freqs_d, wr.model, out_r)
+            torch.cuda.synchronize()
+            r0, r1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            r0.record()
+            for _ in range(5):
+                P.response(pr, main.freqs_d, wr.model, out_r)
+            r1.record()
+            torch.cuda.synchronize()
+            r_ms = r0.elapsed_time(r1) / 5
+            response_info.append({"call": "pespace_response", "mode_mask": wr.model.mode_mask, "batch": wr.B, "N": N,
+                                  "ms_per_call": r_ms, "bin_evals_per_sec": wr.B * N / (r_ms * 1e-3),
+                                  "bytes_written_per_call": out_r.numel() * 8,
+                                  "write_gbs": out_r.numel() * 8 / (r_ms * 1e-3) / 1e9})
+            del out_r
 
     if rank != 0:
         return
 
     # ---- roofline of the dominant kernel (per launch, timed live with CUDA events in the library)
-    kernel = "fisher" if fisher_mode else ("loglike_tab" if tab_mode else ("loglike_mixed" if mixed_mode else "loglike"))
-    metric, unit = (FISHER_METRIC, FISHER_UNIT) if fisher_mode else (METRIC, UNIT)
-    peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * (clocks.get("sm_max_mhz") or 1965.0) * 1e6 / 1e12
+    sm_max = clocks.get("sm_max_mhz") or 1965.0
+    peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     dfma_tflops, _ = P.fp64_peak(8192, mode=0)
     dfma3_tflops, _ = P.fp64_peak(8192, mode=1)
-    n_det = len(wl.model.detectors)
-    kern_ms = main_ms / max(1, main_launches)                 # one launch = one detector, B x N (sample, bin) units
-    cmask = (2 if wl.model.mode_mask & 9 else 0) | (1 if wl.model.mode_mask & 2 else 0) | \
-            (4 if wl.model.mode_mask & 4 else 0) | (8 if wl.model.mode_mask & 16 else 0)
-    per_det = [FP64_OPS_PER_UNIT.get((kernel, d.kind, cmask)) for d in wl.model.detectors]
-    known = [o for o in per_det if o]
-    ops = {k: sum(o[k] for o in known) / len(known) for k in ("dfma", "dmul", "dadd")} if len(known) == n_det else None
-    if fisher_mode and args.grad_only:
-        ops = None                    # no ncu op counts for the gradient-only variant
-    roofline = {"bound": "alu", "kernel": f"{kernel}_kernel", "achieved": None, "peak": peak_tflops,
-                "unit": "TFLOP/s", "frac": None, "traffic": DRAM_TRAFFIC_PER_LAUNCH.get(args.config)}
-    if ops:
-        flop_per_unit = 2.0 * ops["dfma"] + ops["dmul"] + ops["dadd"]
-        inst_per_unit = ops["dfma"] + ops["dmul"] + ops["dadd"]
-        achieved = flop_per_unit * B * N / (kern_ms * 1e-3) / 1e12
-        # issue cost on the FP64 pipe (profiles/r01_fp64_operand_bandwidth.md): one 64-bit register operand
-        # per cycle and SM sub-partition, at least 2 cycles per instruction -> a DFMA with three distinct
-        # register operands takes 3 cycles.  The bound below charges every DFMA 3 cycles and DMUL/DADD 2.
-        cyc = 3.0 * ops["dfma"] + 2.0 * (ops["dmul"] + ops["dadd"])
-        t_operand = cyc * (B * N / 32.0) / (SM_COUNT * 4) / ((clocks.get("sm_max_mhz") or 1965.0) * 1e6)
-        roofline.update({
-            "achieved": achieved, "frac": achieved / peak_tflops,
-            "flop_per_unit": flop_per_unit, "unit_of_work": "(sample, bin, detector)",
-            "flop_per_launch": flop_per_unit * B * N,
-            "fma_share_of_fp64_instructions": ops["dfma"] / inst_per_unit,
-            "fp64_pipe_frac": inst_per_unit * B * N / (kern_ms * 1e-3) / (peak_tflops * 1e12 / 2.0),
-            "operand_bandwidth_bound_ms": t_operand * 1e3,
-            "frac_of_operand_bandwidth_bound": t_operand * 1e3 / kern_ms,
-        })
+    kern_ms = t["kernel_ms_total"] / max(1, t["kernel_launches"])   # one launch = one detector, B x N units
+    B_launch = B / world if strong else B
+    roofline = roofline_of(path, wl, B_launch, N, kern_ms, ops_doc, peak_tflops, sm_max, stale)
     roofline.update({
         "peak_source": "148 SM x 64 FP64 lanes x 2 flop x clocks.max.sm (DESIGN.md; no FP64 entry in "
                        "MEASURED_PEAKS.json); DFMA micro-benchmarks of this library alongside",
         "peak_dfma_measured": dfma_tflops, "peak_dfma_3reg_measured": dfma3_tflops,
         "frac_of_dfma_measured": (roofline["achieved"] / dfma_tflops) if roofline["achieved"] else None,
-        "kernel_ms": kern_ms, "kernel_launches": main_launches, "kernel_share_of_step": main_ms / elapsed_ms,
+        "kernel_launches": t["kernel_launches"], "kernel_share_of_step": t["kernel_ms_total"] / t["elapsed_ms"],
+        "csrc_hash": pbuild.csrc_hash(),
         "flop_basis": "FP64 operations of the reduced algorithm = executed 2*DFMA+DMUL+DADD per unit, averaged over "
-                      f"the detectors, ncu ({OPS_SOURCE})",
-        "hbm_gbs_achieved": (roofline["traffic"] / (kern_ms * 1e-3) / 1e9) if roofline["traffic"] else None,
+                      "the detectors, from the ncu captures listed in profiles/r02_ncu.md",
         "survey_estimate_flop_per_bin_eval": SURVEY_FLOP_PER_BIN_EVAL.get(args.config),
     })
 
     cpu_baseline = None
     if not args.no_cpu_baseline and world == 1:
-        rate, sec, cores, desc = oracle_timed(args.config, args.ref_samples, 1,
-                                              tab_nodes=args.tab_nodes if tab_mode else 0)
+        rate, sec, cores, desc = oracle_timed(args.config, path, args.ref_samples, 1, tab_nodes=args.tab_nodes)
         cpu_baseline = {"value": rate, "unit": unit, "cores": cores, "kind": "oracle", "sample": desc,
                         "value_one_thread": oracle_timed.one_thread}
 
     line = {
         "metric": metric, "value": value, "unit": unit, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f64+f32 (mixed: FP64 phases, FP32 geometry)" if mixed_mode else "f64", "data": "synthetic",
+        "ms_per_step": max_ms / args.steps, "higher_is_better": True, "scaling": args.scaling if world > 1 else "weak",
+        "vs_baseline": None,
+        "dtype": "f64+f32 (mixed: FP64 phases, FP32 geometry)" if path == "mixed" else "f64", "data": "synthetic",
         "bin_evals_per_sec": value * N,
-        "config": workload_config(wl, args, l2="256 MiB buffer rewritten before every step, inside the timed region"),
+        "config": workload_config(wl, args, path, l2="256 MiB buffer rewritten before every step, inside the timed region"),
         "clocks": clocks,
-        "e2e": {"value": e2e["full"], "unit": unit, "h2d_bytes_per_step": int(h2d),
-                "d2h_bytes_per_step": int(d2h), "steps": e2e_steps,
-                "api": ("pespace_session_set_data + pespace_session_loglike_tab per step: theta, the step's waveform "
-                        "tables, data set and PSD copied from pinned host memory, lnL read back" if tab_mode else
-                        "pespace_session_set_data + pespace_session_" + ("fisher" if fisher_mode else "loglike") +
-                        " per step: theta, data set and PSD copied from pinned host memory, result read back"),
-                "precision_note": "pespace_session_loglike_mixed" if mixed_mode else None,
-                "value_resident_data": e2e["resident"],
+        "e2e": {"value": e2e["full"], "unit": unit, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+                "steps": e2e_steps, "api": e2e_api, "value_resident_data": e2e["resident"],
                 "resident_data_note": "same call with the data set copied once (sampler use): theta in, result out"},
-        "gpu_launches": int(launches),
+        "gpu_launches": int(t["launches"]),
         "roofline": roofline,
         "cpu_baseline": cpu_baseline,
         "result_check": {"min": float(last.min()), "max": float(last.max())},
+        "other_configs": others,
         "response": response_info,
     }
     print(json.dumps(line), flush=True)
@@ -450,19 +552,32 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["ours", "reference"], default="ours")
     ap.add_argument("--config", type=int, default=2, choices=[2, 3, 4, 5])
-    ap.add_argument("--precision", choices=["f64", "mixed"], default="f64",
-                    help="mixed: pespace_loglike_mixed (FP64 phases, FP32 geometry; SURVEY 8(f) N2) in the device-timed leg")
+    ap.add_argument("--path", choices=sorted(UNITS), default=None,
+                    help="entry point to time (default: loglike; config 5: fisher)")
+    ap.add_argument("--precision", choices=["f64", "mixed"], default="f64", help="mixed = --path mixed")
+    ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic", help="tab = --path tab")
+    ap.add_argument("--grad-only", action="store_true", help="config 5: forward-mode gradient only (= --path fisher-grad)")
+    ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
+                    help="N > 1: weak = one batch of B per rank; strong = one global batch of B split over the ranks")
     ap.add_argument("--response", action="store_true", help="also time pespace_response on a slice of the batch")
     ap.add_argument("--response-batch", type=int, default=256)
-    ap.add_argument("--grad-only", action="store_true",
-                    help="config 5: d lnL / d theta only (pespace_fisher with d_out_F = NULL)")
-    ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic",
-                    help="tab: pespace_loglike_tab on synthetic tabulated mode waveforms (SURVEY 8(f) N1)")
     ap.add_argument("--tab-nodes", type=int, default=4096, help="nodes K of the waveform tables")
     ap.add_argument("--ref-samples", type=int, default=None,
                     help="samples per oracle pass (default: sized for ~15 s of CPU work)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-others", dest="others", action="store_false",
+                    help="skip the short runs of the other configs / calls (other_configs, response)")
     args = ap.parse_args()
+    if args.path is None:
+        if args.precision == "mixed":
+            args.path = "mixed"
+        elif args.waveform == "tab":
+            args.path = "tab"
+        elif args.grad_only:
+            args.path = "fisher-grad"
+    # the extra short runs belong to the default invocation (the driver's command line) only
+    if args.config != 2 or args.path not in (None, "loglike") or args.scaling != "weak":
+        args.others = False
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3
     if args.impl == "reference":

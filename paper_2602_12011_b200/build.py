@@ -20,6 +20,18 @@ NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", 
               "-Xcompiler", "-fPIC", "--fmad=true", "-Xptxas", "-v"] + os.environ.get("PESPACE_NVCC_EXTRA", "").split()
 
 
+def csrc_hash() -> str:
+    """sha256 over the names and contents of the CUDA sources and the public headers: the stamp that ties
+    profiles/*_ops.json (ncu operation counts) to the kernels they were counted on (bench.py: roofline.stale)."""
+    import hashlib
+    h = hashlib.sha256()
+    for path in sorted(DEPS):
+        h.update(os.path.basename(path).encode())
+        h.update(b"\0")
+        h.update(open(path, "rb").read())
+    return h.hexdigest()[:16]
+
+
 def nvcc() -> str:
     cand = os.path.join(os.environ.get("CUDA_HOME", "/usr/local/cuda"), "bin", "nvcc")
     return cand if os.path.exists(cand) else "nvcc"

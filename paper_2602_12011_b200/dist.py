@@ -93,8 +93,8 @@ class ShardedLikelihood:
         import torch
         import torch.distributed as dist
         B = params.shape[0]
-        if not (dist.is_available() and dist.is_initialized()) or dist.get_world_size() == 1:
-            return self.local_eval(params)
+        if not (dist.is_available() and dist.is_initialized()):
+            return self.local_eval(params)          # (a one-rank group still takes the all-gather path below)
         rank, world = dist.get_rank(), dist.get_world_size()
         lo, hi = shard_bounds(B, rank, world)
         per = -(-B // world)

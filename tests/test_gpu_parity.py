@@ -426,3 +426,32 @@ def test_fisher_full_size_sampled_parity(P):
     wl = W.config(5)
     data, psd = wl.data(oracle_response_fn), wl.psd()
     check_fisher(P, wl, data, psd, subset=[0, 85, 170, 255])
+
+
+# ------------------------------------------------------------------ multi-GPU plumbing on one GPU
+def test_sharded_likelihood_with_the_real_binding_under_nccl(P):
+    """dist.ShardedLikelihood driving binding.Likelihood inside a one-rank NCCL group (the all-gather path is taken
+    even at world size 1): bit-identical to the plain call.  This is as far as one GPU goes; the world-size-2 host
+    logic is covered on gloo (tests/test_dist_gloo.py)."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_2602_12011_b200 import dist as pdist
+    wl = W.config(3, B=70, N=3000)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    lik = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    plain = lik(dev(wl.params)).cpu().numpy()
+    with socket.socket() as s:
+        s.bind(("127.0.0.1", 0))
+        port = s.getsockname()[1]
+    assert not dist.is_initialized()
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
+    try:
+        sharded = pdist.ShardedLikelihood(lambda p: lik(p))
+        got = sharded(dev(wl.params)).cpu().numpy()
+        assert np.array_equal(got, plain)
+        t_max, units = pdist.aggregate(12.5, wl.B, torch.device("cuda", torch.cuda.current_device()))
+        assert t_max == 12.5 and units == wl.B
+        assert np.array_equal(pdist.gather_lnL(plain, torch.device("cuda", torch.cuda.current_device())), plain)
+    finally:
+        dist.destroy_process_group()
