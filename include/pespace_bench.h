@@ -17,7 +17,10 @@ extern "C" {
  *   mode 0: a = a*m + c with m, c shared by the chains (two register operands per DFMA):
  *           the FP64 pipe peak, 1 warp-instruction / 2 cycles / SM sub-partition;
  *   mode 1: a = a*b + c with three distinct register operands per DFMA: the register-file
- *           read bandwidth then limits the pipe to 1 / 3 cycles (profiles/r01_fp64_operand_bandwidth.md). */
+ *           read bandwidth then limits the pipe to 1 / 3 cycles (profiles/r01_fp64_operand_bandwidth.md);
+ *   modes 2-5: FP64 tensor-core probe, `iters` blocks of 8 x NACC mma.sync.m8n8k4.f64 (DMMA, 256 FMAs per warp
+ *           instruction) per warp: 2: NACC = 8 independent accumulators; 3: NACC = 2; 4: NACC = 8 with one
+ *           independent DFMA per DMMA interleaved; 5: with four (profiles/r02_dmma.md). */
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms);
 
 /* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel

@@ -209,7 +209,7 @@ int pespace::host::loglike_impl(const double* d_params, int64_t B, const double*
 extern "C" {
 
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms) {
-  if (iters <= 0 || !h_out_tflops || (mode != 0 && mode != 1)) return PESPACE_EINVAL;
+  if (iters <= 0 || !h_out_tflops || mode < 0 || mode > 5) return PESPACE_EINVAL;
   int dev = 0, sms = 0;
   CU(cudaGetDevice(&dev));
   CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -223,7 +223,11 @@ int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_m
   const int blocks = sms * 8, threads = 256;
   auto go = [&](int n) {
     if (mode == 0) dfma_peak_kernel<false><<<blocks, threads>>>(n, d_in, d_out);
-    else dfma_peak_kernel<true><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 1) dfma_peak_kernel<true><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 2) dmma_peak_kernel<8, 0><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 3) dmma_peak_kernel<2, 0><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 4) dmma_peak_kernel<8, 1><<<blocks, threads>>>(n, d_in, d_out);
+    else dmma_peak_kernel<8, 4><<<blocks, threads>>>(n, d_in, d_out);
     ++g_launches;
   };
   go(iters / 8 + 1);   // warm-up
@@ -233,7 +237,11 @@ int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_m
   CU(cudaEventSynchronize(e1));
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, e0, e1));
-  const double flops = 2.0 * 64.0 * (double)iters * (double)blocks * (double)threads;
+  // per thread and iteration: modes 0, 1: 64 DFMAs; modes 2-5: 8 x NACC DMMAs of 256 FMAs per warp (8 per thread) plus
+  // DFMA_MIX DFMAs per DMMA
+  const double fma_per_thread_iter = mode <= 1 ? 64.0 : mode == 2 ? 8.0 * 8 * 8 : mode == 3 ? 8.0 * 2 * 8
+                                     : mode == 4 ? 8.0 * 8 * (8 + 1) : 8.0 * 8 * (8 + 4);
+  const double flops = 2.0 * fma_per_thread_iter * (double)iters * (double)blocks * (double)threads;
   *h_out_tflops = flops / (ms * 1e-3) / 1e12;
   if (h_out_ms) *h_out_ms = ms;
   cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(d_in); cudaFree(d_out);

@@ -818,4 +818,36 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, const double*
   if (r == 12345.678) out[0] = r;   // never true; keeps the chains alive
 }
 
+// FP64 tensor-core probe: chains of mma.sync.aligned.m8n8k4 (DMMA, 8 x 8 x 4 = 256 FMAs per warp instruction) on NACC
+// independent accumulator fragments per warp; DFMA_MIX > 0 interleaves that many independent DFMAs per DMMA, to see
+// whether the two share the FP64 issue port (profiles/r02_dmma.md)
+template <int NACC, int DFMA_MIX>
+__global__ void __launch_bounds__(256) dmma_peak_kernel(int iters, const double* __restrict__ in,
+                                                        double* __restrict__ out) {
+  double c0[NACC], c1[NACC], x[DFMA_MIX > 0 ? DFMA_MIX : 1];
+  const double a = in[threadIdx.x & 63], b = in[(threadIdx.x + 7) & 63];
+#pragma unroll
+  for (int j = 0; j < NACC; ++j) { c0[j] = in[(threadIdx.x + j) & 63]; c1[j] = in[(threadIdx.x + 2 * j + 1) & 63]; }
+#pragma unroll
+  for (int j = 0; j < (DFMA_MIX > 0 ? DFMA_MIX : 1); ++j) x[j] = in[(threadIdx.x + 3 * j) & 63];
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int r = 0; r < 8; ++r) {
+#pragma unroll
+      for (int j = 0; j < NACC; ++j) {
+        asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0, %1}, {%2}, {%3}, {%0, %1};"
+                     : "+d"(c0[j]), "+d"(c1[j]) : "d"(a), "d"(b));
+#pragma unroll
+        for (int q = 0; q < DFMA_MIX; ++q) x[q] = fma(x[q], a, b);
+      }
+    }
+  }
+  double r = 0.0;
+#pragma unroll
+  for (int j = 0; j < NACC; ++j) r += c0[j] + c1[j];
+#pragma unroll
+  for (int j = 0; j < (DFMA_MIX > 0 ? DFMA_MIX : 1); ++j) r += x[j];
+  if (r == 12345.678) out[0] = r;   // never true; keeps the chains alive
+}
+
 }  // namespace pespace
