@@ -53,6 +53,8 @@ def lib():
         L.pespace_oracle_response_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, i64, C.POINTER(_Model), dp]
         L.pespace_oracle_loglike_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, dp, C.POINTER(_Grid),
                                                  C.POINTER(_Model), dp]
+        L.pespace_oracle_fisher_tab.argtypes = [dp, i64, i64, dp, dp, dp, dp, dp, dp, C.POINTER(_Grid),
+                                                C.POINTER(_Model), dp, dp]
         L.pespace_oracle_tab_waveform.argtypes = [i64, dp, dp, dp, dp, dp, i64, dp, dp, dp]
         dbl = C.c_double
         L.pespace_oracle_response_orb.argtypes = [dp, i64, i64, dbl, dbl, dp, dp, dp, i64, C.POINTER(_Model), dp]
@@ -174,6 +176,23 @@ def loglike_tab(params, table, data, psd, grid, model) -> np.ndarray:
     _check(lib().pespace_oracle_loglike_tab(_dp(p), B, K, _dp(fn), _dp(a), _dp(ph), _dp(tf), _dp(d), _dp(s), C.byref(g),
                                             C.byref(m), _dp(out)), "loglike_tab")
     return out
+
+
+def fisher_tab(params, table, data, psd, grid, model):
+    """T1 x O12: -> (F [B][11][11], grad [B][11] or None when data is None); rows / columns 0-3 are 0"""
+    p = _f64(np.atleast_2d(params))
+    s = _f64(psd)
+    m, keep = _model(model)
+    g = _Grid(float(grid.f0), float(grid.df), int(grid.N))
+    B = p.shape[0]
+    fn, a, ph, tf, K = _table(table, B, model)
+    F = np.empty((B, NPAR, NPAR), dtype=np.float64)
+    d = None if data is None else np.ascontiguousarray(data, dtype=np.complex128).view(np.float64)
+    grad = None if data is None else np.empty((B, NPAR), dtype=np.float64)
+    _check(lib().pespace_oracle_fisher_tab(_dp(p), B, K, _dp(fn), _dp(a), _dp(ph), _dp(tf), None if d is None else _dp(d),
+                                           _dp(s), C.byref(g), C.byref(m), _dp(F), None if grad is None else _dp(grad)),
+           "fisher_tab")
+    return F, grad
 
 
 def tab_waveform(fnodes, amp, phase, tf, freqs):

@@ -576,23 +576,26 @@ bool table_ok(const WaveTable& W) {
   return W.fn[0] > 0.0;
 }
 
-// A, E, T of one detector at one frequency from the tables, summed over the modes of the mask
-void response_bin_tab(const WaveTable& W, int64_t b, const double* th, const Frame<double>& F, double f,
-                      uint32_t mode_mask, const pespace_oracle_detector& D, Cx<double> AET[3]) {
-  for (int c = 0; c < 3; ++c) AET[c] = cx<double>(0.0, 0.0);
-  const double DL = th[4], iota = th[5], phic = th[6], tc = th[10];
+// A, E, T of one detector at one frequency from the tables, summed over the modes of the mask.  T = double, or
+// Dual<11> for the derivatives w.r.t. the parameters this path uses (D_L, iota, phi_c, lambda, beta, psi, t_c): the
+// table values are plain numbers, theta and the frame carry the tangents.
+template <class T>
+void response_bin_tab(const WaveTable& W, int64_t b, const T* th, const Frame<T>& F, double f,
+                      uint32_t mode_mask, const pespace_oracle_detector& D, Cx<T> AET[3]) {
+  for (int c = 0; c < 3; ++c) AET[c] = cx<T>(T(0.0), T(0.0));
+  const T DL = th[4], iota = th[5], phic = th[6], tc = th[10];
   int imode = 0;
   for (int im = 0; im < 5; ++im) {
     if (!(mode_mask & (1u << im))) continue;
     const int l = MODE_TABLE[im].l, m = MODE_TABLE[im].m;
     double a, p, t;
     if (tab_waveform(W, b, imode, f, &a, &p, &t)) {
-      const double amp = a / DL;
-      const double psi = p + 2.0 * K<double>::pi() * f * tc - (double)m * phic;
-      const double tf = t + tc;
-      Cx<double> y[6], XYZ[3], ch[3];
+      const T amp = T(a) / DL;
+      const T psi = T(p) + T(2.0) * K<T>::pi() * T(f) * tc - T((double)m) * phic;
+      const T tf = T(t) + tc;
+      Cx<T> y[6], XYZ[3], ch[3];
       links_from_waveform(iota, F, l, m, f, amp, psi, tf, D, y);
-      tdi_xyz(y, f, D.L_m, D.tdi_gen, XYZ);
+      tdi_xyz(y, T(f), D.L_m, D.tdi_gen, XYZ);
       aet(XYZ, ch);
       for (int c = 0; c < 3; ++c) AET[c] = AET[c] + ch[c];
     }
@@ -600,8 +603,8 @@ void response_bin_tab(const WaveTable& W, int64_t b, const double* th, const Fra
   }
 }
 
-Frame<double> tab_frame(const double* th) {
-  Source<double> s = Source<double>();
+template <class T> Frame<T> tab_frame(const T* th) {
+  Source<T> s = Source<T>();
   s.lam = th[7]; s.bet = th[8]; s.psi = th[9];
   return make_frame(s);
 }
@@ -690,6 +693,61 @@ int pespace_oracle_loglike_tab(const double* params, int64_t B, int64_t K, const
         }
       }
     out_lnL[b] = (double)(-0.5L * 4.0L * (long double)grid->df * sum);
+  }
+  return 0;
+}
+
+// T1 x O12: F_ij and grad_i with tabulated mode waveforms (the paper's own Fisher use: the waveform is
+// fixed and the derivatives are taken w.r.t. extrinsic parameters).  Derivatives w.r.t. the raw theta entries the
+// tabulated path uses (D_L, iota, phi_c, lambda, beta, psi, t_c); rows and columns of M, q, chi1, chi2 are exactly 0.
+int pespace_oracle_fisher_tab(const double* params, int64_t B, int64_t K, const double* fnodes, const double* amp,
+                              const double* phase, const double* tf, const double* data, const double* psd,
+                              const pespace_oracle_grid* grid, const pespace_oracle_model* model, double* out_F,
+                              double* out_grad) {
+  if (!params || !psd || !out_F || B <= 0 || !grid_ok(grid) || !model_ok(model)) return -1;
+  const WaveTable W = {K, fnodes, amp, phase, tf, popcount5(model->mode_mask)};
+  if (!table_ok(W)) return -1;
+  typedef Dual<NPAR> D11;
+  const int nd = model->n_det;
+  const int64_t N = grid->N;
+  const double nan = std::numeric_limits<double>::quiet_NaN();
+#pragma omp parallel for schedule(dynamic, 1) num_threads(g_threads > 0 ? g_threads : omp_get_max_threads())
+  for (int64_t b = 0; b < B; ++b) {
+    const double* th0 = params + b * NPAR;
+    double* Fb = out_F + b * NPAR * NPAR;
+    double* gb = (out_grad && data) ? out_grad + b * NPAR : nullptr;
+    if (!tab_sample_ok(th0)) {
+      for (int i = 0; i < NPAR * NPAR; ++i) Fb[i] = nan;
+      if (gb) for (int i = 0; i < NPAR; ++i) gb[i] = nan;
+      continue;
+    }
+    D11 th[NPAR];
+    for (int i = 0; i < NPAR; ++i) { th[i] = D11(th0[i]); th[i].d[i] = 1.0; }  // identity seed (M, q, chi: unused)
+    const Frame<D11> F = tab_frame(th);
+    long double accF[NPAR][NPAR] = {}, accg[NPAR] = {};
+    for (int d = 0; d < nd; ++d)
+      for (int64_t k = 0; k < N; ++k) {
+        const double f = std::fma((double)k, grid->df, grid->f0);
+        Cx<D11> h[3];
+        response_bin_tab(W, b, th, F, f, model->mode_mask, model->det[d], h);
+        for (int c = 0; c < 3; ++c) {
+          const size_t idx = ((size_t)d * 3 + c) * N + k;
+          const double S = psd[idx];
+          if (!weight_ok(S)) continue;
+          const long double w = 1.0L / (long double)S;
+          for (int i = 0; i < NPAR; ++i)
+            for (int j = i; j < NPAR; ++j)
+              accF[i][j] += w * (long double)(h[c].re.d[i] * h[c].re.d[j] + h[c].im.d[i] * h[c].im.d[j]);
+          if (gb) {
+            const double rr = data[2 * idx] - h[c].re.v, ri = data[2 * idx + 1] - h[c].im.v;
+            for (int i = 0; i < NPAR; ++i) accg[i] += w * (long double)(rr * h[c].re.d[i] + ri * h[c].im.d[i]);
+          }
+        }
+      }
+    const long double norm = 4.0L * (long double)grid->df;
+    for (int i = 0; i < NPAR; ++i)
+      for (int j = i; j < NPAR; ++j) Fb[i * NPAR + j] = Fb[j * NPAR + i] = (double)(norm * accF[i][j]);
+    if (gb) for (int i = 0; i < NPAR; ++i) gb[i] = (double)(norm * accg[i]);
   }
   return 0;
 }

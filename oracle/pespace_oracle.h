@@ -74,6 +74,13 @@ int pespace_oracle_loglike_tab(const double* params, int64_t B, int64_t K, const
                                const double* amp, const double* phase, const double* tf,
                                const double* data_AET, const double* psd, const pespace_oracle_grid* grid,
                                const pespace_oracle_model* model, double* out_lnL);
+/* T1 x O12: Fisher matrix and gradient with tabulated mode waveforms; derivatives w.r.t. the theta entries this path
+ * uses (D_L, iota, phi_c, lambda, beta, psi, t_c), rows / columns of M, q, chi1, chi2 exactly 0.  out_grad may be
+ * NULL; skipped if data_AET is NULL. */
+int pespace_oracle_fisher_tab(const double* params, int64_t B, int64_t K, const double* fnodes,
+                              const double* amp, const double* phase, const double* tf, const double* data_AET,
+                              const double* psd, const pespace_oracle_grid* grid, const pespace_oracle_model* model,
+                              double* out_F, double* out_grad);
 /* the interpolants of ONE (sample, mode) table at freqs[N]; NaN outside the table */
 int pespace_oracle_tab_waveform(int64_t K, const double* fnodes, const double* amp, const double* phase,
                                 const double* tf, const double* freqs, int64_t N, double* out_amp,

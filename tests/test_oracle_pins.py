@@ -843,3 +843,51 @@ def test_T2_response_and_likelihood_with_dense_tables_match_the_analytic_path():
     h = oracle.response_orb(th, tab, fg, model)
     brute = -0.5 * 4.0 * grid.df * (np.abs(data[None] - h) ** 2 / psd[None]).sum(axis=(1, 2, 3))
     assert np.allclose(oracle.loglike_orb(th, tab, data, psd, grid, model), brute, rtol=1e-12, atol=0)
+
+
+# ------------------------------------------------------------------ T1 x O12: Fisher matrix on tabulated waveforms
+@pytest.mark.parametrize("mask,dets", [(1, (LISA,)), (31, (LISA, TQ))])
+def test_T1_fisher_tab_vs_richardson_finite_differences_and_closed_forms(mask, dets):
+    """oracle.fisher_tab (dual numbers through the tabulated path) against Richardson-extrapolated central differences
+    of oracle.response_tab, the D_L / phi_c closed forms, and exact zeros for the parameters the path ignores"""
+    grid, model = small_workload(mask=mask, dets=dets, N=384)
+    f = grid.freqs()
+    psd = np.stack([W.psd_aet(x, f) for x in model.detectors])
+    th = THETA.copy(); th[10] = 3.0e5; th[1] = 2.5
+    table = W.table_from_waveform_fn(th[None], mask, W.log_nodes(f[0], f[-1], 300), oracle.waveform)
+    h = oracle.response_tab(th, table, f, model)[0]
+    d = h + W.coloured_noise(psd, grid.df, np.random.default_rng(3))
+    F, grad = oracle.fisher_tab(th, table, d, psd, grid, model)
+    F, grad = F[0], grad[0]
+    used = [4, 5, 6, 7, 8, 9, 10]
+
+    def dh_tab(j):
+        est = []
+        for div in (1.0, 2.0, 4.0):
+            st = FD_STEPS[j] / div
+            tp, tm = th.copy(), th.copy()
+            tp[j] += st; tm[j] -= st
+            est.append((oracle.response_tab(tp, table, f, model)[0] - oracle.response_tab(tm, table, f, model)[0]) / (2 * st))
+        r1 = [(4 * est[1] - est[0]) / 3, (4 * est[2] - est[1]) / 3]
+        return (16 * r1[1] - r1[0]) / 15
+
+    dh = {j: dh_tab(j) for j in used}
+    hh = inner(h, h, psd, grid.df)
+    for i in used:
+        assert grad[i] == pytest.approx(inner(d - h, dh[i], psd, grid.df), rel=1e-6, abs=1e-6 * math.sqrt(F[i, i]) * math.sqrt(hh))
+        for j in used:
+            assert F[i, j] == F[j, i]
+            assert abs(F[i, j] - inner(dh[i], dh[j], psd, grid.df)) <= 1e-6 * math.sqrt(F[i, i] * F[j, j])
+    assert np.all(F[:4, :] == 0) and np.all(F[:, :4] == 0) and np.all(grad[:4] == 0)       # M, q, chi1, chi2: ignored
+    assert F[4, 4] == pytest.approx(hh / th[4] ** 2, rel=1e-12)
+    assert grad[4] == pytest.approx(-inner(d - h, h, psd, grid.df) / th[4], rel=1e-9)
+    if mask == 1:                                   # (2,2) only: d h / d phi_c = 2 i h
+        assert F[6, 6] == pytest.approx(4 * hh, rel=1e-12)
+        assert abs(F[6, 4]) <= 1e-12 * math.sqrt(F[6, 6] * F[4, 4])
+    F2, g2 = oracle.fisher_tab(th, table, None, psd, grid, model)
+    assert g2 is None and np.array_equal(F2[0], F)
+    # on tables of the analytic modes the extrinsic block approaches the analytic path's (fourth order in the spacing)
+    Fa, _ = oracle.fisher(th, d, psd, grid, model)
+    ix = np.ix_(used, used)
+    dd = np.sqrt(np.diag(Fa[0]))[used]
+    assert (np.abs(F[ix] - Fa[0][ix]) / np.outer(dd, dd)).max() <= 1e-5
