@@ -156,6 +156,17 @@ int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetab
                         const pespace_model* model, double* d_out_lnL, void* d_workspace,
                         size_t workspace_bytes, void* stream);
 
+/* Fisher matrix and gradient on tabulated mode waveforms (T1 x S10).  This is the paper's own Fisher use: the waveform
+ * is fixed and F is taken over extrinsic parameters (PAPER.md:207; Fig. 3 design, :193).  Outputs as pespace_fisher
+ * (F [B][11][11] symmetric full storage, grad [B][11] = <d - h | d_i h>, derivatives w.r.t. the raw theta entries); the
+ * tabulated path depends on D_L, iota, phi_c, lambda, beta, psi, t_c only, so the rows and columns of M, q, chi1, chi2
+ * are exactly 0.  d_data_AET may be NULL (then d_out_grad must be NULL); d_out_F may be NULL (gradient only).
+ * Workspace: pespace_workspace_bytes_fisher_tab. */
+size_t pespace_workspace_bytes_fisher_tab(int64_t B, const pespace_grid* grid, const pespace_model* model);
+int pespace_fisher_tab(const double* d_params, int64_t B, const pespace_wavetable* table, const double* d_data_AET,
+                       const double* d_psd, const pespace_grid* grid, const pespace_model* model, double* d_out_F,
+                       double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream);
+
 /* ---- Tabulated numerical orbits ("Support for high-precision numerical orbits will
  * be extended in future work").  The spacecraft positions at t_lm(f) (Eq. 4, 5) are read from tables instead of the
  * analytic Keplerian orbits: d_pos [n_det][K][3 spacecraft][3] in metres and d_vel [n_det][K][3][3] in m/s on the

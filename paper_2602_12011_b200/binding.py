@@ -18,7 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_loglike_mixed", "pespace_workspace_bytes_grad", "pespace_loglike_grad",
-           "pespace_session_loglike_grad", "pespace_response_orb", "pespace_loglike_orb", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
+           "pespace_session_loglike_grad", "pespace_response_orb", "pespace_loglike_orb",
+           "pespace_workspace_bytes_fisher_tab", "pespace_fisher_tab", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
            "pespace_session_fisher", "pespace_session_loglike_tab", "pespace_session_destroy",
            "pespace_loglike_host", "pespace_fp64_peak", "pespace_profile_enable", "pespace_profile_read",
@@ -73,6 +74,10 @@ def _load():
     L.pespace_workspace_bytes_grad.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
     L.pespace_workspace_bytes_grad.restype = sz
     L.pespace_loglike_grad.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
+    L.pespace_workspace_bytes_fisher_tab.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
+    L.pespace_workspace_bytes_fisher_tab.restype = sz
+    L.pespace_fisher_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp,
+                                     vp, sz, vp]
     L.pespace_response_orb.argtypes = [vp, i64, C.POINTER(_OrbitTable), vp, i64, C.POINTER(_Model), vp, vp]
     L.pespace_loglike_orb.argtypes = [vp, i64, C.POINTER(_OrbitTable), vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp,
                                       vp, sz, vp]
@@ -291,6 +296,37 @@ class Fisher:
                                    None if self.data is None else _dev(out_grad, "out_grad").data_ptr(),
                                    self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_fisher")
         return out_F, (out_grad if self.data is not None else None)
+
+
+class FisherTab(Fisher):
+    """pespace_fisher_tab: Fisher matrix / gradient on tabulated mode waveforms (extrinsic parameters)."""
+
+    def __init__(self, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model, max_batch: int):
+        super().__init__(data, psd, grid, model, max_batch)
+        self.ws_bytes = int(_lib.pespace_workspace_bytes_fisher_tab(max_batch, C.byref(self._g), C.byref(self._m)))
+        self.ws = torch.empty(max(self.ws_bytes, 16), dtype=torch.uint8, device=self.psd.device)
+
+    def __call__(self, params: torch.Tensor, table: WaveTable, grad_only: bool = False):
+        """-> (F or None, grad or None)"""
+        p = _dev(params, "params")
+        B = p.shape[0]
+        if B > self.max_batch:
+            raise PespaceError("batch larger than the workspace was sized for")
+        table.check(B, self.model)
+        if grad_only and self.data is None:
+            raise PespaceError("the gradient needs the data set")
+        F = None if grad_only else torch.empty((B, NPAR, NPAR), dtype=torch.float64, device=p.device)
+        g = None if self.data is None else torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+        _check(_lib.pespace_fisher_tab(p.data_ptr(), B, C.byref(table.c), None if self.data is None else self.data.data_ptr(),
+                                       self.psd.data_ptr(), C.byref(self._g), C.byref(self._m),
+                                       None if F is None else F.data_ptr(), None if g is None else g.data_ptr(),
+                                       self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_fisher_tab")
+        return F, g
+
+
+def fisher_tab(params: torch.Tensor, table: WaveTable, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):
+    """-> (F [B][11][11], grad [B][11] or None) on tabulated mode waveforms"""
+    return FisherTab(data, psd, grid, model, params.shape[0])(params, table)
 
 
 def fisher(params: torch.Tensor, data: Optional[torch.Tensor], psd: torch.Tensor, grid, model):

@@ -178,12 +178,22 @@ __device__ __forceinline__ void jadd(bool first, double* J, int p, int comp, dou
 // Tangent order p = 1..11 follows theta: M, q, chi1, chi2, D_L, iota, phi_c, lambda, beta, psi, t_c
 // (D_L is filled in after the class loop: d h / d D_L = -h / D_L).
 template <int KIND>
+__device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const ClassScal& cs, const BinC& bc,
+                                                const double* __restrict__ sc, const DetC& dc, double* __restrict__ J);
+
+template <int KIND>
 __device__ __forceinline__ void fisher_class(int MC, bool FIRST, const BinC& bc, const double* __restrict__ sc,
                                           const DetC& dc, double ftc4, double* __restrict__ J) {
-  using G = Du<3>;
-  const double MMmc = (double)(MC + 1);
   ClassScal cs;
   fisher_stage_a(MC, bc, sc, ftc4, cs);
+  fisher_class_cs<KIND>((double)(MC + 1), FIRST, cs, bc, sc, dc, J);
+}
+
+// S4-S7 and the tangent assembly of one class (or one tabulated mode) from its phase-like scalars cs; MMmc = m
+template <int KIND>
+__device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const ClassScal& cs, const BinC& bc,
+                                                const double* __restrict__ sc, const DetC& dc, double* __restrict__ J) {
+  using G = Du<3>;
 
   // ---- S4 on (value, d/d alpha [rad], d/d lambda, d/d beta)
   G G1k, G2k, G1u, G2u, G1v, G2v, kR;

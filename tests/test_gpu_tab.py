@@ -179,3 +179,96 @@ def test_tab_session_matches_device_call(P):
     with pytest.raises(P.PespaceError):
         ses.loglike_tab(wl.params, bad)
     ses.close()
+
+
+# ------------------------------------------------------------------ T1 x S10: Fisher matrix / gradient on tables
+TOL_F = 1e-9
+USED = [4, 5, 6, 7, 8, 9, 10]            # D_L, iota, phi_c, lambda, beta, psi, t_c
+
+
+def check_fisher_tab(P, params, table, data, psd, grid, model, with_grad=True):
+    F, g = P.fisher_tab(dev(params), dev_table(P, table), dev(data) if with_grad else None, dev(psd), grid, model)
+    F = F.cpu().numpy()
+    Fo, go = oracle.fisher_tab(params, table, data if with_grad else None, psd, grid, model)
+    assert np.all(F[:, :4, :] == 0) and np.all(F[:, :, :4] == 0)          # M, q, chi1, chi2: not parameters of this path
+    ix = np.ix_(range(params.shape[0]), USED, USED)
+    d = np.sqrt(np.einsum("bii->bi", Fo[ix]))
+    assert np.all(d > 0)
+    errF = np.abs(F[ix] - Fo[ix]) / (d[:, :, None] * d[:, None, :])
+    assert errF.max() <= TOL_F, errF.max()
+    assert np.array_equal(F, F.transpose(0, 2, 1))
+    if with_grad:
+        g = g.cpu().numpy()
+        assert np.all(g[:, :4] == 0)
+        rr = -2.0 * oracle.loglike_tab(params, table, data, psd, grid, model)
+        errg = np.abs(g[:, USED] - go[:, USED]) / (d * np.sqrt(rr)[:, None])
+        assert errg.max() <= TOL_F, errg.max()
+    else:
+        assert g is None
+    return F
+
+
+@pytest.mark.parametrize("idx,B,N,K", [(2, 11, 5000, 700), (3, 6, 2100, 500), (4, 9, 1100, 900)])
+def test_fisher_tab_reduced_configs(P, idx, B, N, K):
+    """several chunks and blocks, ragged tails; tables of the oracle's analytic modes; with and without data"""
+    wl = W.config(idx, B=B, N=N)
+    f = wl.grid.freqs()
+    wl.params[0] = wl.theta_inj
+    table = W.table_from_waveform_fn(wl.params, wl.model.mode_mask, W.log_nodes(f[0], f[-1], K), oracle.waveform)
+    data, psd = noisy_data(wl, table)
+    check_fisher_tab(P, wl.params, table, data, psd, wl.grid, wl.model)
+    check_fisher_tab(P, wl.params, table, data, psd, wl.grid, wl.model, with_grad=False)
+
+
+@pytest.mark.parametrize("gen", [15, 20])
+def test_fisher_tab_random_sky_synthetic_tables(P, gen):
+    rng = np.random.default_rng(6)
+    th = W.draw_prior(7, 4e5, rng)
+    dets = (W.lisa_like(gen), W.taiji_like(gen), W.tianqin_like(gen))
+    model = W.Model(W.MODES_HM, dets)
+    grid = W.Grid(2e-4, 3.1e-5, 600)
+    f = grid.freqs()
+    table = W.chirp_table(th, model.mode_mask, W.log_nodes(1.5 * f[0], 0.8 * f[-1], 200))     # band-limited tables
+    wl = W.Workload("random", grid, model, th, th[2].copy(), 31)
+    data, psd = noisy_data(wl, table)
+    check_fisher_tab(P, th, table, data, psd, grid, model)
+
+
+def test_fisher_tab_gradient_only_edge_cases_and_determinism(P):
+    wl = W.config(4, B=6, N=700)
+    f = wl.grid.freqs()
+    table = W.table_from_waveform_fn(wl.params, wl.model.mode_mask, W.log_nodes(f[0], f[-1], 300), oracle.waveform)
+    data, psd = noisy_data(wl, table)
+    fis = P.FisherTab(dev(data), dev(psd), wl.grid, wl.model, wl.B)
+    F, g = fis(dev(wl.params), dev_table(P, table))
+    none, g1 = fis(dev(wl.params), dev_table(P, table), grad_only=True)
+    assert none is None
+    Fo, go = oracle.fisher_tab(wl.params, table, data, psd, wl.grid, wl.model)
+    d = np.sqrt(np.einsum("bii->bi", Fo[:, 4:, 4:]))
+    rr = -2.0 * oracle.loglike_tab(wl.params, table, data, psd, wl.grid, wl.model)
+    assert (np.abs(g1.cpu().numpy()[:, 4:] - go[:, 4:]) / (d * np.sqrt(rr)[:, None])).max() <= TOL_F
+    F2, g2 = fis(dev(wl.params), dev_table(P, table))
+    assert np.array_equal(F.cpu().numpy(), F2.cpu().numpy()) and np.array_equal(g.cpu().numpy(), g2.cpu().numpy())
+    th = wl.params.copy(); th[1, 4] = -1.0; th[3, 9] = np.nan; th[4, 0] = np.nan      # M is ignored: sample 4 stays valid
+    Fb, gb = fis(dev(th), dev_table(P, table))
+    Fb, gb = Fb.cpu().numpy(), gb.cpu().numpy()
+    assert np.all(np.isnan(Fb[[1, 3]])) and np.all(np.isnan(gb[[1, 3]])) and np.all(np.isfinite(Fb[[0, 2, 4, 5]]))
+    with pytest.raises(P.PespaceError):
+        P.FisherTab(None, dev(psd), wl.grid, wl.model, wl.B)(dev(wl.params), dev_table(P, table), grad_only=True)
+
+
+def test_fisher_tab_full_size_sampled(P):
+    """config 5's workload (three detectors, five modes, N = 262144) at B = 64 on tables; oracle on 3 samples"""
+    wl = W.config(5, B=64)
+    f = wl.grid.freqs()
+    table = W.chirp_table(wl.params, wl.model.mode_mask, W.log_nodes(f[0], f[-1], 2048))
+    data, psd = noisy_data(wl, table)
+    F, g = P.fisher_tab(dev(wl.params), dev_table(P, table), dev(data), dev(psd), wl.grid, wl.model)
+    sub = [0, 31, 63]
+    tsub = tuple(x if x.ndim == 1 else x[sub] for x in table)
+    Fo, go = oracle.fisher_tab(wl.params[sub], tsub, data, psd, wl.grid, wl.model)
+    ix = np.ix_(range(3), USED, USED)
+    d = np.sqrt(np.einsum("bii->bi", Fo[ix]))
+    assert (np.abs(F.cpu().numpy()[sub][ix] - Fo[ix]) / (d[:, :, None] * d[:, None, :])).max() <= TOL_F
+    rr = -2.0 * oracle.loglike_tab(wl.params[sub], tsub, data, psd, wl.grid, wl.model)
+    assert (np.abs(g.cpu().numpy()[sub][:, USED] - go[:, USED]) / (d * np.sqrt(rr)[:, None])).max() <= TOL_F
