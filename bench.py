@@ -335,11 +335,17 @@ def roofline_of(path, wl, B, N, kern_ms, ops_doc, peak_tflops, sm_max_mhz, stale
     no row for one of the kernels involved)"""
     kernel = KERNEL_OF[path]
     cm = class_mask(wl.model.mode_mask)
+    n_det = len(wl.model.detectors)
     rows = []
-    for d in wl.model.detectors:
-        key_mask = 0 if kernel in ("loglike_tab", "loglike_mixed", "loglike_orb") else cm
-        key_kind = 0 if kernel == "loglike_orb" else d.kind
-        rows.append(ops_doc["kernels"].get(f"{kernel}|{key_kind}|{key_mask}"))
+    if kernel == "loglike" and n_det > 1:
+        kernel = "loglike_fused"                       # one launch walks all detectors: n_det x B x N units per launch
+        rows = [ops_doc["kernels"].get(f"loglike_fused|0|{cm}")]
+        B = B * n_det
+    else:
+        for d in wl.model.detectors:
+            key_mask = 0 if kernel in ("loglike_tab", "loglike_mixed", "loglike_orb") else cm
+            key_kind = 0 if kernel == "loglike_orb" else d.kind
+            rows.append(ops_doc["kernels"].get(f"{kernel}|{key_kind}|{key_mask}"))
     out = {"bound": "alu", "kernel": f"{kernel}_kernel", "achieved": None, "peak": peak_tflops, "unit": "TFLOP/s",
            "frac": None, "traffic": None, "kernel_ms": kern_ms, "stale": stale,
            "ops_source": os.path.relpath(OPS_FILE, ROOT), "ops_csrc_hash": ops_doc.get("csrc_hash")}
@@ -503,7 +509,7 @@ def run_ours(args):
     peak_tflops = SM_COUNT * FP64_LANES_PER_SM * 2 * sm_max * 1e6 / 1e12
     dfma_tflops, _ = P.fp64_peak(8192, mode=0)
     dfma3_tflops, _ = P.fp64_peak(8192, mode=1)
-    kern_ms = t["kernel_ms_total"] / max(1, t["kernel_launches"])   # one launch = one detector, B x N units
+    kern_ms = t["kernel_ms_total"] / max(1, t["kernel_launches"])   # one launch = one detector (fused likelihood: all)
     B_launch = B / world if strong else B
     roofline = roofline_of(path, wl, B_launch, N, kern_ms, ops_doc, peak_tflops, sm_max, stale)
     roofline.update({

@@ -191,17 +191,31 @@ int pespace::host::loglike_impl(const double* d_params, int64_t B, const double*
     prep_bins_kernel<<<gb, 256, 0, st>>>((const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
     LAUNCHED();
   }
-  const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
-  for (int d = 0; d < model->n_det; ++d) {
-    const DetC dc = make_det(model->det[d]);
+  int n_slices = (int)(model->n_det * p.nbb);
+  if (model->n_det > 1) {
+    // several detectors: ONE launch, the waveform part (S2/S3) evaluated once per (sample, bin) and shared (pespace_fused.cuh)
+    DetSet D;
+    std::memset(&D, 0, sizeof D);
+    for (int d = 0; d < model->n_det; ++d) D.det[d] = make_det(model->det[d]);
+    const long long ntile = (B + TILE_L - 1) / TILE_L;
+    if (ntile > 65535) return PESPACE_EINVAL;
+    const dim3 g((unsigned)p.nbb, (unsigned)ntile);
     EvPair ev;
     if (int rc2 = prof_begin(ev, st); rc2 != PESPACE_OK) return rc2;
-    CU(loglike_launcher(dc.kind, cm)(g, st, d_consts, d_trig, B, d_bins, G.N, dc, model->n_det, d, d_partial));
+    CU(fused_launcher(cm)(g, st, d_consts, d_trig, B, d_bins, G.N, D, model->n_det, d_partial));
+    LAUNCHED();
+    if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
+    n_slices = (int)p.nbb;
+  } else {
+    const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
+    const DetC dc = make_det(model->det[0]);
+    EvPair ev;
+    if (int rc2 = prof_begin(ev, st); rc2 != PESPACE_OK) return rc2;
+    CU(loglike_launcher(dc.kind, cm)(g, st, d_consts, d_trig, B, d_bins, G.N, dc, 1, 0, d_partial));
     LAUNCHED();
     if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
   }
-  combine_kernel<<<PESPACE_COMBINE_GRID(B), 0, st>>>(d_partial, d_consts, B, (int)(model->n_det * p.nbb),
-                                                                p.stride, d_out_lnL);
+  combine_kernel<<<PESPACE_COMBINE_GRID(B), 0, st>>>(d_partial, d_consts, B, n_slices, p.stride, d_out_lnL);
   LAUNCHED();
   return PESPACE_OK;
 }

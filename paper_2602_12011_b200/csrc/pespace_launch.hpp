@@ -4,6 +4,7 @@
 // compile in parallel.  Not part of the public ABI.
 #pragma once
 #include "pespace_host.hpp"
+#include "pespace_fused.cuh"
 
 namespace pespace {
 namespace host {
@@ -14,6 +15,8 @@ using ResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const doub
                                    long long, const DetC&, int, int, double2*);
 using GradFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*, long long,
                                const DetC&, int, int, double*);
+using FusedFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*, long long,
+                                const DetSet&, int, double*);
 using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&,
                                  int, int, int, double*);
 
@@ -31,6 +34,13 @@ PESPACE_DECLARE_INST(ResponseFn, response_launcher)
 PESPACE_DECLARE_INST(FisherFn, fisher_launcher)
 PESPACE_DECLARE_INST(GradFn, grad_launcher)
 #undef PESPACE_DECLARE_INST
+// fused multi-detector likelihood: specialised on the class mask only
+FusedFn fused_launcher_h0(unsigned cmask);
+FusedFn fused_launcher_h1(unsigned cmask);
+inline FusedFn fused_launcher(unsigned cmask) {
+  if (cmask < 1u || cmask > 15u) return nullptr;
+  return cmask < 8u ? fused_launcher_h0(cmask) : fused_launcher_h1(cmask);
+}
 
 }  // namespace host
 }  // namespace pespace

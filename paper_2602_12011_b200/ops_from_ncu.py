@@ -4,7 +4,8 @@
 
 Each CSV is the `--csv --log-file` output of an `ncu --metrics ...` run of bench.py (the exact command is kept in the
 `.md` beside the CSV under profiles/); B and N are the samples and bins of the profiled launches, so that one launch
-processes B x N units of work (one unit = one (sample, bin, detector)).  For every profiled kernel the script stores,
+processes B x N units of work (one unit = one (sample, bin, detector); for the fused multi-detector kernel, which walks
+the detectors inside one launch, pass B x n_det as B).  For every profiled kernel the script stores,
 per unit, the thread-level FP64 operation counts (DFMA, DMUL, DADD), the FP64-pipe warp instructions, all warp
 instructions, and per launch the DRAM bytes and the duration -- keyed by "<kernel>|<kind>|<class mask>" -- together
 with `csrc_hash`, the content hash of the sources they were counted on (build.csrc_hash()).  bench.py recomputes that
@@ -35,7 +36,7 @@ METRICS = {
 }
 UNIT_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "nsecond": 1.0, "usecond": 1e3, "msecond": 1e6,
               "second": 1e9}
-KERNELS = ("loglike_grad_kernel", "loglike_tab_kernel", "loglike_mixed_kernel", "loglike_orb_kernel", "loglike_kernel",
+KERNELS = ("loglike_fused_kernel", "loglike_grad_kernel", "loglike_tab_kernel", "loglike_mixed_kernel", "loglike_orb_kernel", "loglike_kernel",
            "fisher_kernel", "response_kernel")
 
 
@@ -43,9 +44,11 @@ def kernel_key(name: str):
     """'void pespace::loglike_kernel<0, 2>(...)' -> ('loglike', 0, 2); kernels without a class mask -> (.., kind, 0)"""
     for k in KERNELS:
         if k in name:
-            m = re.search(re.escape(k) + r"<\s*(\d+)\s*(?:,\s*(\d+)u?)?\s*>", name)
+            m = re.search(re.escape(k) + r"<\s*(\d+)u?\s*(?:,\s*(\d+)u?)?\s*>", name)
             kind = int(m.group(1)) if m else 0
             mask = int(m.group(2)) if m and m.group(2) else 0
+            if k == "loglike_fused_kernel":                 # one template argument: the class mask
+                kind, mask = 0, kind
             return k[:-len("_kernel")], kind, mask
     return None
 

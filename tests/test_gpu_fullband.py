@@ -162,6 +162,24 @@ def test_response_tab_full_band_per_bin(P, gen):
     check_response_per_bin(got, want, f, dets, f"tab gen {gen}")
 
 
+def test_response_orb_full_band_per_bin(P):
+    """pespace_response_orb (tabulated orbits, reading T2) over the full band with the same per-bin tolerance: seeded
+    toy ephemeris with breathing arms, five modes, three detectors, the nulls of the NOMINAL arm lengths included"""
+    grid = W.config(2).grid
+    dets = (W.lisa_like(), W.taiji_like(), W.tianqin_like())
+    model = W.Model(W.MODES_HM, dets)
+    idx, _ = band_indices(grid, dets)
+    f = grid.freqs()[idx]
+    th = W.config(4, B=4).params
+    T = 1.0 / grid.df
+    tab = W.synthetic_orbit_table(dets, -16.0 * T, 1800.0, int(18.5 * T / 1800.0) + 2, seed=21)
+    got = P.response_orb(dev(th), P.OrbitTable(tab[0], tab[1], dev(tab[2]), dev(tab[3])), dev(f), model).cpu().numpy()
+    want = oracle.response_orb(th, tab, f, model)
+    assert np.all(np.abs(want[:, :, 0]).max(axis=-1) > 0)
+    worst = check_response_per_bin(got, want, f, dets, "orb")
+    print(f"tabulated orbits, full band: {f.size} bins, worst per-bin error / tolerance {worst:.3f}")
+
+
 def _window_workload(det_list, k0, n, B, mask, seed):
     """an n-bin stretch of the config-2 lattice starting at bin k0: same df, f0 moved"""
     base = W.config(2).grid
@@ -244,7 +262,12 @@ def test_fisher_single_bin_grids_over_the_band(P):
         # the small d_j h_T.)  In sums over many bins the term averages out; here it is the whole result.
         tol_g = tol_F + max(cancel_floor(det, fgrid[k]) * np.sqrt(psd[i].max() / psd[i].min()) for i, det in enumerate(dets))
         assert eF <= tol_F and eg <= tol_g, (k, fgrid[k], eF, eg, tol_F, tol_g)
-        worstF, worstg = max(worstF, eF / tol_F), max(worstg, eg / tol_g)
+        # the reverse-mode gradient (pespace_loglike_grad) of the same single bin, same tolerance; lnL at 1e-9
+        la, ga = P.loglike_grad(dev(th), dev(data), dev(psd), wl.grid, wl.model)
+        ea = (np.abs(ga.cpu().numpy() - go) / (d * np.sqrt(rr)[:, None])).max()
+        assert ea <= tol_g, (k, fgrid[k], ea, tol_g)
+        assert (np.abs(la.cpu().numpy() + 0.5 * rr) / (0.5 * rr)).max() <= TOL_LNL
+        worstF, worstg = max(worstF, eF / tol_F), max(worstg, eg / tol_g, ea / tol_g)
     print(f"single-bin Fisher over the band: {len(ks)} bins, worst F / tolerance {worstF:.2f}, worst grad / tolerance {worstg:.2f}")
 
 

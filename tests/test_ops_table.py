@@ -25,24 +25,30 @@ def add_ops(total, ops, times=1):
         total[k] = total.get(k, 0) + times * v
 
 
-def class_ops(mc: int, kind: int):
-    """one mode class (m = mc + 1) of one (sample, bin, detector): eval_class + eval_geom of pespace_device.cuh"""
+def wave_ops(mc: int):
+    """S2/S3 of one mode class (m = mc + 1): eval_class up to the call of eval_geom (pespace_device.cuh)"""
     t = {"fma": 0, "mul": 0, "add": 0}
-    # S2/S3: v (other classes: one mul), v^2, two Horner polynomials, phase reduction, t_lm
     if mc != 1:
-        add_ops(t, {"mul": 1})
+        add_ops(t, {"mul": 1})                              # v = v_2 (2/m)^{1/3}
     add_ops(t, {"mul": 1})                                  # v^2
     add_ops(t, {"fma": 8 + 7})                              # P (8 incl. the two log terms), Q (7)
     add_ops(t, {"mul": 1, "fma": 1, "add": 2})              # psi = s P; psi -= ((psi + magic) - magic)
     add_ops(t, {"add": 2} if mc == 1 else {"fma": 1, "add": 1})     # + (m/2) PH0 + f t_c
     add_ops(t, {"fma": 2} if mc == 1 else {"mul": 2})       # amplitudes a + b v^2 | v^p a
+    return t
+
+
+def geom_ops(kind: int, tau_cached: bool = False):
+    """S4-S7 of one class for one detector: eval_geom.  tau_cached: the fused kernel keeps tau = s' Q in a register,
+    the per-detector kernel contracts that product into the orbit-angle sum"""
+    t = {"fma": 0, "mul": 0, "add": 0}
     # S4: orbit angle(s) and G1, G2 of k, u', v', Doppler phase of the centre
     if kind == 0:
-        add_ops(t, {"fma": 1}); add_ops(t, SINCOS_TAB)      # alpha = alpha0 + s' Q; sin, cos alpha
+        add_ops(t, {"add": 1} if tau_cached else {"fma": 1}); add_ops(t, SINCOS_TAB)     # alpha = alpha0 + tau; sin, cos
         add_ops(t, {"fma": 1, "add": 2, "mul": 1})          # cos 2a = 2 c c - 1, sin 2a = (s + s) c
         add_ops(t, {"fma": 18})                             # six three-term combinations
     else:
-        add_ops(t, {"mul": 1, "fma": 2}); add_ops(t, SINCOS_TAB, 2)     # tau, alpha_E, phi
+        add_ops(t, {"add": 1, "fma": 1} if tau_cached else {"mul": 1, "fma": 2}); add_ops(t, SINCOS_TAB, 2)
         add_ops(t, {"fma": 6, "mul": 6})
     add_ops(t, {"fma": 1, "mul": 1})                        # k.R
     # projections: k.delta_n, k.n_l, u'.n_l, v'.n_l with literal coefficients
@@ -59,18 +65,38 @@ def class_ops(mc: int, kind: int):
     return t
 
 
+FIRST_CLASS = {"fma": -6, "mul": 6}                         # initialising S: 2 fma + 2 mul instead of 4 fma, x 3
+RESIDUAL = {"add": 2 + 2 + 4 + 6, "fma": 2 + 5, "mul": 4}   # A, E, T, residuals, weighted squares
+
+
 def loglike_ops(classes, kind, single_class):
+    """loglike_kernel<kind, mask>: per (sample, bin) of ONE detector"""
     t = {"fma": 0, "mul": 0, "add": 0}
     add_ops(t, {"mul": 2, "add": 2, "fma": 1})              # f t_c modulo one turn, v = a f^{1/3}
-    first = True
-    for mc in classes:
-        add_ops(t, class_ops(mc, kind))
-        if first:
-            add_ops(t, {"fma": -6, "mul": 6})               # initialising S: 2 fma + 2 mul instead of 4 fma, x 3
-            first = False
-    add_ops(t, {"add": 2 + 2 + 4 + 6, "fma": 2 + 5, "mul": 4})      # A, E, T, residuals, weighted squares
+    for i, mc in enumerate(classes):
+        add_ops(t, wave_ops(mc)); add_ops(t, geom_ops(kind))
+        if i == 0:
+            add_ops(t, FIRST_CLASS)
+    add_ops(t, RESIDUAL)
     add_ops(t, {"add": 1.5 if single_class else 5.0})       # warp reduction per unit
     return t
+
+
+def fused_ops(classes, kinds):
+    """loglike_fused_kernel<mask>: per (sample, bin, detector), averaged over the detectors of the model: the waveform
+    part once per (sample, bin), S4-S8 per detector, one reduction per (sample, bin)"""
+    t = {"fma": 0, "mul": 0, "add": 0}
+    add_ops(t, {"mul": 2, "add": 2, "fma": 1})
+    for mc in classes:
+        add_ops(t, wave_ops(mc)); add_ops(t, {"mul": 1})    # + tau kept as a product of its own
+    for kind in kinds:
+        for i, mc in enumerate(classes):
+            add_ops(t, geom_ops(kind, tau_cached=True))
+            if i == 0:
+                add_ops(t, FIRST_CLASS)
+        add_ops(t, RESIDUAL)
+    add_ops(t, {"add": 5.0})
+    return {k: v / len(kinds) for k, v in t.items()}
 
 
 @pytest.fixture(scope="module")
@@ -80,11 +106,13 @@ def ops():
 
 
 @pytest.mark.parametrize("key,classes,kind", [("loglike|0|2", [1], 0), ("loglike|0|15", [0, 1, 2, 3], 0),
-                                               ("loglike|1|15", [0, 1, 2, 3], 1)])
+                                               ("loglike_fused|0|15", [0, 1, 2, 3], (0, 0, 1))])
 def test_operation_table_sums_to_the_ncu_count(ops, key, classes, kind):
+    """config 2 (one class, LISA-like), config 3 (four classes, LISA-like), config 4 (four classes, two heliocentric
+    detectors and a geocentric one in the fused kernel)"""
     row = ops["kernels"].get(key)
     assert row is not None, key
-    t = loglike_ops(classes, kind, single_class=len(classes) == 1)
+    t = fused_ops(classes, kind) if isinstance(kind, tuple) else loglike_ops(classes, kind, single_class=len(classes) == 1)
     want = sum(t.values())
     got = row["dfma"] + row["dmul"] + row["dadd"]
     assert abs(got - want) <= 0.015 * got, (key, t, row["dfma"], row["dmul"], row["dadd"])
