@@ -53,25 +53,28 @@ constexpr size_t fisher_smem_bytes() {
 // ---- constant accessors: sc points at one sample block [SMEM_STRIDE][DUW]
 __device__ __forceinline__ double cv(const double* sc, int idx) { return sc[idx * DUW]; }
 __device__ __forceinline__ double ct(const double* sc, int idx, int t) { return sc[idx * DUW + 1 + t]; }
-// tangents (M, q, chi1, chi2)
+// tangents (M, q, chi1, chi2).  A constant record is 8 doubles = 64 bytes, 64-byte aligned in shared memory: the
+// tangents are fetched with 128-bit (broadcast) loads
 __device__ __forceinline__ Du<4> c4(const double* sc, int idx) {
   Du<4> r;
-  const double* p = sc + idx * DUW;
-  r.v = p[0]; r.d[0] = p[1]; r.d[1] = p[2]; r.d[2] = p[3]; r.d[3] = p[4];
+  const double2* p = reinterpret_cast<const double2*>(sc + idx * DUW);
+  const double2 a = p[0], b = p[1];
+  r.v = a.x; r.d[0] = a.y; r.d[1] = b.x; r.d[2] = b.y; r.d[3] = sc[idx * DUW + 4];
   return r;
 }
 // geometry directions (orbit angle, lambda, beta): constants carry lambda, beta only
 __device__ __forceinline__ Du<3> cg(const double* sc, int idx) {
   Du<3> r;
-  const double* p = sc + idx * DUW;
-  r.v = p[0]; r.d[0] = 0.0; r.d[1] = p[6]; r.d[2] = p[7];
+  const double2 t = reinterpret_cast<const double2*>(sc + idx * DUW)[3];
+  r.v = sc[idx * DUW]; r.d[0] = 0.0; r.d[1] = t.x; r.d[2] = t.y;
   return r;
 }
 // amplitude directions (M, q, iota)
 __device__ __forceinline__ Du<3> ca3(const double* sc, int idx) {
   Du<3> r;
   const double* p = sc + idx * DUW;
-  r.v = p[0]; r.d[0] = p[1]; r.d[1] = p[2]; r.d[2] = p[5];
+  const double2 a = reinterpret_cast<const double2*>(p)[0];
+  r.v = a.x; r.d[0] = a.y; r.d[1] = p[2]; r.d[2] = p[5];
   return r;
 }
 // a Du<3> with only the orbit-angle tangent
@@ -167,11 +170,12 @@ __device__ __forceinline__ void fisher_stage_a(int MC, const BinC& bc, const dou
   }
 }
 
-// J accumulation: column of this thread in shared memory, J[(p * 6 + comp * 2 + ri) * FBLOCK]
+// J accumulation: column of this thread in shared memory, (re, im) of entry (p, comp) at J[(p * 6 + comp * 2) * FBLOCK]
 __device__ __forceinline__ void jadd(bool first, double* J, int p, int comp, double re, double im) {
-  double* a = J + ((p * 6 + comp * 2) * FBLOCK);
-  if (first) { a[0] = re; a[FBLOCK] = im; }
-  else { a[0] += re; a[FBLOCK] += im; }
+  // (re, im) pairs are adjacent: one 128-bit shared-memory access per entry instead of two 64-bit ones
+  double2* a = reinterpret_cast<double2*>(J + ((p * 6 + comp * 2) * FBLOCK));
+  if (first) { *a = make_double2(re, im); }
+  else { double2 t = *a; t.x += re; t.y += im; *a = t; }
 }
 
 // One mode class of one (sample, bin, detector): adds value and tangents of (X, Y, Z) to J.
@@ -213,12 +217,14 @@ __device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const C
       g2.v = fma(w0[0], s2v, fma(-w1[0], c2v, fma(w2[0], sa, w4[0])));
       g1.d[0] = fma(w0[0], dc2, fma(w1[0], ds2, -w2[0] * sa));
       g2.d[0] = fma(w0[0], ds2, fma(-w1[0], dc2, w2[0] * ca));
-#pragma unroll
-      for (int t = 1; t < 3; ++t) {                             // lambda, beta: slots 6, 7 of the constant record
-        const int q = 5 + t;
-        g1.d[t] = fma(w0[q], c2v, fma(w1[q], s2v, fma(w2[q], ca, w3[q])));
-        g2.d[t] = fma(w0[q], s2v, fma(-w1[q], c2v, fma(w2[q], sa, w4[q])));
-      }
+      // lambda, beta: slots 6, 7 of the constant record, one 128-bit load per constant
+      const double2 t0 = reinterpret_cast<const double2*>(w0)[3], t1 = reinterpret_cast<const double2*>(w1)[3],
+                    t2 = reinterpret_cast<const double2*>(w2)[3], t3 = reinterpret_cast<const double2*>(w3)[3],
+                    t4 = reinterpret_cast<const double2*>(w4)[3];
+      g1.d[1] = fma(t0.x, c2v, fma(t1.x, s2v, fma(t2.x, ca, t3.x)));
+      g2.d[1] = fma(t0.x, s2v, fma(-t1.x, c2v, fma(t2.x, sa, t4.x)));
+      g1.d[2] = fma(t0.y, c2v, fma(t1.y, s2v, fma(t2.y, ca, t3.y)));
+      g2.d[2] = fma(t0.y, s2v, fma(-t1.y, c2v, fma(t2.y, sa, t4.y)));
     };
     rot(S_K, G1k, G2k);
     rot(S_U, G1u, G2u);
@@ -226,8 +232,9 @@ __device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const C
     const double* dx = sc + S_DX * DUW; const double* dy = sc + S_DY * DUW;
     kR.v = fma(dx[0], ca, dy[0] * sa);
     kR.d[0] = fma(dy[0], ca, -dx[0] * sa);
-    kR.d[1] = fma(dx[6], ca, dy[6] * sa);
-    kR.d[2] = fma(dx[7], ca, dy[7] * sa);
+    const double2 dxt = reinterpret_cast<const double2*>(dx)[3], dyt = reinterpret_cast<const double2*>(dy)[3];
+    kR.d[1] = fma(dxt.x, ca, dyt.x * sa);
+    kR.d[2] = fma(dxt.y, ca, dyt.y * sa);
   } else {
     double sE, cE, sp, cp;
     sincos_pu<false>(cv(sc, D_BASE) + cs.tau, nullptr, sE, cE);
@@ -239,12 +246,9 @@ __device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const C
       g2.v = fma(w1[0], cp, -w0[0] * sp);
       g1.d[0] = fma(w0[0], dcp, w1[0] * dsp);
       g2.d[0] = fma(w1[0], dcp, -w0[0] * dsp);
-#pragma unroll
-      for (int t = 1; t < 3; ++t) {
-        const int q = 5 + t;
-        g1.d[t] = fma(w0[q], cp, w1[q] * sp);
-        g2.d[t] = fma(w1[q], cp, -w0[q] * sp);
-      }
+      const double2 t0 = reinterpret_cast<const double2*>(w0)[3], t1 = reinterpret_cast<const double2*>(w1)[3];
+      g1.d[1] = fma(t0.x, cp, t1.x * sp); g2.d[1] = fma(t1.x, cp, -t0.x * sp);
+      g1.d[2] = fma(t0.y, cp, t1.y * sp); g2.d[2] = fma(t1.y, cp, -t0.y * sp);
     };
     rot(D_BASE + 2, G1k, G2k);
     rot(D_BASE + 4, G1u, G2u);
@@ -252,8 +256,9 @@ __device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const C
     const double* dx = sc + S_DX * DUW; const double* dy = sc + S_DY * DUW;
     kR.v = fma(dx[0], cE, dy[0] * sE);
     kR.d[0] = fma(dy[0], cE, -dx[0] * sE);
-    kR.d[1] = fma(dx[6], cE, dy[6] * sE);
-    kR.d[2] = fma(dx[7], cE, dy[7] * sE);
+    const double2 dxt = reinterpret_cast<const double2*>(dx)[3], dyt = reinterpret_cast<const double2*>(dy)[3];
+    kR.d[1] = fma(dxt.x, cE, dyt.x * sE);
+    kR.d[2] = fma(dxt.y, cE, dyt.y * sE);
   }
   // spacecraft at 0, 120, 240 degrees (lambda0 is absorbed by the per-sample constants): same literal
   // coefficients as eval_class
@@ -442,8 +447,9 @@ __device__ __forceinline__ void gram_rows(const double* __restrict__ J, const do
       if (pp == 5) continue;                                  // D_L: from the value, below
       if (pp < P0 && !(pp == 0 && P0 <= 5)) continue;         // not needed by this pass
       const double* jp = J + pp * 6 * FBLOCK;
-      const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
-                   zi = jp[5 * FBLOCK];
+      const double2 X2 = *reinterpret_cast<const double2*>(jp), Y2 = *reinterpret_cast<const double2*>(jp + 2 * FBLOCK),
+                    Z2 = *reinterpret_cast<const double2*>(jp + 4 * FBLOCK);
+      const double xr = X2.x, xi = X2.y, yr = Y2.x, yi = Y2.y, zr = Z2.x, zi = Z2.y;
       if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
       else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
       else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
@@ -487,8 +493,9 @@ __device__ __forceinline__ void gram_row0(const double* __restrict__ J, const do
     for (int pp = 0; pp < NT; ++pp) {
       if (pp == 5) continue;
       const double* jp = J + pp * 6 * FBLOCK;
-      const double xr = jp[0], xi = jp[FBLOCK], yr = jp[2 * FBLOCK], yi = jp[3 * FBLOCK], zr = jp[4 * FBLOCK],
-                   zi = jp[5 * FBLOCK];
+      const double2 X2 = *reinterpret_cast<const double2*>(jp), Y2 = *reinterpret_cast<const double2*>(jp + 2 * FBLOCK),
+                    Z2 = *reinterpret_cast<const double2*>(jp + 4 * FBLOCK);
+      const double xr = X2.x, xi = X2.y, yr = Y2.x, yi = Y2.y, zr = Z2.x, zi = Z2.y;
       if (c == 0) { ar[pp] = zr - xr; ai[pp] = zi - xi; }
       else if (c == 1) { ar[pp] = xr - 2.0 * yr + zr; ai[pp] = xi - 2.0 * yi + zi; }
       else { ar[pp] = xr + yr + zr; ai[pp] = xi + yi + zi; }
@@ -530,8 +537,8 @@ __global__ void __launch_bounds__(FBLOCK, PESPACE_FMINB)
 fisher_kernel(const double* __restrict__ consts, long long B, const double* __restrict__ bins /* [n_det][NBF][N] */,
               long long N, DetC dc, int n_det, int det, int grad_only,
               double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
-  extern __shared__ double fsm[];
-  double* Jsm = fsm;                                   // [NJ][FBLOCK]
+  extern __shared__ __align__(16) double fsm[];
+  double* Jsm = fsm;                                   // [NT x 3][FBLOCK] (re, im) pairs
   double* csm = Jsm + NJ * FBLOCK;                     // [FTILE][SMEM_STRIDE][DUW]
   double* red = csm + FTILE * FS_STRIDE;               // [warps][FTILE][NGP]
   const long long b0 = (long long)blockIdx.y * FTILE;
@@ -539,7 +546,7 @@ fisher_kernel(const double* __restrict__ consts, long long B, const double* __re
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int i = threadIdx.x; i < (FBLOCK / 32) * FTILE * NGP; i += FBLOCK) red[i] = 0.0;
   __syncthreads();
-  double* J = Jsm + threadIdx.x;
+  double* J = Jsm + 2 * threadIdx.x;
   const int ns = (int)min((long long)FTILE, B - b0);
   for (int ch = 0; ch < FCHUNKS; ++ch) {
     const long long kbase = ((long long)blockIdx.x * FCHUNKS + ch) * FBLOCK;

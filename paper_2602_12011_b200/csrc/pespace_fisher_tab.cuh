@@ -76,8 +76,8 @@ __global__ void __launch_bounds__(FBLOCK, PESPACE_FMINB)
 fisher_tab_kernel(const double* __restrict__ consts, long long B, TabC T, const double* __restrict__ bins /* [n_det][NBF][N] */,
                   const double* __restrict__ wt /* [NWT][N] */, long long N, DetC dc, int n_det, int det, int grad_only,
                   double* __restrict__ partial /* [n_det][gridDim.x][B][NG] */) {
-  extern __shared__ double fsm[];
-  double* Jsm = fsm;                                   // [NJ][FBLOCK]
+  extern __shared__ __align__(16) double fsm[];
+  double* Jsm = fsm;                                   // [NT x 3][FBLOCK] (re, im) pairs
   double* csm = Jsm + NJ * FBLOCK;                     // [FTILE][SMEM_STRIDE][DUW]
   double* red = csm + FTILE * FS_STRIDE;               // [warps][FTILE][NGP]
   const long long b0 = (long long)blockIdx.y * FTILE;
@@ -85,7 +85,7 @@ fisher_tab_kernel(const double* __restrict__ consts, long long B, TabC T, const 
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   for (int i = threadIdx.x; i < (FBLOCK / 32) * FTILE * NGP; i += FBLOCK) red[i] = 0.0;
   __syncthreads();
-  double* J = Jsm + threadIdx.x;
+  double* J = Jsm + 2 * threadIdx.x;
   const int ns = (int)min((long long)FTILE, B - b0);
   for (int ch = 0; ch < FCHUNKS; ++ch) {
     const long long kbase = ((long long)blockIdx.x * FCHUNKS + ch) * FBLOCK;
