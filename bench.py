@@ -562,7 +562,9 @@ def main():
                     help="entry point to time (default: loglike; config 5: fisher)")
     ap.add_argument("--precision", choices=["f64", "mixed"], default="f64", help="mixed = --path mixed")
     ap.add_argument("--waveform", choices=["analytic", "tab"], default="analytic", help="tab = --path tab")
-    ap.add_argument("--grad-only", action="store_true", help="config 5: forward-mode gradient only (= --path fisher-grad)")
+    ap.add_argument("--grad-only", action="store_true",
+                    help="lnL + d lnL / d theta by reverse mode, pespace_loglike_grad (= --path grad); the forward-mode "
+                         "gradient of round 1 (pespace_fisher with d_out_F = NULL) is --path fisher-grad")
     ap.add_argument("--scaling", choices=["weak", "strong"], default="weak",
                     help="N > 1: weak = one batch of B per rank; strong = one global batch of B split over the ranks")
     ap.add_argument("--response", action="store_true", help="also time pespace_response on a slice of the batch")
@@ -580,7 +582,7 @@ def main():
         elif args.waveform == "tab":
             args.path = "tab"
         elif args.grad_only:
-            args.path = "fisher-grad"
+            args.path = "grad"
     # the extra short runs belong to the default invocation (the driver's command line) only
     if args.config != 2 or args.path not in (None, "loglike") or args.scaling != "weak":
         args.others = False
