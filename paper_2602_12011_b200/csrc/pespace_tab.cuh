@@ -106,7 +106,25 @@ static __global__ void prep_tab_weights_kernel(GridC G, const double* __restrict
   for (int i = 0; i < NWT; ++i) wt[(size_t)i * (size_t)G.N + (size_t)k] = w[i];
 }
 
-// X, Y, Z of one (sample, bin, detector) summed over the tabulated modes.  Returns (Re, -Im) pairs in S.
+// phase (pu, reduced), tau = kTurn t_tab / yr and amplitude of tabulated mode i of sample b at this bin
+__device__ __forceinline__ void tab_mode(int i, const double (&w)[NWT], long long j, long long j0,
+                                         const double* __restrict__ sc, const TabC& T, long long b, double ftc,
+                                         double& psi, double& tau, double& a) {
+  const size_t base = ((size_t)b * T.n_modes + i) * (size_t)T.K;
+  const double* P = T.phase + base + j;
+  const double* Tt = T.tf + base + j;
+  const double* A = T.amp + base + j0;
+  const double P0 = P[0], dP = P[1] - P0, t0 = Tt[0], t1 = Tt[1];
+  psi = fma(w[WT_H01], dP, P0) * (kTurn / (2.0 * kPi));            // node part of Psi_tab, pu (up to ~1e8)
+  psi -= whole_turns(psi);                                         // mod one turn, exact
+  psi += fma(w[WT_C10], t0, w[WT_C11] * t1);                       // slope part (small)
+  psi += fma((double)T.m[i], sc[W_PH0], ftc);                      // + kTurn [f t_c - m phi_c / 2 pi]
+  tau = fma(w[WT_Q01], dP, fma(w[WT_Q10], t0, w[WT_Q11] * t1));    // kTurn t_tab / yr
+  a = fma(w[WT_L0], A[0], fma(w[WT_L0 + 1], A[1], fma(w[WT_L0 + 2], A[2], w[WT_L0 + 3] * A[3])));
+}
+
+// X, Y, Z of one (sample, bin, detector) summed over the tabulated modes.  Returns (Re, -Im) pairs in S.  ONE = the
+// table holds a single mode (block-uniform): no loop, S initialised by the mode itself.
 template <int KIND>
 __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[NWT], const double* __restrict__ sc,
                                              const DetC& dc, const double2* __restrict__ tab, const TabC& T,
@@ -114,21 +132,18 @@ __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[N
   const double tc = sc[W_TC];
   const double ftc = mul_mod_turn(bc.fT, tc);
   const long long j = (long long)w[WT_J], j0 = (long long)w[WT_J0];
+  if (T.n_modes == 1) {
+    double psi, tau, a;
+    tab_mode(0, w, j, j0, sc, T, b, ftc, psi, tau, a);
+    eval_geom<KIND, true, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA], a * sc[W_KA + 1], S);
+    return;
+  }
 #pragma unroll
   for (int i = 0; i < 6; ++i) S[i] = 0.0;
 #pragma unroll 1
   for (int i = 0; i < T.n_modes; ++i) {
-    const size_t base = ((size_t)b * T.n_modes + i) * (size_t)T.K;
-    const double* P = T.phase + base + j;
-    const double* Tt = T.tf + base + j;
-    const double* A = T.amp + base + j0;
-    const double P0 = P[0], dP = P[1] - P0, t0 = Tt[0], t1 = Tt[1];
-    double psi = fma(w[WT_H01], dP, P0) * (kTurn / (2.0 * kPi));     // node part of Psi_tab, pu (up to ~1e8)
-    psi -= whole_turns(psi);                                         // mod one turn, exact
-    psi += fma(w[WT_C10], t0, w[WT_C11] * t1);                       // slope part (small)
-    psi += fma((double)T.m[i], sc[W_PH0], ftc);                      // + kTurn [f t_c - m phi_c / 2 pi]
-    const double tau = fma(w[WT_Q01], dP, fma(w[WT_Q10], t0, w[WT_Q11] * t1));   // kTurn t_tab / yr
-    const double a = fma(w[WT_L0], A[0], fma(w[WT_L0 + 1], A[1], fma(w[WT_L0 + 2], A[2], w[WT_L0 + 3] * A[3])));
+    double psi, tau, a;
+    tab_mode(i, w, j, j0, sc, T, b, ftc, psi, tau, a);
     eval_geom<KIND, false, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA + 2 * i], a * sc[W_KA + 2 * i + 1], S);
   }
 }
