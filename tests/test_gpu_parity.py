@@ -455,3 +455,24 @@ def test_sharded_likelihood_with_the_real_binding_under_nccl(P):
         assert np.array_equal(pdist.gather_lnL(plain, torch.device("cuda", torch.cuda.current_device())), plain)
     finally:
         dist.destroy_process_group()
+
+
+# ------------------------------------------------------------------ fused multi-detector kernel: model shapes
+@pytest.mark.parametrize("mask,n_det", [(1, 2), (W.MODES_HM, 8), (20, 5), (2, 3)])
+def test_fused_kernel_detector_counts_and_masks(P, mask, n_det):
+    """models with 2 ... PESPACE_MAX_DET detectors of mixed kinds (one launch, waveform part shared): lnL against the
+    oracle, and against the sum of the one-detector calls (each detector alone goes through loglike_kernel)"""
+    import dataclasses
+    protos = [W.lisa_like(), W.tianqin_like(), W.taiji_like(15), dataclasses.replace(W.lisa_like(15), lambda0=0.9),
+              dataclasses.replace(W.tianqin_like(15), lambda0=-0.4), W.taiji_like(),
+              dataclasses.replace(W.lisa_like(), kappa=0.3, L_m=2.0e9), dataclasses.replace(W.tianqin_like(), lon=0.3, lat=0.5)]
+    dets = tuple(protos[:n_det])
+    rng = np.random.default_rng(40 + n_det)
+    th = W.draw_prior(67, 4e5, rng)
+    wl = W.Workload("fused", W.Grid(1.2e-4, 2.7e-5, 700), W.Model(mask, dets), th, th[1].copy(), 50 + n_det)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    got = check_loglike(P, wl, data, psd)
+    one_by_one = np.zeros(wl.B)
+    for d, det in enumerate(dets):
+        one_by_one += P.loglike(dev(th), dev(data[d:d + 1]), dev(psd[d:d + 1]), wl.grid, W.Model(mask, (det,))).cpu().numpy()
+    assert np.allclose(got, one_by_one, rtol=1e-12, atol=0)
