@@ -45,7 +45,9 @@ int run_prep_orb(const double* d_params, long long B, const pespace_model* model
   LAUNCHED();
   return PESPACE_OK;
 }
-SmemOptIn g_cfg_resp, g_cfg_like;
+SmemOptIn g_cfg_resp[3], g_cfg_like[3];
+// kernel variant of a class mask: 1 -> mask 2 unrolled, 2 -> mask 15 unrolled, 0 -> run-time loop
+int variant_of(unsigned cm) { return cm == 2u ? 1 : cm == 15u ? 2 : 0; }
 
 }  // namespace
 
@@ -67,10 +69,17 @@ int pespace_response_orb(const double* d_params, int64_t B, const pespace_orbitt
   const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
     const DetC dc = make_det(model->det[d]);
-    cudaError_t e = opt_in_smem(response_orb_kernel, tab_smem_bytes(), g_cfg_resp);
-    if (e == cudaSuccess)
-      response_orb_kernel<<<grid, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, cm, make_orb(orbit, d), d_freqs, N,
-                                                                 dc, model->n_det, d, (double2*)d_out_AET);
+    cudaError_t e = cudaSuccess;
+    const OrbC O = make_orb(orbit, d);
+#define PESPACE_ORB_RESP(V, CM)                                                                                       \
+    if (variant_of(cm) == V) {                                                                                          \
+      e = opt_in_smem(response_orb_kernel<CM>, tab_smem_bytes(), g_cfg_resp[V]);                                        \
+      if (e == cudaSuccess)                                                                                             \
+        response_orb_kernel<CM><<<grid, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, cm, O, d_freqs, N, dc,      \
+                                                                       model->n_det, d, (double2*)d_out_AET);          \
+    }
+    PESPACE_ORB_RESP(0, 0u) PESPACE_ORB_RESP(1, 2u) PESPACE_ORB_RESP(2, 15u)
+#undef PESPACE_ORB_RESP
     ++g_launches;
     if (e == cudaSuccess) e = cudaGetLastError();
     if (e != cudaSuccess) rc = cuda_fail(e);
@@ -109,9 +118,15 @@ int pespace_loglike_orb(const double* d_params, int64_t B, const pespace_orbitta
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc2 = prof_begin(ev, st); rc2 != PESPACE_OK) return rc2;
-    CU(opt_in_smem(loglike_orb_kernel, tab_smem_bytes(), g_cfg_like));
-    loglike_orb_kernel<<<g, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, cm, make_orb(orbit, d), d_bins, G.N, dc,
-                                                           model->n_det, d, d_partial);
+    const OrbC O = make_orb(orbit, d);
+#define PESPACE_ORB_LIKE(V, CM)                                                                                       \
+    if (variant_of(cm) == V) {                                                                                          \
+      CU(opt_in_smem(loglike_orb_kernel<CM>, tab_smem_bytes(), g_cfg_like[V]));                                         \
+      loglike_orb_kernel<CM><<<g, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, cm, O, d_bins, G.N, dc,           \
+                                                                 model->n_det, d, d_partial);                          \
+    }
+    PESPACE_ORB_LIKE(0, 0u) PESPACE_ORB_LIKE(1, 2u) PESPACE_ORB_LIKE(2, 15u)
+#undef PESPACE_ORB_LIKE
     LAUNCHED();
     if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
   }

@@ -10,7 +10,8 @@
 // combinations G1, G2 of a few sines and cosines, a (sample, bin, class) gathers two nodes of the table (36 doubles;
 // t_lm(f) is smooth in f, so neighbouring bins read the same nodes), interpolates the nine coordinates and projects
 // them on the per-sample vectors k/c, k/L, u'/L, v'/L.  One kernel for both detector kinds (the kind, kappa, lambda0,
-// period and pointing of the description are not used), run-time loop over the mode classes.
+// period and pointing of the description are not used); the class loop is unrolled at compile time for the masks of
+// configs 2-4 ((2,2) only; all five modes) and a run-time loop for the rest.
 #pragma once
 #include "pespace_device.cuh"
 #include "pespace_fisher.cuh"   // kClassCB, kClassLN3, kClassS83
@@ -173,21 +174,32 @@ __device__ __forceinline__ void orb_class(int mc, bool first, const BinC& bc, co
   add(S[4], S[5], 2, 0, kb_, -Wr[1], -Wi[1], false);
 }
 
+// CMASK != 0: the classes of that mask unrolled at compile time (instantiated for the common masks); CMASK == 0: any
+// mask, run-time loop
+template <unsigned CMASK>
 __device__ __forceinline__ void eval_xyz_orb(unsigned cmask, const BinC& bc, const double* __restrict__ sc,
                                              const DetC& dc, const double2* __restrict__ tab, const OrbC& O,
                                              double (&S)[6]) {
   const double ftc = mul_mod_turn(bc.fT, sc[W_TC]);
   const double va = sc[W_A] * bc.cf, La = bc.lnf3;
-  bool first = true;
+  if constexpr (CMASK != 0u) {
+#define PESPACE_ORB_CLASS(MC) \
+    if constexpr ((CMASK >> MC) & 1u) orb_class(MC, !(CMASK & ((1u << MC) - 1u)), bc, sc, dc, tab, O, va, La, ftc, S);
+    PESPACE_ORB_CLASS(0) PESPACE_ORB_CLASS(1) PESPACE_ORB_CLASS(2) PESPACE_ORB_CLASS(3)
+#undef PESPACE_ORB_CLASS
+  } else {
+    bool first = true;
 #pragma unroll 1
-  for (int mc = 0; mc < 4; ++mc) {
-    if (!((cmask >> mc) & 1u)) continue;
-    orb_class(mc, first, bc, sc, dc, tab, O, va, La, ftc, S);
-    first = false;
+    for (int mc = 0; mc < 4; ++mc) {
+      if (!((cmask >> mc) & 1u)) continue;
+      orb_class(mc, first, bc, sc, dc, tab, O, va, La, ftc, S);
+      first = false;
+    }
   }
 }
 
 // likelihood with tabulated orbits: grid (bin blocks, sample tiles of TAB_TILE); one launch per detector
+template <unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK, 1)
 loglike_orb_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, unsigned cmask,
                    OrbC O, const double* __restrict__ bins /* [n_det][NBF][N] */, long long N, DetC dc, int n_det,
@@ -215,7 +227,7 @@ loglike_orb_kernel(const double* __restrict__ consts, const double2* __restrict_
   const int ns = (int)min((long long)TAB_TILE, B - b0);
   for (int s = 0; s < ns; ++s) {
     double S[6];
-    eval_xyz_orb(cmask, bc, smem + s * SMEM_STRIDE, dc, tab, O, S);
+    eval_xyz_orb<CMASK>(cmask, bc, smem + s * SMEM_STRIDE, dc, tab, O, S);
     const double Ar = S[4] - S[0], Ai = S[5] - S[1];
     const double Er_ = S[0] - 2.0 * S[2] + S[4], Ei_ = S[1] - 2.0 * S[3] + S[5];
     const double Tr = S[0] + S[2] + S[4], Ti = S[1] + S[3] + S[5];
@@ -239,6 +251,7 @@ loglike_orb_kernel(const double* __restrict__ consts, const double2* __restrict_
 }
 
 // response with tabulated orbits on an arbitrary frequency array
+template <unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK, 1)
 response_orb_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, unsigned cmask,
                     OrbC O, const double* __restrict__ freqs, long long N, DetC dc, int n_det, int det,
@@ -261,7 +274,7 @@ response_orb_kernel(const double* __restrict__ consts, const double2* __restrict
   for (int s = 0; s < ns; ++s) {
     const double* sc = smem + s * SMEM_STRIDE;
     double S[6];
-    eval_xyz_orb(cmask, bc, sc, dc, tab, O, S);
+    eval_xyz_orb<CMASK>(cmask, bc, sc, dc, tab, O, S);
     double ch[6];                                      // S holds (Re, -Im)
     ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
     ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;
