@@ -129,20 +129,21 @@ int pespace_loglike_tab(const double* d_params, int64_t B, const pespace_wavetab
   LAUNCHED();
   const TabC T = make_tab(table, model->mode_mask);
   const dim3 g((unsigned)p.nbb, (unsigned)p.ntile);
-  static SmemOptIn cfg0, cfg1;
+  static SmemOptIn cfg[2][3];
+  const int v = T.n_modes == 1 ? 1 : T.n_modes == 5 ? 2 : 0;       // kernel variant: single mode, five modes unrolled, any
   for (int d = 0; d < model->n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc2 = prof_begin(ev, st); rc2 != PESPACE_OK) return rc2;
-    if (dc.kind == 0) {
-      CU(opt_in(loglike_tab_kernel<0>, cfg0));
-      loglike_tab_kernel<0><<<g, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, T, d_bins, d_wt, G.N, dc,
-                                                                model->n_det, d, d_partial);
-    } else {
-      CU(opt_in(loglike_tab_kernel<1>, cfg1));
-      loglike_tab_kernel<1><<<g, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, T, d_bins, d_wt, G.N, dc,
-                                                                model->n_det, d, d_partial);
+#define PESPACE_TAB_LAUNCH(KIND, V, NM)                                                                              \
+    if (dc.kind == KIND && v == V) {                                                                                   \
+      CU(opt_in(loglike_tab_kernel<KIND, NM>, cfg[KIND][V]));                                                          \
+      loglike_tab_kernel<KIND, NM><<<g, BLOCK, tab_smem_bytes(), st>>>(d_consts, d_trig, B, T, d_bins, d_wt, G.N, dc,  \
+                                                                       model->n_det, d, d_partial);                   \
     }
+    PESPACE_TAB_LAUNCH(0, 0, 0) PESPACE_TAB_LAUNCH(0, 1, 1) PESPACE_TAB_LAUNCH(0, 2, 5)
+    PESPACE_TAB_LAUNCH(1, 0, 0) PESPACE_TAB_LAUNCH(1, 1, 1) PESPACE_TAB_LAUNCH(1, 2, 5)
+#undef PESPACE_TAB_LAUNCH
     LAUNCHED();
     if (int rc2 = prof_end(ev, st); rc2 != PESPACE_OK) return rc2;
   }

@@ -123,28 +123,32 @@ __device__ __forceinline__ void tab_mode(int i, const double (&w)[NWT], long lon
   a = fma(w[WT_L0], A[0], fma(w[WT_L0 + 1], A[1], fma(w[WT_L0 + 2], A[2], w[WT_L0 + 3] * A[3])));
 }
 
-// X, Y, Z of one (sample, bin, detector) summed over the tabulated modes.  Returns (Re, -Im) pairs in S.  ONE = the
-// table holds a single mode (block-uniform): no loop, S initialised by the mode itself.
-template <int KIND>
+// X, Y, Z of one (sample, bin, detector) summed over the tabulated modes.  Returns (Re, -Im) pairs in S.  NM = number of
+// modes known at compile time (1: no loop; 5: unrolled) or 0: run-time loop over T.n_modes.
+template <int KIND, int NM>
 __device__ __forceinline__ void eval_xyz_tab(const BinC& bc, const double (&w)[NWT], const double* __restrict__ sc,
                                              const DetC& dc, const double2* __restrict__ tab, const TabC& T,
                                              long long b, double (&S)[6]) {
   const double tc = sc[W_TC];
   const double ftc = mul_mod_turn(bc.fT, tc);
   const long long j = (long long)w[WT_J], j0 = (long long)w[WT_J0];
-  if (T.n_modes == 1) {
-    double psi, tau, a;
-    tab_mode(0, w, j, j0, sc, T, b, ftc, psi, tau, a);
-    eval_geom<KIND, true, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA], a * sc[W_KA + 1], S);
-    return;
-  }
+  if constexpr (NM > 0) {
 #pragma unroll
-  for (int i = 0; i < 6; ++i) S[i] = 0.0;
+    for (int i = 0; i < NM; ++i) {
+      double psi, tau, a;
+      tab_mode(i, w, j, j0, sc, T, b, ftc, psi, tau, a);
+      if (i == 0) eval_geom<KIND, true, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA], a * sc[W_KA + 1], S);
+      else eval_geom<KIND, false, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA + 2 * i], a * sc[W_KA + 2 * i + 1], S);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 6; ++i) S[i] = 0.0;
 #pragma unroll 1
-  for (int i = 0; i < T.n_modes; ++i) {
-    double psi, tau, a;
-    tab_mode(i, w, j, j0, sc, T, b, ftc, psi, tau, a);
-    eval_geom<KIND, false, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA + 2 * i], a * sc[W_KA + 2 * i + 1], S);
+    for (int i = 0; i < T.n_modes; ++i) {
+      double psi, tau, a;
+      tab_mode(i, w, j, j0, sc, T, b, ftc, psi, tau, a);
+      eval_geom<KIND, false, true>(bc, sc, dc, tab, psi, tau, a * sc[W_KA + 2 * i], a * sc[W_KA + 2 * i + 1], S);
+    }
   }
 }
 
@@ -171,7 +175,7 @@ __device__ __forceinline__ void stage_tile_n(double* smem, const double* __restr
 #ifndef PESPACE_MINBT
 #define PESPACE_MINBT 2
 #endif
-template <int KIND>
+template <int KIND, int NM>
 __global__ void __launch_bounds__(BLOCK, PESPACE_MINBT)
 loglike_tab_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, TabC T,
                    const double* __restrict__ bins /* [n_det][NBF][N] */, const double* __restrict__ wt /* [NWT][N] */,
@@ -202,7 +206,7 @@ loglike_tab_kernel(const double* __restrict__ consts, const double2* __restrict_
   const int ns = (int)min((long long)TAB_TILE, B - b0);
   for (int s = 0; s < ns; ++s) {
     double S[6];
-    eval_xyz_tab<KIND>(bc, iw, smem + s * SMEM_STRIDE, dc, tab, T, b0 + s, S);
+    eval_xyz_tab<KIND, NM>(bc, iw, smem + s * SMEM_STRIDE, dc, tab, T, b0 + s, S);
     const double Ar = S[4] - S[0], Ai = S[5] - S[1];
     const double Er_ = S[0] - 2.0 * S[2] + S[4], Ei_ = S[1] - 2.0 * S[3] + S[5];
     const double Tr = S[0] + S[2] + S[4], Ti = S[1] + S[3] + S[5];
@@ -255,7 +259,7 @@ response_tab_kernel(const double* __restrict__ consts, const double2* __restrict
   for (int s = 0; s < ns; ++s) {
     const double* sc = smem + s * SMEM_STRIDE;
     double S[6];
-    eval_xyz_tab<KIND>(bc, iw, sc, dc, tab, T, b0 + s, S);
+    eval_xyz_tab<KIND, 0>(bc, iw, sc, dc, tab, T, b0 + s, S);
     double ch[6];                                      // S holds (Re, -Im)
     ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
     ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;

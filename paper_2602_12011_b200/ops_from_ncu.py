@@ -47,7 +47,7 @@ def kernel_key(name: str):
             m = re.search(re.escape(k) + r"<\s*(\d+)u?\s*(?:,\s*(\d+)u?)?\s*>", name)
             kind = int(m.group(1)) if m else 0
             mask = int(m.group(2)) if m and m.group(2) else 0
-            if k == "loglike_fused_kernel":                 # one template argument: the class mask
+            if k in ("loglike_fused_kernel", "loglike_orb_kernel"):     # one template argument: the class mask
                 kind, mask = 0, kind
             return k[:-len("_kernel")], kind, mask
     return None
