@@ -345,7 +345,7 @@ def roofline_of(path, wl, B, N, kern_ms, ops_doc, peak_tflops, sm_max_mhz, stale
         n_modes = bin(wl.model.mode_mask).count("1")
         for d in wl.model.detectors:
             # second key: the compile-time variant of the kernel (class mask; tab: mode count; 0 = run-time loop)
-            key_mask = {"loglike_tab": n_modes if n_modes in (1, 5) else 0, "loglike_mixed": 0,
+            key_mask = {"loglike_tab": n_modes if n_modes in (1, 5) else 0, "loglike_mixed": cm if cm in (2, 15) else 0,
                         "loglike_orb": cm if cm in (2, 15) else 0}.get(kernel, cm)
             key_kind = 0 if kernel == "loglike_orb" else d.kind
             rows.append(ops_doc["kernels"].get(f"{kernel}|{key_kind}|{key_mask}"))

@@ -36,18 +36,21 @@ extern "C" int pespace_loglike_mixed(const double* d_params, int64_t B, const do
   LAUNCHED();
   const unsigned cm = class_mask(model->mode_mask);
   const dim3 g((unsigned)nbb, (unsigned)ntile);
-  static SmemOptIn cfg0, cfg1;
+  static SmemOptIn cfg[2][3];
+  const int v = cm == 2u ? 1 : cm == 15u ? 2 : 0;       // kernel variant: mask 2 / mask 15 unrolled, else run-time loop
   for (int d = 0; d < n_det; ++d) {
     const DetC dc = make_det(model->det[d]);
     EvPair ev;
     if (int rc = prof_begin(ev, st); rc != PESPACE_OK) return rc;
-    if (dc.kind == 0) {
-      CU(opt_in_smem(loglike_mixed_kernel<0>, mixed_smem_bytes(), cfg0));
-      loglike_mixed_kernel<0><<<g, BLOCK, mixed_smem_bytes(), st>>>(d_consts, d_trig, B, cm, d_bins, N, dc, n_det, d, d_partial);
-    } else {
-      CU(opt_in_smem(loglike_mixed_kernel<1>, mixed_smem_bytes(), cfg1));
-      loglike_mixed_kernel<1><<<g, BLOCK, mixed_smem_bytes(), st>>>(d_consts, d_trig, B, cm, d_bins, N, dc, n_det, d, d_partial);
+#define PESPACE_MIX_LAUNCH(KIND, V, CM)                                                                            \
+    if (dc.kind == KIND && v == V) {                                                                                 \
+      CU(opt_in_smem(loglike_mixed_kernel<KIND, CM>, mixed_smem_bytes(), cfg[KIND][V]));                             \
+      loglike_mixed_kernel<KIND, CM><<<g, BLOCK, mixed_smem_bytes(), st>>>(d_consts, d_trig, B, cm, d_bins, N, dc,   \
+                                                                           n_det, d, d_partial);                    \
     }
+    PESPACE_MIX_LAUNCH(0, 0, 0u) PESPACE_MIX_LAUNCH(0, 1, 2u) PESPACE_MIX_LAUNCH(0, 2, 15u)
+    PESPACE_MIX_LAUNCH(1, 0, 0u) PESPACE_MIX_LAUNCH(1, 1, 2u) PESPACE_MIX_LAUNCH(1, 2, 15u)
+#undef PESPACE_MIX_LAUNCH
     LAUNCHED();
     if (int rc = prof_end(ev, st); rc != PESPACE_OK) return rc;
   }

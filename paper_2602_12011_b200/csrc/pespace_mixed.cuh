@@ -176,7 +176,8 @@ constexpr size_t mixed_smem_bytes() { return mixed_smem_used(); }
 #ifndef PESPACE_MINBX
 #define PESPACE_MINBX 2
 #endif
-template <int KIND>
+// CMASK != 0: the classes of that mask unrolled at compile time (the masks of configs 2-4); 0: any mask, run-time loop
+template <int KIND, unsigned CMASK>
 __global__ void __launch_bounds__(BLOCK, PESPACE_MINBX)
 loglike_mixed_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, unsigned cmask,
                      const double* __restrict__ bins /* [n_det][NBF][N], built with fold mode 2 */, long long N, DetC dc,
@@ -225,13 +226,22 @@ loglike_mixed_kernel(const double* __restrict__ consts, const double2* __restric
     const double ftc = mul_mod_turn(fT, sc[W_TC]);
     const double va = sc[W_A] * cf;
     float S[6];
-    bool first = true;
+    if constexpr (CMASK != 0u) {
+#define PESPACE_MIX_CLASS(MC)                                                                                    \
+      if constexpr ((CMASK >> MC) & 1u)                                                                            \
+        eval_class_mixed<KIND>(MC, !(CMASK & ((1u << MC) - 1u)), fT, cf, lnf3, fm53, fm83f, sthf, cthf, omcf, fTLf, sc, sf, \
+                               dc, tabf, tabm1, va, ftc, S);
+      PESPACE_MIX_CLASS(0) PESPACE_MIX_CLASS(1) PESPACE_MIX_CLASS(2) PESPACE_MIX_CLASS(3)
+#undef PESPACE_MIX_CLASS
+    } else {
+      bool first = true;
 #pragma unroll 1
-    for (int mc = 0; mc < 4; ++mc) {
-      if (!((cmask >> mc) & 1u)) continue;
-      eval_class_mixed<KIND>(mc, first, fT, cf, lnf3, fm53, fm83f, sthf, cthf, omcf, fTLf, sc, sf, dc, tabf, tabm1, va,
-                             ftc, S);
-      first = false;
+      for (int mc = 0; mc < 4; ++mc) {
+        if (!((cmask >> mc) & 1u)) continue;
+        eval_class_mixed<KIND>(mc, first, fT, cf, lnf3, fm53, fm83f, sthf, cthf, omcf, fTLf, sc, sf, dc, tabf, tabm1, va,
+                               ftc, S);
+        first = false;
+      }
     }
     const float Ar = S[4] - S[0], Ai = S[5] - S[1];
     const float Er_ = S[0] - 2.0f * S[2] + S[4], Ei_ = S[1] - 2.0f * S[3] + S[5];
