@@ -104,3 +104,16 @@ def test_mixed_full_size_sampled(P):
     rel = np.abs(got[idx] - want) / np.abs(want)
     assert np.all(np.isfinite(got)) and rel.max() <= TOL_MIXED, rel
     print(f"config 2 full size: mixed-precision relative error {rel.max():.2e}")
+
+
+@pytest.mark.parametrize("mask", [W.MODE_33, W.MODE_21 | W.MODE_33, W.MODE_21 | W.MODE_33 | W.MODE_44,
+                                  W.MODE_22 | W.MODE_32 | W.MODE_44])
+def test_mixed_other_mode_masks(P, mask):
+    """mode sets whose class mask is neither config 2's nor config 3's: the kernel variant with the run-time class
+    loop (the compile-time variants cover masks 2 and 15 only)"""
+    base = W.config(4, B=37, N=1100)
+    wl = W.Workload("mask%d" % mask, base.grid, W.Model(mask, base.model.detectors), base.params, base.theta_inj,
+                    base.noise_seed)
+    data = wl.data(lambda p, f, m: oracle.response(p, f, m))
+    err = check(P, wl, data, wl.psd())
+    print(f"mode mask {mask}: max mixed-precision error {err:.2e}")

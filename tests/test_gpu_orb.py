@@ -77,6 +77,23 @@ def test_orb_reduced_configs_synthetic_ephemeris(P, idx, B, N):
     check_response_orb(P, wl.params[:4], tab, f[::5], wl.model)
 
 
+@pytest.mark.parametrize("mask", [W.MODE_33, W.MODE_21 | W.MODE_33 | W.MODE_44, W.MODE_22 | W.MODE_32 | W.MODE_44])
+def test_orb_other_mode_masks(P, mask):
+    """class masks other than configs 2-4's: the kernel variant with the run-time class loop"""
+    base = W.config(4, B=37, N=1100)
+    wl = W.Workload("mask%d" % mask, base.grid, W.Model(mask, base.model.detectors), base.params, base.theta_inj,
+                    base.noise_seed)
+    f = wl.grid.freqs()
+    t_lo, t_hi = time_span(wl.params, W.MODES_HM, f[[0, -1]])
+    dt = 1800.0
+    tab = W.synthetic_orbit_table(wl.model.detectors, t_lo, dt, int((t_hi - t_lo) / dt) + 2, seed=mask)
+    rng = np.random.default_rng(wl.noise_seed)
+    psd = wl.psd()
+    data = oracle.response_orb(wl.theta_inj[None], tab, f, wl.model)[0] + W.coloured_noise(psd, wl.grid.df, rng)
+    check_loglike_orb(P, wl, tab, data, psd)
+    check_response_orb(P, wl.params[:4], tab, f[::5], wl.model)
+
+
 @pytest.mark.parametrize("gen", [15, 20])
 def test_orb_dense_analytic_tables_reproduce_the_analytic_kernels(P, gen):
     """tables sampled from the oracle's analytic orbits: the tabulated-orbit kernels must agree with the oracle on those

@@ -79,6 +79,22 @@ def test_tab_reduced_configs_oracle_tables(P, idx, B, N, K):
     check_response_tab(P, wl.params[:4], tuple(x if x.ndim == 1 else x[:4] for x in table), f[::3], wl.model)
 
 
+@pytest.mark.parametrize("mask", [W.MODE_22 | W.MODE_33, W.MODE_21 | W.MODE_33 | W.MODE_32,
+                                  W.MODE_22 | W.MODE_21 | W.MODE_32 | W.MODE_44])
+def test_tab_two_to_four_modes(P, mask):
+    """mode counts other than 1 and 5: the kernel variant with the run-time mode loop (the compile-time variants
+    cover the mode counts of configs 2-4 only)"""
+    base = W.config(4, B=37, N=1100)
+    wl = W.Workload("mask%d" % mask, base.grid, W.Model(mask, base.model.detectors), base.params, base.theta_inj,
+                    base.noise_seed)
+    f = wl.grid.freqs()
+    wl.params[0] = wl.theta_inj
+    table = W.table_from_waveform_fn(wl.params, mask, W.log_nodes(f[0], f[-1], 600), oracle.waveform)
+    data, psd = noisy_data(wl, table)
+    check_loglike_tab(P, wl.params, table, data, psd, wl.grid, wl.model)
+    check_response_tab(P, wl.params[:4], tuple(x if x.ndim == 1 else x[:4] for x in table), f[::3], wl.model)
+
+
 @pytest.mark.parametrize("gen", [15, 20])
 def test_tab_random_sky_band_limited_table(P, gen):
     """Prior draws through all three detector kinds; synthetic chirp tables that end inside the grid (modes vanish
