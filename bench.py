@@ -484,7 +484,7 @@ def run_ours(args):
     response_info = None
     if (args.response or args.others) and world == 1:
         response_info = []
-        for cfg in (2, 3):
+        for cfg in (2, 3, 4):                         # config 4: three detectors in ONE launch (response_fused_kernel)
             wr = W.config(cfg, B=args.response_batch)
             pr = torch.from_numpy(np.ascontiguousarray(wr.params)).to(device)
             out_r = torch.empty((wr.B, len(wr.model.detectors), 3, N, 2), dtype=torch.float64, device=device)
@@ -499,6 +499,7 @@ def run_ours(args):
             torch.cuda.synchronize()
             r_ms = r0.elapsed_time(r1) / 5
             response_info.append({"call": "pespace_response", "mode_mask": wr.model.mode_mask, "batch": wr.B, "N": N,
+                                  "n_det": len(wr.model.detectors),
                                   "ms_per_call": r_ms, "bin_evals_per_sec": wr.B * N / (r_ms * 1e-3),
                                   "bytes_written_per_call": out_r.numel() * 8,
                                   "write_gbs": out_r.numel() * 8 / (r_ms * 1e-3) / 1e9})

@@ -139,11 +139,26 @@ int pespace_response(const double* d_params, int64_t B, const double* d_freqs, i
   int rc = run_prep(d_params, B, model, d_consts, d_trig, st);
   if (rc == PESPACE_OK) {
     const unsigned cm = class_mask(model->mode_mask);
-    const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
-    for (int d = 0; d < model->n_det && rc == PESPACE_OK; ++d) {
-      const DetC dc = make_det(model->det[d]);
-      cudaError_t e = response_launcher(dc.kind, cm)(grid, st, d_consts, d_trig, B, d_freqs, N, dc, model->n_det, d,
-                                             (double2*)d_out_AET);
+    if (model->n_det > 1) {
+      // several detectors: ONE launch, S2/S3 evaluated once per (sample, bin) and shared (pespace_fused.cuh)
+      DetSet D;
+      std::memset(&D, 0, sizeof D);
+      for (int d = 0; d < model->n_det; ++d) D.det[d] = make_det(model->det[d]);
+      const long long ntile = (B + TILE_L - 1) / TILE_L;
+      if (ntile > 65535) rc = PESPACE_EINVAL;
+      if (rc == PESPACE_OK) {
+        const dim3 grid((unsigned)p.nbb, (unsigned)ntile);
+        cudaError_t e = fused_response_launcher(cm)(grid, st, d_consts, d_trig, B, d_freqs, N, D, model->n_det,
+                                                    (double2*)d_out_AET);
+        ++g_launches;
+        if (e == cudaSuccess) e = cudaGetLastError();
+        if (e != cudaSuccess) rc = cuda_fail(e);
+      }
+    } else {
+      const dim3 grid((unsigned)p.nbb, (unsigned)p.ntile);
+      const DetC dc = make_det(model->det[0]);
+      cudaError_t e = response_launcher(dc.kind, cm)(grid, st, d_consts, d_trig, B, d_freqs, N, dc, 1, 0,
+                                                     (double2*)d_out_AET);
       ++g_launches;
       if (e == cudaSuccess) e = cudaGetLastError();
       if (e != cudaSuccess) rc = cuda_fail(e);

@@ -29,6 +29,9 @@ constexpr int TILE_L = PESPACE_FTILE_L;        // samples per block (the staged 
 __host__ __device__ constexpr size_t fused_smem_bytes(int n_det) {
   return sizeof(double) * ((size_t)2 * NTAB + (size_t)TILE_L * sample_stride(n_det) + (size_t)(BLOCK / 32) * TILE_L);
 }
+__host__ __device__ constexpr size_t fused_response_smem_bytes(int n_det) {
+  return sizeof(double) * ((size_t)2 * NTAB + (size_t)TILE_L * sample_stride(n_det));
+}
 
 // S2/S3 of class m = MC + 1 (the first half of eval_class): phase psi (pu, reduced), tau = kTurn (t_lm - t_c) / yr and
 // the amplitudes of the two polarisation contents
@@ -139,6 +142,74 @@ loglike_fused_kernel(const double* __restrict__ consts, const double2* __restric
 #pragma unroll
     for (int wv = 0; wv < BLOCK / 32; ++wv) t += red[wv][threadIdx.x];
     partial[(size_t)blockIdx.x * (size_t)B + (size_t)(b0 + threadIdx.x)] = t;
+  }
+}
+
+// pespace_response for models with several detectors: the same sharing for the response arrays.  The frequency array is
+// arbitrary here, so the per-bin record is computed in the prologue (make_bin); its detector-dependent part (sin / cos
+// 2 pi f L and the TDI prefactor g z f^{-7/6}, four doubles per detector) is kept per thread in local memory (L1) and
+// read back once per (sample, detector).
+template <unsigned CMASK>
+__global__ void __launch_bounds__(BLOCK, 1)
+response_fused_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
+                      const double* __restrict__ freqs, long long N, DetSet D, int n_det,
+                      double2* __restrict__ out /* [B][n_det][3][N] */) {
+  double2* tab = reinterpret_cast<double2*>(pespace_dyn_smem);
+  double* smem = reinterpret_cast<double*>(tab + NTAB);
+  const int stride = sample_stride(n_det);
+  const long long b0 = (long long)blockIdx.y * TILE_L;
+  const int ns = (int)min((long long)TILE_L, B - b0);
+  stage_trig(tab, trig);
+  for (int i = threadIdx.x; i < ns * stride; i += BLOCK) smem[i] = consts[b0 * stride + i];
+  const long long k = (long long)blockIdx.x * BLOCK + threadIdx.x;
+  const bool live = k < N;
+  const double fraw = freqs[live ? k : N - 1];
+  const bool pos = fraw > 0.0;
+  const BinC bc = make_bin(pos ? fraw : 1.0, D.det[0].Lbar);
+  double pb[PESPACE_MAX_DET][4];                       // sin, cos 2 pi f L_d; prefactor (re, im)
+  for (int d = 0; d < n_det; ++d) {
+    BinC bd = bc;
+    sincospi(2.0 * (pos ? fraw : 1.0) * D.det[d].Lbar, &bd.sth, &bd.cth);
+    pb[d][0] = bd.sth; pb[d][1] = bd.cth;
+    tdi_prefactor(bd, D.det[d].gen, pb[d][2], pb[d][3]);
+  }
+  __syncthreads();
+  const double i2 = 0.70710678118654752440, i6 = 0.40824829046386301637, i3 = 0.57735026918962576451;
+  for (int s = 0; s < ns; ++s) {
+    const double* sc = smem + s * stride;
+    const double ftc = mul_mod_turn(bc.fT, sc[W_TC]);
+    const double va = sc[W_A] * bc.cf, La = bc.lnf3;
+    double psi[4], tau[4], CKp[4], CKc[4];
+    if (CMASK & 1u) eval_wave<0>(bc, sc, va, La, ftc, psi[0], tau[0], CKp[0], CKc[0]);
+    if (CMASK & 2u) eval_wave<1>(bc, sc, va, La, ftc, psi[1], tau[1], CKp[1], CKc[1]);
+    if (CMASK & 4u) eval_wave<2>(bc, sc, va, La, ftc, psi[2], tau[2], CKp[2], CKc[2]);
+    if (CMASK & 8u) eval_wave<3>(bc, sc, va, La, ftc, psi[3], tau[3], CKp[3], CKc[3]);
+    const bool valid = sc[W_VALID] != 0.0;
+#pragma unroll 1
+    for (int d = 0; d < n_det; ++d) {
+      BinC bd = bc;
+      bd.sth = pb[d][0]; bd.cth = pb[d][1];
+      const double gr = pb[d][2], gi = pb[d][3];
+      const DetC& dc = D.det[d];
+      const double* scd = sc + D_STRIDE * d;
+      double S[6];
+      if (dc.kind == 0) geom_classes<0, CMASK>(bd, scd, dc, tab, psi, tau, CKp, CKc, S);
+      else geom_classes<1, CMASK>(bd, scd, dc, tab, psi, tau, CKp, CKc, S);
+      double ch[6];                                    // S holds (Re, -Im)
+      ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
+      ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;
+      ch[4] = (S[0] + S[2] + S[4]) * i3; ch[5] = -(S[1] + S[3] + S[5]) * i3;
+      if (!live) continue;
+#pragma unroll
+      for (int c = 0; c < 3; ++c) {
+        double2 o;
+        o.x = ch[2 * c] * gr - ch[2 * c + 1] * gi;
+        o.y = ch[2 * c] * gi + ch[2 * c + 1] * gr;
+        if (!pos) { o.x = 0.0; o.y = 0.0; }
+        if (!valid) { o.x = CUDART_NAN; o.y = CUDART_NAN; }
+        out[(((size_t)(b0 + s) * n_det + d) * 3 + c) * (size_t)N + (size_t)k] = o;
+      }
+    }
   }
 }
 

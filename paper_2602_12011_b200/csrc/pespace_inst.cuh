@@ -1,5 +1,5 @@
 // pespace_inst.cuh -- body of the pespace_inst_*.cu translation units.  The including file defines
-//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher, 3 adjoint gradient, 4 fused multi-detector likelihood (kind unused)
+//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher, 3 adjoint gradient, 4 fused multi-detector likelihood, 5 fused multi-detector response (kind unused)
 //   PESPACE_INST_KIND  0 heliocentric, 1 geocentric
 //   PESPACE_INST_HALF  0 class masks 1..7, 1 class masks 8..15
 #include "pespace_launch.hpp"
@@ -9,7 +9,7 @@
 #if PESPACE_INST_WHAT == 3
 #include "pespace_grad.cuh"
 #endif
-#if PESPACE_INST_WHAT == 4
+#if PESPACE_INST_WHAT == 4 || PESPACE_INST_WHAT == 5
 #include "pespace_fused.cuh"
 #endif
 
@@ -51,6 +51,18 @@ cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2*
   return cudaSuccess;
 }
 using Fn = FusedFn;
+#elif PESPACE_INST_WHAT == 5
+template <int KIND, unsigned CM>
+cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
+                   const double* freqs, long long N, const DetSet& D, int n_det, double2* out) {
+  static SmemOptIn configured;
+  if (cudaError_t e = opt_in_smem(response_fused_kernel<CM>, fused_response_smem_bytes(PESPACE_MAX_DET), configured);
+      e != cudaSuccess)
+    return e;
+  response_fused_kernel<CM><<<g, BLOCK, fused_response_smem_bytes(n_det), st>>>(consts, trig, B, freqs, N, D, n_det, out);
+  return cudaSuccess;
+}
+using Fn = FusedResponseFn;
 #elif PESPACE_INST_WHAT == 3
 template <int KIND, unsigned CM>
 cudaError_t launch(dim3 g, cudaStream_t st, const double* consts, const double2* trig, long long B,
@@ -94,6 +106,8 @@ constexpr unsigned kBase = 8;
 #define PESPACE_INST_NAME PESPACE_CAT(response_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
 #elif PESPACE_INST_WHAT == 4
 #define PESPACE_INST_NAME PESPACE_CAT(fused_launcher_h, PESPACE_INST_HALF, , , )
+#elif PESPACE_INST_WHAT == 5
+#define PESPACE_INST_NAME PESPACE_CAT(fused_response_launcher_h, PESPACE_INST_HALF, , , )
 #elif PESPACE_INST_WHAT == 3
 #define PESPACE_INST_NAME PESPACE_CAT(grad_launcher_k, PESPACE_INST_KIND, _h, PESPACE_INST_HALF, )
 #else

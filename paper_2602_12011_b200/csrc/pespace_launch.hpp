@@ -17,6 +17,8 @@ using GradFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*
                                const DetC&, int, int, double*);
 using FusedFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*, long long,
                                 const DetSet&, int, double*);
+using FusedResponseFn = cudaError_t (*)(dim3, cudaStream_t, const double*, const double2*, long long, const double*,
+                                        long long, const DetSet&, int, double2*);
 using FisherFn = cudaError_t (*)(dim3, cudaStream_t, const double*, long long, const double*, long long, const DetC&,
                                  int, int, int, double*);
 
@@ -40,6 +42,12 @@ FusedFn fused_launcher_h1(unsigned cmask);
 inline FusedFn fused_launcher(unsigned cmask) {
   if (cmask < 1u || cmask > 15u) return nullptr;
   return cmask < 8u ? fused_launcher_h0(cmask) : fused_launcher_h1(cmask);
+}
+FusedResponseFn fused_response_launcher_h0(unsigned cmask);
+FusedResponseFn fused_response_launcher_h1(unsigned cmask);
+inline FusedResponseFn fused_response_launcher(unsigned cmask) {
+  if (cmask < 1u || cmask > 15u) return nullptr;
+  return cmask < 8u ? fused_response_launcher_h0(cmask) : fused_response_launcher_h1(cmask);
 }
 
 }  // namespace host

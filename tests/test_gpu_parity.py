@@ -476,3 +476,20 @@ def test_fused_kernel_detector_counts_and_masks(P, mask, n_det):
     for d, det in enumerate(dets):
         one_by_one += P.loglike(dev(th), dev(data[d:d + 1]), dev(psd[d:d + 1]), wl.grid, W.Model(mask, (det,))).cpu().numpy()
     assert np.allclose(got, one_by_one, rtol=1e-12, atol=0)
+    # pespace_response of the same model (response_fused_kernel) against the oracle and the one-detector calls
+    # (response_kernel); non-positive and repeated frequencies, out-of-domain sample, ragged bin block
+    f = wl.grid.freqs()[::3].copy()
+    thr = th[:9].copy()
+    resp, _ = check_response(P, thr, f, wl.model)
+    f[5] = 0.0; f[6] = -1e-3; f[7] = f[8]
+    thr[4, 4] = -1.0
+    resp = P.response(dev(thr), dev(f), wl.model).cpu().numpy()
+    assert np.all(np.delete(resp, 4, axis=0)[..., 5:7] == 0.0)          # f <= 0: zeros
+    assert np.all(np.isnan(resp[4])) and np.all(np.isfinite(np.delete(resp, 4, axis=0)))
+    assert np.array_equal(np.delete(resp, 4, axis=0)[..., 7], np.delete(resp, 4, axis=0)[..., 8])
+    for d, det in enumerate(dets):
+        one = P.response(dev(thr), dev(f), W.Model(mask, (det,))).cpu().numpy()[:, 0]
+        ok = np.delete(np.arange(9), 4)
+        scale = np.abs(one[ok]).max(axis=(1, 2), keepdims=True)
+        assert np.all(np.abs(resp[ok, d] - one[ok]) <= 1e-11 * scale)
+    assert np.array_equal(resp[np.isfinite(resp)], P.response(dev(thr), dev(f), wl.model).cpu().numpy()[np.isfinite(resp)])
