@@ -752,9 +752,12 @@ static __global__ void combine_kernel(const double* __restrict__ partial, const 
 // launch configuration of combine_kernel
 #define PESPACE_COMBINE_GRID(B) (unsigned)(((B) + 31) / 32), dim3(32, pespace::CGROUPS)
 
-// pespace_response: same body, writes A, E, T (with the common factor restored).
+// pespace_response: same body, writes A, E, T (with the common factor restored).  Like the likelihood kernel the
+// single-class instantiations evaluate four samples per trip (independent dependency chains for the FP64 pipe) and all
+// instantiations are compiled for the block count per SM that suits their register need.  Non-positive frequencies
+// are handled by a zero prefactor, out-of-domain samples by a block-uniform branch: no selects in the sample loop.
 template <int KIND, unsigned CMASK>
-__global__ void __launch_bounds__(BLOCK)
+__global__ void __launch_bounds__(BLOCK, popc4(CMASK) == 1 ? PESPACE_MINB1 : PESPACE_MINBM)
 response_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B,
                 const double* __restrict__ freqs, long long N, DetC dc, int n_det, int det,
                 double2* __restrict__ out /* [B][n_det][3][N] */) {
@@ -770,28 +773,47 @@ response_kernel(const double* __restrict__ consts, const double2* __restrict__ t
   const BinC bc = make_bin(pos ? fraw : 1.0, dc.Lbar);
   double gr, gi;
   tdi_prefactor(bc, dc.gen, gr, gi);
+  const double i2 = 0.70710678118654752440, i6 = 0.40824829046386301637, i3 = 0.57735026918962576451;
+  // the channel normalisations folded into the prefactor; f <= 0: zeros (the body runs on f = 1 and is finite)
+  const double gA[2] = {pos ? gr * i2 : 0.0, pos ? gi * i2 : 0.0};
+  const double gE[2] = {pos ? gr * i6 : 0.0, pos ? gi * i6 : 0.0};
+  const double gT[2] = {pos ? gr * i3 : 0.0, pos ? gi * i3 : 0.0};
   __syncthreads();
   const int ns = (int)min((long long)TILE, B - b0);
-  const double i2 = 0.70710678118654752440, i6 = 0.40824829046386301637, i3 = 0.57735026918962576451;
-  for (int s = 0; s < ns; ++s) {
-    const double* sc = smem + s * SMEM_STRIDE;
+  double2* const obase = out + ((size_t)b0 * n_det + det) * 3 * (size_t)N + (size_t)(live ? k : 0);
+  const size_t sstride = (size_t)n_det * 3 * (size_t)N;
+  auto eval = [&](int s, double (&ch)[6]) {
     double S[6];
-    eval_xyz<KIND, CMASK, true>(bc, sc, dc, tab, S);
-    double ch[6];                                      // S holds (Re, -Im)
-    ch[0] = (S[4] - S[0]) * i2; ch[1] = (S[1] - S[5]) * i2;
-    ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;
-    ch[4] = (S[0] + S[2] + S[4]) * i3; ch[5] = -(S[1] + S[3] + S[5]) * i3;
-    if (!live) continue;
-    const bool valid = sc[W_VALID] != 0.0;
-#pragma unroll
-    for (int c = 0; c < 3; ++c) {
-      double2 o;
-      o.x = ch[2 * c] * gr - ch[2 * c + 1] * gi;
-      o.y = ch[2 * c] * gi + ch[2 * c + 1] * gr;
-      if (!pos) { o.x = 0.0; o.y = 0.0; }
-      if (!valid) { o.x = CUDART_NAN; o.y = CUDART_NAN; }
-      out[(((size_t)(b0 + s) * n_det + det) * 3 + c) * (size_t)N + (size_t)k] = o;
+    eval_xyz<KIND, CMASK, true>(bc, smem + s * SMEM_STRIDE, dc, tab, S);   // S holds (Re, -Im)
+    ch[0] = S[4] - S[0]; ch[1] = S[1] - S[5];
+    ch[2] = S[0] - 2.0 * S[2] + S[4]; ch[3] = -(S[1] - 2.0 * S[3] + S[5]);
+    ch[4] = S[0] + S[2] + S[4]; ch[5] = -(S[1] + S[3] + S[5]);
+  };
+  auto store = [&](int s, const double (&ch)[6]) {
+    if (!live) return;
+    double2* o = obase + (size_t)s * sstride;
+    if (smem[s * SMEM_STRIDE + W_VALID] != 0.0) {
+      o[0] = make_double2(fma(ch[0], gA[0], -ch[1] * gA[1]), fma(ch[0], gA[1], ch[1] * gA[0]));
+      o[N] = make_double2(fma(ch[2], gE[0], -ch[3] * gE[1]), fma(ch[2], gE[1], ch[3] * gE[0]));
+      o[2 * N] = make_double2(fma(ch[4], gT[0], -ch[5] * gT[1]), fma(ch[4], gT[1], ch[5] * gT[0]));
+    } else {
+      o[0] = o[N] = o[2 * N] = make_double2(CUDART_NAN, CUDART_NAN);
     }
+  };
+  int s = 0;
+  if constexpr (popc4(CMASK) == 1) {
+    for (; s + 4 <= ns; s += 4) {
+      double ch[4][6];
+#pragma unroll
+      for (int j = 0; j < 4; ++j) eval(s + j, ch[j]);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) store(s + j, ch[j]);
+    }
+  }
+  for (; s < ns; ++s) {
+    double ch[6];
+    eval(s, ch);
+    store(s, ch);
   }
 }
 

@@ -172,6 +172,7 @@ response_fused_kernel(const double* __restrict__ consts, const double2* __restri
     sincospi(2.0 * (pos ? fraw : 1.0) * D.det[d].Lbar, &bd.sth, &bd.cth);
     pb[d][0] = bd.sth; pb[d][1] = bd.cth;
     tdi_prefactor(bd, D.det[d].gen, pb[d][2], pb[d][3]);
+    if (!pos) { pb[d][2] = 0.0; pb[d][3] = 0.0; }     // f <= 0: zeros (the body runs on f = 1 and is finite)
   }
   __syncthreads();
   const double i2 = 0.70710678118654752440, i6 = 0.40824829046386301637, i3 = 0.57735026918962576451;
@@ -200,14 +201,13 @@ response_fused_kernel(const double* __restrict__ consts, const double2* __restri
       ch[2] = (S[0] - 2.0 * S[2] + S[4]) * i6; ch[3] = -(S[1] - 2.0 * S[3] + S[5]) * i6;
       ch[4] = (S[0] + S[2] + S[4]) * i3; ch[5] = -(S[1] + S[3] + S[5]) * i3;
       if (!live) continue;
+      double2* o = out + ((size_t)(b0 + s) * n_det + d) * 3 * (size_t)N + (size_t)k;
+      if (valid) {                                     // block-uniform
 #pragma unroll
-      for (int c = 0; c < 3; ++c) {
-        double2 o;
-        o.x = ch[2 * c] * gr - ch[2 * c + 1] * gi;
-        o.y = ch[2 * c] * gi + ch[2 * c + 1] * gr;
-        if (!pos) { o.x = 0.0; o.y = 0.0; }
-        if (!valid) { o.x = CUDART_NAN; o.y = CUDART_NAN; }
-        out[(((size_t)(b0 + s) * n_det + d) * 3 + c) * (size_t)N + (size_t)k] = o;
+        for (int c = 0; c < 3; ++c)
+          o[c * N] = make_double2(fma(ch[2 * c], gr, -ch[2 * c + 1] * gi), fma(ch[2 * c], gi, ch[2 * c + 1] * gr));
+      } else {
+        o[0] = o[N] = o[2 * N] = make_double2(CUDART_NAN, CUDART_NAN);
       }
     }
   }
