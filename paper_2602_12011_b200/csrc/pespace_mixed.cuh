@@ -20,217 +20,285 @@ __constant__ double kMixCB[4] = {1.2599210498948731648, 1.0, 0.87358046473629886
 __constant__ double kMixLN3[4] = {0.23104906018664843647, 0.0, -0.13515503603605479399, -0.23104906018664843647};
 __constant__ double kMixS83[4] = {0.1574901312368591456, 1.0, 2.948334068485008683, 6.349604207872797899};
 
-// sin, cos of a phase a (pu, |a| < 2^22) in FP32 from the float table: first-order sine and second-order cosine
-// correction of the remainder |y| <= 1/2 pu (theta <= 3.1e-3: the dropped terms are < 5e-9)
-__device__ __forceinline__ void sincos_f(float y, int j, const float2* __restrict__ tabf, float& s, float& c) {
-  const float2 T = tabf[j & (NTAB - 1)];
-  const float sl = y * (float)kRadPerPu;
-  const float cl = -0.5f * sl * sl;
-  s = fmaf(T.y, sl, fmaf(T.x, cl, T.x));
-  c = fmaf(-T.x, sl, fmaf(T.y, cl, T.y));
+// ---- packed FP32 arithmetic (Blackwell FFMA2 / FMUL2 / FADD2: one instruction, two lanes).  A thread evaluates TWO
+// samples of its bin at once, lane x = sample s, lane y = sample s + 1: the FP32 part is bound by the issue port, and a
+// packed instruction does the work of two for one issue slot (the FP32 pipe is then busy two cycles, during which the
+// FP64 phase arithmetic, the table loads and the integer work issue for free).
+typedef float2 F2;
+__device__ __forceinline__ F2 bc2(float a) { return make_float2(a, a); }
+__device__ __forceinline__ F2 fma2(F2 a, F2 b, F2 c) { return __ffma2_rn(a, b, c); }
+__device__ __forceinline__ F2 mul2(F2 a, F2 b) { return __fmul2_rn(a, b); }
+__device__ __forceinline__ F2 add2(F2 a, F2 b) { return __fadd2_rn(a, b); }
+__device__ __forceinline__ F2 sub2(F2 a, F2 b) { return __ffma2_rn(b, make_float2(-1.0f, -1.0f), a); }   // a - b
+
+// the three float tables (sin, cos, cos - 1) are separate arrays so that the two lanes' entries load straight into
+// the halves of a register pair
+struct TabF { const float* sn; const float* cs; const float* cm1; };
+
+// sin, cos of the node j plus the remainder y (pu, |y| <= 1/2): first-order sine and second-order cosine correction
+// (theta <= 3.1e-3: the dropped terms are < 5e-9), both lanes
+__device__ __forceinline__ void sincos_f2(F2 y, int j0, int j1, const TabF& T, F2& s, F2& c) {
+  const F2 Tx = make_float2(T.sn[j0 & (NTAB - 1)], T.sn[j1 & (NTAB - 1)]);
+  const F2 Ty = make_float2(T.cs[j0 & (NTAB - 1)], T.cs[j1 & (NTAB - 1)]);
+  const F2 sl = mul2(y, bc2((float)kRadPerPu)), nsl = mul2(y, bc2(-(float)kRadPerPu));
+  const F2 cl = mul2(mul2(sl, sl), bc2(-0.5f));
+  s = fma2(Ty, sl, fma2(Tx, cl, Tx));
+  c = fma2(Tx, nsl, fma2(Ty, cl, Ty));
 }
-__device__ __forceinline__ void sincos_pu_f(float a, const float2* __restrict__ tabf, float& s, float& c) {
-  const float t = a + kMagicF;
-  sincos_f(a - (t - kMagicF), __float_as_int(t), tabf, s, c);
+// phase a in pu, |a| < 2^22
+__device__ __forceinline__ void sincos_pu_f2(F2 a, const TabF& T, F2& s, F2& c) {
+  const F2 t = add2(a, bc2(kMagicF));
+  const F2 y = sub2(a, add2(t, bc2(-kMagicF)));
+  sincos_f2(y, __float_as_int(t.x), __float_as_int(t.y), T, s, c);
 }
 
-// One mode class of one (sample, bin, detector): adds X, Y, Z (whitening and per-bin factor excluded) to S (FP32).
-//   sc: FP64 constants (phase polynomial), sf: FP32 copy of the same block with the amplitudes scaled by 2^64
+// per-bin numbers of the FP32 part, broadcast to both lanes
+struct BinF2 { F2 fm83, sth, nsth, ncth, omc, fTL; };
+
+// One mode class of one (bin, detector) for the sample pair (s, s + 1): adds X, Y, Z (whitening and per-bin factor
+// excluded) to S (FP32 pairs).
+//   sc0, sc1: FP64 constants of the two samples (phase polynomial, Doppler phase of the centre)
+//   sf: FP32 copy of the pair's blocks, constant j of both samples in one float2; amplitudes scaled by 2^64
 template <int KIND>
-__device__ __forceinline__ void eval_class_mixed(int MC, bool first, double fT, double cf, double lnf3, double fm53,
-                                                 float fm83f, float sthf, float cthf, float omcf, float fTLf,
-                                                 const double* __restrict__ sc, const float* __restrict__ sf,
-                                                 const DetC& dc, const float2* __restrict__ tabf,
-                                                 const float2* __restrict__ tabm1, double va, double ftc,
-                                                 float (&S)[6]) {
-  // ---- S2: phase, FP64
-  const double v = va * kMixCB[MC];
+__device__ __forceinline__ void eval_class_mixed(int MC, bool first, double fT, double lnf3, double fm53,
+                                                 const BinF2& bf, const double* __restrict__ sc0,
+                                                 const double* __restrict__ sc1, const F2* __restrict__ sf,
+                                                 const DetC& dc, const TabF& T, double va0, double va1, double ftc0,
+                                                 double ftc1, F2 (&S)[6]) {
+  // ---- S2: phase, FP64, per sample
   const double L = lnf3 + kMixLN3[MC];
-  const double v2 = v * v;
-  double P = fma(sc[W_P7], v, fma(sc[W_P6L], L, sc[W_P6]));
-  P = fma(P, v, fma(sc[W_P5L], L, sc[W_P5]));
-  P = fma(P, v, sc[W_P4]);
-  P = fma(P, v, sc[W_P3]);
-  P = fma(P, v, sc[W_P2]);
-  P = fma(P, v2, sc[W_P0]);
-  double psi = (kMixS83[MC] * fm53) * P;
-  psi -= whole_turns(psi);
-  psi += fma(0.5 * (double)(MC + 1), sc[W_PH0], ftc);
-  // ---- S3: t_lm, FP32
-  const float vf = (float)v, Lf = (float)L, v2f = vf * vf;
-  float Q = fmaf(sf[W_Q7], vf, fmaf(sf[W_Q6L], Lf, sf[W_Q6]));
-  Q = fmaf(Q, vf, sf[W_Q5]);
-  Q = fmaf(Q, vf, sf[W_Q4]);
-  Q = fmaf(Q, vf, sf[W_Q3]);
-  Q = fmaf(Q, vf, sf[W_Q2]);
-  Q = fmaf(Q, v2f, sf[W_Q0]);
-  const float tau = ((float)kMixS83[MC] * fm83f) * Q;
-  const float* ka = sf + W_KA + 4 * MC;
-  float CKp, CKc;
-  if (MC == 1) { CKp = fmaf(ka[1], v2f, ka[0]); CKc = fmaf(ka[3], v2f, ka[2]); }
-  else if (MC == 3) { CKp = v2f * ka[0]; CKc = v2f * ka[2]; }
-  else { CKp = vf * ka[0]; CKc = vf * ka[2]; }
-  // ---- S4: orbit, FP32
-  float G1k, G2k, G1u, G2u, G1v, G2v, cD, sD;      // cD, sD: cos, sin of the guiding-centre (Earth) angle
+  const double s53 = kMixS83[MC] * fm53, mh = 0.5 * (double)(MC + 1);
+  double v[2], psi[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const double* sc = h ? sc1 : sc0;
+    v[h] = (h ? va1 : va0) * kMixCB[MC];
+    const double v2 = v[h] * v[h];
+    double P = fma(sc[W_P7], v[h], fma(sc[W_P6L], L, sc[W_P6]));
+    P = fma(P, v[h], fma(sc[W_P5L], L, sc[W_P5]));
+    P = fma(P, v[h], sc[W_P4]);
+    P = fma(P, v[h], sc[W_P3]);
+    P = fma(P, v[h], sc[W_P2]);
+    P = fma(P, v2, sc[W_P0]);
+    double x = s53 * P;
+    x -= whole_turns(x);
+    psi[h] = x + fma(mh, sc[W_PH0], h ? ftc1 : ftc0);
+  }
+  // ---- S3: t_lm, FP32 pairs
+  const F2 vf = make_float2((float)v[0], (float)v[1]), Lf = bc2((float)L), v2f = mul2(vf, vf);
+  F2 Q = fma2(sf[W_Q7], vf, fma2(sf[W_Q6L], Lf, sf[W_Q6]));
+  Q = fma2(Q, vf, sf[W_Q5]);
+  Q = fma2(Q, vf, sf[W_Q4]);
+  Q = fma2(Q, vf, sf[W_Q3]);
+  Q = fma2(Q, vf, sf[W_Q2]);
+  Q = fma2(Q, v2f, sf[W_Q0]);
+  const F2 tau = mul2(mul2(bc2((float)kMixS83[MC]), bf.fm83), Q);
+  const F2* ka = sf + W_KA + 4 * MC;
+  F2 CKp, CKc;
+  if (MC == 1) { CKp = fma2(ka[1], v2f, ka[0]); CKc = fma2(ka[3], v2f, ka[2]); }
+  else if (MC == 3) { CKp = mul2(v2f, ka[0]); CKc = mul2(v2f, ka[2]); }
+  else { CKp = mul2(vf, ka[0]); CKc = mul2(vf, ka[2]); }
+  // ---- S4: orbit, FP32 pairs
+  F2 G1k, G2k, G1u, G2u, G1v, G2v, cD, sD;         // cD, sD: cos, sin of the guiding-centre (Earth) angle
   if (KIND == 0) {
-    float sa, ca;
-    sincos_pu_f(sf[D_BASE] + tau, tabf, sa, ca);
-    const float c2 = fmaf(2.0f * ca, ca, -1.0f), s2 = 2.0f * sa * ca;
-    const float* w = sf + S_K;
-    G1k = fmaf(w[0], c2, fmaf(w[1], s2, fmaf(w[2], ca, w[3])));
-    G2k = fmaf(w[0], s2, fmaf(-w[1], c2, fmaf(w[2], sa, w[4])));
+    F2 sa, ca;
+    sincos_pu_f2(add2(sf[D_BASE], tau), T, sa, ca);
+    const F2 ca2 = add2(ca, ca);
+    const F2 c2 = fma2(ca2, ca, bc2(-1.0f)), nc2 = fma2(mul2(ca, bc2(-2.0f)), ca, bc2(1.0f)), s2 = mul2(add2(sa, sa), ca);
+    const F2* w = sf + S_K;
+    G1k = fma2(w[0], c2, fma2(w[1], s2, fma2(w[2], ca, w[3])));
+    G2k = fma2(w[0], s2, fma2(w[1], nc2, fma2(w[2], sa, w[4])));
     w = sf + S_U;
-    G1u = fmaf(w[0], c2, fmaf(w[1], s2, fmaf(w[2], ca, w[3])));
-    G2u = fmaf(w[0], s2, fmaf(-w[1], c2, fmaf(w[2], sa, w[4])));
+    G1u = fma2(w[0], c2, fma2(w[1], s2, fma2(w[2], ca, w[3])));
+    G2u = fma2(w[0], s2, fma2(w[1], nc2, fma2(w[2], sa, w[4])));
     w = sf + S_V;
-    G1v = fmaf(w[0], c2, fmaf(w[1], s2, fmaf(w[2], ca, w[3])));
-    G2v = fmaf(w[0], s2, fmaf(-w[1], c2, fmaf(w[2], sa, w[4])));
+    G1v = fma2(w[0], c2, fma2(w[1], s2, fma2(w[2], ca, w[3])));
+    G2v = fma2(w[0], s2, fma2(w[1], nc2, fma2(w[2], sa, w[4])));
     cD = ca; sD = sa;
   } else {
-    float sp, cp;
-    sincos_pu_f(sf[D_BASE] + tau, tabf, sD, cD);
-    sincos_pu_f(fmaf(tau, (float)dc.yr_over_p, sf[D_BASE + 1]), tabf, sp, cp);
-    const float* w = sf + D_BASE + 2;
-    G1k = fmaf(w[0], cp, w[1] * sp); G2k = fmaf(w[1], cp, -w[0] * sp);
-    G1u = fmaf(w[2], cp, w[3] * sp); G2u = fmaf(w[3], cp, -w[2] * sp);
-    G1v = fmaf(w[4], cp, w[5] * sp); G2v = fmaf(w[5], cp, -w[4] * sp);
+    F2 sp, cp;
+    sincos_pu_f2(add2(sf[D_BASE], tau), T, sD, cD);
+    sincos_pu_f2(fma2(tau, bc2((float)dc.yr_over_p), sf[D_BASE + 1]), T, sp, cp);
+    const F2 nsp = mul2(sp, bc2(-1.0f));
+    const F2* w = sf + D_BASE + 2;
+    G1k = fma2(w[0], cp, mul2(w[1], sp)); G2k = fma2(w[1], cp, mul2(w[0], nsp));
+    G1u = fma2(w[2], cp, mul2(w[3], sp)); G2u = fma2(w[3], cp, mul2(w[2], nsp));
+    G1v = fma2(w[4], cp, mul2(w[5], sp)); G2v = fma2(w[5], cp, mul2(w[4], nsp));
   }
   constexpr float R3H = 0.86602540378443864676f;
-  const float tk = R3H * G2k;
-  const float nun[3] = {G1k, fmaf(-0.5f, G1k, tk), fmaf(-0.5f, G1k, -tk)};
-  const float ka_ = tk + tk, kb_ = fmaf(-1.5f, G1k, -tk), kc_ = fmaf(1.5f, G1k, -tk);
-  const float tu = R3H * G2u, tv = R3H * G2v;
-  const float ul[3] = {tu + tu, fmaf(-1.5f, G1u, -tu), fmaf(1.5f, G1u, -tu)};
-  const float vl[3] = {tv + tv, fmaf(-1.5f, G1v, -tv), fmaf(1.5f, G1v, -tv)};
-  // ---- S5: arm weights, FP32
-  float Wr[3], Wi[3];
+  const F2 tk = mul2(bc2(R3H), G2k), ntk = mul2(bc2(-R3H), G2k);
+  const F2 nun[3] = {G1k, fma2(bc2(-0.5f), G1k, tk), fma2(bc2(-0.5f), G1k, ntk)};
+  // -k.n_l for the arms a, b, c
+  const F2 nkap[3] = {add2(ntk, ntk), fma2(bc2(1.5f), G1k, tk), fma2(bc2(-1.5f), G1k, tk)};
+  const F2 tu = mul2(bc2(R3H), G2u), ntu = mul2(bc2(-R3H), G2u), tv = mul2(bc2(R3H), G2v), ntv = mul2(bc2(-R3H), G2v);
+  const F2 ul[3] = {add2(tu, tu), fma2(bc2(-1.5f), G1u, ntu), fma2(bc2(1.5f), G1u, ntu)};
+  const F2 vl[3] = {add2(tv, tv), fma2(bc2(-1.5f), G1v, ntv), fma2(bc2(1.5f), G1v, ntv)};
+  // ---- S5: arm weights, FP32 pairs (the reciprocal is MUFU.RCP per lane, ~1 ulp)
+  F2 Wr[3], Wi[3], nWi[3];
 #pragma unroll
   for (int l = 0; l < 3; ++l) {
-    const float uu = ul[l], vv = vl[l];
-    const float v2_ = vv * vv;
-    const float D = fmaf(uu, uu, v2_);
-    float rD;
-    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rD) : "f"(D));        // MUFU.RCP, ~1 ulp
-    rD = (D > 0.0f) ? rD : 0.0f;
-    Wr[l] = (CKp * rD) * fmaf(uu, uu, -v2_);
-    Wi[l] = (CKc * rD) * (uu * vv);
+    const F2 uu = ul[l], vv = vl[l];
+    const F2 v2_ = mul2(vv, vv);
+    const F2 D = fma2(uu, uu, v2_);
+    F2 rD;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rD.x) : "f"(D.x));
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rD.y) : "f"(D.y));
+    rD.x = (D.x > 0.0f) ? rD.x : 0.0f;
+    rD.y = (D.y > 0.0f) ? rD.y : 0.0f;
+    Wr[l] = mul2(mul2(CKp, rD), fma2(bc2(-2.0f), v2_, D));        // u^2 - v^2 = (u^2 + v^2) - 2 v^2
+    Wi[l] = mul2(mul2(CKc, rD), mul2(uu, vv));
+    nWi[l] = mul2(Wi[l], bc2(-1.0f));
   }
   // ---- S6: exponentials relative to the guiding centre.  E_n = E_c (1 + delta_n), E_c = exp(-i base) with the
   // large phase base = psi + kTurn f k.x_centre reduced in FP64 (Doppler phase of the centre from the FP64 constants),
   // delta_n = exp(-i a_n) - 1 with the arm-scale phase a_n = kTurn f L k.(x_n - x_centre)/L, |a_n| < 1 turn, in FP32
   // from the (sin, cos - 1) table: at low frequency a_n -> 0 and the brackets below are differences of O(2 pi f L)
   // quantities, which this form evaluates without cancelling against 1 (FP32 would lose 1 / (2 pi f L) digits).
-  const double kR = fma(sc[S_DX], (double)cD, sc[S_DY] * (double)sD);
-  const double ub = fma(fT, kR, psi);
-  const double tb = ub + kMagic;
-  float sb, cb;
-  sincos_f((float)(ub - (tb - kMagic)), __double2loint(tb), tabf, sb, cb);
-  float dC[3], dS[3];                 // cos a_n - 1, sin a_n
+  F2 yb;
+  int jb[2];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    const double* sc = h ? sc1 : sc0;
+    const double kR = fma(sc[S_DX], (double)(h ? cD.y : cD.x), sc[S_DY] * (double)(h ? sD.y : sD.x));
+    const double ub = fma(fT, kR, psi[h]);
+    const double tb = ub + kMagic;
+    (h ? yb.y : yb.x) = (float)(ub - (tb - kMagic));
+    jb[h] = __double2loint(tb);
+  }
+  F2 sb, cb;
+  sincos_f2(yb, jb[0], jb[1], T, sb, cb);
+  const F2 nsb = mul2(sb, bc2(-1.0f));
+  F2 dC[3], dS[3];                    // cos a_n - 1, sin a_n
 #pragma unroll
   for (int n = 0; n < 3; ++n) {
-    const float a = fTLf * nun[n];
-    const float t = a + kMagicF;
-    const float y = a - (t - kMagicF);
-    const float2 T = tabm1[__float_as_int(t) & (NTAB - 1)];        // (sin, cos - 1) of the node
-    const float sl = y * (float)kRadPerPu, cl = -0.5f * sl * sl, Ty = 1.0f + T.y;
-    dS[n] = fmaf(Ty, sl, fmaf(T.x, cl, T.x));
-    dC[n] = fmaf(-T.x, sl, fmaf(Ty, cl, T.y));
+    const F2 a = mul2(bf.fTL, nun[n]);
+    const F2 t = add2(a, bc2(kMagicF));
+    const F2 y = sub2(a, add2(t, bc2(-kMagicF)));
+    const int j0 = __float_as_int(t.x) & (NTAB - 1), j1 = __float_as_int(t.y) & (NTAB - 1);
+    const F2 Tx = make_float2(T.sn[j0], T.sn[j1]), Ty = make_float2(T.cs[j0], T.cs[j1]);
+    const F2 Tm = make_float2(T.cm1[j0], T.cm1[j1]);               // cos - 1 of the node, full relative accuracy
+    const F2 sl = mul2(y, bc2((float)kRadPerPu)), nsl = mul2(y, bc2(-(float)kRadPerPu));
+    const F2 cl = mul2(mul2(sl, sl), bc2(-0.5f));
+    dS[n] = fma2(Ty, sl, fma2(Tx, cl, Tx));
+    dC[n] = fma2(Tx, nsl, fma2(Ty, cl, Tm));
   }
-  // ---- S7: brackets in the centre frame, B'(r,s,kap) = kap (delta_s - cos(th) delta_r + (1 - cos th)) - i sin(th) (1 + delta_r)
-  float Sc[6];
-  auto add = [&](float& Sr, float& Si, int r, int s_, float kap, float wr, float wi, bool init) {
-    const float br = fmaf(kap, fmaf(-cthf, dC[r], dC[s_]) + omcf, -sthf * dS[r]);
-    const float bi = fmaf(kap, fmaf(-cthf, dS[r], dS[s_]), fmaf(sthf, dC[r], sthf));
+  // ---- S7: brackets in the centre frame, B'(r,s,kap) = kap (delta_s - cos(th) delta_r + (1 - cos th)) - i sin(th) (1 + delta_r).
+  // The three "minus W" terms of the TDI sums are taken as W times MINUS the bracket, so that only -k.n_l is needed.
+  F2 Ps[3], nPs[3], Qs[3], nQs[3];
+#pragma unroll
+  for (int r = 0; r < 3; ++r) {
+    Ps[r] = mul2(bf.sth, dS[r]); nPs[r] = mul2(bf.nsth, dS[r]);
+    Qs[r] = fma2(bf.sth, dC[r], bf.sth); nQs[r] = fma2(bf.nsth, dC[r], bf.nsth);
+  }
+  F2 Sc[6];
+  // plus = true: + W B(r, s, kap = km);  plus = false: - W B(r, s, kap = -km)
+  auto add = [&](F2& Sr, F2& Si, int r, int s_, F2 km, int l, bool plus, bool init) {
+    const F2 in_r = add2(fma2(bf.ncth, dC[r], dC[s_]), bf.omc), in_i = fma2(bf.ncth, dS[r], dS[s_]);
+    const F2 br = fma2(km, in_r, plus ? nPs[r] : Ps[r]);
+    const F2 bi = fma2(km, in_i, plus ? Qs[r] : nQs[r]);
     if (init) {
-      Sr = fmaf(wr, br, -wi * bi);
-      Si = fmaf(wr, bi, wi * br);
+      Sr = fma2(Wr[l], br, mul2(nWi[l], bi));
+      Si = fma2(Wr[l], bi, mul2(Wi[l], br));
     } else {
-      Sr = fmaf(wr, br, fmaf(-wi, bi, Sr));
-      Si = fmaf(wr, bi, fmaf(wi, br, Si));
+      Sr = fma2(Wr[l], br, fma2(nWi[l], bi, Sr));
+      Si = fma2(Wr[l], bi, fma2(Wi[l], br, Si));
     }
   };
-  add(Sc[0], Sc[1], 0, 2, -kb_, Wr[1], Wi[1], true);
-  add(Sc[0], Sc[1], 0, 1, kc_, -Wr[2], -Wi[2], false);
-  add(Sc[2], Sc[3], 1, 0, -kc_, Wr[2], Wi[2], true);
-  add(Sc[2], Sc[3], 1, 2, ka_, -Wr[0], -Wi[0], false);
-  add(Sc[4], Sc[5], 2, 1, -ka_, Wr[0], Wi[0], true);
-  add(Sc[4], Sc[5], 2, 0, kb_, -Wr[1], -Wi[1], false);
+  // arms: index 0 = a (2-3), 1 = b (3-1), 2 = c (1-2)
+  add(Sc[0], Sc[1], 0, 2, nkap[1], 1, true, true);      // X: + W_b B(1,3,-k.n_b)
+  add(Sc[0], Sc[1], 0, 1, nkap[2], 2, false, false);    //    - W_c B(1,2,+k.n_c)
+  add(Sc[2], Sc[3], 1, 0, nkap[2], 2, true, true);      // Y: + W_c B(2,1,-k.n_c)
+  add(Sc[2], Sc[3], 1, 2, nkap[0], 0, false, false);    //    - W_a B(2,3,+k.n_a)
+  add(Sc[4], Sc[5], 2, 1, nkap[0], 0, true, true);      // Z: + W_a B(3,2,-k.n_a)
+  add(Sc[4], Sc[5], 2, 0, nkap[1], 1, false, false);    //    - W_b B(3,1,+k.n_b)
   // back to the SSB frame: (Sr - i Si) (cb - i sb)
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    const float xr = fmaf(Sc[2 * c], cb, -Sc[2 * c + 1] * sb), xi = fmaf(Sc[2 * c], sb, Sc[2 * c + 1] * cb);
-    if (first) { S[2 * c] = xr; S[2 * c + 1] = xi; }
-    else { S[2 * c] += xr; S[2 * c + 1] += xi; }
+    if (first) {
+      S[2 * c] = fma2(Sc[2 * c], cb, mul2(Sc[2 * c + 1], nsb));
+      S[2 * c + 1] = fma2(Sc[2 * c], sb, mul2(Sc[2 * c + 1], cb));
+    } else {
+      S[2 * c] = fma2(Sc[2 * c], cb, fma2(Sc[2 * c + 1], nsb, S[2 * c]));
+      S[2 * c + 1] = fma2(Sc[2 * c], sb, fma2(Sc[2 * c + 1], cb, S[2 * c + 1]));
+    }
   }
 }
 
-// dynamic shared memory: [float2 (sin, cos) table | float2 (sin, cos - 1) table | FP64 sample constants | FP32 copy |
-// warp partials]
+// dynamic shared memory: [float sin | cos | cos - 1 tables | FP64 sample constants | FP32 copy, the two samples of a
+// pair interleaved | warp partials]
 constexpr int MIX_TILE = 64;
+static_assert(MIX_TILE % 4 == 0, "sample pairs; stage_tile pads the tile to a multiple of four samples");
 constexpr size_t mixed_smem_used() {
-  return 2 * sizeof(float2) * NTAB + sizeof(double) * (size_t)MIX_TILE * SMEM_STRIDE +
+  return 3 * sizeof(float) * NTAB + sizeof(double) * (size_t)MIX_TILE * SMEM_STRIDE +
          sizeof(float) * (size_t)MIX_TILE * SMEM_STRIDE + sizeof(double) * (size_t)(BLOCK / 32) * MIX_TILE;
 }
-constexpr size_t mixed_smem_bytes() { return mixed_smem_used(); }
+constexpr size_t mixed_smem_bytes() { return (mixed_smem_used() + 15) / 16 * 16; }
 
 #ifndef PESPACE_MINBX
 #define PESPACE_MINBX 2
 #endif
 // CMASK != 0: the classes of that mask unrolled at compile time (the masks of configs 2-4); 0: any mask, run-time loop
 template <int KIND, unsigned CMASK>
-__global__ void __launch_bounds__(BLOCK, PESPACE_MINBX)
+__global__ void __launch_bounds__(BLOCK, popc4(CMASK) > 1 ? 1 : PESPACE_MINBX)      // four classes unrolled: 128 registers spill
 loglike_mixed_kernel(const double* __restrict__ consts, const double2* __restrict__ trig, long long B, unsigned cmask,
                      const double* __restrict__ bins /* [n_det][NBF][N], built with fold mode 2 */, long long N, DetC dc,
                      int n_det, int det, double* __restrict__ partial /* [n_det][gridDim.x][B] */) {
-  float2* tabf = reinterpret_cast<float2*>(pespace_dyn_smem);
-  float2* tabm1 = tabf + NTAB;
-  double* smem = reinterpret_cast<double*>(tabm1 + NTAB);
-  float* smf = reinterpret_cast<float*>(smem + MIX_TILE * SMEM_STRIDE);
-  double (*red)[MIX_TILE] = reinterpret_cast<double (*)[MIX_TILE]>(smf + MIX_TILE * SMEM_STRIDE);
+  double* smem = reinterpret_cast<double*>(pespace_dyn_smem);                  // FP64 constants first: 16-byte aligned
+  F2* smf = reinterpret_cast<F2*>(smem + MIX_TILE * SMEM_STRIDE);              // [MIX_TILE / 2][SMEM_STRIDE] pairs
+  double (*red)[MIX_TILE] = reinterpret_cast<double (*)[MIX_TILE]>(smf + (MIX_TILE / 2) * SMEM_STRIDE);
+  float* tsn = reinterpret_cast<float*>(&red[BLOCK / 32][0]);
+  float* tcs = tsn + NTAB;
+  float* tm1 = tcs + NTAB;
+  const TabF T{tsn, tcs, tm1};
   const long long b0 = (long long)blockIdx.y * MIX_TILE;
   for (int i = threadIdx.x; i < NTAB; i += blockDim.x) {
-    const double2 T = trig[i];
-    tabf[i] = make_float2((float)T.x, (float)T.y);
+    const double2 t = trig[i];
+    tsn[i] = (float)t.x;
+    tcs[i] = (float)t.y;
     // cos - 1 = -sin^2 / (1 + cos) where cos > 0, formed in FP64 so that the float keeps full relative accuracy
-    tabm1[i] = make_float2((float)T.x, (float)(T.y > 0.0 ? -T.x * T.x / (1.0 + T.y) : T.y - 1.0));
+    tm1[i] = (float)(t.y > 0.0 ? -t.x * t.x / (1.0 + t.y) : t.y - 1.0);
   }
   stage_tile(smem, consts, b0, B, n_det, det);
   __syncthreads();
   for (int i = threadIdx.x; i < MIX_TILE * SMEM_STRIDE; i += blockDim.x) {
-    const int j = i % SMEM_STRIDE;
+    const int sidx = i / SMEM_STRIDE, j = i % SMEM_STRIDE;
     double x = smem[i];
     if (j >= W_KA && j < W_KA + 16) x *= (double)kAmpScale;       // amplitudes carry the 2^64 scale
-    smf[i] = (float)x;
+    float* dst = reinterpret_cast<float*>(smf + (sidx >> 1) * SMEM_STRIDE + j);
+    dst[sidx & 1] = (float)x;
   }
   const long long k = (long long)blockIdx.x * BLOCK + threadIdx.x;
   const bool live = k < N;
   const double* bp = bins + (size_t)det * NBF * (size_t)N + (size_t)(live ? k : N - 1);
   const double fT = bp[BF_FT * N], cf = bp[BF_CF * N], lnf3 = bp[BF_LNF3 * N], fm53 = bp[BF_FM53 * N];
-  const float fm83f = (float)bp[BF_FM83 * N], sthf = (float)bp[BF_STH * N], cthf = (float)bp[BF_CTH * N];
-  const float fTLf = (float)(fT * dc.Lbar);
   const double sth = bp[BF_STH * N], cth = bp[BF_CTH * N];
-  const float omcf = (float)(cth > 0.0 ? sth * sth / (1.0 + cth) : 1.0 - cth);     // 1 - cos(2 pi f L), no cancellation
-  float dr[3], di[3], sw[3];
+  BinF2 bf;
+  bf.fm83 = bc2((float)bp[BF_FM83 * N]);
+  bf.sth = bc2((float)sth); bf.nsth = bc2(-(float)sth); bf.ncth = bc2(-(float)cth);
+  bf.omc = bc2((float)(cth > 0.0 ? sth * sth / (1.0 + cth) : 1.0 - cth));       // 1 - cos(2 pi f L), no cancellation
+  bf.fTL = bc2((float)(fT * dc.Lbar));
+  F2 dr[3], di[3], nsw[3];
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
-    dr[c] = (float)bp[(BF_DR + c) * N]; di[c] = (float)bp[(BF_DI + c) * N];
-    sw[c] = live ? (float)bp[(BF_W + c) * N] : 0.0f;
-    if (!live) { dr[c] = 0.0f; di[c] = 0.0f; }
+    dr[c] = bc2(live ? (float)bp[(BF_DR + c) * N] : 0.0f);
+    di[c] = bc2(live ? (float)bp[(BF_DI + c) * N] : 0.0f);
+    nsw[c] = bc2(live ? -(float)bp[(BF_W + c) * N] : 0.0f);
   }
   __syncthreads();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int ns = (int)min((long long)MIX_TILE, B - b0);
-  for (int s = 0; s < ns; ++s) {
-    const double* sc = smem + s * SMEM_STRIDE;
-    const float* sf = smf + s * SMEM_STRIDE;
-    const double ftc = mul_mod_turn(fT, sc[W_TC]);
-    const double va = sc[W_A] * cf;
-    float S[6];
+  for (int s = 0; s < ns; s += 2) {          // the pair (s, s + 1); stage_tile pads an odd tail with a copy
+    const double* sc0 = smem + s * SMEM_STRIDE;
+    const double* sc1 = sc0 + SMEM_STRIDE;
+    const F2* sf = smf + (s >> 1) * SMEM_STRIDE;
+    const double ftc0 = mul_mod_turn(fT, sc0[W_TC]), ftc1 = mul_mod_turn(fT, sc1[W_TC]);
+    const double va0 = sc0[W_A] * cf, va1 = sc1[W_A] * cf;
+    F2 S[6];
     if constexpr (CMASK != 0u) {
-#define PESPACE_MIX_CLASS(MC)                                                                                    \
-      if constexpr ((CMASK >> MC) & 1u)                                                                            \
-        eval_class_mixed<KIND>(MC, !(CMASK & ((1u << MC) - 1u)), fT, cf, lnf3, fm53, fm83f, sthf, cthf, omcf, fTLf, sc, sf, \
-                               dc, tabf, tabm1, va, ftc, S);
+#define PESPACE_MIX_CLASS(MC)                                                                                       \
+      if constexpr ((CMASK >> MC) & 1u)                                                                               \
+        eval_class_mixed<KIND>(MC, !(CMASK & ((1u << MC) - 1u)), fT, lnf3, fm53, bf, sc0, sc1, sf, dc, T, va0, va1, ftc0, \
+                               ftc1, S);
       PESPACE_MIX_CLASS(0) PESPACE_MIX_CLASS(1) PESPACE_MIX_CLASS(2) PESPACE_MIX_CLASS(3)
 #undef PESPACE_MIX_CLASS
     } else {
@@ -238,23 +306,25 @@ loglike_mixed_kernel(const double* __restrict__ consts, const double2* __restric
 #pragma unroll 1
       for (int mc = 0; mc < 4; ++mc) {
         if (!((cmask >> mc) & 1u)) continue;
-        eval_class_mixed<KIND>(mc, first, fT, cf, lnf3, fm53, fm83f, sthf, cthf, omcf, fTLf, sc, sf, dc, tabf, tabm1, va,
-                               ftc, S);
+        eval_class_mixed<KIND>(mc, first, fT, lnf3, fm53, bf, sc0, sc1, sf, dc, T, va0, va1, ftc0, ftc1, S);
         first = false;
       }
     }
-    const float Ar = S[4] - S[0], Ai = S[5] - S[1];
-    const float Er_ = S[0] - 2.0f * S[2] + S[4], Ei_ = S[1] - 2.0f * S[3] + S[5];
-    const float Tr = S[0] + S[2] + S[4], Ti = S[1] + S[3] + S[5];
-    float r0 = fmaf(-sw[0], Ar, dr[0]), r1 = fmaf(-sw[0], Ai, di[0]);
-    float acc = fmaf(r0, r0, r1 * r1);
-    r0 = fmaf(-sw[1], Er_, dr[1]); r1 = fmaf(-sw[1], Ei_, di[1]);
-    acc += fmaf(r0, r0, r1 * r1);
-    r0 = fmaf(-sw[2], Tr, dr[2]); r1 = fmaf(-sw[2], Ti, di[2]);
-    acc += fmaf(r0, r0, r1 * r1);
+    const F2 Ar = sub2(S[4], S[0]), Ai = sub2(S[5], S[1]);
+    const F2 Er_ = fma2(bc2(-2.0f), S[2], add2(S[0], S[4])), Ei_ = fma2(bc2(-2.0f), S[3], add2(S[1], S[5]));
+    const F2 Tr = add2(add2(S[0], S[2]), S[4]), Ti = add2(add2(S[1], S[3]), S[5]);
+    F2 r0 = fma2(nsw[0], Ar, dr[0]), r1 = fma2(nsw[0], Ai, di[0]);
+    F2 acc2 = fma2(r0, r0, mul2(r1, r1));
+    r0 = fma2(nsw[1], Er_, dr[1]); r1 = fma2(nsw[1], Ei_, di[1]);
+    acc2 = fma2(r0, r0, fma2(r1, r1, acc2));
+    r0 = fma2(nsw[2], Tr, dr[2]); r1 = fma2(nsw[2], Ti, di[2]);
+    acc2 = fma2(r0, r0, fma2(r1, r1, acc2));
+    // S9: halving butterfly: after the first level the lanes 0-15 hold sample s, the lanes 16-31 sample s + 1
+    const bool up = lane & 16;
+    float acc = (up ? acc2.y : acc2.x) + __shfl_xor_sync(0xffffffffu, up ? acc2.x : acc2.y, 16);
 #pragma unroll
-    for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-    if (lane == 0) red[warp][s] = (double)acc;
+    for (int o = 8; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
+    if ((lane & 15) == 0) red[warp][s + (lane >> 4)] = (double)acc;     // s + 1 <= MIX_TILE - 1 (s even)
   }
   __syncthreads();
   if (threadIdx.x < ns) {
