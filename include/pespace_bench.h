@@ -20,7 +20,12 @@ extern "C" {
  *           read bandwidth then limits the pipe to 1 / 3 cycles (profiles/r01_fp64_operand_bandwidth.md);
  *   modes 2-5: FP64 tensor-core probe, `iters` blocks of 8 x NACC mma.sync.m8n8k4.f64 (DMMA, 256 FMAs per warp
  *           instruction) per warp: 2: NACC = 8 independent accumulators; 3: NACC = 2; 4: NACC = 8 with one
- *           independent DFMA per DMMA interleaved; 5: with four (profiles/r02_dmma.md). */
+ *           independent DFMA per DMMA interleaved; 5: with four (profiles/r02_dmma.md);
+ *   modes 6-10: register-operand probes (profiles/r02_operand_reuse.md): 6: DFMA a_j = a_j m + c_j, one operand
+ *           shared with the preceding instruction; 7: DFMA a_j = a_j b_{j&1} + c_j, shared with the one before
+ *           that; 8: FP32 FFMA with three distinct registers (128 FMAs per thread and block of rounds; the rate
+ *           is returned in FP32 TFLOP/s); 9: packed FFMA2 with three distinct register pairs; 10: FFMA with
+ *           multiplier and addend shared (the FP32 pipe peak). */
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms);
 
 /* Kernel timing for roofline reports.  While enabled, every launch of the dominant kernel

@@ -238,7 +238,7 @@ int pespace::host::loglike_impl(const double* d_params, int64_t B, const double*
 extern "C" {
 
 int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_ms) {
-  if (iters <= 0 || !h_out_tflops || mode < 0 || mode > 5) return PESPACE_EINVAL;
+  if (iters <= 0 || !h_out_tflops || mode < 0 || mode > 10) return PESPACE_EINVAL;
   int dev = 0, sms = 0;
   CU(cudaGetDevice(&dev));
   CU(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
@@ -256,7 +256,12 @@ int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_m
     else if (mode == 2) dmma_peak_kernel<8, 0><<<blocks, threads>>>(n, d_in, d_out);
     else if (mode == 3) dmma_peak_kernel<2, 0><<<blocks, threads>>>(n, d_in, d_out);
     else if (mode == 4) dmma_peak_kernel<8, 1><<<blocks, threads>>>(n, d_in, d_out);
-    else dmma_peak_kernel<8, 4><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 5) dmma_peak_kernel<8, 4><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 6) operand_probe_kernel<0><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 7) operand_probe_kernel<1><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 8) operand_probe_kernel<2><<<blocks, threads>>>(n, d_in, d_out);
+    else if (mode == 9) operand_probe_kernel<3><<<blocks, threads>>>(n, d_in, d_out);
+    else operand_probe_kernel<4><<<blocks, threads>>>(n, d_in, d_out);
     ++g_launches;
   };
   go(iters / 8 + 1);   // warm-up
@@ -266,10 +271,11 @@ int pespace_fp64_peak(int mode, int iters, double* h_out_tflops, double* h_out_m
   CU(cudaEventSynchronize(e1));
   float ms = 0.f;
   CU(cudaEventElapsedTime(&ms, e0, e1));
-  // per thread and iteration: modes 0, 1: 64 DFMAs; modes 2-5: 8 x NACC DMMAs of 256 FMAs per warp (8 per thread) plus
-  // DFMA_MIX DFMAs per DMMA
+  // per thread and iteration: modes 0, 1, 6, 7: 64 DFMAs; modes 2-5: 8 x NACC DMMAs of 256 FMAs per warp (8 per
+  // thread) plus DFMA_MIX DFMAs per DMMA; modes 8-10: 128 FP32 FMAs
   const double fma_per_thread_iter = mode <= 1 ? 64.0 : mode == 2 ? 8.0 * 8 * 8 : mode == 3 ? 8.0 * 2 * 8
-                                     : mode == 4 ? 8.0 * 8 * (8 + 1) : 8.0 * 8 * (8 + 4);
+                                     : mode == 4 ? 8.0 * 8 * (8 + 1) : mode == 5 ? 8.0 * 8 * (8 + 4)
+                                     : mode <= 7 ? 64.0 : 128.0;
   const double flops = 2.0 * fma_per_thread_iter * (double)iters * (double)blocks * (double)threads;
   *h_out_tflops = flops / (ms * 1e-3) / 1e12;
   if (h_out_ms) *h_out_ms = ms;

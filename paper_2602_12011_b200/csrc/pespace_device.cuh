@@ -840,6 +840,58 @@ __global__ void __launch_bounds__(256) dfma_peak_kernel(int iters, const double*
   if (r == 12345.678) out[0] = r;   // never true; keeps the chains alive
 }
 
+// Register-operand probes (profiles/r02_operand_reuse.md).  Eight rounds of 8 FP64 / 16 FP32 / 8 packed-FP32 chains:
+//   MODE 0: DFMA a_j = a_j m + c_j       one operand (m) shared with the preceding instruction
+//   MODE 1: DFMA a_j = a_j b_{j&1} + c_j one operand shared with the instruction before the preceding one
+//   MODE 2: FFMA a_j = a_j b_j + c_j     three distinct registers
+//   MODE 3: FFMA2 (two FP32 lanes per instruction) p_j = p_j q_j + r_j, three distinct register pairs
+//   MODE 4: FFMA a_j = a_j m + c         multiplier and addend shared (the FP32 pipe peak)
+template <int MODE>
+__global__ void __launch_bounds__(256) operand_probe_kernel(int iters, const double* __restrict__ in,
+                                                            double* __restrict__ out) {
+  double a[8], b[8], c[8];
+  float fa[16], fb[16], fc[16];
+  float2 p[8], q[8], r[8];
+  const double m = in[threadIdx.x & 31];
+#pragma unroll
+  for (int j = 0; j < 8; ++j) {
+    a[j] = in[(threadIdx.x + j) & 63]; b[j] = in[(threadIdx.x + 2 * j + 1) & 63]; c[j] = in[(threadIdx.x + 3 * j + 2) & 63];
+  }
+#pragma unroll
+  for (int j = 0; j < 16; ++j) { fa[j] = (float)in[(threadIdx.x + j) & 63]; fb[j] = (float)in[(threadIdx.x + 2 * j + 1) & 63]; fc[j] = (float)in[(threadIdx.x + 3 * j + 2) & 63]; }
+#pragma unroll
+  for (int j = 0; j < 8; ++j) { p[j] = make_float2(fa[2 * j], fa[2 * j + 1]); q[j] = make_float2(fb[2 * j], fb[2 * j + 1]); r[j] = make_float2(fc[2 * j], fc[2 * j + 1]); }
+  const float fm = (float)m, fcc = fc[0];
+  for (int i = 0; i < iters; ++i) {
+#pragma unroll
+    for (int rr = 0; rr < 8; ++rr) {
+      if (MODE == 0) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = fma(a[j], m, c[j]);
+      } else if (MODE == 1) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) a[j] = fma(a[j], b[j & 1], c[j]);
+      } else if (MODE == 2) {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) fa[j] = fmaf(fa[j], fb[j], fc[j]);
+      } else if (MODE == 3) {
+#pragma unroll
+        for (int j = 0; j < 8; ++j) p[j] = __ffma2_rn(p[j], q[j], r[j]);
+      } else {
+#pragma unroll
+        for (int j = 0; j < 16; ++j) fa[j] = fmaf(fa[j], fm, fcc);
+      }
+    }
+  }
+  double t = 0.0;
+#pragma unroll
+  for (int j = 0; j < 8; ++j) t += a[j] + (double)p[j].x + (double)p[j].y;
+#pragma unroll
+  for (int j = 0; j < 16; ++j) t += (double)fa[j];
+  if (t == 12345.678) out[0] = t;
+}
+
+
 // FP64 tensor-core probe: chains of mma.sync.aligned.m8n8k4 (DMMA, 8 x 8 x 4 = 256 FMAs per warp instruction) on NACC
 // independent accumulator fragments per warp; DFMA_MIX > 0 interleaves that many independent DFMAs per DMMA, to see
 // whether the two share the FP64 issue port (profiles/r02_dmma.md)
