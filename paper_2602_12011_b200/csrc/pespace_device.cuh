@@ -738,8 +738,18 @@ static __global__ void combine_kernel(const double* __restrict__ partial, const 
   const int x = threadIdx.x, g = threadIdx.y;
   const long long b = (long long)blockIdx.x * 32 + x;
   double t = 0.0;
-  if (b < B)
-    for (int i = g; i < n_slices; i += CGROUPS) t += partial[(size_t)i * (size_t)B + (size_t)b];
+  if (b < B) {
+    // the loads of eight slices are issued together, the additions keep the order g, g + CGROUPS, ...
+    int i = g;
+    for (; i + 7 * CGROUPS < n_slices; i += 8 * CGROUPS) {
+      double v[8];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) v[u] = partial[(size_t)(i + u * CGROUPS) * (size_t)B + (size_t)b];
+#pragma unroll
+      for (int u = 0; u < 8; ++u) t += v[u];
+    }
+    for (; i < n_slices; i += CGROUPS) t += partial[(size_t)i * (size_t)B + (size_t)b];
+  }
   part[g][x] = t;
   __syncthreads();
   if (g == 0 && b < B) {
