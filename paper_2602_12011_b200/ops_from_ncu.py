@@ -36,8 +36,8 @@ METRICS = {
 }
 UNIT_SCALE = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "nsecond": 1.0, "usecond": 1e3, "msecond": 1e6,
               "second": 1e9}
-KERNELS = ("loglike_fused_kernel", "loglike_grad_kernel", "loglike_tab_kernel", "loglike_mixed_kernel", "loglike_orb_kernel", "loglike_kernel",
-           "fisher_kernel", "response_kernel")
+KERNELS = ("loglike_fused_kernel", "loglike_grad_kernel", "loglike_tab_kernel", "loglike_mixed_kernel",
+           "loglike_orb_kernel", "loglike_kernel", "fisher_kernel", "response_fused_kernel", "response_kernel")
 
 
 def kernel_key(name: str):
@@ -47,7 +47,7 @@ def kernel_key(name: str):
             m = re.search(re.escape(k) + r"<\s*(\d+)u?\s*(?:,\s*(\d+)u?)?\s*>", name)
             kind = int(m.group(1)) if m else 0
             mask = int(m.group(2)) if m and m.group(2) else 0
-            if k in ("loglike_fused_kernel", "loglike_orb_kernel"):     # one template argument: the class mask
+            if k in ("loglike_fused_kernel", "loglike_orb_kernel", "response_fused_kernel"):   # one argument: the mask
                 kind, mask = 0, kind
             return k[:-len("_kernel")], kind, mask
     return None

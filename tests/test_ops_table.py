@@ -127,3 +127,17 @@ def test_ops_file_is_stamped(ops):
     assert ops["unit"] == "(sample, bin, detector)"
     # not asserted equal to build.csrc_hash(): bench.py reports roofline.stale when the kernels moved on
     assert len(build.csrc_hash()) == 16
+
+
+def test_kernel_names_map_to_table_keys():
+    """ops_from_ncu.kernel_key: demangled ncu kernel names -> (kernel, kind, class mask) of the table keys bench.py reads"""
+    from paper_2602_12011_b200.ops_from_ncu import kernel_key
+    assert kernel_key("void pespace::loglike_kernel<0, 2>(const double *, ...)") == ("loglike", 0, 2)
+    assert kernel_key("void pespace::loglike_kernel<1, 15u>(const double *)") == ("loglike", 1, 15)
+    assert kernel_key("void pespace::loglike_fused_kernel<15>(const double *)") == ("loglike_fused", 0, 15)
+    assert kernel_key("void pespace::response_fused_kernel<15u>(const double *)") == ("response_fused", 0, 15)
+    assert kernel_key("void pespace::response_kernel<0, 2>(const double *)") == ("response", 0, 2)
+    assert kernel_key("void pespace::loglike_orb_kernel<2>(const double *)") == ("loglike_orb", 0, 2)
+    assert kernel_key("void pespace::loglike_tab_kernel<0, 5>(const double *)") == ("loglike_tab", 0, 5)
+    assert kernel_key("void pespace::fisher_kernel<1, 15>(const double *)") == ("fisher", 1, 15)
+    assert kernel_key("void pespace::combine_kernel(const double *)") is None
