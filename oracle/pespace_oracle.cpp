@@ -20,10 +20,10 @@
 // position / velocity tables; pinned by the T2 tests (exact on cubic trajectories, reproduces the analytic orbit and
 // its response when fed dense samples of it, rigid arms between nodes, zero outside the table).
 //
-// Pins (tests/test_oracle_pins.py): P1-P16 of SURVEY.md 8(c).  "Parity
-// unpinned": absolute values of the Taiji-/TianQin-like results (G8, G13 are
-// proposals, not in the paper) and the spin terms of G3 beyond "vanish at
-// chi = 0" and the finite-difference check.
+// Pins (tests/test_oracle_pins.py): P1-P16 of SURVEY.md 8(c), the spin terms of G3 against the Poisson-Will forms
+// of beta and sigma (phase and time series), the c_lm v^p table of O5 against point-mass multipole moments and the
+// test-mass mode fluxes.  "Parity unpinned": the absolute values of the Taiji-/TianQin-like results (G8, G13 are
+// proposals, not in the paper) and the constant per-mode phase -m pi/8 of reading G5.
 //
 // Build: g++ -O2 -std=gnu++17 -ffp-contract=off -fopenmp -shared -fPIC (oracle/build.py)
 
