@@ -79,17 +79,19 @@ def gather_lnL(local: "np.ndarray", device=None) -> "np.ndarray":
     return torch.cat(out).cpu().numpy()
 
 
-class ShardedLikelihood:
-    """Strong scaling over samples: every rank holds the same data set and the same batch of theta,
-    evaluates the samples [lo, hi) of `shard_bounds` with `local_eval` (e.g. a `binding.Likelihood`: tensor of
-    theta [b][11] -> tensor of lnL [b]) and one all-gather of ceil(B / G) doubles per rank restores the full lnL
-    vector on every rank, in sample order.  No other collective touches the data path; the result of each sample is
-    bit-identical to the single-GPU one (the reduction of a sample never crosses ranks)."""
+class ShardedCall:
+    """Strong scaling over samples for ANY per-sample call of the library: every rank holds the same
+    data set and the same batch of theta, evaluates the samples [lo, hi) of `shard_bounds` with `local_eval` (theta
+    [b][11] -> a tensor [b][...] or a tuple of such tensors, `None` entries allowed: e.g. a `binding.Likelihood`
+    (lnL), a `binding.LikelihoodGrad` (lnL, gradient) or a `binding.Fisher` (F, gradient)), and one all-gather of
+    ceil(B / G) rows per output restores the full arrays on every rank, in sample order.  No other collective touches
+    the data path; the result of each sample is bit-identical to the single-GPU one (the reduction of a sample never
+    crosses ranks)."""
 
     def __init__(self, local_eval):
         self.local_eval = local_eval
 
-    def __call__(self, params: "torch.Tensor") -> "torch.Tensor":
+    def __call__(self, params: "torch.Tensor"):
         import torch
         import torch.distributed as dist
         B = params.shape[0]
@@ -98,13 +100,27 @@ class ShardedLikelihood:
         rank, world = dist.get_rank(), dist.get_world_size()
         lo, hi = shard_bounds(B, rank, world)
         per = -(-B // world)
-        mine = torch.full((per,), float("nan"), dtype=torch.float64, device=params.device)
-        if hi > lo:
-            mine[:hi - lo] = self.local_eval(params[lo:hi].contiguous())
-        parts = [torch.empty_like(mine) for _ in range(world)]
-        dist.all_gather(parts, mine)
-        out = torch.empty(B, dtype=torch.float64, device=params.device)
-        for r, part in enumerate(parts):
-            rlo, rhi = shard_bounds(B, r, world)
-            out[rlo:rhi] = part[:rhi - rlo]
-        return out
+        # every rank evaluates at least one sample so that the shapes of the outputs are known everywhere (a rank
+        # whose slice is empty -- more ranks than samples -- evaluates sample 0 and discards it)
+        local = self.local_eval(params[lo:hi].contiguous() if hi > lo else params[:1].contiguous())
+        single = not isinstance(local, (tuple, list))
+        outs = []
+        for res in ((local,) if single else local):
+            if res is None:
+                outs.append(None)
+                continue
+            mine = torch.full((per,) + tuple(res.shape[1:]), float("nan"), dtype=res.dtype, device=res.device)
+            if hi > lo:
+                mine[:hi - lo] = res
+            parts = [torch.empty_like(mine) for _ in range(world)]
+            dist.all_gather(parts, mine)
+            out = torch.empty((B,) + tuple(res.shape[1:]), dtype=res.dtype, device=res.device)
+            for r, part in enumerate(parts):
+                rlo, rhi = shard_bounds(B, r, world)
+                out[rlo:rhi] = part[:rhi - rlo]
+            outs.append(out)
+        return outs[0] if single else tuple(outs)
+
+
+class ShardedLikelihood(ShardedCall):
+    """`ShardedCall` for a call that returns lnL [b] (kept under its round-1 name)."""

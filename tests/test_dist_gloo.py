@@ -40,8 +40,15 @@ def _worker(rank: int, world: int, port: int, B: int, out_dir: str) -> None:
     sharded = pdist.ShardedLikelihood(lambda p: torch.from_numpy(_stand_in_lnL(p.numpy())))
     strong = sharded(torch.from_numpy(wl.params)).numpy()          # same batch on every rank, split and gathered
     tiny = sharded(torch.from_numpy(wl.params[:1])).numpy()        # fewer samples than ranks: one rank idles
+    # a call with several outputs (lnL, gradient-like [b][11], nothing, Fisher-like [b][11][11])
+    multi = pdist.ShardedCall(lambda p: (torch.from_numpy(_stand_in_lnL(p.numpy())), -p, None,
+                                         p[:, :, None] * p[:, None, :]))
+    m_lnL, m_grad, m_none, m_F = multi(torch.from_numpy(wl.params))
+    assert m_none is None
+    t_lnL, t_grad, _, t_F = multi(torch.from_numpy(wl.params[:1]))
     np.savez(os.path.join(out_dir, f"r{rank}.npz"), full=full, t_max=t_max, units=units, mine=mine, lo=lo, hi=hi,
-             strong=strong, tiny=tiny)
+             strong=strong, tiny=tiny, m_lnL=m_lnL.numpy(), m_grad=m_grad.numpy(), m_F=m_F.numpy(),
+             t_grad=t_grad.numpy(), t_F=t_F.numpy())
     import torch.distributed as dist
     dist.destroy_process_group()
 
@@ -59,6 +66,10 @@ def test_sample_sharding_world_size_2(tmp_path):
         assert np.array_equal(got, want)                        # gather restores sample order, bit for bit
         assert float(r["t_max"]) == 11.0 and float(r["units"]) == B      # MAX of times, SUM of units
         assert np.array_equal(r["strong"], want) and np.array_equal(r["tiny"], want[:1])   # ShardedLikelihood
+        p = W.config(2, B=B, N=8).params
+        assert np.array_equal(r["m_lnL"], want) and np.array_equal(r["m_grad"], -p)            # ShardedCall, tuples
+        assert np.array_equal(r["m_F"], p[:, :, None] * p[:, None, :])
+        assert np.array_equal(r["t_grad"], -p[:1]) and r["t_F"].shape == (1, 11, 11)
     assert int(res[0]["lo"]) == 0 and int(res[0]["hi"]) == int(res[1]["lo"]) and int(res[1]["hi"]) == B
     assert not np.array_equal(res[0]["mine"], res[1]["mine"])    # different batches per rank
     assert np.array_equal(res[0]["mine"], W.config(2, B=4, N=8, param_seed=1000).params)   # rank 0 keeps the seed

@@ -453,6 +453,18 @@ def test_sharded_likelihood_with_the_real_binding_under_nccl(P):
         t_max, units = pdist.aggregate(12.5, wl.B, torch.device("cuda", torch.cuda.current_device()))
         assert t_max == 12.5 and units == wl.B
         assert np.array_equal(pdist.gather_lnL(plain, torch.device("cuda", torch.cuda.current_device())), plain)
+        # the calls with several outputs: adjoint gradient (lnL, grad) and Fisher matrix (F, grad)
+        th = dev(wl.params[:9])
+        lg = P.LikelihoodGrad(dev(data), dev(psd), wl.grid, wl.model, 9)
+        want_l, want_g = (x.clone() for x in lg(th))
+        got_l, got_g = pdist.ShardedCall(lambda p: lg(p))(th)
+        assert torch.equal(got_l, want_l) and torch.equal(got_g, want_g)
+        fi = P.Fisher(dev(data), dev(psd), wl.grid, wl.model, 9)
+        want_F, want_fg = (x.clone() for x in fi(th))
+        got_F, got_fg = pdist.ShardedCall(lambda p: fi(p))(th)
+        assert torch.equal(got_F, want_F) and torch.equal(got_fg, want_fg)
+        none_F, only_g = pdist.ShardedCall(lambda p: fi(p, grad_only=True))(th)
+        assert none_F is None and only_g.shape == (9, 11)
     finally:
         dist.destroy_process_group()
 
