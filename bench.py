@@ -16,7 +16,8 @@ e2e            the same metric through the C ABI with HOST buffers (pespace_sess
 roofline       the dominant kernel against the FP64 ALU peak; operation counts from profiles/r02_ops.json (ncu),
                marked stale when the kernel sources have changed since they were counted
 other_configs  (default run only) short device-timed runs of configs 3, 4, 5 (Fisher), the adjoint gradient and
-               pespace_response, so that every BASELINE.json config and every north-star call is in the driver's line
+               pespace_response, so that every BASELINE.json config and every north-star call is in the driver's line;
+               single_theta_latency: one sample x N bins per call, plain and with pespace_prepare (wall clock, us)
 cpu_baseline / --impl reference   the oracle, as it stands, on the box's host cores
 
 --path selects the entry point that is timed: loglike (default; config 5: fisher), mixed, tab, orb, grad (adjoint
@@ -505,6 +506,34 @@ def run_ours(args):
                                   "write_gbs": out_r.numel() * 8 / (r_ms * 1e-3) / 1e9})
             del out_r
 
+    # ---- single-theta latency (one sample x N bins; a sampler that walks one chain): the plain call rebuilds the
+    # per-bin table on every call, the prepared call (pespace_prepare once) does not
+    latency_info = None
+    if args.others and world == 1:
+        latency_info = []
+        for cfg in (2, 4):
+            wq = W.config(cfg, B=1)
+            psd_q = wq.psd()
+            data_q = W.coloured_noise(psd_q, wq.grid.df, np.random.default_rng(5))
+            lq = P.Likelihood(torch.from_numpy(np.ascontiguousarray(data_q)).to(device),
+                              torch.from_numpy(psd_q).to(device), wq.grid, wq.model, 1)
+            pq = torch.from_numpy(np.ascontiguousarray(wq.params)).to(device)
+            oq = torch.empty(1, dtype=torch.float64, device=device)
+            row = {"config": cfg, "B": 1, "N": wq.grid.N, "n_det": len(wq.model.detectors)}
+            for key in ("pespace_loglike_us", "pespace_loglike_prepared_us"):
+                if key.endswith("prepared_us"):
+                    lq.prepare()
+                for _ in range(20):
+                    lq(pq, oq)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(200):
+                    lq(pq, oq)
+                torch.cuda.synchronize()
+                row[key] = (time.perf_counter() - t0) / 200 * 1e6
+            latency_info.append(row)
+            del lq
+
     if rank != 0:
         return
 
@@ -551,6 +580,7 @@ def run_ours(args):
         "result_check": {"min": float(last.min()), "max": float(last.max())},
         "other_configs": others,
         "response": response_info,
+        "single_theta_latency": latency_info,
     }
     print(json.dumps(line), flush=True)
 

@@ -114,6 +114,27 @@ int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data
                          const pespace_grid* grid, const pespace_model* model, double* d_out_lnL /* [B] */,
                          double* d_out_grad /* [B][11] */, void* d_workspace, size_t workspace_bytes, void* stream);
 
+/* Prepared data ("a persistent prepared-data handle, S0 tables cached across calls from a
+ * sampler") for callers that keep theta on the device.  pespace_prepare runs step S0 alone: it folds the data set and
+ * the PSD into the per-bin table at the head of the workspace (the same bytes pespace_loglike / pespace_loglike_grad
+ * write there on every call).  pespace_loglike_prepared / pespace_loglike_grad_prepared then evaluate batches of
+ * theta against that table without reading d_data_AET / d_psd again: same results, bit for bit, as the plain calls
+ * on the same inputs.  The table stays valid while the SAME workspace is used with the SAME grid and model and only
+ * by these two calls (any other entry point given this workspace may overwrite it; results are then undefined --
+ * call pespace_prepare again).  Its position does not depend on B: one workspace sized for the largest batch serves
+ * every smaller one.  The plain and the gradient call lay the table out identically, so one pespace_prepare on a
+ * workspace of max(pespace_workspace_bytes, pespace_workspace_bytes_grad) bytes serves both.
+ *   pespace_prepare: workspace_bytes >= pespace_workspace_bytes(1, grid, model, 0).
+ * Errors as for the plain calls. */
+int pespace_prepare(const double* d_data_AET, const double* d_psd, const pespace_grid* grid, const pespace_model* model,
+                    void* d_workspace, size_t workspace_bytes, void* stream);
+int pespace_loglike_prepared(const double* d_params, int64_t B, const pespace_grid* grid, const pespace_model* model,
+                             double* d_out_lnL, void* d_workspace, size_t workspace_bytes, void* stream);
+int pespace_loglike_grad_prepared(const double* d_params, int64_t B, const pespace_grid* grid,
+                                  const pespace_model* model, double* d_out_lnL /* [B] or NULL */,
+                                  double* d_out_grad /* [B][11] or NULL */, void* d_workspace, size_t workspace_bytes,
+                                  void* stream);
+
 /* Mixed-precision twin of pespace_loglike (the paper's float32 mode for searches and coarse
  * maximisation).  Same arguments, same workspace size.  Every phase that enters an exponential
  * (PN phase, 2 pi f t_c, Doppler phases, their sum and its reduction modulo one turn) stays FP64; the t_lm polynomial,

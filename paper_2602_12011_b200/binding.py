@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_loglike_mixed", "pespace_workspace_bytes_grad", "pespace_loglike_grad",
+           "pespace_prepare", "pespace_loglike_prepared", "pespace_loglike_grad_prepared",
            "pespace_session_loglike_grad", "pespace_response_orb", "pespace_loglike_orb",
            "pespace_workspace_bytes_fisher_tab", "pespace_fisher_tab", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
@@ -74,6 +75,9 @@ def _load():
     L.pespace_workspace_bytes_grad.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
     L.pespace_workspace_bytes_grad.restype = sz
     L.pespace_loglike_grad.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
+    L.pespace_prepare.argtypes = [vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, sz, vp]
+    L.pespace_loglike_prepared.argtypes = [vp, i64, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
+    L.pespace_loglike_grad_prepared.argtypes = [vp, i64, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, vp, sz, vp]
     L.pespace_workspace_bytes_fisher_tab.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model)]
     L.pespace_workspace_bytes_fisher_tab.restype = sz
     L.pespace_fisher_tab.argtypes = [vp, i64, C.POINTER(_WaveTable), vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp,
@@ -179,6 +183,19 @@ class Likelihood:
         self._g = _grid(grid)
         self.ws_bytes = workspace_bytes(max_batch, grid, model)
         self.ws = torch.empty(self.ws_bytes, dtype=torch.uint8, device=self.data.device)
+        self.prepared = False
+
+    _has_prepared = True                     # pespace_loglike and pespace_loglike_grad have a *_prepared twin
+
+    def prepare(self) -> "Likelihood":
+        """pespace_prepare: fold data and PSD into the per-bin table of the workspace once; later calls skip step S0
+        (pespace_loglike_prepared / pespace_loglike_grad_prepared) until a call of another kind rewrites the table."""
+        if not self._has_prepared:
+            raise PespaceError("this call has no prepared variant")
+        _check(_lib.pespace_prepare(self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g), C.byref(self._m),
+                                    self.ws.data_ptr(), self.ws_bytes, _stream_ptr()), "pespace_prepare")
+        self.prepared = True
+        return self
 
     def __call__(self, params: torch.Tensor, out: Optional[torch.Tensor] = None, mixed: bool = False) -> torch.Tensor:
         """mixed=True: pespace_loglike_mixed (FP64 phases, FP32 geometry; ~1e-6 relative accuracy)."""
@@ -188,6 +205,12 @@ class Likelihood:
             raise PespaceError("batch larger than the workspace was sized for")
         if out is None:
             out = torch.empty(B, dtype=torch.float64, device=p.device)
+        if self.prepared and not mixed and type(self) is Likelihood:
+            _check(_lib.pespace_loglike_prepared(p.data_ptr(), B, C.byref(self._g), C.byref(self._m),
+                                                 _dev(out, "out").data_ptr(), self.ws.data_ptr(), self.ws_bytes,
+                                                 _stream_ptr()), "pespace_loglike_prepared")
+            return out
+        self.prepared = False                # the mixed kernel keeps its own (whitened) table in the same place
         fn, name = (_lib.pespace_loglike_mixed, "pespace_loglike_mixed") if mixed else \
             (_lib.pespace_loglike, "pespace_loglike")
         _check(fn(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g), C.byref(self._m),
@@ -235,6 +258,7 @@ def response_tab(params: torch.Tensor, table: WaveTable, freqs: torch.Tensor, mo
 
 class LikelihoodTab(Likelihood):
     """pespace_loglike_tab with data, PSD and workspace resident on the device."""
+    _has_prepared = False
 
     def __init__(self, data: torch.Tensor, psd: torch.Tensor, grid, model, max_batch: int):
         super().__init__(data, psd, grid, model, max_batch)
@@ -366,6 +390,7 @@ def response_orb(params: torch.Tensor, orbit: OrbitTable, freqs: torch.Tensor, m
 
 class LikelihoodOrb(Likelihood):
     """pespace_loglike_orb: likelihood with tabulated orbits; data, PSD and workspace resident."""
+    _has_prepared = False
 
     def __call__(self, params: torch.Tensor, orbit: OrbitTable, out: Optional[torch.Tensor] = None) -> torch.Tensor:
         p = _dev(params, "params")
@@ -402,6 +427,12 @@ class LikelihoodGrad(Likelihood):
             out_lnL = torch.empty(B, dtype=torch.float64, device=p.device)
         if out_grad is None:
             out_grad = torch.empty((B, NPAR), dtype=torch.float64, device=p.device)
+        if self.prepared:
+            _check(_lib.pespace_loglike_grad_prepared(p.data_ptr(), B, C.byref(self._g), C.byref(self._m),
+                                                      _dev(out_lnL, "out_lnL").data_ptr(),
+                                                      _dev(out_grad, "out_grad").data_ptr(), self.ws.data_ptr(),
+                                                      self.ws_bytes, _stream_ptr()), "pespace_loglike_grad_prepared")
+            return out_lnL, out_grad
         _check(_lib.pespace_loglike_grad(p.data_ptr(), B, self.data.data_ptr(), self.psd.data_ptr(), C.byref(self._g),
                                          C.byref(self._m), _dev(out_lnL, "out_lnL").data_ptr(),
                                          _dev(out_grad, "out_grad").data_ptr(), self.ws.data_ptr(), self.ws_bytes,

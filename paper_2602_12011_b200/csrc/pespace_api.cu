@@ -176,6 +176,27 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
                                      stream, false);
 }
 
+int pespace_prepare(const double* d_data_AET, const double* d_psd, const pespace_grid* grid, const pespace_model* model,
+                    void* d_workspace, size_t workspace_bytes, void* stream) {
+  if (!d_data_AET || !d_psd || !d_workspace || !grid_ok(grid) || !model_ok(model)) return PESPACE_EINVAL;
+  if (workspace_bytes < pespace_workspace_bytes(1, grid, model, 0) || ((uintptr_t)d_workspace & 15u)) return PESPACE_EINVAL;
+  cudaStream_t st = (cudaStream_t)stream;
+  const Plan p = make_plan(1, grid->N, model->n_det);
+  double* d_bins = (double*)((char*)d_workspace + p.trig_bytes);
+  const GridC G = {grid->f0, grid->df, (long long)grid->N};
+  const PrepArgs A = make_prep_args(model);
+  prep_bins_kernel<<<dim3((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det), 256, 0, st>>>(
+      (const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
+  LAUNCHED();
+  return PESPACE_OK;
+}
+
+int pespace_loglike_prepared(const double* d_params, int64_t B, const pespace_grid* grid, const pespace_model* model,
+                             double* d_out_lnL, void* d_workspace, size_t workspace_bytes, void* stream) {
+  return pespace::host::loglike_impl(d_params, B, nullptr, nullptr, grid, model, d_out_lnL, d_workspace, workspace_bytes,
+                                     stream, true);
+}
+
 }  // extern "C"
 
 // pespace_loglike with one extra switch for the session calls: bins_ready = the per-bin table (S0) at the head of the
@@ -183,7 +204,7 @@ int pespace_loglike(const double* d_params, int64_t B, const double* d_data_AET,
 int pespace::host::loglike_impl(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
                                 const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
                                 void* d_workspace, size_t workspace_bytes, void* stream, bool bins_ready) {
-  if (!d_params || !d_data_AET || !d_psd || !d_out_lnL || !d_workspace || B <= 0 || !grid_ok(grid) ||
+  if (!d_params || (!bins_ready && (!d_data_AET || !d_psd)) || !d_out_lnL || !d_workspace || B <= 0 || !grid_ok(grid) ||
       !model_ok(model))
     return PESPACE_EINVAL;
   if (workspace_bytes < pespace_workspace_bytes(B, grid, model, 0) || ((uintptr_t)d_workspace & 15u))

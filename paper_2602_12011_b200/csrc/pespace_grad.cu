@@ -37,8 +37,27 @@ size_t pespace_workspace_bytes_grad(int64_t B, const pespace_grid* grid, const p
 int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
                          const pespace_grid* grid, const pespace_model* model, double* d_out_lnL, double* d_out_grad,
                          void* d_workspace, size_t workspace_bytes, void* stream) {
-  if (!d_params || !d_data_AET || !d_psd || (!d_out_lnL && !d_out_grad) || !d_workspace || B <= 0 || !grid_ok(grid) ||
-      !model_ok(model))
+  return loglike_grad_impl(d_params, B, d_data_AET, d_psd, grid, model, d_out_lnL, d_out_grad, d_workspace,
+                           workspace_bytes, stream, false);
+}
+
+int pespace_loglike_grad_prepared(const double* d_params, int64_t B, const pespace_grid* grid,
+                                  const pespace_model* model, double* d_out_lnL, double* d_out_grad, void* d_workspace,
+                                  size_t workspace_bytes, void* stream) {
+  return loglike_grad_impl(d_params, B, nullptr, nullptr, grid, model, d_out_lnL, d_out_grad, d_workspace,
+                           workspace_bytes, stream, true);
+}
+
+}  // extern "C"
+
+// bins_ready: the per-bin table at the head of the workspace was written by pespace_prepare (or an earlier call) for
+// the same data set, PSD, grid and model
+int pespace::host::loglike_grad_impl(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                                     const pespace_grid* grid, const pespace_model* model, double* d_out_lnL,
+                                     double* d_out_grad, void* d_workspace, size_t workspace_bytes, void* stream,
+                                     bool bins_ready) {
+  if (!d_params || (!bins_ready && (!d_data_AET || !d_psd)) || (!d_out_lnL && !d_out_grad) || !d_workspace || B <= 0 ||
+      !grid_ok(grid) || !model_ok(model))
     return PESPACE_EINVAL;
   if (workspace_bytes < pespace_workspace_bytes_grad(B, grid, model) || ((uintptr_t)d_workspace & 15u))
     return PESPACE_EINVAL;
@@ -58,9 +77,11 @@ int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data
   prep_samples_du_kernel<<<(unsigned)((B + 63) / 64), 64, 0, st>>>(d_params, B, A, d_du);
   LAUNCHED();
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
-  prep_bins_kernel<<<dim3((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det), 256, 0, st>>>(
-      (const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
-  LAUNCHED();
+  if (!bins_ready) {
+    prep_bins_kernel<<<dim3((unsigned)((grid->N + 255) / 256), (unsigned)model->n_det), 256, 0, st>>>(
+        (const double2*)d_data_AET, d_psd, G, A, 1, d_bins);
+    LAUNCHED();
+  }
   const unsigned cm = class_mask(model->mode_mask);
   const dim3 g((unsigned)p.nbx, (unsigned)p.ntile);
   for (int d = 0; d < model->n_det; ++d) {
@@ -76,5 +97,3 @@ int pespace_loglike_grad(const double* d_params, int64_t B, const double* d_data
   LAUNCHED();
   return PESPACE_OK;
 }
-
-}  // extern "C"

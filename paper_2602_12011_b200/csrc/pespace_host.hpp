@@ -95,6 +95,11 @@ int loglike_impl(const double* d_params, int64_t B, const double* d_data_AET, co
                  const pespace_grid* grid, const pespace_model* model, double* d_out_lnL, void* d_workspace,
                  size_t workspace_bytes, void* stream, bool bins_ready);
 
+// pespace_loglike_grad with the same switch (pespace_grad.cu)
+int loglike_grad_impl(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,
+                      const pespace_grid* grid, const pespace_model* model, double* d_out_lnL, double* d_out_grad,
+                      void* d_workspace, size_t workspace_bytes, void* stream, bool bins_ready);
+
 // Fisher path (pespace_fisher.cu)
 size_t fisher_workspace_bytes(long long B, long long N, int n_det);
 

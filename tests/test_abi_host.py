@@ -62,6 +62,16 @@ def test_argument_validation_without_a_device():
     bad_m3, keep4 = P._model(W.Model(1, (W.Detector("x", 0, 17, 1e9),)))
     assert L.pespace_fisher(fake, 4, None, fake, C.byref(g), C.byref(bad_m3), fake, None, fake, 1 << 30, None) == EINVAL
     assert L.pespace_loglike_host(None, 4, fake, fake, C.byref(g), C.byref(m), fake) == EINVAL
+    # prepared-data entry points: the same checks, before any CUDA call
+    assert L.pespace_prepare(None, fake, C.byref(g), C.byref(m), fake, 1 << 30, None) == EINVAL
+    assert L.pespace_prepare(fake, fake, C.byref(g), C.byref(m), fake, 8, None) == EINVAL                 # ws too small
+    assert L.pespace_prepare(fake, fake, C.byref(g), C.byref(m), 0x1008, 1 << 30, None) == EINVAL          # alignment
+    assert L.pespace_prepare(fake, fake, C.byref(bad_g), C.byref(m), fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike_prepared(None, 4, C.byref(g), C.byref(m), fake, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike_prepared(fake, 0, C.byref(g), C.byref(m), fake, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike_prepared(fake, 4, C.byref(g), C.byref(m), fake, fake, 8, None) == EINVAL
+    assert L.pespace_loglike_grad_prepared(fake, 4, C.byref(g), C.byref(m), None, None, fake, 1 << 30, None) == EINVAL
+    assert L.pespace_loglike_grad_prepared(fake, 4, C.byref(g), C.byref(m), fake, fake, fake, 8, None) == EINVAL
     assert L.pespace_fp64_peak(0, 0, None, None) == EINVAL
     assert L.pespace_workspace_bytes(0, C.byref(g), C.byref(m), 0) == 0
     assert L.pespace_workspace_bytes(4096, C.byref(g), C.byref(m), 0) > 4096 * 8

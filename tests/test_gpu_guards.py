@@ -83,11 +83,21 @@ def test_loglike_response_fisher_grad_stay_inside_their_arrays(P, B, N, n_det, m
     gw.check("pespace_loglike workspace"); go.check("pespace_loglike out")
     lik(d_th, out=go.f64(B), mixed=True)
     gw.check("pespace_loglike_mixed workspace"); go.check("pespace_loglike_mixed out")
+    # pespace_prepare + pespace_loglike_prepared
+    lik.prepare()
+    gw.check("pespace_prepare workspace")
+    lik(d_th, out=go.f64(B))
+    assert lik.prepared
+    gw.check("pespace_loglike_prepared workspace"); go.check("pespace_loglike_prepared out")
     # pespace_loglike_grad
     lg = P.LikelihoodGrad(d_data, d_psd, wl.grid, wl.model, B)
     gw, go, gg = guard_workspace(lg), Guarded(8 * B), Guarded(8 * B * 11)
     lg(d_th, out_lnL=go.f64(B), out_grad=gg.f64(B, 11))
     gw.check("pespace_loglike_grad workspace"); go.check("pespace_loglike_grad lnL"); gg.check("pespace_loglike_grad grad")
+    lg.prepare()
+    lg(d_th, out_lnL=go.f64(B), out_grad=gg.f64(B, 11))
+    gw.check("pespace_loglike_grad_prepared workspace"); go.check("pespace_loglike_grad_prepared lnL")
+    gg.check("pespace_loglike_grad_prepared grad")
     # pespace_fisher (matrix + gradient, gradient only)
     fi = P.Fisher(d_data, d_psd, wl.grid, wl.model, B)
     gw, gF, gg = guard_workspace(fi), Guarded(8 * B * 121), Guarded(8 * B * 11)

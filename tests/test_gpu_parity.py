@@ -505,3 +505,39 @@ def test_fused_kernel_detector_counts_and_masks(P, mask, n_det):
         scale = np.abs(one[ok]).max(axis=(1, 2), keepdims=True)
         assert np.all(np.abs(resp[ok, d] - one[ok]) <= 1e-11 * scale)
     assert np.array_equal(resp[np.isfinite(resp)], P.response(dev(thr), dev(f), wl.model).cpu().numpy()[np.isfinite(resp)])
+
+
+# ------------------------------------------------------------------ prepared data
+@pytest.mark.parametrize("idx,B,N", [(2, 70, 3000), (4, 67, 1100)])
+def test_prepared_calls_are_bit_identical_to_the_plain_ones(P, idx, B, N):
+    """pespace_prepare once, then pespace_loglike_prepared / pespace_loglike_grad_prepared for several batches
+    (full, smaller, one sample) against the same workspace: bit-identical to pespace_loglike / pespace_loglike_grad,
+    which rebuild the per-bin table on every call; the table survives the calls, a mixed-precision call in between
+    invalidates it and the binding falls back to the plain call."""
+    import torch
+    wl = W.config(idx, B=B, N=N)
+    data, psd = wl.data(oracle_response_fn), wl.psd()
+    th = dev(wl.params)
+    plain = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, B)
+    want = plain(th).clone()
+    prep = P.Likelihood(dev(data), dev(psd), wl.grid, wl.model, B).prepare()
+    n0 = P.launch_count()
+    got = prep(th).clone()
+    assert P.launch_count() - n0 == 3                                     # prep_samples, main kernel, combine
+    assert prep.prepared and torch.equal(got, want)
+    for b in (B - 7, 1):
+        assert torch.equal(prep(th[:b].contiguous()), want[:b])
+    check_loglike(P, wl, data, psd)                                       # and the oracle agrees (plain path)
+    mixed = prep(th, mixed=True)
+    assert not prep.prepared and torch.isfinite(mixed).all()
+    assert torch.equal(prep(th), want)                                    # plain call again (rebuilds the table)
+    # gradient twin: one pespace_prepare on the larger workspace serves it
+    pg = P.LikelihoodGrad(dev(data), dev(psd), wl.grid, wl.model, B)
+    want_l, want_g = (x.clone() for x in pg(th))
+    pg.prepare()
+    got_l, got_g = pg(th)
+    assert torch.equal(got_l, want_l) and torch.equal(got_g, want_g)
+    got_l, got_g = pg(th[:5].contiguous())
+    assert torch.equal(got_l, want_l[:5]) and torch.equal(got_g, want_g[:5])
+    with pytest.raises(P.PespaceError):
+        P.LikelihoodOrb(dev(data), dev(psd), wl.grid, wl.model, B).prepare()
