@@ -45,6 +45,8 @@ extern "C" {
                                unknown mode_mask, n_det outside 1..PESPACE_MAX_DET, workspace too small */
 #define PESPACE_ECUDA (-2)  /* CUDA launch / runtime error; text via pespace_strerror() */
 #define PESPACE_ENOMEM (-3) /* device or pinned-host allocation failed (host-buffer calls only) */
+#define PESPACE_ETOOBIG (-4) /* pespace_response_noalloc: the batch needs more scratch than the static array holds;
+                                text via pespace_strerror() */
 
 #define PESPACE_NPAR 11
 #define PESPACE_MAX_DET 8
@@ -77,6 +79,23 @@ typedef struct {
  *   d_params [B][11], d_freqs [N] (Hz; bins with f <= 0 produce 0), d_out_AET [B][n_det][3][N][2]. */
 int pespace_response(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
                      const pespace_model* model, double* d_out_AET, void* stream);
+
+/* pespace_response without any allocation, for callers that cannot call cudaMalloc (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid it).  Same arguments, same kernels and bit-identical output; the scratch
+ * of step S1 (per-sample constants and the sine / cosine table) lives in ONE static device array of
+ * PESPACE_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.  The call
+ * allocates and frees nothing (no cudaMalloc / cudaMallocAsync / cudaFree, no allocating library routine).
+ *   Limit: pespace_noalloc_scratch_needed(B, model) = 16384 + 8 B (40 + 24 n_det) bytes (rounded up to 256) must not
+ *   exceed PESPACE_NOALLOC_SCRATCH_BYTES: B <= 2016 samples for one detector, 1152 for three, 556 for eight; N is
+ *   not limited.  A larger batch is rejected with PESPACE_ETOOBIG before anything is launched (pespace_strerror
+ *   names the sizes); pespace_noalloc_scratch_needed returns 0 for invalid arguments.
+ *   Sharing: every call uses the same array and finds the previous call's contents there; nothing has to start at
+ *   zero (the prep kernel of a call writes every word its response kernels read).  Calls on ONE stream are ordered
+ *   and safe; calls that overlap on the GPU (several streams or host threads) RACE on the array -- serialise them. */
+#define PESPACE_NOALLOC_SCRATCH_BYTES (1 << 20)
+size_t pespace_noalloc_scratch_needed(int64_t B, const pespace_model* model);
+int pespace_response_noalloc(const double* d_params, int64_t B, const double* d_freqs, int64_t N,
+                             const pespace_model* model, double* d_out_AET, void* stream);
 
 /* Scratch the likelihood / Fisher calls need for (B, grid, model). */
 size_t pespace_workspace_bytes(int64_t B, const pespace_grid* grid, const pespace_model* model,

@@ -19,6 +19,7 @@ LIB_PATH = os.path.join(_HERE, "libpespace.so")
 EXPORTS = ("pespace_response", "pespace_workspace_bytes", "pespace_loglike", "pespace_fisher",
            "pespace_loglike_mixed", "pespace_workspace_bytes_grad", "pespace_loglike_grad",
            "pespace_prepare", "pespace_loglike_prepared", "pespace_loglike_grad_prepared",
+           "pespace_response_noalloc", "pespace_noalloc_scratch_needed",
            "pespace_session_loglike_grad", "pespace_response_orb", "pespace_loglike_orb",
            "pespace_workspace_bytes_fisher_tab", "pespace_fisher_tab", "pespace_response_tab", "pespace_workspace_bytes_tab", "pespace_loglike_tab",
            "pespace_session_create", "pespace_session_set_data", "pespace_session_loglike", "pespace_session_loglike_mixed",
@@ -67,6 +68,9 @@ def _load():
     L = C.CDLL(LIB_PATH)
     vp, i64, sz = C.c_void_p, C.c_int64, C.c_size_t
     L.pespace_response.argtypes = [vp, i64, vp, i64, C.POINTER(_Model), vp, vp]
+    L.pespace_response_noalloc.argtypes = [vp, i64, vp, i64, C.POINTER(_Model), vp, vp]
+    L.pespace_noalloc_scratch_needed.argtypes = [i64, C.POINTER(_Model)]
+    L.pespace_noalloc_scratch_needed.restype = sz
     L.pespace_workspace_bytes.argtypes = [i64, C.POINTER(_Grid), C.POINTER(_Model), C.c_int]
     L.pespace_workspace_bytes.restype = sz
     L.pespace_loglike.argtypes = [vp, i64, vp, vp, C.POINTER(_Grid), C.POINTER(_Model), vp, vp, sz, vp]
@@ -166,6 +170,28 @@ def response(params: torch.Tensor, freqs: torch.Tensor, model, out: Optional[tor
     _check(_lib.pespace_response(p.data_ptr(), B, f.data_ptr(), N, C.byref(m), _dev(out, "out").data_ptr(),
                                  _stream_ptr()), "pespace_response")
     return torch.view_as_complex(out)
+
+
+NOALLOC_SCRATCH_BYTES = 1 << 20      # PESPACE_NOALLOC_SCRATCH_BYTES of include/pespace.h
+
+
+def noalloc_scratch_needed(B: int, model) -> int:
+    m, keep = _model(model)
+    return int(_lib.pespace_noalloc_scratch_needed(int(B), C.byref(m)))
+
+
+def response_noalloc(params: torch.Tensor, freqs: torch.Tensor, model, out: torch.Tensor) -> torch.Tensor:
+    """pespace_response_noalloc: as `response`, scratch in the library's static device array (no allocation inside
+    the call, so `out` [B][n_det][3][N][2] f64 is the caller's; batches beyond the array raise PespaceError)."""
+    p, f = _dev(params, "params"), _dev(freqs, "freqs")
+    B, N, nd = p.shape[0], f.shape[0], len(model.detectors)
+    o = _dev(out, "out")
+    if tuple(o.shape) != (B, nd, 3, N, 2):
+        raise PespaceError("out must be [B][n_det][3][N][2]")
+    m, keep = _model(model)
+    _check(_lib.pespace_response_noalloc(p.data_ptr(), B, f.data_ptr(), N, C.byref(m), o.data_ptr(), _stream_ptr()),
+           "pespace_response_noalloc")
+    return torch.view_as_complex(o)
 
 
 class Likelihood:

@@ -89,6 +89,7 @@ const char* pespace_strerror(int code) {
     case PESPACE_EINVAL: return "invalid argument";
     case PESPACE_ECUDA: return cuda_msg()[0] ? cuda_msg() : "CUDA error";
     case PESPACE_ENOMEM: return "out of memory";
+    case PESPACE_ETOOBIG: return cuda_msg()[0] ? cuda_msg() : "batch beyond the static scratch array";
     default: return "unknown error code";
   }
 }
