@@ -202,6 +202,11 @@ def run_reference(args):
     rank, _, world = pdist.env_world()
     if rank != 0:
         return
+    if world > 1:
+        # torchrun sets OMP_NUM_THREADS=1 for every rank when it starts several; the other ranks have exited, so rank 0
+        # gives the oracle the host cores it has under plain `python bench.py --impl reference`
+        import oracle
+        oracle.set_threads(len(os.sched_getaffinity(0)))
     path = default_path(args)
     wl = W.config(args.config)
     metric, unit = UNITS[path]
