@@ -17,7 +17,8 @@ roofline       the dominant kernel against the FP64 ALU peak; operation counts f
                marked stale when the kernel sources have changed since they were counted
 other_configs  (default run only) short device-timed runs of configs 3, 4, 5 (Fisher), the adjoint gradient and
                pespace_response, so that every BASELINE.json config and every north-star call is in the driver's line;
-               single_theta_latency: one sample x N bins per call, plain and with pespace_prepare (wall clock, us)
+               single_theta_latency: one sample x N bins per call, plain, with pespace_prepare, and the prepared call
+               replayed from a CUDA graph (wall clock, us)
 cpu_baseline / --impl reference   the oracle, as it stands, on the box's host cores
 
 --path selects the entry point that is timed: loglike (default; config 5: fisher), mixed, tab, orb, grad (adjoint
@@ -536,6 +537,23 @@ def run_ours(args):
                     lq(pq, oq)
                 torch.cuda.synchronize()
                 row[key] = (time.perf_counter() - t0) / 200 * 1e6
+            # the prepared call replayed from a CUDA graph (three kernel nodes; no host-side launch work)
+            try:
+                gq = torch.cuda.CUDAGraph()
+                with torch.cuda.graph(gq):
+                    lq(pq, oq)
+                for _ in range(20):
+                    gq.replay()
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(200):
+                    gq.replay()
+                torch.cuda.synchronize()
+                row["pespace_loglike_prepared_graph_replay_us"] = (time.perf_counter() - t0) / 200 * 1e6
+                del gq
+            except RuntimeError as exc:                      # reported, never fatal for the bench line
+                row["pespace_loglike_prepared_graph_replay_us"] = None
+                row["graph_error"] = str(exc)[:200]
             latency_info.append(row)
             del lq
 
