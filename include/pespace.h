@@ -158,7 +158,10 @@ int pespace_loglike_grad_prepared(const double* d_params, int64_t B, const pespa
  * maximisation).  Same arguments, same workspace size.  Every phase that enters an exponential
  * (PN phase, 2 pi f t_c, Doppler phases, their sum and its reduction modulo one turn) stays FP64; the t_lm polynomial,
  * orbit, projections, arm weights, sines / cosines of the reduced phases, TDI sums and the whitened residual run in
- * FP32.  Accuracy ~1e-6 relative on the response, a few 1e-6 of max(|lnL|, <h|h>/2) on lnL (tests/test_gpu_mixed.py):
+ * FP32.  Accuracy ~1e-6 relative on the response, a few 1e-6 of max(|lnL|, <h|h>/2) on lnL for the BASELINE configs
+ * (tests/test_gpu_mixed.py); over random models the error is 2e-7 in the median and below 1.2e-5 in 99 % of them, and
+ * it grows like 5e-7 / (2 pi f L / c) where a detector's arm is short against the wavelength: up to 4e-4 for a
+ * TianQin-like detector ALONE in a band below 0.3 mHz (tests/test_gpu_random_sweep.py).
  * NOT a substitute for pespace_loglike where |delta lnL| << 1 matters.  Inputs must be detector-like in magnitude:
  * sqrt(4 df / S_n) |h| x 2^-64 and x 2^64 must both be representable in FP32 (not checked). */
 int pespace_loglike_mixed(const double* d_params, int64_t B, const double* d_data_AET, const double* d_psd,

@@ -6,7 +6,8 @@
 // A/E/T and the residual.  Data and template are whitened per bin and channel (r_c = sqrt(w_c) (d_c - h_c)) and the
 // amplitudes carry a fixed scale 2^64, so that every FP32 quantity is of order 1e-3..1e3 for detector-like inputs
 // (|sqrt(4 df / S_n) h| between ~1e-19 x 2^64 and 1e19 x 2^64 overflow / underflow is NOT detected).
-// Accuracy: ~1e-6 relative on h (measured against the oracle in tests/test_gpu_mixed.py), i.e. NOT a substitute for
+// Accuracy: ~1e-6 relative on h for the BASELINE configs (tests/test_gpu_mixed.py), growing like 5e-7 / (2 pi f L / c)
+// for arms that are short against the wavelength (tests/test_gpu_random_sweep.py), i.e. NOT a substitute for
 // pespace_loglike in parameter estimation of SNR ~ 1e3 signals; throughput: DESIGN.md 8c.
 #pragma once
 #include "pespace_device.cuh"
