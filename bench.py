@@ -517,15 +517,18 @@ def run_ours(args):
     latency_info = None
     if args.others and world == 1:
         latency_info = []
-        for cfg in (2, 4):
-            wq = W.config(cfg, B=1)
+        # (config, N): the full one-month grids, and the paper's own protocol -- one theta per call against the number
+        # of frequency samples (Fig. 4; its PE runs use ~32.7 k bins) -- for one and five modes
+        for cfg, nq in ((2, None), (4, None), (2, 4096), (2, 32768), (3, 4096), (3, 32768), (3, None)):
+            wq = W.config(cfg, B=1, N=nq)
             psd_q = wq.psd()
             data_q = W.coloured_noise(psd_q, wq.grid.df, np.random.default_rng(5))
             lq = P.Likelihood(torch.from_numpy(np.ascontiguousarray(data_q)).to(device),
                               torch.from_numpy(psd_q).to(device), wq.grid, wq.model, 1)
             pq = torch.from_numpy(np.ascontiguousarray(wq.params)).to(device)
             oq = torch.empty(1, dtype=torch.float64, device=device)
-            row = {"config": cfg, "B": 1, "N": wq.grid.N, "n_det": len(wq.model.detectors)}
+            row = {"config": cfg, "B": 1, "N": wq.grid.N, "n_det": len(wq.model.detectors),
+                   "mode_mask": wq.model.mode_mask}
             for key in ("pespace_loglike_us", "pespace_loglike_prepared_us"):
                 if key.endswith("prepared_us"):
                     lq.prepare()
