@@ -393,7 +393,9 @@ __device__ __forceinline__ bool sample_in_domain(const double* th) {
 // Frame and detector blocks of the per-sample constants (O7, O8): the sky basis with the polarisation angle
 // absorbed, projected on the orbit basis of every detector, and the orbital phases at t_c.
 template <class T, class Put>
-__device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc, const PrepArgs& A, Put put) {
+__device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc, const PrepArgs& A, Put put,
+                           int det_lo = 0, int det_hi = PESPACE_MAX_DET) {
+  // detectors det_lo <= d < min(det_hi, n_det): all of them by default; one per thread in prep_samples_kernel
   // frame (O7) with the polarisation angle absorbed into the basis: u' = cos(psi) u + sin(psi) v, ...
   const T cl = p_cos(lam), sl = p_sin(lam), cb = p_cos(bet), sb = p_sin(bet), cp = p_cos(pol), sp = p_sin(pol);
   const T k[3] = {-(cb * cl), -(cb * sl), -sb};
@@ -405,7 +407,7 @@ __device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc
   const T* W3[3] = {k, up, vp};
   const int off[3] = {S_K - D_BASE, S_U - D_BASE, S_V - D_BASE};
   const double tcv = p_val(tc);
-  for (int dI = 0; dI < A.n_det; ++dI) {
+  for (int dI = det_lo; dI < A.n_det && dI < det_hi; ++dI) {
     const DetC& D = A.det[dI];
     const int base = D_BASE + D_STRIDE * dI;
     for (int i = 0; i < D_STRIDE; ++i) put(base + i, T(0.0));
@@ -446,14 +448,25 @@ __device__ void prep_frame(const T& lam, const T& bet, const T& pol, const T& tc
   }
 }
 
+// sec < 0: the whole block of constants (one thread per sample: the Fisher / gradient tangents, the orbit-table path).
+// sec >= 0: one of its 2 + n_det independent SECTIONS -- 0: phase and time polynomials, 1: mode amplitudes and
+// polarisation content, 2 + d: sky basis on the orbit basis of detector d -- so that prep_samples_kernel can give a
+// sample to 2 + n_det threads: the one-thread version is a chain of ~20 dependent library calls (cbrt, log, ten
+// divisions, eight sine / cosine pairs), 9.6 us for a single sample, which is the floor of the single-theta regime
+// (DESIGN.md 5.5).  Every constant is computed by the same expression in either mode.
 template <class T, class Put>
-__device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
+__device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put, int sec = -1) {
   const T M = th[0], q = th[1], chi1 = th[2], chi2 = th[3], DL = th[4], iota = th[5], phic = th[6],
           lam = th[7], bet = th[8], pol = th[9], tc = th[10];
+  if (sec >= 2) {
+    prep_frame(lam, bet, pol, tc, A, put, sec - 2, sec - 1);
+    return;
+  }
   const T Ms = M * (kGMsun / (kC * kC * kC));
   const T eta = q / ((1.0 + q) * (1.0 + q)), delta = (q - 1.0) / (q + 1.0);
   const T mu1 = q / (1.0 + q), mu2 = 1.0 / (1.0 + q);
   const T Ds = DL * (kGpc / kC);
+  if (sec <= 0) {                                        // ---- section 0: phase and time polynomials
   const T a = p_cbrt(kPi * Ms);
   const T lna = p_log(a);
   put(W_A, a); put(W_LNA, lna); put(W_TC, tc);
@@ -483,7 +496,10 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
   put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
   put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l) + cQ * ph6l * lna); put(W_Q6L, cQ * ph6l);
   put(W_Q7, 2.0 * cQ * ph7);
-  // amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
+  put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
+  }
+  if (sec == 0) return;
+  // ---- section 1: amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
   const T amp0 = p_sqrt(2.0 * eta / 3.0) * 0.82630748711075811083 * (Ms * Ms / Ds) / (Ms * p_sqrt(p_cbrt(Ms)));
   const double s57 = sqrt(5.0 / 7.0);
   const T clm[5] = {T(1.0), delta / 3.0, 0.75 * sqrt(15.0 / 14.0) * delta, s57 / 3.0 * (1.0 - 3.0 * eta),
@@ -505,8 +521,8 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put) {
     kam[4 * (m - 1) + 2 + slot] = 2.0 * Alm * Kc;      // factor 2 of n.e_x.n = 2 (n.u)(n.v)
   }
   for (int i = 0; i < 16; ++i) put(W_KA + i, kam[i]);
-  put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
-  prep_frame(lam, bet, pol, tc, A, put);
+  if (sec == 1) return;
+  prep_frame(lam, bet, pol, tc, A, put);                 // ---- sections 2 + d (all of them here: sec < 0)
 }
 
 // sine/cosine table of sincos_tab: trig[j] = (sin, cos)(2 pi j / NTAB), |error| <= 1 ulp (sincospi)
@@ -518,24 +534,36 @@ __device__ __forceinline__ void fill_trig_entry(double2* __restrict__ trig, long
   }
 }
 __host__ __device__ constexpr long long prep_threads(long long B) { return B > NTAB ? B : (long long)NTAB; }
+// threads of prep_samples_kernel: 2 + n_det sections per sample (prep_sample), each section of 32 samples in a warp of
+// its own (sections in one warp would run one after the other), at least NTAB threads for the table
+__host__ __device__ constexpr long long prep_threads(long long B, int n_det) {
+  return ((B + 31) / 32) * 32 * (2 + n_det) > NTAB ? ((B + 31) / 32) * 32 * (2 + n_det) : (long long)NTAB;
+}
 
-// grid covers prep_threads(B) threads: thread j < NTAB also writes table entry j (trig may be null)
+// grid covers prep_threads(B, n_det) threads: thread j < NTAB also writes table entry j (trig may be null); warp w
+// works on section w % (2 + n_det) of the samples 32 (w / (2 + n_det)) + lane
 static __global__ void prep_samples_kernel(const double* __restrict__ params, long long B, PrepArgs A,
                                     double* __restrict__ consts, double2* __restrict__ trig) {
-  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  fill_trig_entry(trig, b);
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  fill_trig_entry(trig, t);
+  const int nsec = 2 + A.n_det;
+  const long long w = t >> 5;
+  const int sec = (int)(w % nsec);
+  const long long b = (w / nsec) * 32 + (t & 31);
   if (b >= B) return;
   const double* thp = params + b * NPAR;
   const int stride = sample_stride(A.n_det);
   double* o = consts + b * stride;
   if (!sample_in_domain(thp)) {
-    for (int i = 0; i < stride; ++i) o[i] = 0.0;
-    o[W_A] = 1.0; o[W_VALID] = 0.0;
+    if (sec == 0) {
+      for (int i = 0; i < stride; ++i) o[i] = 0.0;
+      o[W_A] = 1.0; o[W_VALID] = 0.0;
+    }
     return;
   }
   double th[NPAR];
   for (int i = 0; i < NPAR; ++i) th[i] = thp[i];
-  prep_sample<double>(th, A, [o](int idx, double val) { o[idx] = val; });
+  prep_sample<double>(th, A, [o](int idx, double val) { o[idx] = val; }, sec);
 }
 
 // ---------------------------------------------------------------------------------------------

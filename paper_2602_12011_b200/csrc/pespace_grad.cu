@@ -72,7 +72,8 @@ int pespace::host::loglike_grad_impl(const double* d_params, int64_t B, const do
   double* d_partial = (double*)(ws + p.trig_bytes + p.bins_bytes + p.consts_bytes + p.du_bytes);
   const PrepArgs A = make_prep_args(model);
   // S1 twice: the plain constants the sweep reads, and their tangents for the chain rule of the second pass
-  prep_samples_kernel<<<(unsigned)((prep_threads(B) + 127) / 128), 128, 0, st>>>(d_params, B, A, d_consts, d_trig);
+  prep_samples_kernel<<<(unsigned)((prep_threads(B, model->n_det) + 127) / 128), 128, 0, st>>>(d_params, B, A, d_consts,
+                                                                                             d_trig);
   LAUNCHED();
   prep_samples_du_kernel<<<(unsigned)((B + 63) / 64), 64, 0, st>>>(d_params, B, A, d_du);
   LAUNCHED();

@@ -28,7 +28,7 @@ extern "C" int pespace_loglike_mixed(const double* d_params, int64_t B, const do
   double* d_bins = (double*)(ws + trig_bytes + consts_bytes + partial_bytes);
   const PrepArgs A = make_prep_args(model);
   const int th = 128;
-  prep_samples_kernel<<<(unsigned)((prep_threads(B) + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts, d_trig);
+  prep_samples_kernel<<<(unsigned)((prep_threads(B, n_det) + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts, d_trig);
   LAUNCHED();
   const GridC G = {grid->f0, grid->df, N};
   prep_bins_kernel<<<dim3((unsigned)((N + 255) / 256), (unsigned)n_det), 256, 0, st>>>((const double2*)d_data_AET, d_psd, G,

@@ -78,7 +78,8 @@ int pespace_response_noalloc(const double* d_params, int64_t B, const double* d_
   double2* d_trig = reinterpret_cast<double2*>(scratch);
   double* d_consts = reinterpret_cast<double*>(scratch + trig_bytes());
   const PrepArgs A = make_prep_args(model);
-  prep_samples_kernel<<<(unsigned)((prep_threads(B) + 127) / 128), 128, 0, st>>>(d_params, B, A, d_consts, d_trig);
+  prep_samples_kernel<<<(unsigned)((prep_threads(B, model->n_det) + 127) / 128), 128, 0, st>>>(d_params, B, A, d_consts,
+                                                                                             d_trig);
   LAUNCHED();
   const unsigned cm = class_mask(model->mode_mask);
   if (model->n_det > 1) {
