@@ -49,7 +49,8 @@ extern "C" int pespace_fisher(const double* d_params, int64_t B, const double* d
   double* d_bins = (double*)((char*)d_workspace + p.consts_bytes + p.partial_bytes);
   const PrepArgs A = make_prep_args(model);
   const int th = 64;
-  prep_samples_du_kernel<<<(unsigned)((B + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts);
+  prep_samples_du_kernel<<<(unsigned)((prep_du_threads(B, model->n_det) + th - 1) / th), th, 0, st>>>(d_params, B, A,
+                                                                                                    d_consts);
   LAUNCHED();
   const unsigned cm = class_mask(model->mode_mask);
   const GridC G = {grid->f0, grid->df, (long long)grid->N};

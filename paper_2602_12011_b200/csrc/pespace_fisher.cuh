@@ -362,17 +362,28 @@ __device__ __forceinline__ void fisher_class_cs(double MMmc, bool FIRST, const C
   component(2, 2, 1, -kap[0], 0, 0, kap[1], 1);    // Z = W_a B(3,2,k32) - W_b B(3,1,k31)
 }
 
-// ---- per-sample constants with tangents: consts_du [B][sample_stride(n_det)][DUW]
+// ---- per-sample constants with tangents: consts_du [B][sample_stride(n_det)][DUW].  Like prep_samples_kernel the
+// grid covers prep_du_threads(B, n_det) threads: warp w works on section w % (2 + n_det) (prep_sample) of the samples
+// 32 (w / (2 + n_det)) + lane
+__host__ __device__ constexpr long long prep_du_threads(long long B, int n_det) {
+  return ((B + 31) / 32) * 32 * (2 + n_det);
+}
 static __global__ void prep_samples_du_kernel(const double* __restrict__ params, long long B, PrepArgs A,
                                        double* __restrict__ consts) {
-  const long long b = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const int nsec = 2 + A.n_det;
+  const long long w = t >> 5;
+  const int sec = (int)(w % nsec);
+  const long long b = (w / nsec) * 32 + (t & 31);
   if (b >= B) return;
   const double* thp = params + b * NPAR;
   const int stride = sample_stride(A.n_det);
   double* o = consts + b * (long long)stride * DUW;
   if (!sample_in_domain(thp)) {
-    for (int i = 0; i < stride * DUW; ++i) o[i] = 0.0;
-    o[W_A * DUW] = 1.0;
+    if (sec == 0) {
+      for (int i = 0; i < stride * DUW; ++i) o[i] = 0.0;
+      o[W_A * DUW] = 1.0;
+    }
     return;
   }
   // tangent slots: M, q, chi1, chi2, iota, lambda, beta.  D_L, phi_c, psi and t_c are closed form.
@@ -386,7 +397,7 @@ static __global__ void prep_samples_du_kernel(const double* __restrict__ params,
     double* p = o + idx * DUW;
     p[0] = val.v;
     for (int t = 0; t < 7; ++t) p[1 + t] = val.d[t];
-  });
+  }, sec);
 }
 
 __device__ __forceinline__ void stage_tile_du(double* smem, const double* __restrict__ consts, long long b0,

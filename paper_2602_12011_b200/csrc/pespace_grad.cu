@@ -75,7 +75,7 @@ int pespace::host::loglike_grad_impl(const double* d_params, int64_t B, const do
   prep_samples_kernel<<<(unsigned)((prep_threads(B, model->n_det) + 127) / 128), 128, 0, st>>>(d_params, B, A, d_consts,
                                                                                              d_trig);
   LAUNCHED();
-  prep_samples_du_kernel<<<(unsigned)((B + 63) / 64), 64, 0, st>>>(d_params, B, A, d_du);
+  prep_samples_du_kernel<<<(unsigned)((prep_du_threads(B, model->n_det) + 63) / 64), 64, 0, st>>>(d_params, B, A, d_du);
   LAUNCHED();
   const GridC G = {grid->f0, grid->df, (long long)grid->N};
   if (!bins_ready) {

@@ -79,6 +79,19 @@ def gather_lnL(local: "np.ndarray", device=None) -> "np.ndarray":
     return torch.cat(out).cpu().numpy()
 
 
+def replicate(*tensors, src: int = 0):
+    """Replication of the data set, the PSD (and, for strong scaling, the theta batch) from rank `src` to every rank
+    ("data, weights and per-bin tables are replicated once (ncclBroadcast)"): one broadcast per
+    tensor, in place; every rank passes tensors of the same shape and dtype.  Returns the tensors.  Done once per
+    data set -- the hot loop has no collective besides the all-gather of ShardedCall."""
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        import torch
+        for t in tensors:
+            dist.broadcast(torch.view_as_real(t) if t.is_complex() else t, src=src)     # (re, im) pairs: same memory
+    return tensors if len(tensors) != 1 else tensors[0]
+
+
 class ShardedCall:
     """Strong scaling over samples for ANY per-sample call of the library: every rank holds the same
     data set and the same batch of theta, evaluates the samples [lo, hi) of `shard_bounds` with `local_eval` (theta

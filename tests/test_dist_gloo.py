@@ -40,6 +40,11 @@ def _worker(rank: int, world: int, port: int, B: int, out_dir: str) -> None:
     sharded = pdist.ShardedLikelihood(lambda p: torch.from_numpy(_stand_in_lnL(p.numpy())))
     strong = sharded(torch.from_numpy(wl.params)).numpy()          # same batch on every rank, split and gathered
     tiny = sharded(torch.from_numpy(wl.params[:1])).numpy()        # fewer samples than ranks: one rank idles
+    # replication of the data set from rank 0: rank 1 starts with zeros
+    d_ = torch.arange(24.0).reshape(2, 3, 4) if rank == 0 else torch.zeros(2, 3, 4)
+    p_ = torch.full((5,), 7.0) if rank == 0 else torch.zeros(5)
+    d_, p_ = pdist.replicate(d_, p_)
+    assert torch.equal(d_, torch.arange(24.0).reshape(2, 3, 4)) and torch.equal(p_, torch.full((5,), 7.0))
     # a call with several outputs (lnL, gradient-like [b][11], nothing, Fisher-like [b][11][11])
     multi = pdist.ShardedCall(lambda p: (torch.from_numpy(_stand_in_lnL(p.numpy())), -p, None,
                                          p[:, :, None] * p[:, None, :]))
@@ -91,3 +96,6 @@ def test_single_process_fallbacks():
     assert (t, u) == (3.5, 12.0)
     x = np.arange(5.0)
     assert np.array_equal(pdist.gather_lnL(x), x)
+    import torch
+    y = torch.ones(3)
+    assert pdist.replicate(y) is y                              # no process group: nothing to do

@@ -447,6 +447,8 @@ def test_sharded_likelihood_with_the_real_binding_under_nccl(P):
     assert not dist.is_initialized()
     dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1)
     try:
+        rep_d, rep_p = pdist.replicate(dev(data), dev(psd))                     # NCCL broadcast (one rank: identity)
+        assert torch.equal(torch.view_as_real(rep_d), torch.view_as_real(dev(data))) and torch.equal(rep_p, dev(psd))
         sharded = pdist.ShardedLikelihood(lambda p: lik(p))
         got = sharded(dev(wl.params)).cpu().numpy()
         assert np.array_equal(got, plain)
