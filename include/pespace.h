@@ -217,7 +217,8 @@ int pespace_fisher_tab(const double* d_params, int64_t B, const pespace_wavetabl
  * is the cubic Hermite interpolant with the node velocities as slopes.  Eq. 5 / Eq. 6 keep the nominal constant arm
  * length L_m of the detector description in the delays (the paper's formalism assumes rigid equal arms, PAPER.md:55,
  * :61); the link directions n_rs = (x_r - x_s) / |x_r - x_s| (unit vectors: the arms of a numerical orbit breathe) and
- * k.(x_r + x_s) come from the table; kind, kappa, lambda0, period_s, lon, lat of the description are ignored.  A mode whose t_lm(f) lies outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.  Waveform:
+ * k.(x_r + x_s) come from the table; kind, kappa, lambda0, period_s, lon, lat of the description are ignored.  A mode
+ * whose t_lm(f) lies outside [t0, t0 + (K-1) dt] contributes 0 at that frequency.  Waveform:
  * the analytic TaylorF2 modes of pespace_loglike.  Workspace of pespace_loglike_orb: pespace_workspace_bytes(B, grid,
  * model, 0).  Errors and per-sample domain as pespace_loglike. */
 typedef struct {

@@ -48,7 +48,8 @@ int run_prep(const double* d_params, long long B, const pespace_model* model, do
              cudaStream_t st) {
   const PrepArgs A = make_prep_args(model);
   const int th = 128;
-  prep_samples_kernel<<<(unsigned)((prep_threads(B, model->n_det) + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts, d_trig);
+  prep_samples_kernel<<<(unsigned)((prep_threads(B, model->n_det) + th - 1) / th), th, 0, st>>>(d_params, B, A, d_consts,
+                                                                                                d_trig);
   LAUNCHED();
   return PESPACE_OK;
 }

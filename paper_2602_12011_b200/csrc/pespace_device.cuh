@@ -467,36 +467,36 @@ __device__ void prep_sample(const T (&th)[NPAR], const PrepArgs& A, Put put, int
   const T mu1 = q / (1.0 + q), mu2 = 1.0 / (1.0 + q);
   const T Ds = DL * (kGpc / kC);
   if (sec <= 0) {                                        // ---- section 0: phase and time polynomials
-  const T a = p_cbrt(kPi * Ms);
-  const T lna = p_log(a);
-  put(W_A, a); put(W_LNA, lna); put(W_TC, tc);
-  put(W_PH0, -kTurn * (phic / kPi + 0.125));            // pu, for m/2 = 1
-  put(W_VALID, T(1.0));
-  // TaylorF2 3.5PN coefficients, spin terms per G3
-  const double pi2 = kPi * kPi;
-  const T bso = (113.0 / 12.0 * (mu1 * mu1) + 6.25 * eta) * chi1 + (113.0 / 12.0 * (mu2 * mu2) + 6.25 * eta) * chi2;
-  const T sss = 79.0 / 8.0 * (eta * chi1 * chi2);
-  const T ph2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
-  const T ph3 = -16.0 * kPi + 4.0 * bso;
-  const T ph4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * (eta * eta) - 10.0 * sss;
-  const T ph5a = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);          // phi5 = ph5a (1 + 3 ln v)
-  const T ph6a = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * pi2 - 6848.0 / 21.0 * kEuler +
-                 eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi2) + 76055.0 / 1728.0 * (eta * eta) -
-                 127825.0 / 1296.0 * (eta * eta * eta) - 6848.0 / 21.0 * log(4.0);   // phi6 = ph6a - 6848/21 ln v
-  const double ph6l = -6848.0 / 21.0;
-  const T ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * (eta * eta));
-  const T a5 = 1.0 / (a * a * a * a * a);
-  const T cP = kTurn * 3.0 / (256.0 * kPi * eta) * a5;  // kTurn Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
-  put(W_P0, cP); put(W_P2, cP * ph2); put(W_P3, cP * ph3); put(W_P4, cP * ph4);
-  // ln v = ln (pi Ms)^{1/3} + ln f'^{1/3}: the sample part of the logarithm is folded into the constant terms, so
-  // the kernels multiply the *L coefficients by ln f'^{1/3} only (one add less per bin, no tangent on L)
-  put(W_P5, cP * ph5a + cP * 3.0 * ph5a * lna); put(W_P5L, cP * 3.0 * ph5a);
-  put(W_P6, cP * ph6a + cP * ph6l * lna); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
-  const T cQ = cP / (3.0 * kYear);                       // kTurn (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
-  put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
-  put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l) + cQ * ph6l * lna); put(W_Q6L, cQ * ph6l);
-  put(W_Q7, 2.0 * cQ * ph7);
-  put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
+    const T a = p_cbrt(kPi * Ms);
+    const T lna = p_log(a);
+    put(W_A, a); put(W_LNA, lna); put(W_TC, tc);
+    put(W_PH0, -kTurn * (phic / kPi + 0.125));            // pu, for m/2 = 1
+    put(W_VALID, T(1.0));
+    // TaylorF2 3.5PN coefficients, spin terms per G3
+    const double pi2 = kPi * kPi;
+    const T bso = (113.0 / 12.0 * (mu1 * mu1) + 6.25 * eta) * chi1 + (113.0 / 12.0 * (mu2 * mu2) + 6.25 * eta) * chi2;
+    const T sss = 79.0 / 8.0 * (eta * chi1 * chi2);
+    const T ph2 = 3715.0 / 756.0 + 55.0 / 9.0 * eta;
+    const T ph3 = -16.0 * kPi + 4.0 * bso;
+    const T ph4 = 15293365.0 / 508032.0 + 27145.0 / 504.0 * eta + 3085.0 / 72.0 * (eta * eta) - 10.0 * sss;
+    const T ph5a = kPi * (38645.0 / 756.0 - 65.0 / 9.0 * eta);          // phi5 = ph5a (1 + 3 ln v)
+    const T ph6a = 11583231236531.0 / 4694215680.0 - 640.0 / 3.0 * pi2 - 6848.0 / 21.0 * kEuler +
+                   eta * (-15737765635.0 / 3048192.0 + 2255.0 / 12.0 * pi2) + 76055.0 / 1728.0 * (eta * eta) -
+                   127825.0 / 1296.0 * (eta * eta * eta) - 6848.0 / 21.0 * log(4.0);   // phi6 = ph6a - 6848/21 ln v
+    const double ph6l = -6848.0 / 21.0;
+    const T ph7 = kPi * (77096675.0 / 254016.0 + 378515.0 / 1512.0 * eta - 74045.0 / 756.0 * (eta * eta));
+    const T a5 = 1.0 / (a * a * a * a * a);
+    const T cP = kTurn * 3.0 / (256.0 * kPi * eta) * a5;  // kTurn Psi/(2 pi) = f'^{-5/3} * sum (cP phi_k) v^k
+    put(W_P0, cP); put(W_P2, cP * ph2); put(W_P3, cP * ph3); put(W_P4, cP * ph4);
+    // ln v = ln (pi Ms)^{1/3} + ln f'^{1/3}: the sample part of the logarithm is folded into the constant terms, so
+    // the kernels multiply the *L coefficients by ln f'^{1/3} only (one add less per bin, no tangent on L)
+    put(W_P5, cP * ph5a + cP * 3.0 * ph5a * lna); put(W_P5L, cP * 3.0 * ph5a);
+    put(W_P6, cP * ph6a + cP * ph6l * lna); put(W_P6L, cP * ph6l); put(W_P7, cP * ph7);
+    const T cQ = cP / (3.0 * kYear);                       // kTurn (t - t_c)/yr = f'^{-8/3} * sum (cQ q_k) v^k
+    put(W_Q0, -5.0 * cQ); put(W_Q2, -3.0 * cQ * ph2); put(W_Q3, -2.0 * cQ * ph3); put(W_Q4, -(cQ * ph4));
+    put(W_Q5, 3.0 * cQ * ph5a); put(W_Q6, cQ * (ph6a + ph6l) + cQ * ph6l * lna); put(W_Q6L, cQ * ph6l);
+    put(W_Q7, 2.0 * cQ * ph7);
+    put(W_MDL, -1.0 / DL); put(W_PAD, T(0.0));
   }
   if (sec == 0) return;
   // ---- section 1: amplitudes (O4, O5) and polarisation content (O6) per mode, gathered per class m
@@ -893,12 +893,22 @@ __global__ void __launch_bounds__(256) operand_probe_kernel(int iters, const dou
   const double m = in[threadIdx.x & 31];
 #pragma unroll
   for (int j = 0; j < 8; ++j) {
-    a[j] = in[(threadIdx.x + j) & 63]; b[j] = in[(threadIdx.x + 2 * j + 1) & 63]; c[j] = in[(threadIdx.x + 3 * j + 2) & 63];
+    a[j] = in[(threadIdx.x + j) & 63];
+    b[j] = in[(threadIdx.x + 2 * j + 1) & 63];
+    c[j] = in[(threadIdx.x + 3 * j + 2) & 63];
   }
 #pragma unroll
-  for (int j = 0; j < 16; ++j) { fa[j] = (float)in[(threadIdx.x + j) & 63]; fb[j] = (float)in[(threadIdx.x + 2 * j + 1) & 63]; fc[j] = (float)in[(threadIdx.x + 3 * j + 2) & 63]; }
+  for (int j = 0; j < 16; ++j) {
+    fa[j] = (float)in[(threadIdx.x + j) & 63];
+    fb[j] = (float)in[(threadIdx.x + 2 * j + 1) & 63];
+    fc[j] = (float)in[(threadIdx.x + 3 * j + 2) & 63];
+  }
 #pragma unroll
-  for (int j = 0; j < 8; ++j) { p[j] = make_float2(fa[2 * j], fa[2 * j + 1]); q[j] = make_float2(fb[2 * j], fb[2 * j + 1]); r[j] = make_float2(fc[2 * j], fc[2 * j + 1]); }
+  for (int j = 0; j < 8; ++j) {
+    p[j] = make_float2(fa[2 * j], fa[2 * j + 1]);
+    q[j] = make_float2(fb[2 * j], fb[2 * j + 1]);
+    r[j] = make_float2(fc[2 * j], fc[2 * j + 1]);
+  }
   const float fm = (float)m, fcc = fc[0];
   for (int i = 0; i < iters; ++i) {
 #pragma unroll

@@ -92,8 +92,14 @@ __device__ __forceinline__ double p_log(double x) { return log(x); }
 __device__ __forceinline__ double p_sin(double x) { return sin(x); }
 __device__ __forceinline__ double p_cos(double x) { return cos(x); }
 __device__ __forceinline__ double p_val(double x) { return x; }
-template <int N> __device__ __forceinline__ Du<N> p_sqrt(const Du<N>& a) { const double s = sqrt(a.v); return chain(a, s, 0.5 / s); }
-template <int N> __device__ __forceinline__ Du<N> p_cbrt(const Du<N>& a) { const double c = cbrt(a.v); return chain(a, c, c / (3.0 * a.v)); }
+template <int N> __device__ __forceinline__ Du<N> p_sqrt(const Du<N>& a) {
+  const double s = sqrt(a.v);
+  return chain(a, s, 0.5 / s);
+}
+template <int N> __device__ __forceinline__ Du<N> p_cbrt(const Du<N>& a) {
+  const double c = cbrt(a.v);
+  return chain(a, c, c / (3.0 * a.v));
+}
 template <int N> __device__ __forceinline__ Du<N> p_log(const Du<N>& a) { return chain(a, log(a.v), 1.0 / a.v); }
 template <int N> __device__ __forceinline__ Du<N> p_sin(const Du<N>& a) { return chain(a, sin(a.v), cos(a.v)); }
 template <int N> __device__ __forceinline__ Du<N> p_cos(const Du<N>& a) { return chain(a, cos(a.v), -sin(a.v)); }

@@ -1,5 +1,6 @@
 // pespace_inst.cuh -- body of the pespace_inst_*.cu translation units.  The including file defines
-//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher, 3 adjoint gradient, 4 fused multi-detector likelihood, 5 fused multi-detector response (kind unused)
+//   PESPACE_INST_WHAT  0 likelihood, 1 response, 2 Fisher, 3 adjoint gradient, 4 fused multi-detector likelihood,
+//                      5 fused multi-detector response (4, 5: kind unused)
 //   PESPACE_INST_KIND  0 heliocentric, 1 geocentric
 //   PESPACE_INST_HALF  0 class masks 1..7, 1 class masks 8..15
 #include "pespace_launch.hpp"

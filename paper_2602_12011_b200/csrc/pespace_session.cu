@@ -37,7 +37,8 @@ namespace {
 void release(pespace_session* s) {
   if (!s) return;
   cudaFree(s->d_params); cudaFree(s->d_data); cudaFree(s->d_psd); cudaFree(s->d_lnL); cudaFree(s->d_F);
-  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab); cudaFree(s->d_ws_g); cudaFree(s->d_grad_g);
+  cudaFree(s->d_grad); cudaFree(s->d_ws); cudaFree(s->d_ws_f); cudaFree(s->d_ws_t); cudaFree(s->d_tab);
+  cudaFree(s->d_ws_g); cudaFree(s->d_grad_g);
   if (s->h_lnL_pin) cudaFreeHost(s->h_lnL_pin);
   if (s->h_par_pin) cudaFreeHost(s->h_par_pin);
   if (s->st) cudaStreamDestroy(s->st);
