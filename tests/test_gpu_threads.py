@@ -79,3 +79,34 @@ def test_concurrent_host_threads_on_their_own_streams():
     for i in range(N_THREADS):
         for w, g in zip(want[i], got[i]):
             assert torch.equal(w, g), f"thread {i}: concurrent result differs from the serial one"
+
+
+def test_sessions_and_repeated_calls_do_not_leak_device_memory():
+    """100 session create / set_data / call / destroy cycles and 500 calls of the allocating pespace_response leave the
+    free device memory where it was (sessions own a stream, device and pinned buffers; pespace_response takes its
+    scratch from the stream-ordered pool)."""
+    import torch
+    from paper_2602_12011_b200 import binding as P
+    wl = W.config(4, B=8, N=4000)
+    psd = wl.psd()
+    data = W.coloured_noise(psd, wl.grid.df, np.random.default_rng(1))
+    th, f = dev(wl.params), dev(wl.grid.freqs())
+    out = torch.empty((wl.B, 3, 3, wl.grid.N, 2), dtype=torch.float64, device="cuda")
+
+    def cycle(n_sessions, n_calls):
+        for _ in range(n_sessions):
+            ses = P.Session(wl.grid, wl.model, wl.B, want_fisher=True)
+            ses.set_data(data, psd)
+            ses.loglike(wl.params)
+            ses.loglike_grad(wl.params)
+            ses.fisher(wl.params[:2])
+            ses.close()
+        for _ in range(n_calls):
+            P.response(th, f, wl.model, out)
+        torch.cuda.synchronize()
+
+    cycle(3, 10)                                              # first use: modules, pools
+    free0 = torch.cuda.mem_get_info()[0]
+    cycle(100, 500)
+    free1 = torch.cuda.mem_get_info()[0]
+    assert free1 >= free0 - (8 << 20), (free0, free1)         # nothing accumulates (8 MiB of slack for pool granularity)
