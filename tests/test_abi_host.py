@@ -204,3 +204,43 @@ def test_orb_argument_validation_without_a_device():
     assert L.pespace_loglike_orb(fake, 4, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 8, None) == -1
     assert L.pespace_loglike_orb(fake, 0, C.byref(good), fake, fake, C.byref(g), C.byref(m), fake, fake, 1 << 30,
                                  None) == -1
+
+
+def test_a_c_program_links_against_the_library(tmp_path):
+    """a caller written in C (not C++, no torch, no Python): includes include/pespace.h, links libpespace.so, asks for
+    the workspace size of BASELINE config 2, checks the no-allocation limits and that a bad call is refused with
+    PESPACE_EINVAL and a message -- everything that works without a GPU"""
+    import subprocess
+    from paper_2602_12011_b200 import binding as P     # builds the library if it is missing
+    src = tmp_path / "caller.c"
+    src.write_text(r'''
+#include <stdio.h>
+#include <string.h>
+#include "pespace.h"
+int main(void) {
+  pespace_detector det = {0};
+  det.kind = 0; det.tdi_gen = 20; det.L_m = 2.5e9; det.kappa = -0.349;
+  pespace_model model = {PESPACE_MODE_22, 1, &det};
+  pespace_grid grid = {1e-4, 1.0 / (30.0 * 86400.0), 262144};
+  size_t ws = pespace_workspace_bytes(4096, &grid, &model, 0);
+  size_t wg = pespace_workspace_bytes_grad(4096, &grid, &model);
+  if (ws == 0 || wg <= ws) return 1;
+  if (pespace_noalloc_scratch_needed(2016, &model) > PESPACE_NOALLOC_SCRATCH_BYTES) return 2;
+  if (pespace_noalloc_scratch_needed(2017, &model) <= PESPACE_NOALLOC_SCRATCH_BYTES) return 3;
+  if (pespace_loglike(NULL, 4096, NULL, NULL, &grid, &model, NULL, NULL, ws, NULL) != PESPACE_EINVAL) return 4;
+  if (strcmp(pespace_strerror(PESPACE_EINVAL), "invalid argument") != 0) return 5;
+  det.tdi_gen = 17;                                  /* unknown TDI generation */
+  if (pespace_workspace_bytes(4096, &grid, &model, 0) != 0) return 6;
+  printf("%s %zu %zu\n", pespace_version(), ws, wg);
+  return 0;
+}
+''')
+    exe = tmp_path / "caller"
+    libdir = os.path.dirname(P.LIB_PATH)
+    res = subprocess.run(["gcc", "-std=c99", "-Wall", "-Werror", "-I", os.path.join(ROOT, "include"), str(src), "-o", str(exe),
+                          "-L", libdir, "-lpespace", "-Wl,-rpath," + libdir], capture_output=True, text=True)
+    assert res.returncode == 0, res.stderr
+    run = subprocess.run([str(exe)], capture_output=True, text=True)
+    assert run.returncode == 0, (run.returncode, run.stdout, run.stderr)
+    version, ws, wg = run.stdout.strip().rsplit(" ", 2)
+    assert version == P.version() and int(ws) > 0 and int(wg) > int(ws)
