@@ -557,6 +557,22 @@ def run_ours(args):
             except RuntimeError as exc:                      # reported, never fatal for the bench line
                 row["pespace_loglike_prepared_graph_replay_us"] = None
                 row["graph_error"] = str(exc)[:200]
+            # lnL + reverse-mode gradient for one theta (a gradient-based sampler's step), prepared call
+            try:
+                gq_ = P.LikelihoodGrad(lq.data, lq.psd, wq.grid, wq.model, 1).prepare()
+                lo_, go_ = torch.empty(1, dtype=torch.float64, device=device), torch.empty((1, 11), dtype=torch.float64, device=device)
+                for _ in range(20):
+                    gq_(pq, lo_, go_)
+                torch.cuda.synchronize()
+                t0 = time.perf_counter()
+                for _ in range(200):
+                    gq_(pq, lo_, go_)
+                torch.cuda.synchronize()
+                row["pespace_loglike_grad_prepared_us"] = (time.perf_counter() - t0) / 200 * 1e6
+                del gq_
+            except RuntimeError as exc:
+                row["pespace_loglike_grad_prepared_us"] = None
+                row["grad_error"] = str(exc)[:200]
             latency_info.append(row)
             del lq
 
