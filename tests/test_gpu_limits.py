@@ -1,7 +1,7 @@
 """Maximum batch sizes (include/pespace.h: the sample tiles of a call fill gridDim.y = 65535): the largest accepted batch
 is evaluated correctly -- first, last and interior samples against the oracle, every result finite -- and one sample
 more is refused with PESPACE_EINVAL before anything is launched.  Likelihood: 65535 x 64 samples; reverse-mode
-gradient of a multi-class model: 65535 x 16."""
+gradient of a multi-class model: 65535 x 16; Fisher matrix: 65535 x 4."""
 import numpy as np
 import pytest
 
@@ -75,3 +75,29 @@ def test_largest_gradient_batch_and_one_more():
     assert (np.abs(grad.cpu().numpy()[idx] - go) / scale).max() <= TOL
     with pytest.raises(P.PespaceError, match="invalid argument"):
         lg(d_th)
+
+
+def test_largest_fisher_batch_and_one_more():
+    import torch
+    from paper_2602_12011_b200 import binding as P
+    grid = W.Grid(1.3e-4, 1.1e-5, 96)
+    model = W.Model(W.MODE_22 | W.MODE_21 | W.MODE_44, (W.lisa_like(15),))
+    rng = np.random.default_rng(8)
+    b_max = 65535 * 4
+    th = big_batch(b_max + 1, grid, rng)
+    wl = W.Workload("limits", grid, model, th[:8], th[0].copy(), 5)
+    psd, data = wl.psd(), wl.data(lambda p, f, m: oracle.response(p, f, m))
+    d_th = dev(th)
+    fi = P.Fisher(dev(data), dev(psd), grid, model, b_max + 1)
+    F, g = fi(d_th[:b_max])
+    assert bool(torch.isfinite(F).all()) and bool(torch.isfinite(g).all())
+    idx = np.array([0, 3, 4, 4099, 100001, b_max - 5, b_max - 1])
+    Fo, go = oracle.fisher(th[idx], data, psd, grid, model)
+    d = np.sqrt(np.einsum("bii->bi", Fo))
+    assert (np.abs(F.cpu().numpy()[idx] - Fo) / (d[:, :, None] * d[:, None, :])).max() <= TOL
+    want = oracle.loglike(th[idx], data, psd, grid, model)
+    hh = -2.0 * oracle.loglike(th[idx], np.zeros_like(data), psd, grid, model)
+    scale = d * np.sqrt(np.maximum(-2.0 * want, hh))[:, None]
+    assert (np.abs(g.cpu().numpy()[idx] - go) / scale).max() <= TOL
+    with pytest.raises(P.PespaceError, match="invalid argument"):
+        fi(d_th)
